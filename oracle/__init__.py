@@ -1,0 +1,160 @@
+"""CPU oracle for the FD EMRI harmonic sum -- TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package.  It shares no code with paper_2307_12585_b200 and never imports it.
+
+`load()` compiles oracle/fdemri_oracle.cpp with g++ (once) and returns a thin ctypes/numpy wrapper.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "fdemri_oracle.cpp")
+_HDR = os.path.join(_HERE, "fdemri_oracle.h")
+_LIB = os.path.join(_HERE, "libfdemri_oracle.so")
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int32)
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 -std=c++17 -fopenmp -ffp-contract=off -> oracle/libfdemri_oracle.so"""
+    stale = (not os.path.exists(_LIB)) or any(
+        os.path.getmtime(s) > os.path.getmtime(_LIB) for s in (_SRC, _HDR))
+    if force or stale:
+        cmd = ["g++", "-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC",
+               "-o", _LIB, _SRC]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+    return _LIB
+
+
+def _d(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(_dp)
+
+
+class Oracle:
+    def __init__(self, lib):
+        self.lib = lib
+        lib.fdemri_oracle_num_threads.restype = C.c_int
+
+    @property
+    def num_threads(self) -> int:
+        return int(self.lib.fdemri_oracle_num_threads())
+
+    def set_explicit(self, on: bool):
+        """Pin P7 switch: list voices stand for themselves only (no implied (l,-m,-n) partner)."""
+        self.lib.fdemri_oracle_set_explicit(C.c_int(1 if on else 0))
+
+    def build_splines(self, t, y):
+        """y: [n_comp][n_knots] -> (coef_hi, coef_lo) each [n_comp][n_knots-1][4]."""
+        t, tp = _d(t)
+        y = np.atleast_2d(np.ascontiguousarray(y, dtype=np.float64))
+        n_comp, N = y.shape
+        hi = np.empty((n_comp, N - 1, 4))
+        lo = np.empty((n_comp, N - 1, 4))
+        rc = self.lib.fdemri_oracle_build_splines(C.c_int(N), tp, C.c_int(n_comp), y.ctypes.data_as(_dp),
+                                                  hi.ctypes.data_as(_dp), lo.ctypes.data_as(_dp))
+        if rc:
+            raise ValueError(f"fdemri_oracle_build_splines -> {rc}")
+        return hi, lo
+
+    def ylm(self, l, m, theta, phi) -> complex:
+        re, im = C.c_double(), C.c_double()
+        rc = self.lib.fdemri_oracle_ylm(C.c_int(l), C.c_int(m), C.c_double(theta), C.c_double(phi),
+                                        C.byref(re), C.byref(im))
+        if rc:
+            raise ValueError("fdemri_oracle_ylm")
+        return complex(re.value, im.value)
+
+    def g(self, X) -> complex:
+        re, im = C.c_double(), C.c_double()
+        if self.lib.fdemri_oracle_g(C.c_double(X), C.byref(re), C.byref(im)):
+            raise ValueError("fdemri_oracle_g")
+        return complex(re.value, im.value)
+
+    def g_over_sqrt(self, Fdot, Fddot) -> complex:
+        re, im = C.c_double(), C.c_double()
+        if self.lib.fdemri_oracle_g_over_sqrt(C.c_double(Fdot), C.c_double(Fddot), C.byref(re), C.byref(im)):
+            raise ValueError("no term")
+        return complex(re.value, im.value)
+
+    def _outs(self, n_freq, want_extra):
+        hp = np.empty((n_freq, 2))
+        hx = np.empty((n_freq, 2))
+        nterms = np.zeros(n_freq, dtype=np.int32) if want_extra else None
+        amb = np.zeros(n_freq, dtype=np.uint8) if want_extra else None
+        return hp, hx, nterms, amb
+
+    def waveform(self, lmn, t, f_phi, f_r, Phi_phi, Phi_r, amp, freq, theta, phi, extra=True, n_threads=0):
+        """Level-C oracle: build splines in long double, then sum.  Single waveform (no batch axis).
+        Returns dict(hplus, hcross complex128[n_freq], n_evals, nterms, ambiguous, max_roots)."""
+        lmn = np.ascontiguousarray(lmn, dtype=np.int32)
+        t, tp = _d(t)
+        a1, p1 = _d(f_phi); a2, p2 = _d(f_r); a3, p3 = _d(Phi_phi); a4, p4 = _d(Phi_r)
+        amp, ap = _d(amp)
+        freq, fp = _d(freq)
+        n_modes, N, n_freq = lmn.shape[0], t.shape[0], freq.shape[0]
+        assert amp.shape == (n_modes, N, 2)
+        hp, hx, nterms, amb = self._outs(n_freq, extra)
+        ne = C.c_int64(0)
+        mr = C.c_int32(0)
+        rc = self.lib.fdemri_oracle_waveform(
+            C.c_int(n_modes), lmn.ctypes.data_as(_ip), C.c_int(N), tp, p1, p2, p3, p4, ap,
+            C.c_int64(n_freq), fp, C.c_double(theta), C.c_double(phi),
+            hp.ctypes.data_as(_dp), hx.ctypes.data_as(_dp), C.byref(ne),
+            nterms.ctypes.data_as(_ip) if extra else None,
+            amb.ctypes.data_as(C.POINTER(C.c_uint8)) if extra else None,
+            C.byref(mr), C.c_int(n_threads))
+        if rc:
+            raise ValueError(f"fdemri_oracle_waveform -> {rc}")
+        return dict(hplus=hp.view(np.complex128)[:, 0], hcross=hx.view(np.complex128)[:, 0],
+                    n_evals=int(ne.value), nterms=nterms, ambiguous=amb, max_roots=int(mr.value))
+
+    def sum(self, lmn, t, fphi_k, fr_k, sh_hi, sh_lo, am_hi, am_lo, freq, theta, phi, extra=True, n_threads=0):
+        """Level-A oracle: sum from given spline coefficients (hi + optional lo parts)."""
+        lmn = np.ascontiguousarray(lmn, dtype=np.int32)
+        t, tp = _d(t)
+        a1, p1 = _d(fphi_k); a2, p2 = _d(fr_k)
+        sh_hi, shp = _d(sh_hi)
+        am_hi, amp_ = _d(am_hi)
+        if sh_lo is not None:
+            sh_lo, slp = _d(sh_lo)
+        else:
+            slp = None
+        if am_lo is not None:
+            am_lo, alp = _d(am_lo)
+        else:
+            alp = None
+        freq, fp = _d(freq)
+        n_modes, N, n_freq = lmn.shape[0], t.shape[0], freq.shape[0]
+        assert sh_hi.shape == (4, N - 1, 4) and am_hi.shape == (n_modes, 2, N - 1, 4)
+        hp, hx, nterms, amb = self._outs(n_freq, extra)
+        ne = C.c_int64(0)
+        mr = C.c_int32(0)
+        rc = self.lib.fdemri_oracle_sum(
+            C.c_int(n_modes), lmn.ctypes.data_as(_ip), C.c_int(N), tp, p1, p2, shp, slp, amp_, alp,
+            C.c_int64(n_freq), fp, C.c_double(theta), C.c_double(phi),
+            hp.ctypes.data_as(_dp), hx.ctypes.data_as(_dp), C.byref(ne),
+            nterms.ctypes.data_as(_ip) if extra else None,
+            amb.ctypes.data_as(C.POINTER(C.c_uint8)) if extra else None,
+            C.byref(mr), C.c_int(n_threads))
+        if rc:
+            raise ValueError(f"fdemri_oracle_sum -> {rc}")
+        return dict(hplus=hp.view(np.complex128)[:, 0], hcross=hx.view(np.complex128)[:, 0],
+                    n_evals=int(ne.value), nterms=nterms, ambiguous=amb, max_roots=int(mr.value))
+
+
+_ORACLE = None
+
+
+def load() -> Oracle:
+    global _ORACLE
+    if _ORACLE is None:
+        _ORACLE = Oracle(C.CDLL(build()))
+    return _ORACLE
