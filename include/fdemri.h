@@ -1,0 +1,117 @@
+/* fdemri.h -- C ABI of libfdemri: the frequency-domain EMRI harmonic sum of arXiv:2307.12585 on one
+ * NVIDIA B200 (sm_100a), FP64.
+ *
+ * What it computes (PAPER.md = /root/reference/PAPER.md of the build; see DESIGN.md for the readings):
+ *   S1  not-a-knot cubic splines of f_phi, f_r, Phi_phi, Phi_r and of Re/Im A_lmn over the sparse
+ *       trajectory;
+ *   S2  per voice (l,m,n) and segment, the cubic  f = A + B tau + C tau^2 + D tau^3  (Eq. 6) and
+ *       the contiguous range of frequency bins it covers, "predetermined before the summation" (L105);
+ *   S3  per bin and root t_j(f) the term of Eq. 9 (L107-119):
+ *         A(t) g(X)/sqrt|Fdot| exp{i[2 pi f t - Phi(t)]},  X = 2 pi Fdot^3 / (3 Fddot^2),
+ *       summed over voices with the spin-weighted harmonics (Eq. 1) into h~+(f), h~x(f), the
+ *       (l,-m,-n) partner of every m>0 voice taken from the symmetry A -> (-1)^l conj A;
+ *   S4  one coalesced store per bin (no atomics; the paper's kernel adds atomically, L121).
+ *
+ * Conventions
+ *   - "dev" pointers are CUDA device pointers, "host" pointers are host pointers.  The caller owns every
+ *     buffer, including the work space; the plan owns only small host metadata.
+ *   - Nothing here allocates device memory, and build_splines / sum do not synchronise: they enqueue
+ *     kernels on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ *   - Every function returns a status: 0 = FDEMRI_OK, >0 = error.  No exceptions, no printing.
+ *   - Asynchronous CUDA errors surface in the next call or in fdemri_get_stats (which synchronises).
+ */
+#ifndef FDEMRI_H
+#define FDEMRI_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    FDEMRI_OK = 0,
+    FDEMRI_ERR_INVALID_ARG = 1, /* bad size, NULL pointer, l<2, m<0, m>l, unsorted knots ...            */
+    FDEMRI_ERR_WORKSPACE = 2,   /* work space missing or too small                                        */
+    FDEMRI_ERR_CUDA = 3,        /* a CUDA runtime call or kernel failed                                   */
+    FDEMRI_ERR_NOT_BUILT = 4,   /* fdemri_sum / get_coeffs before fdemri_build_splines                    */
+    FDEMRI_ERR_UNSUPPORTED = 5  /* input violates an assumption of the method (see fdemri_stats.flags)    */
+};
+
+/* plan flags */
+enum {
+    FDEMRI_FLAG_NONE = 0
+};
+
+/* bits of fdemri_stats.flags (device-side validation, read back by fdemri_get_stats) */
+enum {
+    FDEMRI_BAD_TWO_EXTREMA = 1,   /* a segment cubic has two interior extrema (paper assumes <= 1, L105)   */
+    FDEMRI_BAD_STRIP_OVERFLOW = 2,/* a voice has more monotone branches than the map holds                 */
+    FDEMRI_BAD_NONFINITE = 4,     /* NaN/Inf met in the inputs or spline coefficients                      */
+    FDEMRI_BAD_NEWTON = 8         /* a root iteration hit its iteration cap                                */
+};
+
+typedef struct fdemri_plan_s* fdemri_plan_t;
+
+typedef struct {
+    uint64_t n_items;        /* non-empty (voice, sign, segment-branch) items of the last sum (S2)            */
+    uint64_t n_strips;       /* monotone branches ("strips") those items form                               */
+    uint64_t n_evals;        /* accumulated (voice, sign, root, bin) terms = "mode-bin evaluations" (P9)      */
+    uint64_t n_turnover;     /* segments with an interior extremum of F (Fdot = 0, L92, L105)                 */
+    uint64_t n_airy;         /* evaluations that took the small-|X| (Airy) path                              */
+    uint64_t flags;          /* OR of FDEMRI_BAD_*                                                            */
+} fdemri_stats;
+
+/* Create a plan.
+ *  lmn_host    [n_modes][3] int32 (l, m, n) with l >= 2, 0 <= m <= l; copied.  The partner (l,-m,-n) of every
+ *              m > 0 voice is implied (L64-66 + symmetry); m = 0 voices stand for themselves.
+ *  n_batch     number of independent parameter sets evaluated per call (>= 1)
+ *  n_knots     points of the sparse trajectory (4..512), the same for every batch item (L58: ~100)
+ *  t_knots_dev [n_batch][n_knots] seconds, strictly increasing; borrowed until fdemri_build_splines returns
+ *  n_freq      number of frequency bins
+ *  freq_dev    [n_freq] Hz, sorted ascending, >= 0, shared by the batch; borrowed for the plan's life.
+ *              NULL selects the uniform grid  f_i = f0 + (double)i*df  (product rounded, then sum rounded) --
+ *              with f0 = 0, df = 1/T the DFT grid of L141.
+ */
+int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, int n_batch, int n_knots,
+                const double* t_knots_dev, int64_t n_freq, const double* freq_dev, double f0, double df,
+                uint32_t flags);
+
+/* Device work space the plan needs (bytes); the caller allocates it (256-byte aligned) and hands it over.
+ * The work space holds the spline records and the segment->bin map; it must stay valid and untouched
+ * between build_splines and the last sum. */
+size_t fdemri_workspace_bytes(fdemri_plan_t plan);
+int fdemri_set_workspace(fdemri_plan_t plan, void* dev_ptr, size_t bytes);
+
+/* S1.  All inputs are device pointers, borrowed until the enqueued kernels have run.
+ *  f_phi, f_r      [n_batch][n_knots] Hz      fundamental frequencies Omega/(2 pi M) at the knots (L94)
+ *  Phi_phi, Phi_r  [n_batch][n_knots] rad     fundamental phases at the knots (L56)
+ *  amp             [n_batch][n_modes][n_knots][2] (re, im) mode amplitudes at the knots (L60), with mu/d_L of
+ *                  Eq. 1 folded in by the caller */
+int fdemri_build_splines(fdemri_plan_t plan, const double* f_phi, const double* f_r, const double* Phi_phi,
+                         const double* Phi_r, const double* amp, void* cuda_stream);
+
+/* S0 + S2 + S3 + S4.
+ *  theta_host, phi_host  source-frame viewing angles (L66), [n_angles] on the host, n_angles = 1 or n_batch
+ *  hplus_dev, hcross_dev [n_batch][n_freq][2] (re, im) FP64, fully overwritten (zeros where no voice has
+ *                        support, L147; the bin f = 0 is always zero) */
+int fdemri_sum(fdemri_plan_t plan, int n_angles, const double* theta_host, const double* phi_host,
+               double* hplus_dev, double* hcross_dev, void* cuda_stream);
+
+/* Counters of the last fdemri_sum (synchronises the stream used by that call). */
+int fdemri_get_stats(fdemri_plan_t plan, fdemri_stats* out);
+
+/* Spline coefficients as built on the device, for parity level A (oracle fed the GPU's coefficients).
+ *  shared_hi, shared_lo [n_batch][4][n_knots-1][4]  (a,b,c,d) of f_phi, f_r, Phi_phi, Phi_r as hi + lo doubles
+ *  amp_coef             [n_batch][n_modes][2][n_knots-1][4]  (a,b,c,d) of Re A, Im A
+ * Device pointers; any may be NULL.  Enqueued on the stream of the last build_splines. */
+int fdemri_get_coeffs(fdemri_plan_t plan, double* shared_hi_dev, double* shared_lo_dev, double* amp_coef_dev);
+
+int fdemri_destroy(fdemri_plan_t plan);
+const char* fdemri_strerror(int status);
+/* Library version string, e.g. "fdemri 0.1 sm_100a". */
+const char* fdemri_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

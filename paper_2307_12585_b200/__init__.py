@@ -1,0 +1,9 @@
+"""fdemri: B200-native frequency-domain EMRI harmonic sum (arXiv:2307.12585), FP64, sm_100a.
+
+The product is the C-ABI CUDA library libfdemri.so (include/fdemri.h); this package is its thin binding
+plus the seeded input generator (`synth`).  There is no CPU fallback.
+"""
+from . import synth  # noqa: F401
+from .binding import (FdemriError, Waveform, fdemri_build_splines, fdemri_destroy, fdemri_get_coeffs,  # noqa: F401
+                      fdemri_get_stats, fdemri_plan, fdemri_set_workspace, fdemri_sum, fdemri_version,
+                      fdemri_workspace_bytes, waveform_from_workload)

@@ -1,0 +1,290 @@
+// fdemri.cu -- host side of libfdemri (C ABI of include/fdemri.h).  One translation unit: the kernels live
+// in the .cuh files included below.  Build: see paper_2307_12585_b200/build.py
+//   nvcc -O3 -std=c++17 -gencode arch=compute_100a,code=sm_100a -lineinfo -Xcompiler -fPIC -shared
+#include "../../include/fdemri.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "fdemri_common.cuh"
+#include "fdemri_map.cuh"
+#include "fdemri_splines.cuh"
+#include "fdemri_strips.cuh"
+#include "fdemri_sum.cuh"
+
+struct fdemri_plan_s {
+    FdemriDims d;
+    std::vector<int32_t> lmn;
+    const double* t_knots_dev;
+    // work space carve-up (device pointers)
+    void* ws;
+    size_t ws_bytes;
+    int* lmn_dev;
+    SplineFac* fac;
+    double *sh_hi, *sh_lo, *rec;
+    int2* ent;
+    StripRaw* strips;
+    int* n_strips;
+    int4* dense;
+    int* n_dense;
+    int dense_cap;
+    double4* wts;
+    double* angles;
+    unsigned long long* stats;     // [0..5] = fdemri_stats, [6] = tile counter (low 32 bits)
+    std::vector<double> angle_stage;
+    bool built;
+    cudaStream_t last_stream;
+    int sm_count;
+};
+
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// walks the carve-up; with base == nullptr only sizes are computed
+static size_t carve(fdemri_plan_s* p, char* base) {
+    const FdemriDims& d = p->d;
+    size_t off = 0;
+    const size_t B = d.n_batch, V = d.n_modes, N = d.n_knots, S = d.n_seg;
+    auto take = [&](size_t bytes) {
+        char* ptr = base ? base + off : nullptr;
+        off += align_up(bytes);
+        return ptr;
+    };
+    p->lmn_dev = (int*)take(V * 3 * sizeof(int));
+    p->fac = (SplineFac*)take(B * N * sizeof(SplineFac));
+    p->sh_hi = (double*)take(B * 4 * S * 4 * sizeof(double));
+    p->sh_lo = (double*)take(B * 4 * S * 4 * sizeof(double));
+    p->rec = (double*)take(B * V * S * R_DOUBLES * sizeof(double));
+    p->ent = (int2*)take(B * V * 2 * (size_t)d.ent_max * sizeof(int2));
+    p->strips = (StripRaw*)take(B * V * 2 * FDEMRI_MAX_STRIPS * sizeof(StripRaw));
+    p->n_strips = (int*)take(B * V * 2 * sizeof(int));
+    p->dense_cap = (int)(2 * V * FDEMRI_MAX_STRIPS);
+    p->dense = (int4*)take(B * (size_t)p->dense_cap * sizeof(int4));
+    p->n_dense = (int*)take(B * sizeof(int));
+    p->wts = (double4*)take(B * V * sizeof(double4));
+    p->angles = (double*)take(B * 2 * sizeof(double));
+    p->stats = (unsigned long long*)take(8 * sizeof(unsigned long long));
+    return off;
+}
+
+extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, int n_batch, int n_knots,
+                           const double* t_knots_dev, int64_t n_freq, const double* freq_dev, double f0, double df,
+                           uint32_t flags) {
+    (void)flags;
+    if (!out) return FDEMRI_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (n_modes < 1 || n_modes > (1 << 20) || !lmn_host || n_batch < 1 || n_knots < 4 || n_knots > FDEMRI_MAX_KNOTS ||
+        !t_knots_dev || n_freq < 1 || n_freq >= ((int64_t)1 << 31) - FDEMRI_TILE)
+        return FDEMRI_ERR_INVALID_ARG;
+    if (!freq_dev && !(df > 0.0 && std::isfinite(df) && std::isfinite(f0) && f0 >= 0.0)) return FDEMRI_ERR_INVALID_ARG;
+    for (int v = 0; v < n_modes; ++v) {
+        int l = lmn_host[3 * v], m = lmn_host[3 * v + 1], n = lmn_host[3 * v + 2];
+        if (l < 2 || l > 60 || m < 0 || m > l || n < -100000 || n > 100000) return FDEMRI_ERR_INVALID_ARG;
+    }
+    int64_t n_tiles = (n_freq + FDEMRI_TILE - 1) / FDEMRI_TILE;
+    if (n_tiles * (int64_t)n_batch >= ((int64_t)1 << 31)) return FDEMRI_ERR_INVALID_ARG;
+    fdemri_plan_s* p = new (std::nothrow) fdemri_plan_s();
+    if (!p) return FDEMRI_ERR_INVALID_ARG;
+    p->d.n_modes = n_modes;
+    p->d.n_batch = n_batch;
+    p->d.n_knots = n_knots;
+    p->d.n_seg = n_knots - 1;
+    p->d.ent_max = n_knots - 1 + FDEMRI_ENT_EXTRA;
+    p->d.n_freq = n_freq;
+    p->d.n_tiles = (int)n_tiles;
+    p->d.f0 = f0;
+    p->d.df = df;
+    p->d.freq = freq_dev;
+    p->lmn.assign(lmn_host, lmn_host + (size_t)3 * n_modes);
+    p->t_knots_dev = t_knots_dev;
+    p->ws = nullptr;
+    p->ws_bytes = 0;
+    p->built = false;
+    p->last_stream = nullptr;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        delete p;
+        return FDEMRI_ERR_CUDA;
+    }
+    p->sm_count = prop.multiProcessorCount;
+    carve(p, nullptr);
+    *out = p;
+    return FDEMRI_OK;
+}
+
+extern "C" size_t fdemri_workspace_bytes(fdemri_plan_t p) {
+    if (!p) return 0;
+    fdemri_plan_s tmp = *p;
+    return carve(&tmp, nullptr);
+}
+
+extern "C" int fdemri_set_workspace(fdemri_plan_t p, void* dev_ptr, size_t bytes) {
+    if (!p || !dev_ptr) return FDEMRI_ERR_INVALID_ARG;
+    if (((uintptr_t)dev_ptr & 255) != 0) return FDEMRI_ERR_INVALID_ARG;
+    if (bytes < fdemri_workspace_bytes(p)) return FDEMRI_ERR_WORKSPACE;
+    p->ws = dev_ptr;
+    p->ws_bytes = bytes;
+    carve(p, (char*)dev_ptr);
+    p->built = false;
+    if (cudaMemcpy(p->lmn_dev, p->lmn.data(), p->lmn.size() * sizeof(int32_t), cudaMemcpyHostToDevice) != cudaSuccess)
+        return FDEMRI_ERR_CUDA;
+    if (cudaMemset(p->stats, 0, 8 * sizeof(unsigned long long)) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    return FDEMRI_OK;
+}
+
+template <int MAXN>
+static void launch_splines(fdemri_plan_s* p, const double* f_phi, const double* f_r, const double* Phi_phi,
+                           const double* Phi_r, const double* amp, cudaStream_t st) {
+    const FdemriDims& d = p->d;
+    int nb = (d.n_batch * 4 + 63) / 64;
+    k_spline_shared<MAXN><<<nb, 64, 0, st>>>(d.n_batch, d.n_knots, f_phi, f_r, Phi_phi, Phi_r, p->fac, p->sh_hi,
+                                             p->sh_lo, p->stats + 5);
+    size_t nt = (size_t)d.n_batch * d.n_modes * 2;
+    k_spline_amp<MAXN><<<(unsigned)((nt + 127) / 128), 128, 0, st>>>(d.n_batch, d.n_modes, d.n_knots, amp, p->fac,
+                                                                      p->rec, p->stats + 5);
+}
+
+extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const double* f_r, const double* Phi_phi,
+                                    const double* Phi_r, const double* amp, void* cuda_stream) {
+    if (!p || !f_phi || !f_r || !Phi_phi || !Phi_r || !amp) return FDEMRI_ERR_INVALID_ARG;
+    if (!p->ws) return FDEMRI_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const FdemriDims& d = p->d;
+    p->last_stream = st;
+    if (cudaMemsetAsync(p->stats, 0, 8 * sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    k_spline_factor<<<(d.n_batch + 63) / 64, 64, 0, st>>>(d.n_batch, d.n_knots, p->t_knots_dev, p->fac, p->stats + 5);
+    if (d.n_knots <= 128) launch_splines<128>(p, f_phi, f_r, Phi_phi, Phi_r, amp, st);
+    else if (d.n_knots <= 256) launch_splines<256>(p, f_phi, f_r, Phi_phi, Phi_r, amp, st);
+    else launch_splines<FDEMRI_MAX_KNOTS>(p, f_phi, f_r, Phi_phi, Phi_r, amp, st);
+    size_t nrec = (size_t)d.n_batch * d.n_modes * d.n_seg;
+    k_records<<<(unsigned)((nrec + 127) / 128), 128, 0, st>>>(d, p->lmn_dev, p->t_knots_dev, p->sh_hi, p->sh_lo, p->rec,
+                                                              p->stats);
+    size_t nvs = (size_t)d.n_batch * d.n_modes * 2;
+    k_strips<<<(unsigned)((nvs + 63) / 64), 64, 0, st>>>(d, p->lmn_dev, f_phi, f_r, p->rec, p->ent, p->strips,
+                                                         p->n_strips, p->stats);
+    k_strip_compact<<<d.n_batch, 1024, 0, st>>>(d.n_modes, p->dense_cap, p->strips, p->n_strips, p->dense, p->n_dense);
+    if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
+    p->built = true;
+    return FDEMRI_OK;
+}
+
+extern "C" int fdemri_sum(fdemri_plan_t p, int n_angles, const double* theta_host, const double* phi_host,
+                          double* hplus_dev, double* hcross_dev, void* cuda_stream) {
+    if (!p || !theta_host || !phi_host || !hplus_dev || !hcross_dev) return FDEMRI_ERR_INVALID_ARG;
+    if (!p->ws) return FDEMRI_ERR_WORKSPACE;
+    if (!p->built) return FDEMRI_ERR_NOT_BUILT;
+    const FdemriDims& d = p->d;
+    if (n_angles != 1 && n_angles != d.n_batch) return FDEMRI_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    p->last_stream = st;
+    p->angle_stage.resize((size_t)2 * n_angles);
+    for (int i = 0; i < n_angles; ++i) {
+        if (!std::isfinite(theta_host[i]) || !std::isfinite(phi_host[i])) return FDEMRI_ERR_INVALID_ARG;
+        p->angle_stage[2 * i] = theta_host[i];
+        p->angle_stage[2 * i + 1] = phi_host[i];
+    }
+    if (cudaMemcpyAsync(p->angles, p->angle_stage.data(), p->angle_stage.size() * sizeof(double),
+                        cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return FDEMRI_ERR_CUDA;
+    // S0
+    int nw = n_angles * d.n_modes;
+    k_weights<<<(nw + 127) / 128, 128, 0, st>>>(n_angles, d.n_modes, p->lmn_dev, p->angles, p->wts);
+    // reset the per-sum counters: n_airy (slot 4) and the tile counter (slot 6)
+    if (cudaMemsetAsync(p->stats + 4, 0, sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    if (cudaMemsetAsync(p->stats + 6, 0, sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    SumArgs a;
+    a.d = d;
+    a.rec = p->rec;
+    a.ent = p->ent;
+    a.dense = p->dense;
+    a.n_dense = p->n_dense;
+    a.dense_cap = p->dense_cap;
+    a.wts = p->wts;
+    a.n_angles = n_angles;
+    a.hp = hplus_dev;
+    a.hx = hcross_dev;
+    a.tile_counter = (unsigned int*)(p->stats + 6);
+    a.stats = p->stats;
+    a.total_tiles = d.n_tiles * d.n_batch;
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_tile_sum, FDEMRI_TILE, 0) != cudaSuccess || per_sm < 1)
+        per_sm = 1;
+    long long grid = (long long)p->sm_count * per_sm;
+    if (grid > a.total_tiles) grid = a.total_tiles;
+    k_tile_sum<<<(unsigned)grid, FDEMRI_TILE, 0, st>>>(a);
+    if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
+    return FDEMRI_OK;
+}
+
+extern "C" int fdemri_get_stats(fdemri_plan_t p, fdemri_stats* out) {
+    if (!p || !out) return FDEMRI_ERR_INVALID_ARG;
+    if (!p->ws) return FDEMRI_ERR_WORKSPACE;
+    unsigned long long h[8];
+    if (cudaStreamSynchronize(p->last_stream) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    if (cudaMemcpy(h, p->stats, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    out->n_items = h[0];
+    out->n_strips = h[1];
+    out->n_evals = h[2];
+    out->n_turnover = h[3];
+    out->n_airy = h[4];
+    out->flags = h[5];
+    if (h[5] & (FDEMRI_BAD_TWO_EXTREMA | FDEMRI_BAD_STRIP_OVERFLOW)) return FDEMRI_ERR_UNSUPPORTED;
+    if (h[5] & FDEMRI_BAD_NONFINITE) return FDEMRI_ERR_INVALID_ARG;
+    return FDEMRI_OK;
+}
+
+// amp_coef[b][v][c][k][j] <- rec[b][v][k][R_AR + 4c + j]
+__global__ void k_gather_amp(size_t total, int S, const double* __restrict__ rec, double* __restrict__ out) {
+    size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= total) return;
+    int j = (int)(id & 3);
+    size_t r = id >> 2;
+    int k = (int)(r % S);
+    r /= S;
+    int c = (int)(r & 1);
+    size_t bv = r >> 1;
+    out[id] = rec[(bv * S + k) * R_DOUBLES + (c ? R_AI : R_AR) + j];
+}
+
+extern "C" int fdemri_get_coeffs(fdemri_plan_t p, double* shared_hi_dev, double* shared_lo_dev, double* amp_coef_dev) {
+    if (!p) return FDEMRI_ERR_INVALID_ARG;
+    if (!p->ws) return FDEMRI_ERR_WORKSPACE;
+    if (!p->built) return FDEMRI_ERR_NOT_BUILT;
+    const FdemriDims& d = p->d;
+    cudaStream_t st = p->last_stream;
+    size_t nsh = (size_t)d.n_batch * 4 * d.n_seg * 4 * sizeof(double);
+    if (shared_hi_dev && cudaMemcpyAsync(shared_hi_dev, p->sh_hi, nsh, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+        return FDEMRI_ERR_CUDA;
+    if (shared_lo_dev && cudaMemcpyAsync(shared_lo_dev, p->sh_lo, nsh, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+        return FDEMRI_ERR_CUDA;
+    if (amp_coef_dev) {
+        size_t total = (size_t)d.n_batch * d.n_modes * 2 * d.n_seg * 4;
+        k_gather_amp<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(total, d.n_seg, p->rec, amp_coef_dev);
+        if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
+    }
+    return FDEMRI_OK;
+}
+
+extern "C" int fdemri_destroy(fdemri_plan_t p) {
+    if (!p) return FDEMRI_ERR_INVALID_ARG;
+    delete p;
+    return FDEMRI_OK;
+}
+
+extern "C" const char* fdemri_strerror(int status) {
+    switch (status) {
+        case FDEMRI_OK: return "ok";
+        case FDEMRI_ERR_INVALID_ARG: return "invalid argument";
+        case FDEMRI_ERR_WORKSPACE: return "work space missing or too small";
+        case FDEMRI_ERR_CUDA: return "CUDA error";
+        case FDEMRI_ERR_NOT_BUILT: return "splines not built";
+        case FDEMRI_ERR_UNSUPPORTED: return "input violates an assumption of the method";
+        default: return "unknown status";
+    }
+}
+
+extern "C" const char* fdemri_version(void) { return "fdemri 0.1 sm_100a"; }

@@ -1,0 +1,115 @@
+// fdemri_common.cuh -- layouts and small device helpers shared by the kernels of libfdemri.
+// Product code: nothing here comes from (or is shared with) oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define FDEMRI_MAX_KNOTS 512
+#define FDEMRI_MAX_STRIPS 8          // monotone branches kept per (voice, sign)
+#define FDEMRI_ENT_EXTRA 8           // entries per (voice, sign) = (n_knots-1) + FDEMRI_ENT_EXTRA
+#define FDEMRI_TILE 256              // bins per tile = threads per CTA of the sum kernel
+
+// ------------------------------------------------------------------------------------------------
+// Record of one (voice, segment): everything the sum needs about that piece of trajectory.
+// 24 doubles = 192 B.  tau = t - t_k.
+// ------------------------------------------------------------------------------------------------
+enum {
+    R_FA = 0,   // F(tau) = FA + FB tau + FC tau^2 + FD tau^3  (Eq. 6); FA is the knot value F_k (R6)
+    R_FB = 1,
+    R_FC = 2,
+    R_FD = 3,
+    R_PC = 4,   // phase constant in cycles: -frac(Phi_v(t_k)/2pi) + m*phi/2pi
+    R_BH = 5,   // b' = b_Phi/2pi as hi + lo
+    R_BL = 6,
+    R_NC = 7,   // -c_Phi/2pi
+    R_AR = 8,   // Re A coefficients a,b,c,d  (8..11)   (32-byte aligned: written as one double4)
+    R_AI = 12,  // Im A coefficients a,b,c,d  (12..15)
+    R_ND = 16,  // -d_Phi/2pi
+    R_TK = 17,  // t_k
+    R_Q1 = 18,  // normal segment: seed tau0 = x (Q1 + x (Q2 + x Q3)), x = s f - FA
+    R_Q2 = 19,  // turnover segment: Q1 = tau_e, Q2 = F_e, Q3 = C + 3 D tau_e
+    R_Q3 = 20,
+    R_H = 21,   // segment length h_k
+    R_TYPE = 22,// 0.0 normal, 1.0 turnover (one interior extremum)
+    R_SPARE = 23,
+    R_DOUBLES = 24
+};
+
+struct FdemriDims {
+    int n_modes, n_batch, n_knots, n_seg;   // n_seg = n_knots - 1
+    int ent_max;                            // entries per (voice, sign)
+    int64_t n_freq;
+    int n_tiles;                            // tiles per batch item
+    double f0, df;
+    const double* freq;                     // NULL => uniform grid
+};
+
+// frequency of bin i: explicit array, or the uniform grid f0 + i*df with a rounded product and a rounded sum
+__device__ __forceinline__ double fdemri_freq(const FdemriDims& d, int64_t i) {
+    if (d.freq) return __ldg(d.freq + i);
+    return __dadd_rn(d.f0, __dmul_rn((double)i, d.df));
+}
+
+// ------------------------------------------------------------------------------------------------
+// double-double arithmetic (hi + lo, |lo| <= ulp(hi)/2) for the phase path (R9)
+// ------------------------------------------------------------------------------------------------
+struct dd {
+    double hi, lo;
+};
+__host__ __device__ __forceinline__ dd dd_make(double a) { return dd{a, 0.0}; }
+__device__ __forceinline__ dd two_sum(double a, double b) {
+    double s = __dadd_rn(a, b);
+    double bb = __dadd_rn(s, -a);
+    double e = __dadd_rn(__dadd_rn(a, -__dadd_rn(s, -bb)), __dadd_rn(b, -bb));
+    return dd{s, e};
+}
+__device__ __forceinline__ dd quick_two_sum(double a, double b) {   // |a| >= |b|
+    double s = __dadd_rn(a, b);
+    double e = __dadd_rn(b, -__dadd_rn(s, -a));
+    return dd{s, e};
+}
+__device__ __forceinline__ dd two_prod(double a, double b) {
+    double p = __dmul_rn(a, b);
+    double e = __fma_rn(a, b, -p);
+    return dd{p, e};
+}
+__device__ __forceinline__ dd dd_add(dd a, dd b) {
+    dd s = two_sum(a.hi, b.hi);
+    dd t = two_sum(a.lo, b.lo);
+    s.lo = __dadd_rn(s.lo, t.hi);
+    s = quick_two_sum(s.hi, s.lo);
+    s.lo = __dadd_rn(s.lo, t.lo);
+    return quick_two_sum(s.hi, s.lo);
+}
+__device__ __forceinline__ dd dd_neg(dd a) { return dd{-a.hi, -a.lo}; }
+__device__ __forceinline__ dd dd_sub(dd a, dd b) { return dd_add(a, dd_neg(b)); }
+__device__ __forceinline__ dd dd_mul(dd a, dd b) {
+    dd p = two_prod(a.hi, b.hi);
+    p.lo = __dadd_rn(p.lo, __dadd_rn(__dmul_rn(a.hi, b.lo), __dmul_rn(a.lo, b.hi)));
+    return quick_two_sum(p.hi, p.lo);
+}
+__device__ __forceinline__ dd dd_mul_d(dd a, double b) {
+    dd p = two_prod(a.hi, b);
+    p.lo = __dadd_rn(p.lo, __dmul_rn(a.lo, b));
+    return quick_two_sum(p.hi, p.lo);
+}
+__device__ __forceinline__ dd dd_div(dd a, dd b) {
+    double q1 = __ddiv_rn(a.hi, b.hi);
+    dd r = dd_sub(a, dd_mul_d(b, q1));
+    double q2 = __ddiv_rn(r.hi, b.hi);
+    r = dd_sub(r, dd_mul_d(b, q2));
+    double q3 = __ddiv_rn(r.hi, b.hi);
+    dd q = quick_two_sum(q1, q2);
+    return dd_add(q, dd_make(q3));
+}
+// fractional part in [-0.5, 0.5] of a double-double
+__device__ __forceinline__ double dd_frac(dd a) {
+    double r = rint(a.hi);
+    dd f = dd_add(dd{__dadd_rn(a.hi, -r), 0.0}, dd{a.lo, 0.0});   // a.hi - r is exact
+    double g = __dadd_rn(f.hi, f.lo);
+    return __dadd_rn(g, -rint(g));
+}
+
+// 1/(2 pi) as a double-double
+#define FDEMRI_INV2PI_HI 0.15915494309189535
+#define FDEMRI_INV2PI_LO (-9.839338337591243e-18)

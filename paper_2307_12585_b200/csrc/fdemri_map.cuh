@@ -1,0 +1,178 @@
+// fdemri_map.cuh -- S0 (harmonic weights) and S2 (segment records + segment->bin-range map).
+//
+// S2 follows PAPER.md L103 (A..D = mode-number-weighted sums of the fundamental-frequency spline
+// coefficients) and L105 ("the spline segment in which each value of f falls is predetermined before the
+// summation").  The map is inverted with respect to the paper: instead of a segment index per (f, voice) it
+// stores, per (voice, sign, segment-branch), the contiguous interval of bins the branch covers.  Along a
+// monotone run of branches these intervals are adjacent, so runs are kept as "strips" [lo, hi] and a bin
+// finds its segment inside a strip by a short search over the branch start bins.
+#pragma once
+#include "fdemri_common.cuh"
+
+// ------------------------------------------------------------------------------------------------
+// S0: weights.  -2Y_lm(theta, phi) = sqrt((2l+1)/4pi) d^l_{m,2}(theta) e^{i m phi}  (Wigner small-d), hence
+//   W+ = e^{i m phi} w+,  Wx = i e^{i m phi} wx   with real  w+ = (y+ + (-1)^l y-)/2,  wx = (y+ - (-1)^l y-)/2,
+//   y+- = -2Y_{l,+-m}(theta, 0);  m = 0: w+ = wx = y/2 (R1, R2).
+// The factor e^{i m phi} goes into the phase as m*phi/2pi cycles.
+// ------------------------------------------------------------------------------------------------
+__device__ double fdemri_wigner_d(int l, int mp, int m, double ch, double sh) {
+    // d^l_{mp,m} = sqrt((l+mp)!(l-mp)!(l+m)!(l-m)!) sum_k (-1)^{mp-m+k} ch^{2l+m-mp-2k} sh^{mp-m+2k}
+    //              / [(l+m-k)! k! (mp-m+k)! (l-mp-k)!]
+    double lf[4] = {lgamma((double)(l + mp + 1)), lgamma((double)(l - mp + 1)), lgamma((double)(l + m + 1)),
+                    lgamma((double)(l - m + 1))};
+    double lpref = 0.5 * (lf[0] + lf[1] + lf[2] + lf[3]);
+    double tot = 0.0;
+    for (int k = 0; k <= 2 * l; ++k) {
+        int a = l + m - k, b = mp - m + k, d = l - mp - k;
+        if (a < 0 || b < 0 || d < 0) continue;
+        double lt = lpref - lgamma((double)(a + 1)) - lgamma((double)(k + 1)) - lgamma((double)(b + 1)) -
+                    lgamma((double)(d + 1));
+        double term = exp(lt) * pow(ch, (double)(2 * l + m - mp - 2 * k)) * pow(sh, (double)(mp - m + 2 * k));
+        tot += ((mp - m + k) & 1) ? -term : term;
+    }
+    return tot;
+}
+
+// wts: [n_angles][V] double4 {w+, wx, m*phi/2pi (cycles, reduced), 0}
+__global__ void k_weights(int n_angles, int V, const int* __restrict__ lmn, const double* __restrict__ angles,
+                          double4* __restrict__ wts) {
+    int id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= n_angles * V) return;
+    int a = id / V, v = id - a * V;
+    int l = lmn[3 * v], m = lmn[3 * v + 1];
+    double theta = angles[2 * a], phi = angles[2 * a + 1];
+    double ch = cos(0.5 * theta), sh = sin(0.5 * theta);
+    double norm = sqrt((2.0 * l + 1.0) / (4.0 * 3.14159265358979323846));
+    double yp = norm * fdemri_wigner_d(l, m, 2, ch, sh);
+    double wp, wx;
+    if (m > 0) {
+        double ym = norm * fdemri_wigner_d(l, -m, 2, ch, sh);
+        if (l & 1) ym = -ym;
+        wp = 0.5 * (yp + ym);
+        wx = 0.5 * (yp - ym);
+    } else {
+        wp = 0.5 * yp;
+        wx = 0.5 * yp;
+    }
+    double cyc = (double)m * phi * 0.15915494309189535;
+    cyc -= rint(cyc);
+    wts[id] = make_double4(wp, wx, cyc, 0.0);
+}
+
+// ------------------------------------------------------------------------------------------------
+// S2a: records.  One thread per (batch item, voice, segment).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double fdemri_knotF(int m, int n, double fphi, double fr) {
+    // knot value of F_v as plainly rounded doubles (R6): products rounded, then the sum rounded
+    return __dadd_rn(__dmul_rn((double)m, fphi), __dmul_rn((double)n, fr));
+}
+
+__device__ __forceinline__ dd fdemri_combine(int m, int n, double ahi, double alo, double bhi, double blo) {
+    dd x = dd_mul_d(dd{ahi, alo}, (double)m);
+    dd y = dd_mul_d(dd{bhi, blo}, (double)n);
+    return dd_add(x, y);
+}
+
+// root of the monotone cubic  FB t + FC t^2 + FD t^3 = x  on [0, h]  (safeguarded Newton; build time only)
+__device__ double fdemri_root_build(double FB, double FC, double FD, double x, double h) {
+    double lo = 0.0, hi = h;
+    double Gh = h * (FB + h * (FC + h * FD)) - x;
+    bool inc = Gh > -x;                      // G(h) > G(0)
+    double t = (Gh != -x) ? h * (x / (Gh + x)) : 0.5 * h;   // secant seed
+    t = fmin(fmax(t, 0.0), h);
+    for (int it = 0; it < 80; ++it) {
+        double G = t * (FB + t * (FC + t * FD)) - x;
+        double dG = FB + t * (2.0 * FC + 3.0 * FD * t);
+        if (G == 0.0) break;
+        if ((G > 0.0) == inc) hi = t; else lo = t;
+        double tn = t - G / dG;
+        if (!(tn > lo && tn < hi)) tn = 0.5 * (lo + hi);
+        if (fabs(tn - t) <= 1e-15 * h) { t = tn; break; }
+        t = tn;
+    }
+    return t;
+}
+
+__global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ t_knots,
+                          const double* __restrict__ sh_hi, const double* __restrict__ sh_lo,
+                          double* __restrict__ rec, unsigned long long* __restrict__ stats) {
+    size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    size_t total = (size_t)d.n_batch * d.n_modes * d.n_seg;
+    if (id >= total) return;
+    int k = (int)(id % d.n_seg);
+    size_t bv = id / d.n_seg;
+    int v = (int)(bv % d.n_modes);
+    int b = (int)(bv / d.n_modes);
+    int m = lmn[3 * v + 1], n = lmn[3 * v + 2];
+    const size_t per = (size_t)d.n_seg * 4;
+    const double* hi = sh_hi + (size_t)b * 4 * per + (size_t)k * 4;
+    const double* lo = sh_lo + (size_t)b * 4 * per + (size_t)k * 4;
+    double* R = rec + id * R_DOUBLES;
+    // F cubic (Eq. 6)
+    double FA = fdemri_knotF(m, n, hi[0], hi[per]);
+    dd FBd = fdemri_combine(m, n, hi[1], lo[1], hi[per + 1], lo[per + 1]);
+    dd FCd = fdemri_combine(m, n, hi[2], lo[2], hi[per + 2], lo[per + 2]);
+    dd FDd = fdemri_combine(m, n, hi[3], lo[3], hi[per + 3], lo[per + 3]);
+    double FB = FBd.hi, FC = FCd.hi, FD = FDd.hi;
+    // phase spline of the voice, in cycles (R9)
+    const dd inv2pi = dd{FDEMRI_INV2PI_HI, FDEMRI_INV2PI_LO};
+    dd Pa = dd_add(two_prod((double)m, hi[2 * per]), two_prod((double)n, hi[3 * per]));   // knot values: exact
+    dd Pb = fdemri_combine(m, n, hi[2 * per + 1], lo[2 * per + 1], hi[3 * per + 1], lo[3 * per + 1]);
+    dd Pc = fdemri_combine(m, n, hi[2 * per + 2], lo[2 * per + 2], hi[3 * per + 2], lo[3 * per + 2]);
+    dd Pd = fdemri_combine(m, n, hi[2 * per + 3], lo[2 * per + 3], hi[3 * per + 3], lo[3 * per + 3]);
+    double pc = -dd_frac(dd_mul(Pa, inv2pi));
+    dd bq = dd_mul(Pb, inv2pi);
+    double tk = t_knots[(size_t)b * d.n_knots + k];
+    double h = __dadd_rn(t_knots[(size_t)b * d.n_knots + k + 1], -tk);
+    R[R_FA] = FA; R[R_FB] = FB; R[R_FC] = FC; R[R_FD] = FD;
+    R[R_PC] = pc; R[R_BH] = bq.hi; R[R_BL] = bq.lo;
+    R[R_NC] = -dd_mul(Pc, inv2pi).hi;
+    R[R_ND] = -dd_mul(Pd, inv2pi).hi;
+    R[R_TK] = tk; R[R_H] = h; R[R_SPARE] = 0.0;
+    // interior extrema of F on (0, h): roots of FB + 2 FC t + 3 FD t^2
+    double ext[2]; int ne = 0;
+    {
+        double qa = 3.0 * FD, qb = 2.0 * FC, qc = FB;
+        if (qa == 0.0) {
+            if (qb != 0.0) { double r = -qc / qb; if (r > 0.0 && r < h) ext[ne++] = r; }
+        } else {
+            double disc = qb * qb - 4.0 * qa * qc;
+            if (disc > 0.0) {
+                double sq = sqrt(disc);
+                double qq = -0.5 * (qb + (qb >= 0.0 ? sq : -sq));
+                double r1 = qq / qa, r2 = (qq != 0.0) ? qc / qq : r1;
+                if (r1 > r2) { double tmp = r1; r1 = r2; r2 = tmp; }
+                if (r1 > 0.0 && r1 < h) ext[ne++] = r1;
+                if (r2 > 0.0 && r2 < h && r2 != r1) ext[ne++] = r2;
+            }
+        }
+    }
+    bool bad = !(isfinite(FA) && isfinite(FB) && isfinite(FC) && isfinite(FD) && isfinite(pc) && isfinite(bq.hi));
+    if (ne == 0) {
+        // seed of the inverse: cubic through tau(x) at x = dF {0, 1/3, 2/3, 1}, x = s f - FA
+        double dF = h * (FB + h * (FC + h * FD));
+        double q1 = 0.0, q2 = 0.0, q3 = 0.0;
+        if (dF != 0.0 && isfinite(dF)) {
+            double t1 = fdemri_root_build(FB, FC, FD, dF * (1.0 / 3.0), h);
+            double t2 = fdemri_root_build(FB, FC, FD, dF * (2.0 / 3.0), h);
+            double g1 = 3.0 * t1, g2 = 1.5 * t2, g3 = h;
+            double gam = 4.5 * (g1 - 2.0 * g2 + g3);
+            double bet = 3.0 * (g2 - g1) - gam;
+            double alp = g1 - bet * (1.0 / 3.0) - gam * (1.0 / 9.0);
+            double idF = 1.0 / dF;
+            q1 = alp * idF; q2 = bet * idF * idF; q3 = gam * idF * idF * idF;
+        }
+        R[R_Q1] = q1; R[R_Q2] = q2; R[R_Q3] = q3; R[R_TYPE] = 0.0;
+    } else if (ne == 1) {
+        double te = ext[0];
+        R[R_Q1] = te;
+        R[R_Q2] = FA + te * (FB + te * (FC + te * FD));     // F_e (R7)
+        R[R_Q3] = FC + 3.0 * FD * te;                        // F(t) - F_e = z^2 (Q3 + FD z), z = t - te
+        R[R_TYPE] = 1.0;
+        atomicAdd(stats + 3, 1ull);
+    } else {
+        R[R_Q1] = 0.0; R[R_Q2] = 0.0; R[R_Q3] = 0.0; R[R_TYPE] = 2.0;
+        atomicOr(stats + 5, 1ull);                           // FDEMRI_BAD_TWO_EXTREMA
+    }
+    if (bad) atomicOr(stats + 5, 4ull);
+}

@@ -1,0 +1,231 @@
+"""GPU parity: libfdemri (through the C ABI) against the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star): per bin |delta h| <= 1e-10 max|h|, and 1 - overlap <= 1e-12 (flat noise,
+both polarisations).  Bins the oracle marks boundary-ambiguous (R8) are excluded from the per-bin
+check (expected count: 0).  Level C = independent spline builds; level A = oracle fed the GPU's coefficients.
+"""
+import functools
+import math
+
+import numpy as np
+import pytest
+
+from helpers import max_rel_err, one_minus_overlap
+
+pytestmark = pytest.mark.gpu
+
+TOL_BIN = 1e-10
+TOL_MISMATCH = 1e-12
+
+
+@pytest.fixture(scope="module")
+def fd():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2307_12585_b200 as pkg
+    return pkg
+
+
+@functools.lru_cache(maxsize=None)
+def workload(idx):
+    from paper_2307_12585_b200 import synth
+    return synth.CONFIGS[idx]()
+
+
+def oracle_c(orc, w, freq, b=0):
+    return orc.waveform(w.lmn, w.t_knots[b], w.f_phi[b], w.f_r[b], w.Phi_phi[b], w.Phi_r[b], w.amp[b], freq,
+                        w.theta, w.phi)
+
+
+def check(gp, gx, ref, label):
+    keep = ref["ambiguous"] == 0
+    assert (~keep).sum() <= 2, f"{label}: {(~keep).sum()} ambiguous bins"
+    err = max_rel_err(gp, gx, ref["hplus"], ref["hcross"], mask=keep)
+    mm = one_minus_overlap(gp[keep], gx[keep], ref["hplus"][keep], ref["hcross"][keep])
+    print(f"[parity] {label}: max|dh|/max|h| = {err:.3e}, 1-overlap = {mm:.3e}, bins = {keep.sum()}")
+    assert np.all(np.isfinite(gp)) and np.all(np.isfinite(gx))
+    assert err <= TOL_BIN, f"{label}: per-bin {err}"
+    assert mm <= TOL_MISMATCH, f"{label}: mismatch {mm}"
+    # exact zeros where the oracle has no term (P8)
+    zero = (ref["nterms"] == 0) & keep
+    assert np.all(gp[zero] == 0) and np.all(gx[zero] == 0), f"{label}: non-zero outside support"
+    return err, mm
+
+
+def run_gpu(fd, w):
+    wf = fd.waveform_from_workload(w)
+    wf.sum(w.theta, w.phi)
+    hp, hx = wf.result()
+    st = wf.stats()
+    return wf, hp, hx, st
+
+
+def test_small_case_levels_A_and_C(fd, orc):
+    from paper_2307_12585_b200 import synth
+    w = synth.small_case(seed=2, n_knots=14)
+    wf, hp, hx, st = run_gpu(fd, w)
+    freq = w.freq_array()
+    ref = oracle_c(orc, w, freq)
+    assert ref["max_roots"] == 2
+    check(hp[0], hx[0], ref, "small level C")
+    assert st["n_evals"] == ref["n_evals"]                      # P9
+    assert st["n_airy"] > 0 and st["n_turnover"] > 0
+    # level A: the oracle's sum on the GPU-built coefficients
+    hi, lo, am = wf.coeffs()
+    refA = orc.sum(w.lmn, w.t_knots[0], w.f_phi[0], w.f_r[0], hi[0], lo[0], am[0], None, freq, w.theta, w.phi)
+    check(hp[0], hx[0], refA, "small level A")
+    # level B: coefficients themselves (phase increments over a segment, relative amplitude deviation)
+    ohi, olo = orc.build_splines(w.t_knots[0], np.stack([w.f_phi[0], w.f_r[0], w.Phi_phi[0], w.Phi_r[0]]))
+    h = np.diff(w.t_knots[0])
+    dco = (hi[0] - ohi) + (lo[0] - olo)
+    for c in (2, 3):
+        inc = np.abs(dco[c, :, 1] * h) + np.abs(dco[c, :, 2] * h ** 2) + np.abs(dco[c, :, 3] * h ** 3)
+        assert inc.max() < 1e-12, f"phase-increment deviation {inc.max()} rad"
+    wf.close()
+
+
+def test_small_case_no_turnover_other_angles(fd, orc):
+    from paper_2307_12585_b200 import synth
+    w = synth.small_case(seed=5, n_knots=9, turnover=False, modes=((2, 2, 0), (3, 1, 2), (4, 0, 3), (5, 5, -1), (10, 7, -2)))
+    w.theta, w.phi = 2.1, -0.7
+    wf, hp, hx, st = run_gpu(fd, w)
+    ref = oracle_c(orc, w, w.freq_array())
+    check(hp[0], hx[0], ref, "no-turnover")
+    assert st["n_evals"] == ref["n_evals"]
+    wf.close()
+
+
+def test_config0_full(fd, orc):
+    w = workload(0)
+    wf, hp, hx, st = run_gpu(fd, w)
+    ref = oracle_c(orc, w, w.freq_array())
+    check(hp[0], hx[0], ref, "config0")
+    assert st["n_evals"] == ref["n_evals"]
+    wf.close()
+
+
+def test_config1_full(fd, orc):
+    w = workload(1)
+    wf, hp, hx, st = run_gpu(fd, w)
+    ref = oracle_c(orc, w, w.freq_array())
+    check(hp[0], hx[0], ref, "config1")
+    assert st["n_evals"] == ref["n_evals"]
+    assert ref["max_roots"] == 2
+    wf.close()
+
+
+def _sampled_bins(n_freq, n, seed, hi_frac=0.36):
+    rng = np.random.default_rng(seed)
+    a = rng.integers(1, int(n_freq * hi_frac), size=n)
+    edge = np.array([0, 1, 2, 255, 256, 257, n_freq - 2, n_freq - 1])
+    return np.unique(np.concatenate([a, edge]))
+
+
+def test_config2_sampled_bins_full_size(fd, orc):
+    """BASELINE config 2 at full size in the launch configuration bench.py times; the oracle computes sampled
+    bins one by one (an arbitrary grid holding exactly those frequencies)."""
+    w = workload(2)
+    wf, hp, hx, st = run_gpu(fd, w)
+    idx = _sampled_bins(w.n_freq, 6000, 11)
+    freq = w.freq_array()[idx]
+    ref = oracle_c(orc, w, freq)
+    # scale by the full waveform's maximum, as the tolerance is stated
+    scale = max(np.abs(hp[0]).max(), np.abs(hx[0]).max())
+    keep = ref["ambiguous"] == 0
+    dp = np.abs(hp[0][idx] - ref["hplus"])[keep].max() / scale
+    dx = np.abs(hx[0][idx] - ref["hcross"])[keep].max() / scale
+    mm = one_minus_overlap(hp[0][idx][keep], hx[0][idx][keep], ref["hplus"][keep], ref["hcross"][keep])
+    print(f"[parity] config2 sampled: {dp:.3e} {dx:.3e} mismatch {mm:.3e}; evals {st['n_evals']:.4g} items {st['n_items']}")
+    assert max(dp, dx) <= TOL_BIN and mm <= TOL_MISMATCH
+    assert 2.5e8 < st["n_evals"] < 4e8            # ~3.15e8 evaluations
+    # properties that hold at any size: zero beyond the highest voice frequency, f = 0 bin zero
+    assert hp[0][0] == 0 and hx[0][0] == 0
+    assert np.all(hp[0][int(0.5 * w.n_freq):] == 0)
+    wf.close()
+
+
+def test_config3_arbitrary_grid(fd, orc):
+    w = workload(3)
+    wf, hp, hx, st = run_gpu(fd, w)
+    ref = oracle_c(orc, w, w.freq_array())
+    check(hp[0], hx[0], ref, "config3")
+    assert st["n_evals"] == ref["n_evals"]
+    wf.close()
+
+
+def test_deterministic_bitwise(fd):
+    w = workload(1)
+    wf = fd.waveform_from_workload(w)
+    wf.sum(w.theta, w.phi)
+    a = [x.copy() for x in wf.result()]
+    for _ in range(2):
+        wf.sum(w.theta, w.phi)
+        b = wf.result()
+        assert np.array_equal(a[0].view(np.uint64), b[0].view(np.uint64))
+        assert np.array_equal(a[1].view(np.uint64), b[1].view(np.uint64))
+    wf.close()
+
+
+def test_batched_config4_subset(fd, orc):
+    """Config 4 on a seeded subset of its 1024 parameter sets spanning the M range, per-item angles."""
+    from paper_2307_12585_b200 import synth
+    M, e0, _ = synth.config4_params()
+    order = np.argsort(M)
+    items = [int(order[3]), int(order[len(order) // 2]), int(order[-3])]
+    w = synth.config4(items=items, substeps=40)
+    wf = fd.waveform_from_workload(w)
+    th = np.array([w.theta, 1.0, 2.5])
+    ph = np.array([w.phi, -2.0, 0.3])
+    wf.sum(th, ph)
+    hp, hx = wf.result()
+    st = wf.stats()
+    total = 0
+    for b in range(len(items)):
+        idx = _sampled_bins(w.n_freq, 1500, 20 + b, hi_frac=0.9)
+        freq = w.freq_array()[idx]
+        ref = orc.waveform(w.lmn, w.t_knots[b], w.f_phi[b], w.f_r[b], w.Phi_phi[b], w.Phi_r[b], w.amp[b], freq,
+                           float(th[b]), float(ph[b]))
+        scale = max(np.abs(hp[b]).max(), np.abs(hx[b]).max())
+        keep = ref["ambiguous"] == 0
+        err = max(np.abs(hp[b][idx] - ref["hplus"])[keep].max(), np.abs(hx[b][idx] - ref["hcross"])[keep].max()) / scale
+        mm = one_minus_overlap(hp[b][idx][keep], hx[b][idx][keep], ref["hplus"][keep], ref["hcross"][keep])
+        print(f"[parity] config4 item {items[b]} (M={M[items[b]]:.3g}): {err:.3e}, mismatch {mm:.3e}")
+        assert err <= TOL_BIN and mm <= TOL_MISMATCH
+        total += 1
+    assert total == 3 and st["n_evals"] > 0
+    wf.close()
+
+
+def test_edge_cases(fd, orc):
+    import torch
+    from paper_2307_12585_b200 import synth
+    w = synth.small_case(seed=6, n_knots=4, n_freq=1)           # minimum knots; only the f = 0 bin
+    wf, hp, hx, st = run_gpu(fd, w)
+    assert hp.shape == (1, 1) and hp[0, 0] == 0 and hx[0, 0] == 0 and st["n_evals"] == 0
+    wf.close()
+    w = synth.small_case(seed=6, n_knots=4, n_freq=777)         # ragged tile; grid entirely below every voice
+    wf, hp, hx, st = run_gpu(fd, w)
+    ref = oracle_c(orc, w, w.freq_array())
+    assert ref["n_evals"] == st["n_evals"]
+    check(hp[0], hx[0], ref, "ragged")
+    wf.close()
+    w = synth.small_case(seed=7, n_knots=5, n_freq=20001)       # 4 segments, ragged tail, turnover
+    wf, hp, hx, st = run_gpu(fd, w)
+    ref = oracle_c(orc, w, w.freq_array())
+    check(hp[0], hx[0], ref, "n_knots=5")
+    assert ref["n_evals"] == st["n_evals"] and st["n_evals"] > 0
+    wf.close()
+    # error behaviour
+    t = torch.zeros((1, 3), dtype=torch.float64, device="cuda")
+    with pytest.raises(fd.FdemriError):
+        fd.fdemri_plan(np.array([[2, 2, 0]], np.int32), 1, 3, t, 10, None, 0.0, 1e-6)      # n_knots < 4
+    t = torch.zeros((1, 8), dtype=torch.float64, device="cuda")
+    with pytest.raises(fd.FdemriError):
+        fd.fdemri_plan(np.array([[2, 3, 0]], np.int32), 1, 8, t, 10, None, 0.0, 1e-6)      # m > l
+    p = fd.fdemri_plan(np.array([[2, 2, 0]], np.int32), 1, 8, t, 10, None, 0.0, 1e-6)
+    out = torch.zeros((1, 10, 2), dtype=torch.float64, device="cuda")
+    with pytest.raises(fd.FdemriError) as ei:
+        fd.fdemri_sum(p, 0.1, 0.2, out, out)                                               # no work space
+    assert ei.value.status == 2
+    fd.fdemri_destroy(p)
