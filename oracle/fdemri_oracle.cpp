@@ -432,12 +432,17 @@ static int sum_impl(int n_modes, const int32_t* lmn, int N, const double* t,
                     const double* pb = flo_incl ? std::lower_bound(fb, fe, flo) : std::upper_bound(fb, fe, flo);
                     const double* pe = fhi_incl ? std::upper_bound(fb, fe, fhi) : std::lower_bound(fb, fe, fhi);
                     if (ambiguous) {
-                        // R8: bins within a few ulp of a boundary value (only extremum values can differ
-                        // between implementations; knot values are shared doubles, but flag both)
-                        for (const double* q = pb - 1; q <= pb; ++q)
-                            if (q >= fb && q < fe && fabs(*q - flo) <= 16.0 * ulp_of(flo) && *q > 0.0) ambiguous[q - freq] = 1;
-                        for (const double* q = pe - 1; q <= pe; ++q)
-                            if (q >= fb && q < fe && fabs(*q - fhi) <= 16.0 * ulp_of(fhi) && *q > 0.0) ambiguous[q - freq] = 1;
+                        // R8: bins within a few ulp of an extremum value F_e -- the only boundary value that an
+                        // independent implementation computes itself (knot values are the same doubles everywhere,
+                        // so comparisons against them are exact and never ambiguous)
+                        bool lo_ext = (P.Va < P.Vb) ? P.a_ext : P.b_ext, hi_ext = (P.Va < P.Vb) ? P.b_ext : P.a_ext;
+                        bool flo_ext = sgn > 0 ? lo_ext : hi_ext, fhi_ext = sgn > 0 ? hi_ext : lo_ext;
+                        if (flo_ext)
+                            for (const double* q = pb - 1; q <= pb; ++q)
+                                if (q >= fb && q < fe && fabs(*q - flo) <= 16.0 * ulp_of(flo) && *q > 0.0) ambiguous[q - freq] = 1;
+                        if (fhi_ext)
+                            for (const double* q = pe - 1; q <= pe; ++q)
+                                if (q >= fb && q < fe && fabs(*q - fhi) <= 16.0 * ulp_of(fhi) && *q > 0.0) ambiguous[q - freq] = 1;
                     }
                     const ld* cF = &V.cF[4 * P.seg];
                     const ld* cP = &V.cP[4 * P.seg];
