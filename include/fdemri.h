@@ -39,7 +39,9 @@ enum {
 
 /* plan flags */
 enum {
-    FDEMRI_FLAG_NONE = 0
+    FDEMRI_FLAG_NONE = 0,
+    FDEMRI_FLAG_TIMING = 1     /* record CUDA events around the S3 tile kernel of every fdemri_sum (see
+                                  fdemri_get_kernel_ms); costs two event records per call                  */
 };
 
 /* bits of fdemri_stats.flags (device-side validation, read back by fdemri_get_stats) */
@@ -105,6 +107,14 @@ int fdemri_get_stats(fdemri_plan_t plan, fdemri_stats* out);
  *  amp_coef             [n_batch][n_modes][2][n_knots-1][4]  (a,b,c,d) of Re A, Im A
  * Device pointers; any may be NULL.  Enqueued on the stream of the last build_splines. */
 int fdemri_get_coeffs(fdemri_plan_t plan, double* shared_hi_dev, double* shared_lo_dev, double* amp_coef_dev);
+
+/* Device time in ms of the S3/S4 tile kernel of the last fdemri_sum, from CUDA events recorded on that call's
+ * stream (plan created with FDEMRI_FLAG_TIMING).  Synchronises on the stop event. */
+int fdemri_get_kernel_ms(fdemri_plan_t plan, float* ms_out);
+
+/* FP64 FMA peak of the current device measured with a register-resident DFMA loop (the roofline denominator
+ * of the ALU-bound tile kernel): writes TFLOP/s (2 flop per DFMA).  Synchronous; n_iters ~ 1<<16. */
+int fdemri_measure_fp64_peak(int n_iters, double* tflops_out);
 
 int fdemri_destroy(fdemri_plan_t plan);
 const char* fdemri_strerror(int status);

@@ -399,7 +399,7 @@ static int sum_impl(int n_modes, const int32_t* lmn, int N, const double* t,
     int64_t n_evals = 0;
     int max_roots = 0;
 #ifdef _OPENMP
-    if (n_threads > 0) omp_set_num_threads(n_threads);
+    omp_set_num_threads(n_threads > 0 ? n_threads : omp_get_num_procs());
     const int n_thr = omp_get_max_threads();
 #else
     const int n_thr = 1;

@@ -20,7 +20,7 @@ STATUS = {0: "FDEMRI_OK", 1: "FDEMRI_ERR_INVALID_ARG", 2: "FDEMRI_ERR_WORKSPACE"
           4: "FDEMRI_ERR_NOT_BUILT", 5: "FDEMRI_ERR_UNSUPPORTED"}
 
 EXPORTS = ["fdemri_plan", "fdemri_workspace_bytes", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum",
-           "fdemri_get_stats", "fdemri_get_coeffs", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
+           "fdemri_get_stats", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
 
 
 class FdemriStats(C.Structure):
@@ -61,6 +61,10 @@ def lib() -> C.CDLL:
         L.fdemri_get_stats.argtypes = [vp, C.POINTER(FdemriStats)]
         L.fdemri_get_coeffs.restype = C.c_int
         L.fdemri_get_coeffs.argtypes = [vp, dp, dp, dp]
+        L.fdemri_get_kernel_ms.restype = C.c_int
+        L.fdemri_get_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
+        L.fdemri_measure_fp64_peak.restype = C.c_int
+        L.fdemri_measure_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
         L.fdemri_destroy.restype = C.c_int
         L.fdemri_destroy.argtypes = [vp]
         L.fdemri_strerror.restype = C.c_char_p
@@ -138,6 +142,18 @@ def fdemri_get_coeffs(plan, shared_hi=None, shared_lo=None, amp_coef=None):
     _chk("fdemri_get_coeffs", lib().fdemri_get_coeffs(plan, _ptr(shared_hi), _ptr(shared_lo), _ptr(amp_coef)))
 
 
+def fdemri_get_kernel_ms(plan) -> float:
+    ms = C.c_float()
+    _chk("fdemri_get_kernel_ms", lib().fdemri_get_kernel_ms(plan, C.byref(ms)))
+    return float(ms.value)
+
+
+def fdemri_measure_fp64_peak(n_iters=1 << 16) -> float:
+    tf = C.c_double()
+    _chk("fdemri_measure_fp64_peak", lib().fdemri_measure_fp64_peak(int(n_iters), C.byref(tf)))
+    return float(tf.value)
+
+
 def fdemri_destroy(plan):
     _chk("fdemri_destroy", lib().fdemri_destroy(plan))
 
@@ -150,7 +166,7 @@ def fdemri_version() -> str:
 class Waveform:
     """Owns the device buffers of one plan.  `w` is a synth.Workload-like object (numpy, host)."""
 
-    def __init__(self, lmn, t_knots, n_freq, freqs=None, f0=0.0, df=0.0, device="cuda:0"):
+    def __init__(self, lmn, t_knots, n_freq, freqs=None, f0=0.0, df=0.0, device="cuda:0", flags=0):
         import torch
         self.torch = torch
         self.dev = torch.device(device)
@@ -161,7 +177,7 @@ class Waveform:
         self.n_modes = self.lmn.shape[0]
         self.t_knots = torch.from_numpy(t_knots).to(self.dev)
         self.freqs = None if freqs is None else torch.from_numpy(np.ascontiguousarray(freqs, dtype=np.float64)).to(self.dev)
-        self.plan = fdemri_plan(self.lmn, self.n_batch, self.n_knots, self.t_knots, self.n_freq, self.freqs, f0, df)
+        self.plan = fdemri_plan(self.lmn, self.n_batch, self.n_knots, self.t_knots, self.n_freq, self.freqs, f0, df, flags)
         nbytes = fdemri_workspace_bytes(self.plan)
         self.ws = torch.empty((nbytes + 255) // 8 + 32, dtype=torch.float64, device=self.dev)
         off = (-self.ws.data_ptr()) % 256
@@ -214,7 +230,7 @@ class Waveform:
             pass
 
 
-def waveform_from_workload(w, device="cuda:0") -> Waveform:
-    wf = Waveform(w.lmn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df, device=device)
+def waveform_from_workload(w, device="cuda:0", flags=0) -> Waveform:
+    wf = Waveform(w.lmn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df, device=device, flags=flags)
     wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)
     return wf

@@ -39,6 +39,9 @@ struct fdemri_plan_s {
     bool built;
     cudaStream_t last_stream;
     int sm_count;
+    uint32_t flags;
+    cudaEvent_t ev0, ev1;
+    bool ev_valid;
 };
 
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -73,7 +76,6 @@ static size_t carve(fdemri_plan_s* p, char* base) {
 extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, int n_batch, int n_knots,
                            const double* t_knots_dev, int64_t n_freq, const double* freq_dev, double f0, double df,
                            uint32_t flags) {
-    (void)flags;
     if (!out) return FDEMRI_ERR_INVALID_ARG;
     *out = nullptr;
     if (n_modes < 1 || n_modes > (1 << 20) || !lmn_host || n_batch < 1 || n_knots < 4 || n_knots > FDEMRI_MAX_KNOTS ||
@@ -111,6 +113,15 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
         return FDEMRI_ERR_CUDA;
     }
     p->sm_count = prop.multiProcessorCount;
+    p->flags = flags;
+    p->ev_valid = false;
+    p->ev0 = p->ev1 = nullptr;
+    if (flags & FDEMRI_FLAG_TIMING) {
+        if (cudaEventCreate(&p->ev0) != cudaSuccess || cudaEventCreate(&p->ev1) != cudaSuccess) {
+            delete p;
+            return FDEMRI_ERR_CUDA;
+        }
+    }
     carve(p, nullptr);
     *out = p;
     return FDEMRI_OK;
@@ -215,7 +226,9 @@ extern "C" int fdemri_sum(fdemri_plan_t p, int n_angles, const double* theta_hos
         per_sm = 1;
     long long grid = (long long)p->sm_count * per_sm;
     if (grid > a.total_tiles) grid = a.total_tiles;
+    if (p->ev0) cudaEventRecord(p->ev0, st);
     k_tile_sum<<<(unsigned)grid, FDEMRI_TILE, 0, st>>>(a);
+    if (p->ev1) { cudaEventRecord(p->ev1, st); p->ev_valid = true; }
     if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
     return FDEMRI_OK;
 }
@@ -269,8 +282,62 @@ extern "C" int fdemri_get_coeffs(fdemri_plan_t p, double* shared_hi_dev, double*
     return FDEMRI_OK;
 }
 
+extern "C" int fdemri_get_kernel_ms(fdemri_plan_t p, float* ms_out) {
+    if (!p || !ms_out) return FDEMRI_ERR_INVALID_ARG;
+    if (!p->ev0 || !p->ev_valid) return FDEMRI_ERR_NOT_BUILT;
+    if (cudaEventSynchronize(p->ev1) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    if (cudaEventElapsedTime(ms_out, p->ev0, p->ev1) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    return FDEMRI_OK;
+}
+
+// 8 independent DFMA chains per thread, all in registers
+__global__ void __launch_bounds__(512) k_dfma_peak(int n_iters, double seed, double* sink) {
+    double a0 = seed + threadIdx.x, a1 = a0 + 1.0, a2 = a0 + 2.0, a3 = a0 + 3.0, a4 = a0 + 4.0, a5 = a0 + 5.0,
+           a6 = a0 + 6.0, a7 = a0 + 7.0;
+    const double m = 0.999999, c = 1e-9;
+    for (int i = 0; i < n_iters; ++i) {
+        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+    double r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+    if (r == 12345.678) sink[0] = r;     // never true; keeps the chains alive
+}
+
+extern "C" int fdemri_measure_fp64_peak(int n_iters, double* tflops_out) {
+    if (!tflops_out || n_iters < 1) return FDEMRI_ERR_INVALID_ARG;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    double* sink = nullptr;
+    if (cudaMalloc(&sink, sizeof(double)) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int threads = 512, blocks = prop.multiProcessorCount * 4;
+    k_dfma_peak<<<blocks, threads>>>(n_iters / 8 + 1, 1.0, sink);    // warm-up
+    float best = 1e30f;
+    for (int rep = 0; rep < 3; ++rep) {
+        cudaEventRecord(e0);
+        k_dfma_peak<<<blocks, threads>>>(n_iters, 1.0, sink);
+        cudaEventRecord(e1);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
+    double flops = 2.0 * 8.0 * (double)n_iters * threads * (double)blocks;
+    *tflops_out = flops / (best * 1e-3) * 1e-12;
+    return FDEMRI_OK;
+}
+
 extern "C" int fdemri_destroy(fdemri_plan_t p) {
     if (!p) return FDEMRI_ERR_INVALID_ARG;
+    if (p->ev0) cudaEventDestroy(p->ev0);
+    if (p->ev1) cudaEventDestroy(p->ev1);
     delete p;
     return FDEMRI_OK;
 }

@@ -11,7 +11,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def declared_symbols():
     src = open(os.path.join(ROOT, "include", "fdemri.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(fdemri_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(fdemri_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_library_builds_and_exports_all_declared_symbols():
