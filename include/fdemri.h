@@ -61,6 +61,7 @@ typedef struct {
     uint64_t n_turnover;     /* segments with an interior extremum of F (Fdot = 0, L92, L105)                 */
     uint64_t n_airy;         /* evaluations that took the small-|X| (Airy) path                              */
     uint64_t flags;          /* OR of FDEMRI_BAD_*                                                            */
+    uint64_t n_slow;         /* evaluations whose root needed the safeguarded (division) Newton fallback      */
 } fdemri_stats;
 
 /* Create a plan.
@@ -115,6 +116,12 @@ int fdemri_get_kernel_ms(fdemri_plan_t plan, float* ms_out);
 /* FP64 FMA peak of the current device measured with a register-resident DFMA loop (the roofline denominator
  * of the ALU-bound tile kernel): writes TFLOP/s (2 flop per DFMA).  Synchronous; n_iters ~ 1<<16. */
 int fdemri_measure_fp64_peak(int n_iters, double* tflops_out);
+
+/* Diagnostic: runs the device root finder of the monotone-segment path (Eq. 6 inverted) on n independent
+ * problems.  in_host [n][8] = {x, FB, FC, FD, q1, q2, q3, h}: solve FB tau + FC tau^2 + FD tau^3 = x on [0,h] from
+ * the seed tau0 = x(q1 + x(q2 + x q3)).  out_host [n][6] = {tau, F', F'', |F'|^(-1/2), slow-path flag, error bits}.
+ * Host pointers; synchronous. */
+int fdemri_debug_root_monotone(int n, const double* in_host, double* out_host);
 
 int fdemri_destroy(fdemri_plan_t plan);
 const char* fdemri_strerror(int status);

@@ -32,6 +32,7 @@ def is_stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False, extra=()) -> str:
     if force or is_stale():
+        extra = list(extra) + os.environ.get("FDEMRI_NVCC_EXTRA", "").split()
         cmd = [nvcc_path(), *NVCC_FLAGS, *extra, "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
         if verbose:
             cmd.insert(1, "-Xptxas")

@@ -31,6 +31,7 @@ struct fdemri_plan_s {
     int* n_strips;
     int4* dense;
     int* n_dense;
+    int2* bin_range;
     int dense_cap;
     double4* wts;
     double* angles;
@@ -67,6 +68,7 @@ static size_t carve(fdemri_plan_s* p, char* base) {
     p->dense_cap = (int)(2 * V * FDEMRI_MAX_STRIPS);
     p->dense = (int4*)take(B * (size_t)p->dense_cap * sizeof(int4));
     p->n_dense = (int*)take(B * sizeof(int));
+    p->bin_range = (int2*)take(B * sizeof(int2));
     p->wts = (double4*)take(B * V * sizeof(double4));
     p->angles = (double*)take(B * 2 * sizeof(double));
     p->stats = (unsigned long long*)take(8 * sizeof(unsigned long long));
@@ -88,6 +90,7 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
     }
     int64_t n_tiles = (n_freq + FDEMRI_TILE - 1) / FDEMRI_TILE;
     if (n_tiles * (int64_t)n_batch >= ((int64_t)1 << 31)) return FDEMRI_ERR_INVALID_ARG;
+    if ((int64_t)n_batch * n_modes * (n_knots - 1) >= ((int64_t)1 << 31)) return FDEMRI_ERR_INVALID_ARG;   /* 32-bit record index */
     fdemri_plan_s* p = new (std::nothrow) fdemri_plan_s();
     if (!p) return FDEMRI_ERR_INVALID_ARG;
     p->d.n_modes = n_modes;
@@ -177,7 +180,8 @@ extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const 
     size_t nvs = (size_t)d.n_batch * d.n_modes * 2;
     k_strips<<<(unsigned)((nvs + 63) / 64), 64, 0, st>>>(d, p->lmn_dev, f_phi, f_r, p->rec, p->ent, p->strips,
                                                          p->n_strips, p->stats);
-    k_strip_compact<<<d.n_batch, 1024, 0, st>>>(d.n_modes, p->dense_cap, p->strips, p->n_strips, p->dense, p->n_dense);
+    k_strip_compact<<<d.n_batch, 1024, 0, st>>>(d.n_modes, p->dense_cap, p->strips, p->n_strips, p->dense, p->n_dense,
+                                                p->bin_range);
     if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
     p->built = true;
     return FDEMRI_OK;
@@ -206,13 +210,14 @@ extern "C" int fdemri_sum(fdemri_plan_t p, int n_angles, const double* theta_hos
     k_weights<<<(nw + 127) / 128, 128, 0, st>>>(n_angles, d.n_modes, p->lmn_dev, p->angles, p->wts);
     // reset the per-sum counters: n_airy (slot 4) and the tile counter (slot 6)
     if (cudaMemsetAsync(p->stats + 4, 0, sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
-    if (cudaMemsetAsync(p->stats + 6, 0, sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    if (cudaMemsetAsync(p->stats + 6, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
     SumArgs a;
     a.d = d;
     a.rec = p->rec;
     a.ent = p->ent;
     a.dense = p->dense;
     a.n_dense = p->n_dense;
+    a.bin_range = p->bin_range;
     a.dense_cap = p->dense_cap;
     a.wts = p->wts;
     a.n_angles = n_angles;
@@ -245,6 +250,7 @@ extern "C" int fdemri_get_stats(fdemri_plan_t p, fdemri_stats* out) {
     out->n_turnover = h[3];
     out->n_airy = h[4];
     out->flags = h[5];
+    out->n_slow = h[7];
     if (h[5] & (FDEMRI_BAD_TWO_EXTREMA | FDEMRI_BAD_STRIP_OVERFLOW)) return FDEMRI_ERR_UNSUPPORTED;
     if (h[5] & FDEMRI_BAD_NONFINITE) return FDEMRI_ERR_INVALID_ARG;
     return FDEMRI_OK;
@@ -332,6 +338,31 @@ extern "C" int fdemri_measure_fp64_peak(int n_iters, double* tflops_out) {
     double flops = 2.0 * 8.0 * (double)n_iters * threads * (double)blocks;
     *tflops_out = flops / (best * 1e-3) * 1e-12;
     return FDEMRI_OK;
+}
+
+// diagnostic: the device root finder of the monotone path on n independent problems (host arrays in and out)
+__global__ void k_debug_root(int n, const double* __restrict__ in, double* __restrict__ out) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double* a = in + 8 * i;     // x FB FC FD q1 q2 q3 h
+    double tau, Fd, Fdd, y;
+    unsigned int bad = 0, slow = 0;
+    fdemri_root_monotone(a[0], a[1], a[2], a[3], a[4], a[5], a[6], a[7], tau, Fd, Fdd, y, bad, slow);
+    out[6 * i + 0] = tau; out[6 * i + 1] = Fd; out[6 * i + 2] = Fdd; out[6 * i + 3] = y;
+    out[6 * i + 4] = (double)slow; out[6 * i + 5] = (double)bad;
+}
+
+extern "C" int fdemri_debug_root_monotone(int n, const double* in_host, double* out_host) {
+    if (n < 1 || !in_host || !out_host) return FDEMRI_ERR_INVALID_ARG;
+    double *din = nullptr, *dout = nullptr;
+    if (cudaMalloc(&din, sizeof(double) * 8 * n) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    if (cudaMalloc(&dout, sizeof(double) * 6 * n) != cudaSuccess) { cudaFree(din); return FDEMRI_ERR_CUDA; }
+    cudaMemcpy(din, in_host, sizeof(double) * 8 * n, cudaMemcpyHostToDevice);
+    k_debug_root<<<(n + 127) / 128, 128>>>(n, din, dout);
+    cudaMemcpy(out_host, dout, sizeof(double) * 6 * n, cudaMemcpyDeviceToHost);
+    cudaFree(din);
+    cudaFree(dout);
+    return cudaGetLastError() == cudaSuccess ? FDEMRI_OK : FDEMRI_ERR_CUDA;
 }
 
 extern "C" int fdemri_destroy(fdemri_plan_t p) {

@@ -126,9 +126,12 @@ __global__ void k_strips(FdemriDims d, const int* __restrict__ lmn, const double
 // Dense per-item strip list in (voice, sign, time) order: one CTA per batch item.
 // dense: [B][cap] int4 {lo, hi, (vs << 1) | dir, e0 | (n << 16)};  n_dense: [B]
 __global__ void k_strip_compact(int V, int cap, const StripRaw* __restrict__ strips, const int* __restrict__ n_strips,
-                                int4* __restrict__ dense, int* __restrict__ n_dense) {
+                                int4* __restrict__ dense, int* __restrict__ n_dense, int2* __restrict__ bin_range) {
     __shared__ int s_scan[1024];
     __shared__ int s_base;
+    __shared__ int s_min, s_max;
+    if (threadIdx.x == 0) { s_min = 0x7fffffff; s_max = -1; }
+    int my_min = 0x7fffffff, my_max = -1;
     int b = blockIdx.x;
     int nvs = 2 * V;
     if (threadIdx.x == 0) s_base = 0;
@@ -149,6 +152,8 @@ __global__ void k_strip_compact(int V, int cap, const StripRaw* __restrict__ str
             const StripRaw* ST = strips + ((size_t)b * nvs + vs) * FDEMRI_MAX_STRIPS;
             for (int j = 0; j < cnt; ++j) {
                 StripRaw r = ST[j];
+                my_min = min(my_min, r.lo);
+                my_max = max(my_max, r.hi);
                 if (pos + j < cap)
                     dense[(size_t)b * cap + pos + j] = make_int4(r.lo, r.hi, (vs << 1) | (r.n_dir & 1), r.e0 | ((r.n_dir >> 1) << 16));
             }
@@ -157,5 +162,11 @@ __global__ void k_strip_compact(int V, int cap, const StripRaw* __restrict__ str
         if (threadIdx.x == blockDim.x - 1) s_base += s_scan[threadIdx.x];
         __syncthreads();
     }
-    if (threadIdx.x == 0) n_dense[b] = min(s_base, cap);
+    atomicMin(&s_min, my_min);
+    atomicMax(&s_max, my_max);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        n_dense[b] = min(s_base, cap);
+        bin_range[b] = make_int2(s_min, s_max);
+    }
 }
