@@ -117,12 +117,6 @@ int fdemri_get_kernel_ms(fdemri_plan_t plan, float* ms_out);
  * of the ALU-bound tile kernel): writes TFLOP/s (2 flop per DFMA).  Synchronous; n_iters ~ 1<<16. */
 int fdemri_measure_fp64_peak(int n_iters, double* tflops_out);
 
-/* Diagnostic: runs the device root finder of the monotone-segment path (Eq. 6 inverted) on n independent
- * problems.  in_host [n][8] = {x, FB, FC, FD, q1, q2, q3, h}: solve FB tau + FC tau^2 + FD tau^3 = x on [0,h] from
- * the seed tau0 = x(q1 + x(q2 + x q3)).  out_host [n][6] = {tau, F', F'', |F'|^(-1/2), slow-path flag, error bits}.
- * Host pointers; synchronous. */
-int fdemri_debug_root_monotone(int n, const double* in_host, double* out_host);
-
 int fdemri_destroy(fdemri_plan_t plan);
 const char* fdemri_strerror(int status);
 /* Library version string, e.g. "fdemri 0.1 sm_100a". */

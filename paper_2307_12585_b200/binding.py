@@ -20,7 +20,7 @@ STATUS = {0: "FDEMRI_OK", 1: "FDEMRI_ERR_INVALID_ARG", 2: "FDEMRI_ERR_WORKSPACE"
           4: "FDEMRI_ERR_NOT_BUILT", 5: "FDEMRI_ERR_UNSUPPORTED"}
 
 EXPORTS = ["fdemri_plan", "fdemri_workspace_bytes", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum",
-           "fdemri_get_stats", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_debug_root_monotone", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
+           "fdemri_get_stats", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
 
 
 class FdemriStats(C.Structure):
@@ -65,8 +65,6 @@ def lib() -> C.CDLL:
         L.fdemri_get_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
         L.fdemri_measure_fp64_peak.restype = C.c_int
         L.fdemri_measure_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
-        L.fdemri_debug_root_monotone.restype = C.c_int
-        L.fdemri_debug_root_monotone.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.fdemri_destroy.restype = C.c_int
         L.fdemri_destroy.argtypes = [vp]
         L.fdemri_strerror.restype = C.c_char_p
@@ -154,15 +152,6 @@ def fdemri_measure_fp64_peak(n_iters=1 << 16) -> float:
     tf = C.c_double()
     _chk("fdemri_measure_fp64_peak", lib().fdemri_measure_fp64_peak(int(n_iters), C.byref(tf)))
     return float(tf.value)
-
-
-def fdemri_debug_root_monotone(problems):
-    """problems [n][8] = {x, FB, FC, FD, q1, q2, q3, h} -> [n][6] = {tau, F', F'', y, slow, bad}."""
-    a = np.ascontiguousarray(problems, dtype=np.float64)
-    out = np.empty((a.shape[0], 6))
-    dp = C.POINTER(C.c_double)
-    _chk("fdemri_debug_root_monotone", lib().fdemri_debug_root_monotone(a.shape[0], a.ctypes.data_as(dp), out.ctypes.data_as(dp)))
-    return out
 
 
 def fdemri_destroy(plan):

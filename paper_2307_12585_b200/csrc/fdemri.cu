@@ -40,6 +40,7 @@ struct fdemri_plan_s {
     bool built;
     cudaStream_t last_stream;
     int sm_count;
+    int sum_blocks_per_sm;         // resident CTAs of k_tile_sum per SM (0: not queried yet)
     uint32_t flags;
     cudaEvent_t ev0, ev1;
     bool ev_valid;
@@ -116,6 +117,7 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
         return FDEMRI_ERR_CUDA;
     }
     p->sm_count = prop.multiProcessorCount;
+    p->sum_blocks_per_sm = 0;
     p->flags = flags;
     p->ev_valid = false;
     p->ev0 = p->ev1 = nullptr;
@@ -226,13 +228,20 @@ extern "C" int fdemri_sum(fdemri_plan_t p, int n_angles, const double* theta_hos
     a.tile_counter = (unsigned int*)(p->stats + 6);
     a.stats = p->stats;
     a.total_tiles = d.n_tiles * d.n_batch;
-    int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_tile_sum, FDEMRI_TILE, 0) != cudaSuccess || per_sm < 1)
-        per_sm = 1;
-    long long grid = (long long)p->sm_count * per_sm;
+    const size_t smem = sizeof(FdemriRing);
+    if (p->sum_blocks_per_sm == 0) {
+        if (cudaFuncSetAttribute(k_tile_sum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            return FDEMRI_ERR_CUDA;
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_tile_sum, FDEMRI_SUM_THREADS, smem) != cudaSuccess ||
+            per_sm < 1)
+            per_sm = 1;
+        p->sum_blocks_per_sm = per_sm;
+    }
+    long long grid = (long long)p->sm_count * p->sum_blocks_per_sm;
     if (grid > a.total_tiles) grid = a.total_tiles;
     if (p->ev0) cudaEventRecord(p->ev0, st);
-    k_tile_sum<<<(unsigned)grid, FDEMRI_TILE, 0, st>>>(a);
+    k_tile_sum<<<(unsigned)grid, FDEMRI_SUM_THREADS, smem, st>>>(a);
     if (p->ev1) { cudaEventRecord(p->ev1, st); p->ev_valid = true; }
     if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
     return FDEMRI_OK;
@@ -338,31 +347,6 @@ extern "C" int fdemri_measure_fp64_peak(int n_iters, double* tflops_out) {
     double flops = 2.0 * 8.0 * (double)n_iters * threads * (double)blocks;
     *tflops_out = flops / (best * 1e-3) * 1e-12;
     return FDEMRI_OK;
-}
-
-// diagnostic: the device root finder of the monotone path on n independent problems (host arrays in and out)
-__global__ void k_debug_root(int n, const double* __restrict__ in, double* __restrict__ out) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const double* a = in + 8 * i;     // x FB FC FD q1 q2 q3 h
-    double tau, Fd, Fdd, y;
-    unsigned int bad = 0, slow = 0;
-    fdemri_root_monotone(a[0], a[1], a[2], a[3], a[4], a[5], a[6], a[7], tau, Fd, Fdd, y, bad, slow);
-    out[6 * i + 0] = tau; out[6 * i + 1] = Fd; out[6 * i + 2] = Fdd; out[6 * i + 3] = y;
-    out[6 * i + 4] = (double)slow; out[6 * i + 5] = (double)bad;
-}
-
-extern "C" int fdemri_debug_root_monotone(int n, const double* in_host, double* out_host) {
-    if (n < 1 || !in_host || !out_host) return FDEMRI_ERR_INVALID_ARG;
-    double *din = nullptr, *dout = nullptr;
-    if (cudaMalloc(&din, sizeof(double) * 8 * n) != cudaSuccess) return FDEMRI_ERR_CUDA;
-    if (cudaMalloc(&dout, sizeof(double) * 6 * n) != cudaSuccess) { cudaFree(din); return FDEMRI_ERR_CUDA; }
-    cudaMemcpy(din, in_host, sizeof(double) * 8 * n, cudaMemcpyHostToDevice);
-    k_debug_root<<<(n + 127) / 128, 128>>>(n, din, dout);
-    cudaMemcpy(out_host, dout, sizeof(double) * 6 * n, cudaMemcpyDeviceToHost);
-    cudaFree(din);
-    cudaFree(dout);
-    return cudaGetLastError() == cudaSuccess ? FDEMRI_OK : FDEMRI_ERR_CUDA;
 }
 
 extern "C" int fdemri_destroy(fdemri_plan_t p) {

@@ -7,32 +7,72 @@
 #define FDEMRI_MAX_KNOTS 512
 #define FDEMRI_MAX_STRIPS 8          // monotone branches kept per (voice, sign)
 #define FDEMRI_ENT_EXTRA 8           // entries per (voice, sign) = (n_knots-1) + FDEMRI_ENT_EXTRA
-#define FDEMRI_TILE 256              // bins per tile = threads per CTA of the sum kernel
+#define FDEMRI_CWARPS 8              // consumer (evaluating) warps per CTA of the sum kernel
+#define FDEMRI_BPL 2                 // bins per lane: a consumer warp owns 32*FDEMRI_BPL consecutive bins
+#define FDEMRI_TILE (FDEMRI_CWARPS * 32 * FDEMRI_BPL)     // bins per tile (512)
+#define FDEMRI_SUM_THREADS ((FDEMRI_CWARPS + 1) * 32)     // + one producer warp
+#define FDEMRI_CHUNK 64              // staged items per ring stage
+#define FDEMRI_STAGES 4              // ring depth
 
 // ------------------------------------------------------------------------------------------------
-// Record of one (voice, segment): everything the sum needs about that piece of trajectory.
-// 24 doubles = 192 B.  tau = t - t_k.
+// Record of one (voice, segment) in global memory: everything the sum needs about that piece of
+// trajectory that depends neither on the sign s nor on the viewing angles.  24 doubles = 192 B.  tau = t - t_k.
 // ------------------------------------------------------------------------------------------------
 enum {
     R_FA = 0,   // F(tau) = FA + FB tau + FC tau^2 + FD tau^3  (Eq. 6); FA is the knot value F_k (R6)
     R_FB = 1,
     R_FC = 2,
     R_FD = 3,
-    R_PC = 4,   // phase constant in cycles: -frac(Phi_v(t_k)/2pi) + m*phi/2pi
-    R_BH = 5,   // b' = b_Phi/2pi as hi + lo
-    R_BL = 6,
-    R_NC = 7,   // -c_Phi/2pi
+    R_Q1 = 4,   // normal segment: seed tau0 = x (Q1 + x (Q2 + x Q3)), x = s f - FA
+    R_Q2 = 5,   // turnover segment: Q1 = tau_e, Q2 = F_e, Q3 = C + 3 D tau_e
+    R_Q3 = 6,
+    R_H = 7,    // segment length h_k
     R_AR = 8,   // Re A coefficients a,b,c,d  (8..11)   (32-byte aligned: written as one double4)
     R_AI = 12,  // Im A coefficients a,b,c,d  (12..15)
-    R_ND = 16,  // -d_Phi/2pi
-    R_TK = 17,  // t_k
-    R_Q1 = 18,  // normal segment: seed tau0 = x (Q1 + x (Q2 + x Q3)), x = s f - FA
-    R_Q2 = 19,  // turnover segment: Q1 = tau_e, Q2 = F_e, Q3 = C + 3 D tau_e
-    R_Q3 = 20,
-    R_H = 21,   // segment length h_k
-    R_TYPE = 22,// 0.0 normal, 1.0 turnover (one interior extremum)
-    R_SPARE = 23,
+    R_PC = 16,  // phase constant in cycles: -frac(Phi_v(t_k)/2pi)
+    R_BH = 17,  // b' = b_Phi/2pi as hi + lo
+    R_BL = 18,
+    R_NC = 19,  // -c_Phi/2pi
+    R_ND = 20,  // -d_Phi/2pi
+    R_TK = 21,  // t_k
+    R_TYPE = 22,// 0.0 normal, 1.0 turnover (one interior extremum), 2.0 unsupported (two)
+    R_SF = 23,  // sign (+-1.0) of dF/dtau on the segment (turnover: on its first branch)
     R_DOUBLES = 24
+};
+
+// ------------------------------------------------------------------------------------------------
+// Staged item in shared memory: one (voice, sign, segment-branch) x tile, written by the producer warp of the
+// sum kernel from the record, the sign and the harmonic weights.  Phases are in QUARTER cycles.
+// 32 doubles = 256 B; consumers read it with broadcast LDS.
+// ------------------------------------------------------------------------------------------------
+enum {
+    S_META = 0, // int2 {lo | hi << 16 (tile-relative bins), type | branchB << 1 | sign << 2}
+    S_HSF = 1,  // 0.5 * sign of dF/dtau on this branch (folded into S_PC4; the slow path adds it back)
+    S_NFA = 2,  // -FA
+    S_FB = 3,
+    S_FC = 4,
+    S_FD = 5,
+    S_Q1 = 6,
+    S_Q2 = 7,
+    S_Q3 = 8,
+    S_TOLH = 9, // acceptance threshold of the last Newton correction, 3e-8 h
+    S_HH = 10,  // h/2
+    S_HH1 = 11, // h/2 (1 + 1e-9)
+    S_CU = 12,  // 1/X = CU * (F''/2)^2 / |F'|^3,  CU = sign(F') 6/pi
+    S_TK4 = 13, // 4 t_k
+    S_NBH4 = 14,// -4 b'_hi
+    S_NBL4 = 15,// -4 b'_lo
+    S_NC4 = 16, // 4 (-c_Phi/2pi)
+    S_ND4 = 17, // 4 (-d_Phi/2pi)
+    S_PC4 = 18, // 4 (PC + m phi/2pi) - 0.5 sign(F')     (the e^{-+i pi/4} of the standard SPA, L119)
+    S_SPARE = 19,
+    S_AR = 20,  // 20..23
+    S_AI = 24,  // 24..27
+    S_WP = 28,  // w+
+    S_SWP = 29, // s w+
+    S_NWX = 30, // -wx
+    S_SWX = 31, // s wx
+    S_DOUBLES = 32
 };
 
 struct FdemriDims {

@@ -128,7 +128,7 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
     R[R_PC] = pc; R[R_BH] = bq.hi; R[R_BL] = bq.lo;
     R[R_NC] = -dd_mul(Pc, inv2pi).hi;
     R[R_ND] = -dd_mul(Pd, inv2pi).hi;
-    R[R_TK] = tk; R[R_H] = h; R[R_SPARE] = 0.0;
+    R[R_TK] = tk; R[R_H] = h;
     // interior extrema of F on (0, h): roots of FB + 2 FC t + 3 FD t^2
     double ext[2]; int ne = 0;
     {
@@ -163,15 +163,17 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
             q1 = alp * idF; q2 = bet * idF * idF; q3 = gam * idF * idF * idF;
         }
         R[R_Q1] = q1; R[R_Q2] = q2; R[R_Q3] = q3; R[R_TYPE] = 0.0;
+        R[R_SF] = (dF < 0.0) ? -1.0 : 1.0;
     } else if (ne == 1) {
         double te = ext[0];
         R[R_Q1] = te;
         R[R_Q2] = FA + te * (FB + te * (FC + te * FD));     // F_e (R7)
         R[R_Q3] = FC + 3.0 * FD * te;                        // F(t) - F_e = z^2 (Q3 + FD z), z = t - te
         R[R_TYPE] = 1.0;
+        R[R_SF] = (R[R_Q2] < FA) ? -1.0 : 1.0;               // first branch runs from F_k to F_e
         atomicAdd(stats + 3, 1ull);
     } else {
-        R[R_Q1] = 0.0; R[R_Q2] = 0.0; R[R_Q3] = 0.0; R[R_TYPE] = 2.0;
+        R[R_Q1] = 0.0; R[R_Q2] = 0.0; R[R_Q3] = 0.0; R[R_TYPE] = 2.0; R[R_SF] = 1.0;
         atomicOr(stats + 5, 1ull);                           // FDEMRI_BAD_TWO_EXTREMA
     }
     if (bad) atomicOr(stats + 5, 4ull);

@@ -1,19 +1,30 @@
 // fdemri_sum.cuh -- S3 + S4: the output-tiled harmonic sum (the hot loop).
 //
-// Each CTA owns a tile of FDEMRI_TILE consecutive bins of one batch item (one bin per thread, accumulators in
-// registers).  It scans the item's strips in their fixed (voice, sign, time) order, turns every strip that
-// intersects the tile into "items" -- (voice, sign, segment-branch) with the sub-range of the tile they cover
-// and the index of their record -- in shared memory, and every thread whose bin lies in an item's sub-range
-// evaluates the term of Eq. 9:
-//     A(t) g(X)/sqrt|Fdot| exp{i[2 pi s f t - Phi(t)]},   t = t_k + tau,  F(tau) = s f  (Eq. 6)
-// and adds it with the harmonic weights (Eq. 1).  Every bin is written once (S4): no atomics, and the
-// summation order of a bin depends only on the data, never on scheduling: results are bitwise reproducible.
+// A CTA owns a tile of FDEMRI_TILE consecutive bins of one batch item at a time (tiles are handed out by an
+// atomic counter).  It is warp-specialised:
+//   * one PRODUCER warp scans the item's strips in their fixed (voice, sign, time) order, turns every strip that
+//     intersects the tile into "items" -- (voice, sign, segment-branch) with the sub-range of the tile they
+//     cover -- reads their records and weights from global memory, folds everything that does not depend on
+//     the bin into a 256-byte staged item, and pushes chunks of staged items through a shared-memory ring
+//     (full/empty mbarriers);
+//   * FDEMRI_CWARPS CONSUMER warps each own 64 consecutive bins of the tile, two per lane (lane, lane + 32),
+//     with the eight accumulators in registers.  For every staged item that overlaps its bins a consumer warp
+//     evaluates the term of Eq. 9 for both of its bins at once (two independent
+//     dependency chains per thread hide the 8-cycle FP64 latency):
+//         A(t) g(X)/sqrt|Fdot| exp{i[2 pi s f t - Phi(t)]},   t = t_k + tau,  F(tau) = s f  (Eq. 6)
+//     and adds it with the harmonic weights (Eq. 1).
+// Every bin is written once (S4): no atomics on the data path, and the summation order of a bin depends only
+// on the data, never on scheduling: results are bitwise reproducible.
 // The paper's own layout -- one block per (voice, segment), atomicAdd into global memory (L121) -- is prior art.
+//
+// Fast path (monotone segment, |X| >= 400, > 99 % of the evaluations): division-free inversion of the segment
+// cubic -- stored inverse-cubic seed, one Halley step, one Newton correction whose size is the acceptance test --
+// then the polar form of the asymptotic g(X) series and a polynomial sincos of the phase in quarter turns.
+// Everything else (turnover segments, small |X|, rejected iterations) goes to fdemri_term_slow.
 #pragma once
 #include "fdemri_common.cuh"
 #include "airy_tables.inc"
-
-#define FDEMRI_LCAP (3 * FDEMRI_TILE)     // items per round: each candidate strip emits at most 3
+#include "poly_tables.inc"
 
 struct SumArgs {
     FdemriDims d;
@@ -32,57 +43,31 @@ struct SumArgs {
     int total_tiles;
 };
 
-// constants as c[][] operands (no immediate materialisation in the loop)
-// sin(pi r/2) = r * sum_k S_k r^2k,  cos(pi r/2) = sum_k C_k r^2k,  |r| <= 1/2: truncation 5e-17 / 2e-18
-__constant__ double c_sinq[8] = {1.5707963267948966192, -0.64596409750624625366, 0.079692626246167045121,
-                                 -0.0046817541353186881007, 0.00016044118478735982187, -3.5988432352120853405e-6,
-                                 5.6921729219679268118e-8, -6.6880351098114672325e-10};
-__constant__ double c_cosq[9] = {1.0, -1.2337005501361698274, 0.25366950790104801364, -0.020863480763352960873,
-                                 0.00091926027483942658024, -0.000025202042373060605481, 4.7108747788181715037e-7,
-                                 -6.3866030837918522411e-9, 6.5659631149794723622e-11};
 // asymptotic series of g(X) e^{+i pi/4 sgn X} = sum_k i^k a_k u^k, u = 1/X, a_k = prod_j (4/9-(2j-1)^2)/(k! 8^k)
 __constant__ double c_gre[7] = {1.0, -0.037133487654320986, 0.05764919041266972, -0.2915913992307505,
                                 3.079453030173167, -55.62278536591708, 1533.1694320127956};
 __constant__ double c_gim[6] = {-0.06944444444444445, 0.03799305912780064, -0.11609906402551541,
                                 0.8776669695100169, -12.341573332345238, 278.46508077760257};
 
-__device__ __forceinline__ void fdemri_g_series(double u, double& re, double& im) {
-    const double u2 = u * u;
-    if (fabs(u) <= 2.5e-3) {          // |X| >= 400: through a_4, error < 1.2e-14
-        re = fma(u2, fma(u2, c_gre[2], c_gre[1]), c_gre[0]);
-        im = u * fma(u2, c_gim[1], c_gim[0]);
-    } else {                          // 28 <= |X| < 400: through a_12, error < 2e-15
-        double r = c_gre[6];
-#pragma unroll
-        for (int i = 5; i >= 0; --i) r = fma(r, u2, c_gre[i]);
-        re = r;
-        double q = c_gim[5];
-#pragma unroll
-        for (int i = 4; i >= 0; --i) q = fma(q, u2, c_gim[i]);
-        im = q * u;
-    }
-}
-
 // x with its sign bit XORed by `mask` (0 or 0x80000000): one integer op on the high word
 __device__ __forceinline__ double fdemri_xorsign(double x, unsigned mask) {
     return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));
 }
 
-// sin(2 pi c), cos(2 pi c) for |c| up to ~1e3 cycles (absolute error ~1e-16 + 2 pi ulp(c))
-__device__ __forceinline__ void fdemri_sincos_cycles(double c, double& sn, double& cs) {
-    const double q = 4.0 * c;
+// sin, cos of q quarter turns (|q| up to ~1e4; absolute error ~1e-14 + (pi/2) ulp(q))
+__device__ __forceinline__ void fdemri_sincos_quarter(double q, double& sn, double& cs) {
     const double big = 6755399441055744.0;             // 1.5 * 2^52: adding it rounds to the nearest integer
     const double t = q + big;
     const int k = __double2loint(t);                   // low word of the sum = the integer (two's complement)
     const double r = q - (t - big);                    // in [-1/2, 1/2], exact
     const double r2 = r * r;
-    double s = c_sinq[7];
+    double s = c_sinq[FDEMRI_NSIN - 1];
 #pragma unroll
-    for (int i = 6; i >= 0; --i) s = fma(s, r2, c_sinq[i]);
+    for (int i = FDEMRI_NSIN - 2; i >= 0; --i) s = fma(s, r2, c_sinq[i]);
     s *= r;
-    double co = c_cosq[8];
+    double co = c_cosq[FDEMRI_NCOS - 1];
 #pragma unroll
-    for (int i = 7; i >= 0; --i) co = fma(co, r2, c_cosq[i]);
+    for (int i = FDEMRI_NCOS - 2; i >= 0; --i) co = fma(co, r2, c_cosq[i]);
     // rotate by k quarter turns: swap for odd k, then flip signs
     const bool odd = k & 1;
     const double a = odd ? co : s;
@@ -120,168 +105,182 @@ __device__ __forceinline__ double fdemri_rsqrt_seed(double a) {      // ~21 good
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
     return y;
 }
-// one Newton step of y ~ a^(-1/2):  y <- y + (y/2)(1 - a y^2)
-__device__ __forceinline__ double fdemri_rsqrt_step(double y, double a) {
-    const double t = a * y;
-    const double e = fma(-t, y, 1.0);
-    return fma(0.5 * y, e, y);
+
+// ---- mbarrier helpers (shared::cta) ----------------------------------------------------------------------
+__device__ __forceinline__ unsigned fdemri_smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void fdemri_mbar_init(uint64_t* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(fdemri_smem_addr(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fdemri_mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(fdemri_smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void fdemri_mbar_wait(uint64_t* bar, unsigned parity) {
+    const unsigned addr = fdemri_smem_addr(bar);
+    unsigned done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(addr), "r"(parity)
+            : "memory");
+    } while (!done);
 }
 
-// Root of the monotone segment cubic  FB tau + FC tau^2 + FD tau^3 = x  and 1/sqrt|Fdot| there, without a division.
-// Newton with the reciprocal slope taken as +-y^2, y ~ |F'|^(-1/2) refined alongside (the final y is needed anyway).
-__device__ __forceinline__ void fdemri_root_monotone(double x, double FB, double FC, double FD, double q1, double q2,
-                                                     double q3, double h, double& tau_out, double& Fd_out,
-                                                     double& Fdd_out, double& y_out, unsigned int& bad,
-                                                     unsigned int& bad_slow) {
-    double tau = x * fma(x, fma(x, q3, q2), q1);                 // seed: stored inverse cubic
-    double b2, b1, G, c2, dG, y, r;
-    // iteration 0
+// ---------------------------------------------------------------------------------------------------------
+// Fast path of one term.  it: the staged item (shared memory); sf = s f.  Returns T = A g/sqrt|F'| e^{i psi}
+// and ok = the inversion was accepted and |X| >= 400.  Branch-free, so two calls interleave.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool fdemri_term_fast(const double* __restrict__ it, double sf, double& Tre, double& Tim) {
+    const double FB = it[S_FB], FC = it[S_FC], FD = it[S_FD];
+    const double x = sf + it[S_NFA];
+    double tau = x * fma(x, fma(x, it[S_Q3], it[S_Q2]), it[S_Q1]);          // seed: stored inverse cubic
+    // Halley step:  tau <- tau - d (1 + d F''/(2 F')),  d = G/F',  1/F' from the 64-bit rsqrt seed squared
+    double b2 = fma(tau, FD, FC), b1 = fma(tau, b2, FB), G = fma(tau, b1, -x);
+    double c2 = fma(tau, FD, b2), dG = fma(tau, c2, b1), Fh = fma(tau, FD, c2);   // Fh = F''/2
+    double y = fdemri_rsqrt_seed(fabs(dG));
+    double r = copysign(y * y, dG);
+    const double d0 = G * r;
+    tau = fma(-d0, d0 * (Fh * r), tau - d0);
+    // Newton correction at the new point; its size is the acceptance test
     b2 = fma(tau, FD, FC); b1 = fma(tau, b2, FB); G = fma(tau, b1, -x);
-    c2 = fma(tau, FD, b2); dG = fma(tau, c2, b1);
+    c2 = fma(tau, FD, b2); dG = fma(tau, c2, b1); Fh = fma(tau, FD, c2);
     y = fdemri_rsqrt_seed(fabs(dG));
-    r = copysign(y * y, dG);
-    tau = fma(-G, r, tau);
-    // iteration 1
-    b2 = fma(tau, FD, FC); b1 = fma(tau, b2, FB); G = fma(tau, b1, -x);
-    c2 = fma(tau, FD, b2); dG = fma(tau, c2, b1);
-    y = fdemri_rsqrt_step(y, fabs(dG));
-    r = copysign(y * y, dG);
-    tau = fma(-G, r, tau);
-    // final evaluation and half step
-    b2 = fma(tau, FD, FC); b1 = fma(tau, b2, FB); G = fma(tau, b1, -x);
-    c2 = fma(tau, FD, b2); dG = fma(tau, c2, b1);
-    double Fdd = 2.0 * fma(tau, FD, c2);
-    const double ty = fabs(dG) * y;
-    const double ey = fma(-ty, y, 1.0);                          // residual of y before this step
-    y = fma(0.5 * y, ey, y);
-    r = copysign(y * y, dG);
-    double delta = G * r;
-    // accept when the neglected second-order term is below rounding: in tau (|delta| <= 3e-8 h) and, more
-    // demanding near a turnover just outside the segment, in the slope (|F'' delta| <= 1e-6 |F'|); and the
-    // iterate must sit in the segment (the root does, by membership R6); and the reciprocal slope r = y^2 that
-    // scaled delta must itself be good (|1 - |F'| y^2| <= 1e-3 before its last refinement)
-    const double hh = 0.5 * h;
-#ifdef FDEMRI_DBG_SLOW
-    if (true) {
-#else
-    if (!(fabs(ey) <= 1e-3 && fabs(delta) <= 6e-8 * hh && fabs(Fdd * delta) <= 1e-6 * fabs(dG) && fabs(tau - hh) <= 1.000000001 * hh)) {
-#endif
-        // rare: poor seed or nearly flat slope -- plain safeguarded Newton with a true division
+    {   // third-order refinement of y ~ |F'|^(-1/2): relative error 2^-22 -> < 1e-17
+        const double t = fabs(dG) * y;
+        const double e = fma(-t, y, 1.0);
+        y = fma(y, e * fma(e, 0.375, 0.5), y);
+    }
+    r = y * y;                                         // 1/|F'|
+    const double rs = copysign(r, dG);
+    const double delta = G * rs;
+    tau -= delta;
+    const double tq = (delta * Fh) * rs;               // relative change of F' over the correction, halved
+    y = fma(y, tq, y);                                 // |F'(tau)|^(-1/2) to first order in delta
+    // accept: the neglected second-order terms are below rounding (|F'' delta / F'| <= 1e-6 and |delta| <= 3e-8 h)
+    // and the iterate sits in the segment (the root does, by membership R6)
+    bool ok = (fabs(tq) <= 5e-7) && (fabs(delta) <= it[S_TOLH]) && (fabs(tau - it[S_HH]) <= it[S_HH1]);
+    // 1/X = 3 F''^2 / (2 pi F'^3)
+    const double pq = Fh * r;
+    const double u = (pq * pq) * (r * it[S_CU]);
+    ok = ok && (fabs(u) <= 2.5e-3);
+    const double u2 = u * u;
+    const double dq = u * fma(u2, FDEMRI_G_DQ3, FDEMRI_G_DQ1);
+    const double yr = y * fma(u2, fma(u2, FDEMRI_G_R4, FDEMRI_G_R2), 1.0);
+    // amplitude (two cubics)
+    const double Are = fma(tau, fma(tau, fma(tau, it[S_AR + 3], it[S_AR + 2]), it[S_AR + 1]), it[S_AR]);
+    const double Aim = fma(tau, fma(tau, fma(tau, it[S_AI + 3], it[S_AI + 2]), it[S_AI + 1]), it[S_AI]);
+    // phase in quarter turns (R9): (s f)(4 t_k) exactly as P + e, P reduced modulo 4; local cubic in tau
+    const double TK4 = it[S_TK4];
+    const double P = __dmul_rn(sf, TK4);
+    const double e = __fma_rn(sf, TK4, -P);
+    const double big4 = 27021597764222976.0;           // 1.5 * 2^54: adding it rounds to a multiple of 4
+    const double pr = P - ((P + big4) - big4);
+    const double wv = fma(sf, 4.0, it[S_NBH4]) + it[S_NBL4];
+    const double loc = tau * fma(tau, fma(tau, it[S_ND4], it[S_NC4]), wv);
+    const double q = ((pr + e) + it[S_PC4]) + (loc + dq);
+    double sn, cs;
+    fdemri_sincos_quarter(q, sn, cs);
+    const double Er = yr * cs, Ei = yr * sn;
+    Tre = Are * Er - Aim * Ei;
+    Tim = Are * Ei + Aim * Er;
+    return ok;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Slow path of one term: turnover segments, small |X| (long series or Airy form), rejected fast iterations.
+// flags: bit 0 type (1 = turnover), bit 1 second branch, bit 2 sign.  Returns T and counters in `info`:
+// bit 0 Airy form used, bit 1 monotone fallback Newton, bits 4.. error bits (FDEMRI_BAD_NEWTON << 4).
+// ---------------------------------------------------------------------------------------------------------
+struct FdemriSlowOut {
+    double tre, tim;
+    unsigned info;
+};
+
+__device__ __noinline__ FdemriSlowOut fdemri_term_slow(const double* it, double sf, unsigned flags) {
+    FdemriSlowOut out;
+    out.tre = 0.0; out.tim = 0.0; out.info = 0u;
+    const double FB = it[S_FB], FC = it[S_FC], FD = it[S_FD];
+    const double h = 2.0 * it[S_HH];
+    double tau, Fd, Fdd;
+    if (!(flags & 1u)) {
+        // monotone segment: safeguarded Newton with a true division from the stored seed
+        const double x = sf + it[S_NFA];
+        tau = x * fma(x, fma(x, it[S_Q3], it[S_Q2]), it[S_Q1]);
         tau = fmin(fmax(tau, 0.0), h);
-        int it = 0;
-        for (; it < 60; ++it) {
-            b2 = fma(tau, FD, FC); b1 = fma(tau, b2, FB); G = fma(tau, b1, -x);
+        double dG = 0.0, c2 = 0.0;
+        int n = 0;
+        for (; n < 60; ++n) {
+            const double b2 = fma(tau, FD, FC), b1 = fma(tau, b2, FB), G = fma(tau, b1, -x);
             c2 = fma(tau, FD, b2); dG = fma(tau, c2, b1);
-            delta = G / dG;
-            if (fabs(delta) <= 1e-14 * h) break;
+            const double delta = G / dG;
+            if (!(fabs(delta) > 1e-14 * h)) { if (fabs(delta) <= h) tau -= delta; break; }
             tau = fmin(fmax(tau - delta, 0.0), h);
         }
-        if (it == 60) bad |= 8u;
+        if (n == 60) out.info |= (8u << 4);
+        tau = fmin(fmax(tau, 0.0), h);
+        {
+            const double b2 = fma(tau, FD, FC), b1 = fma(tau, b2, FB);
+            c2 = fma(tau, FD, b2); Fd = fma(tau, c2, b1);
+        }
         Fdd = 2.0 * fma(tau, FD, c2);
-        y = rsqrt(fabs(dG));
-        ++bad_slow;
-    }
-    tau = tau - delta;
-    const double Fd = fma(-delta, Fdd, dG);                      // F'(tau - delta) to first order in delta
-    Fdd = fma(-6.0 * FD, delta, Fdd);                            // F''(tau - delta), exact for a cubic (the Airy
-                                                                 // form near a turnover needs it to 1e-12)
-    {
-        // last refinement of y = |F'|^(-1/2); its residual e = 1 - |F'| y^2 tells whether y had converged
-        const double aFd = fabs(Fd);
-        const double t = aFd * y;
-        const double e = fma(-t, y, 1.0);
-        y = fma(0.5 * y, e, y);                                  // error after the step: 3/8 e^2
-        if (!(fabs(e) <= 2e-7)) y = rsqrt(aFd);                  // rare: the slope moved a lot between iterations
-    }
-    tau_out = tau; Fd_out = Fd; Fdd_out = Fdd; y_out = y;
-}
-
-// One term.  R: the (voice, segment) record (24 doubles, 32-byte aligned); sbit = 0 for s=+1, 0x80000000 for s=-1;
-// f the bin frequency; brB: second branch of a turnover segment; w = {w+, wx, m phi/2pi}.
-// acc = {Re h+, Im h+, Re hx, Im hx}.  cnt = {airy evaluations, slow Newton, error bits}.
-__device__ __forceinline__ void fdemri_term(const double* __restrict__ R, unsigned sbit, double f, int brB,
-                                            const double4 w, double acc[4], unsigned int cnt[3]) {
-    const double4* R4 = reinterpret_cast<const double4*>(R);
-    const double4 rF = fdemri_ld4(R4 + 0);       // FA FB FC FD
-    const double4 rP = fdemri_ld4(R4 + 1);       // PC BH BL NC
-    const double4 rA = fdemri_ld4(R4 + 2);       // Re A
-    const double4 rB = fdemri_ld4(R4 + 3);       // Im A
-    const double4 rQ = fdemri_ld4(R4 + 4);       // ND TK Q1 Q2
-    const double4 rT = fdemri_ld4(R4 + 5);       // Q3 H TYPE spare
-    const double FC = rF.z, FD = rF.w;
-    const double h = rT.y;
-    const double sf = fdemri_xorsign(f, sbit);
-    double tau, Fd, Fdd, y, u;
-    bool series;                                   // |X| >= 28: asymptotic series, else Airy form
-    if (rT.z == 0.0) {
-        fdemri_root_monotone(sf - rF.x, rF.y, FC, FD, rQ.z, rQ.w, rT.x, h, tau, Fd, Fdd, y, cnt[2], cnt[1]);
-        const double y2 = y * y;
-        const double pq = Fdd * y2;
-        u = copysign(0.477464829275686 * pq * pq * y2, Fd);      // 1/X = 3 Fdd^2 / (2 pi Fd^3)
-        series = fabs(u) <= 0.03571428571428571;
-#ifdef FDEMRI_DBG_AIRYTH
-        { const double aFd = fabs(Fd); series = 6.283185307179586 * aFd * aFd * aFd >= 84.0 * Fdd * Fdd; }
-#endif
+        out.info |= 2u;
     } else {
         // turnover segment: F(tau) - F_e = z^2 (c2 + FD z), z = tau - tau_e; branch A: z < 0, branch B: z > 0
-        const double te = rQ.z, Fe = rQ.w, c2 = rT.x;
+        const double te = it[S_Q1], Fe = it[S_Q2], c2 = it[S_Q3];
+        const bool brB = flags & 2u;
         const double Delta = sf - Fe;
         double z = sqrt(fmax(Delta / c2, 0.0));
         if (!brB) z = -z;
         const double tol = 1e-14 * h;
-        int it = 0;
-        for (; it < 40; ++it) {
-            double H = fma(z * z, fma(FD, z, c2), -Delta);
-            double dH = z * fma(3.0 * FD, z, 2.0 * c2);
+        int n = 0;
+        for (; n < 40; ++n) {
+            const double H = fma(z * z, fma(FD, z, c2), -Delta);
+            const double dH = z * fma(3.0 * FD, z, 2.0 * c2);
             if (dH == 0.0) break;
-            double delta = H / dH;
+            const double delta = H / dH;
             z -= delta;
             if (fabs(delta) <= tol) break;
         }
-        if (it == 40) cnt[2] |= 8u;
+        if (n == 40) out.info |= (8u << 4);
         z = brB ? fmin(fmax(z, 0.0), h - te) : fmax(fmin(z, 0.0), -te);
         tau = te + z;
         Fd = z * fma(3.0 * FD, z, 2.0 * c2);          // exact factorisation, no cancellation near Fdot = 0
         Fdd = fma(6.0 * FD, tau, 2.0 * FC);
-        if (Fd == 0.0 && Fdd == 0.0) return;           // R10: no term
-        const double aFd = fabs(Fd);
-        series = 6.283185307179586 * aFd * aFd * aFd >= 84.0 * Fdd * Fdd;
-        y = 0.0; u = 0.0;
-        if (series) {
-            y = rsqrt(aFd);
-            const double y2 = y * y;
-            const double pq = Fdd * y2;
-            u = copysign(0.477464829275686 * pq * pq * y2, Fd);
-        }
     }
-    // amplitude (two cubics)
-    const double Are = fma(tau, fma(tau, fma(tau, rA.w, rA.z), rA.y), rA.x);
-    const double Aim = fma(tau, fma(tau, fma(tau, rB.w, rB.z), rB.y), rB.x);
-    // phase in cycles (R9): (s f) t_k exactly as p + e, local cubic in tau, knot phase from the record
-    const double tk = rQ.y;
-    const double p = __dmul_rn(sf, tk);
-    const double e = __fma_rn(sf, tk, -p);
-    const double big = 6755399441055744.0;
-#ifdef FDEMRI_DBG_RINT
-    const double pr = p - rint(p);
-#else
-    const double pr = p - ((p + big) - big);           // p - rint(p), |p| < 2^51
-#endif
-    const double wv = (sf - rP.y) - rP.z;
-    const double loc = tau * fma(tau, fma(tau, rQ.x, rP.w), wv);
-    double cyc = ((pr + e) + (rP.x + w.z)) + loc;
-    // g(X)/sqrt|Fdot|
+    if (Fd == 0.0 && Fdd == 0.0) return out;           // R10: no term
+    const double aFd = fabs(Fd);
+    const bool series = 6.283185307179586 * aFd * aFd * aFd >= 84.0 * Fdd * Fdd;      // |X| >= 28
+    // amplitude
+    const double Are = fma(tau, fma(tau, fma(tau, it[S_AR + 3], it[S_AR + 2]), it[S_AR + 1]), it[S_AR]);
+    const double Aim = fma(tau, fma(tau, fma(tau, it[S_AI + 3], it[S_AI + 2]), it[S_AI + 1]), it[S_AI]);
+    // phase in quarter turns, the folded -+1/2 of the standard SPA taken out again
+    const double TK4 = it[S_TK4];
+    const double P = __dmul_rn(sf, TK4);
+    const double e = __fma_rn(sf, TK4, -P);
+    const double big4 = 27021597764222976.0;
+    const double pr = P - ((P + big4) - big4);
+    const double wv = fma(sf, 4.0, it[S_NBH4]) + it[S_NBL4];
+    const double loc = tau * fma(tau, fma(tau, it[S_ND4], it[S_NC4]), wv);
+    double q = ((pr + e) + (it[S_PC4] + it[S_HSF])) + loc;
     double Sre, Sim;
     if (series) {
-        // the e^{-+ i pi/4} of the standard SPA goes into the phase
-        double gr, gi;
-        fdemri_g_series(u, gr, gi);
+        const double y = rsqrt(aFd);
+        const double y2 = y * y;
+        const double pq = Fdd * y2;
+        const double u = copysign(0.477464829275686 * pq * pq * y2, Fd);      // 1/X
+        const double u2 = u * u;
+        double gr = c_gre[6];
+#pragma unroll
+        for (int i = 5; i >= 0; --i) gr = fma(gr, u2, c_gre[i]);
+        double gi = c_gim[5];
+#pragma unroll
+        for (int i = 4; i >= 0; --i) gi = fma(gi, u2, c_gim[i]);
+        gi *= u;
         Sre = gr * y;
         Sim = gi * y;
-        cyc -= copysign(0.125, Fd);
+        q -= copysign(0.5, Fd);
     } else {
         // |X| < 28: regular Airy form  e^{-iX} pi kap [Ai(-yy) -+ i Bi(-yy)],  kap = (pi|Fddot|)^(-1/3)
-        if (Fd == 0.0 && Fdd == 0.0) return;           // R10 (monotone type with a flat cubic)
         const double sig = (Fd >= 0.0) ? 1.0 : -1.0;
         const double kap = rcbrt(3.141592653589793 * fabs(Fdd));
         const double k2 = kap * kap;
@@ -289,68 +288,106 @@ __device__ __forceinline__ void fdemri_term(const double* __restrict__ R, unsign
         double ai, bi;
         fdemri_airy_neg(yy, ai, bi);
         const double X = 0.6666666666666666 * sig * yy * sqrt(yy);
-        cyc -= X * 0.15915494309189535;
+        q -= X * 0.6366197723675814;                   // X / (pi/2) quarter turns
         Sre = 3.141592653589793 * kap * ai;
         Sim = -sig * 3.141592653589793 * kap * bi;
-        ++cnt[0];
+        out.info |= 1u;
     }
     double sn, cs;
-#ifdef FDEMRI_DBG_SINCOSPI
-    sincospi(2.0 * cyc, &sn, &cs);
-#else
-    fdemri_sincos_cycles(cyc, sn, cs);
-#endif
+    fdemri_sincos_quarter(q, sn, cs);
     const double Ere = Sre * cs - Sim * sn, Eim = Sre * sn + Sim * cs;
-    const double Tre = Are * Ere - Aim * Eim, Tim = Are * Eim + Aim * Ere;
-    // weights (O2): s=+1: h+ += w+ T, hx += i wx T;  s=-1: h+ += w+ conj(T), hx += conj(i wx T)
-    acc[0] = fma(w.x, Tre, acc[0]);
-    acc[1] = fma(fdemri_xorsign(w.x, sbit), Tim, acc[1]);
-    acc[2] = fma(-w.y, Tim, acc[2]);
-    acc[3] = fma(fdemri_xorsign(w.y, sbit), Tre, acc[3]);
+    out.tre = Are * Ere - Aim * Eim;
+    out.tim = Are * Eim + Aim * Ere;
+    return out;
 }
 
-// item in shared memory: x = lo | hi << 16 (tile-relative bins), y = global record index
-// ((item * V + voice) * n_seg + segment), z = global weight index, w = sign << 30 | branchB << 31
-#ifndef FDEMRI_MINBLOCKS
-#define FDEMRI_MINBLOCKS 3
-#endif
-__global__ void __launch_bounds__(FDEMRI_TILE, FDEMRI_MINBLOCKS) k_tile_sum(SumArgs a) {
-    __shared__ int4 s_list[FDEMRI_LCAP];
-    __shared__ int s_wsum[FDEMRI_TILE / 32];
-    __shared__ int s_tile;
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+// ---------------------------------------------------------------------------------------------------------
+// Shared-memory ring between the producer warp and the consumer warps
+// ---------------------------------------------------------------------------------------------------------
+struct FdemriStage {
+    double items[FDEMRI_CHUNK][S_DOUBLES];
+    int hdr[4];                  // {global tile index (-1: no more work), item count, last chunk of the tile, 0}
+};
+struct FdemriRing {
+    FdemriStage st[FDEMRI_STAGES];
+    uint64_t full[FDEMRI_STAGES];
+    uint64_t empty[FDEMRI_STAGES];
+};
+
+// Producer lane: folds record + weights + sign into the staged item `dst` (shared memory)
+__device__ __forceinline__ void fdemri_stage_item(double* dst, const double* __restrict__ R, const double4 w, int lo,
+                                                  int hi, unsigned sg, unsigned brB) {
+    const double4* R4 = reinterpret_cast<const double4*>(R);
+    const double4 r0 = fdemri_ld4(R4 + 0);       // FA FB FC FD
+    const double4 r1 = fdemri_ld4(R4 + 1);       // Q1 Q2 Q3 H
+    const double4 r2 = fdemri_ld4(R4 + 2);       // Re A
+    const double4 r3 = fdemri_ld4(R4 + 3);       // Im A
+    const double4 r4 = fdemri_ld4(R4 + 4);       // PC BH BL NC
+    const double4 r5 = fdemri_ld4(R4 + 5);       // ND TK TYPE SF
+    const unsigned type = (unsigned)r5.z;
+    const double s = sg ? -1.0 : 1.0;
+    const double sF = (type == 1u && brB) ? -r5.w : r5.w;
+    const double h = r1.w;
+    double2* d2 = reinterpret_cast<double2*>(dst);
+    int2 meta = make_int2(lo | (hi << 16), (int)((type & 1u) | (brB << 1) | (sg << 2)));
+    d2[0] = make_double2(__hiloint2double(meta.y, meta.x), 0.5 * sF);
+    d2[1] = make_double2(-r0.x, r0.y);
+    d2[2] = make_double2(r0.z, r0.w);
+    d2[3] = make_double2(r1.x, r1.y);
+    d2[4] = make_double2(r1.z, 3e-8 * h);
+    d2[5] = make_double2(0.5 * h, 0.5 * h * 1.000000001);
+    d2[6] = make_double2(sF * 1.9098593171027440, 4.0 * r5.y);
+    d2[7] = make_double2(-4.0 * r4.y, -4.0 * r4.z);
+    d2[8] = make_double2(4.0 * r4.w, 4.0 * r5.x);
+    d2[9] = make_double2(fma(4.0, r4.x + w.z, -0.5 * sF), 0.0);
+    d2[10] = make_double2(r2.x, r2.y);
+    d2[11] = make_double2(r2.z, r2.w);
+    d2[12] = make_double2(r3.x, r3.y);
+    d2[13] = make_double2(r3.z, r3.w);
+    d2[14] = make_double2(w.x, s * w.x);
+    d2[15] = make_double2(-w.y, s * w.y);
+}
+
+__device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ring, int lane) {
     const FdemriDims& d = a.d;
     const int V = d.n_modes;
-    unsigned int cnt[3] = {0u, 0u, 0u};          // airy evaluations, slow Newton, error bits
+    int stage = 0;
+    unsigned phase = 0;
     for (;;) {
-        __syncthreads();
-        if (tid == 0) s_tile = (int)atomicAdd(a.tile_counter, 1u);
-        __syncthreads();
-        const int gt = s_tile;
-        if (gt >= a.total_tiles) break;
+        int gt = 0;
+        if (lane == 0) gt = (int)atomicAdd(a.tile_counter, 1u);
+        gt = __shfl_sync(0xffffffffu, gt, 0);
+        const bool done = gt >= a.total_tiles;
+        // a fresh stage for this tile
+        fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u);
+        if (done) {
+            if (lane == 0) {
+                ring->st[stage].hdr[0] = -1; ring->st[stage].hdr[1] = 0; ring->st[stage].hdr[2] = 1;
+                fdemri_mbar_arrive(&ring->full[stage]);
+            }
+            return;
+        }
+        int fill = 0;
         const int b = gt / d.n_tiles, tile = gt - b * d.n_tiles;
         const int64_t bin0 = (int64_t)tile * FDEMRI_TILE;
-        const int64_t bin = bin0 + tid;
-        const bool valid = bin < d.n_freq;
-        const double f = valid ? fdemri_freq(d, bin) : 0.0;
         const int tile_lo = (int)bin0;
         const int tile_hi = (int)min(bin0 + FDEMRI_TILE - 1, d.n_freq - 1);
-        double acc[4] = {0.0, 0.0, 0.0, 0.0};
         const int2 br = a.bin_range[b];
         const int nd = (br.y < tile_lo || br.x > tile_hi) ? 0 : a.n_dense[b];
         const int4* dense_b = a.dense + (size_t)b * a.dense_cap;
         const int wbase = (a.n_angles > 1 ? b : 0) * V;
-        const int rbase = b * V * d.n_seg;
-        for (int base = 0; base < nd; base += FDEMRI_TILE) {
-            // ---- candidate strip of this thread ----
-            const int c = base + tid;
-            int remaining = 0, e_next = 0, e0 = 0, ne = 0, dir = 0, vs = 0, s_lo = 0, s_hi = 0;
+        const size_t rbase = (size_t)b * V * d.n_seg;
+        for (int base = 0; base < nd; base += 32) {
+            // ---- candidate strip of this lane ----
+            const int c = base + lane;
+            int remaining = 0, e_next = 0, ne = 0, dir = 0, vs = 0, s_lo = 0, s_hi = 0;
             const int2* E = nullptr;
             if (c < nd) {
                 const int4 s = dense_b[c];
                 if (s.x <= tile_hi && s.y >= tile_lo) {
                     vs = s.z >> 1; dir = s.z & 1;
-                    e0 = s.w & 0xffff; ne = s.w >> 16;
+                    const int e0 = s.w & 0xffff;
+                    ne = s.w >> 16;
                     s_lo = s.x; s_hi = s.y;
                     E = a.ent + ((size_t)b * 2 * V + vs) * d.ent_max + e0;
                     const int clo = max(s.x, tile_lo), chi = min(s.y, tile_hi);
@@ -375,26 +412,29 @@ __global__ void __launch_bounds__(FDEMRI_TILE, FDEMRI_MINBLOCKS) k_tile_sum(SumA
                     remaining = eb - ea + 1;
                 }
             }
-            // ---- rounds: every candidate emits up to 3 items per round, in candidate order ----
+            // ---- rounds: every candidate emits up to 2 items per round, in candidate order ----
             for (;;) {
-                const int n_emit = min(remaining, 3);
+                const int n_emit = min(remaining, 2);
                 int incl = n_emit;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
                     int t = __shfl_up_sync(0xffffffffu, incl, o);
                     if (lane >= o) incl += t;
                 }
-                if (lane == 31) s_wsum[wid] = incl;
-                __syncthreads();
-                int woff = 0, total = 0;
-#pragma unroll
-                for (int i = 0; i < FDEMRI_TILE / 32; ++i) {
-                    int ci = s_wsum[i];
-                    if (i < wid) woff += ci;
-                    total += ci;
+                const int total = __shfl_sync(0xffffffffu, incl, 31);
+                if (total == 0) break;
+                if (fill + total > FDEMRI_CHUNK) {
+                    // publish the chunk and take the next stage
+                    __syncwarp();
+                    if (lane == 0) {
+                        ring->st[stage].hdr[0] = gt; ring->st[stage].hdr[1] = fill; ring->st[stage].hdr[2] = 0;
+                        fdemri_mbar_arrive(&ring->full[stage]);
+                    }
+                    if (++stage == FDEMRI_STAGES) { stage = 0; phase ^= 1u; }
+                    fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u);
+                    fill = 0;
                 }
-                if (total == 0) { __syncthreads(); break; }
-                int off = woff + incl - n_emit;
+                const int off = fill + incl - n_emit;
                 for (int i = 0; i < n_emit; ++i) {
                     const int e = e_next + i;
                     const int2 en = E[e];
@@ -405,39 +445,130 @@ __global__ void __launch_bounds__(FDEMRI_TILE, FDEMRI_MINBLOCKS) k_tile_sum(SumA
                     hi_e = min(min(hi_e, s_hi), tile_hi) - tile_lo;
                     const int seg = en.y & 0x3fffffff;
                     const int v = vs >> 1;
-                    s_list[off + i] = make_int4(lo_e | (hi_e << 16), rbase + v * d.n_seg + seg, wbase + v,
-                                                ((vs & 1) << 30) | (((en.y >> 30) & 1) << 31));
+                    fdemri_stage_item(ring->st[stage].items[off + i],
+                                      a.rec + (rbase + (size_t)v * d.n_seg + seg) * R_DOUBLES, a.wts[wbase + v], lo_e, hi_e,
+                                      (unsigned)(vs & 1), (unsigned)((en.y >> 30) & 1));
                 }
+                fill += total;
                 e_next += n_emit;
                 remaining -= n_emit;
-                __syncthreads();
-                // ---- evaluate ----
-                for (int j = 0; j < total; ++j) {
-                    const int4 it = s_list[j];
-                    const int lo = it.x & 0xffff, hi = it.x >> 16;
-                    if (tid < lo || tid > hi) continue;
-                    const unsigned fl = (unsigned)it.w;
-                    fdemri_term(a.rec + (size_t)(unsigned)it.y * R_DOUBLES, (fl & 0x40000000u) << 1, f, (int)(fl >> 31),
-                                a.wts[(unsigned)it.z], acc, cnt);
-                }
-                __syncthreads();
             }
         }
-        if (valid) {
-            const size_t o = ((size_t)b * d.n_freq + bin) * 2;
-            *reinterpret_cast<double2*>(a.hp + o) = make_double2(acc[0], acc[1]);
-            *reinterpret_cast<double2*>(a.hx + o) = make_double2(acc[2], acc[3]);
+        // last chunk of the tile (possibly empty)
+        __syncwarp();
+        if (lane == 0) {
+            ring->st[stage].hdr[0] = gt; ring->st[stage].hdr[1] = fill; ring->st[stage].hdr[2] = 1;
+            fdemri_mbar_arrive(&ring->full[stage]);
         }
+        if (++stage == FDEMRI_STAGES) { stage = 0; phase ^= 1u; }
+    }
+}
+
+__device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ring, int cw, int lane) {
+    const FdemriDims& d = a.d;
+    int stage = 0;
+    unsigned phase = 0;
+    int cur = -1;
+    int b = 0;
+    int64_t bin_a = 0;                            // first bin of this lane (second: + 32)
+    double f0 = 0.0, f1 = 0.0;
+    double a00 = 0.0, a01 = 0.0, a02 = 0.0, a03 = 0.0, a10 = 0.0, a11 = 0.0, a12 = 0.0, a13 = 0.0;
+    unsigned n_airy = 0, n_slow = 0, errs = 0;
+    const int wb = cw * 32 * FDEMRI_BPL;          // first tile-relative bin of this warp
+    const int rel0 = wb + lane, rel1 = rel0 + 32;
+    for (;;) {
+        fdemri_mbar_wait(&ring->full[stage], phase);
+        const FdemriStage* S = &ring->st[stage];
+        const int gt = S->hdr[0], cnt = S->hdr[1], last = S->hdr[2];
+        if (gt < 0) break;
+        if (gt != cur) {
+            cur = gt;
+            b = gt / d.n_tiles;
+            const int tile = gt - b * d.n_tiles;
+            bin_a = (int64_t)tile * FDEMRI_TILE + rel0;
+            f0 = (bin_a < d.n_freq) ? fdemri_freq(d, bin_a) : 0.0;
+            f1 = (bin_a + 32 < d.n_freq) ? fdemri_freq(d, bin_a + 32) : 0.0;
+            a00 = a01 = a02 = a03 = a10 = a11 = a12 = a13 = 0.0;
+        }
+        for (int j = 0; j < cnt; ++j) {
+            const double* it = S->items[j];
+            const int2 meta = *reinterpret_cast<const int2*>(it);        // {lo | hi << 16, flags}
+            const int lo = meta.x & 0xffff, hi = meta.x >> 16;
+            if (hi < wb || lo > wb + 32 * FDEMRI_BPL - 1) continue;      // warp-uniform
+            const unsigned flags = (unsigned)meta.y;
+            const unsigned sbit = (flags & 4u) << 29;
+            const bool act0 = rel0 >= lo && rel0 <= hi;
+            const bool act1 = rel1 >= lo && rel1 <= hi;
+            const double sf0 = fdemri_xorsign(f0, sbit), sf1 = fdemri_xorsign(f1, sbit);
+            double T0r = 0.0, T0i = 0.0, T1r = 0.0, T1i = 0.0;
+            bool ok0 = false, ok1 = false;
+            if (!(flags & 1u)) {
+                ok0 = fdemri_term_fast(it, sf0, T0r, T0i);
+                ok1 = fdemri_term_fast(it, sf1, T1r, T1i);
+            }
+            if (act0 && !ok0) {
+                const FdemriSlowOut o = fdemri_term_slow(it, sf0, flags);
+                T0r = o.tre; T0i = o.tim;
+                n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+            }
+            if (act1 && !ok1) {
+                const FdemriSlowOut o = fdemri_term_slow(it, sf1, flags);
+                T1r = o.tre; T1i = o.tim;
+                n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+            }
+            // weights (O2): s=+1: h+ += w+ T, hx += i wx T;  s=-1: h+ += w+ conj(T), hx += conj(i wx T)
+            const double wp = it[S_WP], swp = it[S_SWP], nwx = it[S_NWX], swx = it[S_SWX];
+            if (act0) {
+                a00 = fma(wp, T0r, a00); a01 = fma(swp, T0i, a01); a02 = fma(nwx, T0i, a02); a03 = fma(swx, T0r, a03);
+            }
+            if (act1) {
+                a10 = fma(wp, T1r, a10); a11 = fma(swp, T1i, a11); a12 = fma(nwx, T1i, a12); a13 = fma(swx, T1r, a13);
+            }
+        }
+        if (last) {
+            if (bin_a < d.n_freq) {
+                const size_t o = ((size_t)b * d.n_freq + bin_a) * 2;
+                *reinterpret_cast<double2*>(a.hp + o) = make_double2(a00, a01);
+                *reinterpret_cast<double2*>(a.hx + o) = make_double2(a02, a03);
+            }
+            if (bin_a + 32 < d.n_freq) {
+                const size_t o = ((size_t)b * d.n_freq + bin_a + 32) * 2;
+                *reinterpret_cast<double2*>(a.hp + o) = make_double2(a10, a11);
+                *reinterpret_cast<double2*>(a.hx + o) = make_double2(a12, a13);
+            }
+        }
+        // release the stage
+        __syncwarp();
+        if (lane == 0) fdemri_mbar_arrive(&ring->empty[stage]);
+        if (++stage == FDEMRI_STAGES) { stage = 0; phase ^= 1u; }
     }
     // counters: one atomic per warp
     for (int o = 16; o; o >>= 1) {
-        cnt[0] += __shfl_xor_sync(0xffffffffu, cnt[0], o);
-        cnt[1] += __shfl_xor_sync(0xffffffffu, cnt[1], o);
-        cnt[2] |= __shfl_xor_sync(0xffffffffu, cnt[2], o);
+        n_airy += __shfl_xor_sync(0xffffffffu, n_airy, o);
+        n_slow += __shfl_xor_sync(0xffffffffu, n_slow, o);
+        errs |= __shfl_xor_sync(0xffffffffu, errs, o);
     }
     if (lane == 0) {
-        if (cnt[0]) atomicAdd(a.stats + 4, (unsigned long long)cnt[0]);
-        if (cnt[1]) atomicAdd(a.stats + 7, (unsigned long long)cnt[1]);
-        if (cnt[2]) atomicOr(a.stats + 5, (unsigned long long)cnt[2]);
+        if (n_airy) atomicAdd(a.stats + 4, (unsigned long long)n_airy);
+        if (n_slow) atomicAdd(a.stats + 7, (unsigned long long)n_slow);
+        if (errs) atomicOr(a.stats + 5, (unsigned long long)errs);
     }
+}
+
+#ifndef FDEMRI_MINBLOCKS
+#define FDEMRI_MINBLOCKS 2
+#endif
+__global__ void __launch_bounds__(FDEMRI_SUM_THREADS, FDEMRI_MINBLOCKS) k_tile_sum(SumArgs a) {
+    extern __shared__ __align__(16) unsigned char fdemri_smem[];
+    FdemriRing* ring = reinterpret_cast<FdemriRing*>(fdemri_smem);
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (tid == 0) {
+        for (int i = 0; i < FDEMRI_STAGES; ++i) {
+            fdemri_mbar_init(&ring->full[i], 1u);
+            fdemri_mbar_init(&ring->empty[i], FDEMRI_CWARPS);
+        }
+    }
+    __syncthreads();
+    if (wid == FDEMRI_CWARPS) fdemri_producer(a, ring, lane);
+    else fdemri_consumer(a, ring, wid, lane);
 }
