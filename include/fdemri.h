@@ -49,7 +49,10 @@ enum {
     FDEMRI_BAD_TWO_EXTREMA = 1,   /* a segment cubic has two interior extrema (paper assumes <= 1, L105)   */
     FDEMRI_BAD_STRIP_OVERFLOW = 2,/* a voice has more monotone branches than the map holds                 */
     FDEMRI_BAD_NONFINITE = 4,     /* NaN/Inf met in the inputs or spline coefficients                      */
-    FDEMRI_BAD_NEWTON = 8         /* a root iteration hit its iteration cap                                */
+    FDEMRI_BAD_NEWTON = 8,        /* a root iteration hit its iteration cap                                */
+    FDEMRI_BAD_LIST_OVERFLOW = 16 /* not an error: the per-tile work list did not fit the work space (n_pairs
+                                     entries of 4 bytes needed) or a tile held too many items; fdemri_sum then
+                                     scans the map inside the kernel instead (same results, slower)           */
 };
 
 typedef struct fdemri_plan_s* fdemri_plan_t;
@@ -61,7 +64,9 @@ typedef struct {
     uint64_t n_turnover;     /* segments with an interior extremum of F (Fdot = 0, L92, L105)                 */
     uint64_t n_airy;         /* evaluations that took the small-|X| (Airy) path                              */
     uint64_t flags;          /* OR of FDEMRI_BAD_*                                                            */
-    uint64_t n_slow;         /* evaluations whose root needed the safeguarded (division) Newton fallback      */
+    uint64_t n_slow;         /* evaluations of monotone segments that left the fast path (small |X| or a
+                                rejected iteration) and took the safeguarded Newton with a division           */
+    uint64_t n_pairs;        /* (item, tile) pairs of the work list built by the last fdemri_build_splines    */
 } fdemri_stats;
 
 /* Create a plan.
@@ -80,8 +85,10 @@ int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, int n_
                 uint32_t flags);
 
 /* Device work space the plan needs (bytes); the caller allocates it (256-byte aligned) and hands it over.
- * The work space holds the spline records and the segment->bin map; it must stay valid and untouched
- * between build_splines and the last sum. */
+ * The work space holds the spline records, the segment->bin map and the per-tile work list; it must stay valid
+ * and untouched between build_splines and the last sum.  The size returned includes a default capacity for the
+ * work list (4 bytes per (item, tile) pair); whatever the caller gives beyond the fixed part is used for it, and
+ * fdemri_stats.n_pairs reports what the last build needed (see FDEMRI_BAD_LIST_OVERFLOW). */
 size_t fdemri_workspace_bytes(fdemri_plan_t plan);
 int fdemri_set_workspace(fdemri_plan_t plan, void* dev_ptr, size_t bytes);
 

@@ -10,7 +10,7 @@ CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libfdemri.so")
 SOURCES = ["fdemri.cu"]
 DEPS = ["fdemri.cu", "fdemri_common.cuh", "fdemri_map.cuh", "fdemri_splines.cuh", "fdemri_strips.cuh",
-        "fdemri_sum.cuh", "airy_tables.inc", "poly_tables.inc", os.path.join("..", "..", "include", "fdemri.h")]
+        "fdemri_sum.cuh", "fdemri_pairs.cuh", "airy_tables.inc", "poly_tables.inc", os.path.join("..", "..", "include", "fdemri.h")]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "--fmad=true"]

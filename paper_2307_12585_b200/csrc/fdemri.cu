@@ -6,6 +6,8 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -14,6 +16,7 @@
 #include "fdemri_map.cuh"
 #include "fdemri_splines.cuh"
 #include "fdemri_strips.cuh"
+#include "fdemri_pairs.cuh"
 #include "fdemri_sum.cuh"
 
 struct fdemri_plan_s {
@@ -26,7 +29,12 @@ struct fdemri_plan_s {
     int* lmn_dev;
     SplineFac* fac;
     double *sh_hi, *sh_lo, *rec;
-    int2* ent;
+    int4* ent;
+    int* n_ent;
+    int* tile_cnt;                 // [B * n_tiles] pairs per tile, then [B * n_tiles] fill cursors
+    unsigned int* tile_off;        // [B * n_tiles + 1]
+    unsigned int* pairs;           // [pair_cap]
+    unsigned long long pair_cap;
     StripRaw* strips;
     int* n_strips;
     int4* dense;
@@ -35,7 +43,7 @@ struct fdemri_plan_s {
     int dense_cap;
     double4* wts;
     double* angles;
-    unsigned long long* stats;     // [0..5] = fdemri_stats, [6] = tile counter (low 32 bits)
+    unsigned long long* stats;     // [0..5], [7], [8] = fdemri_stats, [6] = tile counter (low 32 bits); 16 slots
     std::vector<double> angle_stage;
     bool built;
     cudaStream_t last_stream;
@@ -63,7 +71,11 @@ static size_t carve(fdemri_plan_s* p, char* base) {
     p->sh_hi = (double*)take(B * 4 * S * 4 * sizeof(double));
     p->sh_lo = (double*)take(B * 4 * S * 4 * sizeof(double));
     p->rec = (double*)take(B * V * S * R_DOUBLES * sizeof(double));
-    p->ent = (int2*)take(B * V * 2 * (size_t)d.ent_max * sizeof(int2));
+    p->ent = (int4*)take(B * V * 2 * (size_t)d.ent_max * sizeof(int4));
+    p->n_ent = (int*)take(B * V * 2 * sizeof(int));
+    const size_t NT = B * (size_t)d.n_tiles;
+    p->tile_cnt = (int*)take(2 * NT * sizeof(int));
+    p->tile_off = (unsigned int*)take((NT + 1) * sizeof(unsigned int));
     p->strips = (StripRaw*)take(B * V * 2 * FDEMRI_MAX_STRIPS * sizeof(StripRaw));
     p->n_strips = (int*)take(B * V * 2 * sizeof(int));
     p->dense_cap = (int)(2 * V * FDEMRI_MAX_STRIPS);
@@ -72,7 +84,9 @@ static size_t carve(fdemri_plan_s* p, char* base) {
     p->bin_range = (int2*)take(B * sizeof(int2));
     p->wts = (double4*)take(B * V * sizeof(double4));
     p->angles = (double*)take(B * 2 * sizeof(double));
-    p->stats = (unsigned long long*)take(8 * sizeof(unsigned long long));
+    p->stats = (unsigned long long*)take(16 * sizeof(unsigned long long));
+    // the pair list takes what is left of the work space (default: see fdemri_workspace_bytes)
+    p->pairs = (unsigned int*)take(0);
     return off;
 }
 
@@ -135,20 +149,26 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
 extern "C" size_t fdemri_workspace_bytes(fdemri_plan_t p) {
     if (!p) return 0;
     fdemri_plan_s tmp = *p;
-    return carve(&tmp, nullptr);
+    // default capacity of the pair list: every entry once plus an eighth of the band per (voice, sign)
+    const size_t pairs = (size_t)p->d.n_batch * p->d.n_modes * 2 * ((size_t)p->d.n_seg + (size_t)p->d.n_tiles / 8 + 1);
+    return carve(&tmp, nullptr) + align_up(pairs * sizeof(unsigned int));
 }
 
 extern "C" int fdemri_set_workspace(fdemri_plan_t p, void* dev_ptr, size_t bytes) {
     if (!p || !dev_ptr) return FDEMRI_ERR_INVALID_ARG;
     if (((uintptr_t)dev_ptr & 255) != 0) return FDEMRI_ERR_INVALID_ARG;
-    if (bytes < fdemri_workspace_bytes(p)) return FDEMRI_ERR_WORKSPACE;
+    fdemri_plan_s tmp = *p;
+    const size_t fixed = carve(&tmp, nullptr);
+    if (bytes < fixed + 256) return FDEMRI_ERR_WORKSPACE;
     p->ws = dev_ptr;
     p->ws_bytes = bytes;
     carve(p, (char*)dev_ptr);
+    p->pair_cap = (bytes - fixed) / sizeof(unsigned int);
+    if (p->pair_cap > 0xffffffffull) p->pair_cap = 0xffffffffull;
     p->built = false;
     if (cudaMemcpy(p->lmn_dev, p->lmn.data(), p->lmn.size() * sizeof(int32_t), cudaMemcpyHostToDevice) != cudaSuccess)
         return FDEMRI_ERR_CUDA;
-    if (cudaMemset(p->stats, 0, 8 * sizeof(unsigned long long)) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    if (cudaMemset(p->stats, 0, 16 * sizeof(unsigned long long)) != cudaSuccess) return FDEMRI_ERR_CUDA;
     return FDEMRI_OK;
 }
 
@@ -171,7 +191,7 @@ extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const 
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const FdemriDims& d = p->d;
     p->last_stream = st;
-    if (cudaMemsetAsync(p->stats, 0, 8 * sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    if (cudaMemsetAsync(p->stats, 0, 16 * sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
     k_spline_factor<<<(d.n_batch + 63) / 64, 64, 0, st>>>(d.n_batch, d.n_knots, p->t_knots_dev, p->fac, p->stats + 5);
     if (d.n_knots <= 128) launch_splines<128>(p, f_phi, f_r, Phi_phi, Phi_r, amp, st);
     else if (d.n_knots <= 256) launch_splines<256>(p, f_phi, f_r, Phi_phi, Phi_r, amp, st);
@@ -180,10 +200,24 @@ extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const 
     k_records<<<(unsigned)((nrec + 127) / 128), 128, 0, st>>>(d, p->lmn_dev, p->t_knots_dev, p->sh_hi, p->sh_lo, p->rec,
                                                               p->stats);
     size_t nvs = (size_t)d.n_batch * d.n_modes * 2;
-    k_strips<<<(unsigned)((nvs + 63) / 64), 64, 0, st>>>(d, p->lmn_dev, f_phi, f_r, p->rec, p->ent, p->strips,
-                                                         p->n_strips, p->stats);
+    k_strips<<<(unsigned)((nvs + 63) / 64), 64, 0, st>>>(d, p->lmn_dev, f_phi, f_r, p->rec, p->ent, p->n_ent,
+                                                         p->strips, p->n_strips, p->stats);
     k_strip_compact<<<d.n_batch, 1024, 0, st>>>(d.n_modes, p->dense_cap, p->strips, p->n_strips, p->dense, p->n_dense,
                                                 p->bin_range);
+    // S2c: per-tile pair lists (count, prefix sum, fill, sort)
+    {
+        const size_t NT = (size_t)d.n_batch * d.n_tiles;
+        if (cudaMemsetAsync(p->tile_cnt, 0, 2 * NT * sizeof(int), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
+        const size_t nslots = nvs * (size_t)d.ent_max;
+        const unsigned nb = (unsigned)((nslots + 255) / 256);
+        k_pair_pass<0><<<nb, 256, 0, st>>>(d, p->ent, p->n_ent, p->tile_cnt, p->tile_off, p->tile_cnt + NT, p->pairs,
+                                          p->pair_cap, p->stats);
+        k_pair_scan<<<1, 1024, 0, st>>>(NT, p->tile_cnt, p->tile_off, p->pair_cap, p->stats);
+        k_pair_pass<1><<<nb, 256, 0, st>>>(d, p->ent, p->n_ent, p->tile_cnt, p->tile_off, p->tile_cnt + NT, p->pairs,
+                                          p->pair_cap, p->stats);
+        k_pair_sort<<<(unsigned)NT, 256, FDEMRI_SORT_MAX * sizeof(unsigned int), st>>>(NT, p->tile_off, p->pairs,
+                                                                                     p->pair_cap, p->stats);
+    }
     if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
     p->built = true;
     return FDEMRI_OK;
@@ -217,6 +251,8 @@ extern "C" int fdemri_sum(fdemri_plan_t p, int n_angles, const double* theta_hos
     a.d = d;
     a.rec = p->rec;
     a.ent = p->ent;
+    a.tile_off = p->tile_off;
+    a.pairs = p->pairs;
     a.dense = p->dense;
     a.n_dense = p->n_dense;
     a.bin_range = p->bin_range;
@@ -237,20 +273,28 @@ extern "C" int fdemri_sum(fdemri_plan_t p, int n_angles, const double* theta_hos
             per_sm < 1)
             per_sm = 1;
         p->sum_blocks_per_sm = per_sm;
+        if (getenv("FDEMRI_DEBUG"))
+            fprintf(stderr, "[fdemri] k_tile_sum: %d threads, %zu B smem, %d CTAs/SM\n", FDEMRI_SUM_THREADS, smem, per_sm);
     }
     long long grid = (long long)p->sm_count * p->sum_blocks_per_sm;
     if (grid > a.total_tiles) grid = a.total_tiles;
     if (p->ev0) cudaEventRecord(p->ev0, st);
     k_tile_sum<<<(unsigned)grid, FDEMRI_SUM_THREADS, smem, st>>>(a);
     if (p->ev1) { cudaEventRecord(p->ev1, st); p->ev_valid = true; }
-    if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
+    {
+        const cudaError_t err = cudaGetLastError();
+        if (err != cudaSuccess) {
+            if (getenv("FDEMRI_DEBUG")) fprintf(stderr, "[fdemri] fdemri_sum: %s\n", cudaGetErrorString(err));
+            return FDEMRI_ERR_CUDA;
+        }
+    }
     return FDEMRI_OK;
 }
 
 extern "C" int fdemri_get_stats(fdemri_plan_t p, fdemri_stats* out) {
     if (!p || !out) return FDEMRI_ERR_INVALID_ARG;
     if (!p->ws) return FDEMRI_ERR_WORKSPACE;
-    unsigned long long h[8];
+    unsigned long long h[16];
     if (cudaStreamSynchronize(p->last_stream) != cudaSuccess) return FDEMRI_ERR_CUDA;
     if (cudaMemcpy(h, p->stats, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess) return FDEMRI_ERR_CUDA;
     out->n_items = h[0];
@@ -260,6 +304,7 @@ extern "C" int fdemri_get_stats(fdemri_plan_t p, fdemri_stats* out) {
     out->n_airy = h[4];
     out->flags = h[5];
     out->n_slow = h[7];
+    out->n_pairs = h[8];
     if (h[5] & (FDEMRI_BAD_TWO_EXTREMA | FDEMRI_BAD_STRIP_OVERFLOW)) return FDEMRI_ERR_UNSUPPORTED;
     if (h[5] & FDEMRI_BAD_NONFINITE) return FDEMRI_ERR_INVALID_ARG;
     return FDEMRI_OK;

@@ -7,12 +7,15 @@
 #define FDEMRI_MAX_KNOTS 512
 #define FDEMRI_MAX_STRIPS 8          // monotone branches kept per (voice, sign)
 #define FDEMRI_ENT_EXTRA 8           // entries per (voice, sign) = (n_knots-1) + FDEMRI_ENT_EXTRA
-#define FDEMRI_CWARPS 8              // consumer (evaluating) warps per CTA of the sum kernel
+#ifndef FDEMRI_CWARPS
+#define FDEMRI_CWARPS 12             // consumer (evaluating) warps per CTA of the sum kernel
+#endif
 #define FDEMRI_BPL 2                 // bins per lane: a consumer warp owns 32*FDEMRI_BPL consecutive bins
 #define FDEMRI_TILE (FDEMRI_CWARPS * 32 * FDEMRI_BPL)     // bins per tile (512)
 #define FDEMRI_SUM_THREADS ((FDEMRI_CWARPS + 1) * 32)     // + one producer warp
-#define FDEMRI_CHUNK 64              // staged items per ring stage
-#define FDEMRI_STAGES 4              // ring depth
+#define FDEMRI_CHUNK 32              // staged items per ring stage (one per producer lane)
+#define FDEMRI_STAGES 8              // ring depth
+#define FDEMRI_BAD_LIST_OVERFLOW_BIT 16ull   // = FDEMRI_BAD_LIST_OVERFLOW of fdemri.h
 
 // ------------------------------------------------------------------------------------------------
 // Record of one (voice, segment) in global memory: everything the sum needs about that piece of

@@ -1,0 +1,128 @@
+// fdemri_pairs.cuh -- S2c: the balanced work list.  For every tile of FDEMRI_TILE bins, the list of entries
+// (voice, sign, segment-branch) whose bin interval intersects it, in the fixed order (voice, sign, time).
+//
+// "the spline segment in which each value of f falls is predetermined before the summation";
+// here the predetermined map is per tile: count -> prefix sum -> fill -> sort.  The fill uses atomic cursors, so
+// the order inside a tile is arbitrary until k_pair_sort puts the keys (unique, = entry index) in ascending
+// order: the sum kernel then walks every tile in a data-determined order (bitwise reproducible results).
+//   key = (voice*2 + sign) * ent_max + e                (32 bits; the batch item is implied by the tile)
+// If the pair list does not fit the work space, or a tile holds more keys than the sorter takes, the flag
+// FDEMRI_BAD_LIST_OVERFLOW is raised and fdemri_sum falls back to scanning the strips inside the kernel.
+#pragma once
+#include "fdemri_common.cuh"
+
+#define FDEMRI_SORT_MAX 8192         // keys per tile the shared-memory sorter takes
+
+// One thread per (batch item, voice, sign, entry slot).  mode 0: count per tile;  mode 1: fill.
+template <int MODE>
+__global__ void k_pair_pass(FdemriDims d, const int4* __restrict__ ent, const int* __restrict__ n_ent,
+                            int* __restrict__ tile_cnt, const unsigned int* __restrict__ tile_off,
+                            int* __restrict__ tile_cur, unsigned int* __restrict__ pairs, unsigned long long cap,
+                            unsigned long long* __restrict__ stats) {
+    const size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t total = (size_t)d.n_batch * d.n_modes * 2 * d.ent_max;
+    if (id >= total) return;
+    const int e = (int)(id % d.ent_max);
+    const size_t bvs = id / d.ent_max;                 // (batch item, voice, sign)
+    if (e >= n_ent[bvs]) return;
+    const int4 en = ent[id];
+    const int b = (int)(bvs / ((size_t)2 * d.n_modes));
+    const unsigned key = (unsigned)((bvs - (size_t)b * 2 * d.n_modes) * d.ent_max + e);
+    const int t0 = en.x / FDEMRI_TILE, t1 = en.y / FDEMRI_TILE;
+    for (int t = t0; t <= t1; ++t) {
+        const size_t gt = (size_t)b * d.n_tiles + t;
+        if (MODE == 0) {
+            atomicAdd(tile_cnt + gt, 1);
+        } else {
+            const unsigned long long pos = (unsigned long long)tile_off[gt] + (unsigned)atomicAdd(tile_cur + gt, 1);
+            if (pos < cap) pairs[pos] = key;
+        }
+    }
+}
+
+// Exclusive prefix sum of cnt[0..n) into off[0..n], off[n] = total.  One CTA (n is a few thousand per waveform).
+// Raises FDEMRI_BAD_LIST_OVERFLOW when the total exceeds the capacity of the pair list.
+__global__ void __launch_bounds__(1024) k_pair_scan(size_t n, const int* __restrict__ cnt, unsigned int* __restrict__ off,
+                                                    unsigned long long cap, unsigned long long* __restrict__ stats) {
+    __shared__ unsigned int s_w[32];
+    __shared__ unsigned long long s_base;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (tid == 0) s_base = 0ull;
+    __syncthreads();
+    for (size_t start = 0; start < n; start += 4096) {
+        // four consecutive elements per thread
+        const size_t i0 = start + (size_t)tid * 4;
+        unsigned int v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) v[k] = (i0 + k < n) ? (unsigned)cnt[i0 + k] : 0u;
+        const unsigned int mine = v[0] + v[1] + v[2] + v[3];
+        unsigned int incl = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            unsigned int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        if (lane == 31) s_w[wid] = incl;
+        __syncthreads();
+        if (wid == 0) {
+            unsigned int w = s_w[lane], wi = w;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                unsigned int t = __shfl_up_sync(0xffffffffu, wi, o);
+                if (lane >= o) wi += t;
+            }
+            s_w[lane] = wi - w;                       // exclusive over warps
+        }
+        __syncthreads();
+        const unsigned long long base = s_base;
+        unsigned long long run = base + s_w[wid] + (incl - mine);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (i0 + k < n) off[i0 + k] = (unsigned int)(run > 0xffffffffull ? 0xffffffffull : run);
+            run += v[k];
+        }
+        __syncthreads();
+        if (tid == 1023) s_base = run;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        const unsigned long long tot = s_base;
+        off[n] = (unsigned int)(tot > 0xffffffffull ? 0xffffffffull : tot);
+        stats[8] = tot;                                // n_pairs
+        if (tot > cap || tot > 0xffffffffull) atomicOr(stats + 5, (unsigned long long)FDEMRI_BAD_LIST_OVERFLOW_BIT);
+    }
+}
+
+// One CTA per tile: ascending bitonic sort of the tile's keys in shared memory.
+__global__ void __launch_bounds__(256) k_pair_sort(size_t n_tiles_total, const unsigned int* __restrict__ tile_off,
+                                                   unsigned int* __restrict__ pairs, unsigned long long cap,
+                                                   unsigned long long* __restrict__ stats) {
+    extern __shared__ unsigned int s_key[];
+    const size_t gt = blockIdx.x;
+    if (gt >= n_tiles_total) return;
+    const unsigned int o0 = tile_off[gt], o1 = tile_off[gt + 1];
+    const unsigned int n = o1 - o0;
+    if (n < 2u || (unsigned long long)o1 > cap) return;
+    if (n > FDEMRI_SORT_MAX) {
+        if (threadIdx.x == 0) atomicOr(stats + 5, (unsigned long long)FDEMRI_BAD_LIST_OVERFLOW_BIT);
+        return;
+    }
+    unsigned int np = 2;
+    while (np < n) np <<= 1;
+    for (unsigned int i = threadIdx.x; i < np; i += blockDim.x) s_key[i] = (i < n) ? pairs[o0 + i] : 0xffffffffu;
+    __syncthreads();
+    for (unsigned int k = 2; k <= np; k <<= 1) {
+        for (unsigned int j = k >> 1; j > 0; j >>= 1) {
+            for (unsigned int i = threadIdx.x; i < (np >> 1); i += blockDim.x) {
+                // i-th compare-exchange of this stage: partner indices a < b = a + j
+                const unsigned int a = ((i & ~(j - 1)) << 1) | (i & (j - 1));
+                const unsigned int bb = a + j;
+                const bool up = (a & k) == 0;
+                const unsigned int x = s_key[a], y = s_key[bb];
+                if ((x > y) == up) { s_key[a] = y; s_key[bb] = x; }
+            }
+            __syncthreads();
+        }
+    }
+    for (unsigned int i = threadIdx.x; i < n; i += blockDim.x) pairs[o0 + i] = s_key[i];
+}

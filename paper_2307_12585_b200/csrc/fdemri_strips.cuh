@@ -45,10 +45,11 @@ struct StripRaw {   // per (item, voice, sign), FDEMRI_MAX_STRIPS of them
     int n_dir;      // (number of entries << 1) | (1 if bins increase with time)
 };
 
-// One thread per (batch item, voice, sign).  ent: [B][V][2][ent_max] int2 {first bin of the branch, seg | branchB<<30}
+// One thread per (batch item, voice, sign).  ent: [B][V][2][ent_max] int4 {first bin, last bin, seg | branchB<<30, 0}
+// of every non-empty (segment, branch), in time order;  n_ent: [B][V][2] their number
 __global__ void k_strips(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ f_phi,
-                         const double* __restrict__ f_r, const double* __restrict__ rec, int2* __restrict__ ent,
-                         StripRaw* __restrict__ strips, int* __restrict__ n_strips,
+                         const double* __restrict__ f_r, const double* __restrict__ rec, int4* __restrict__ ent,
+                         int* __restrict__ n_ent, StripRaw* __restrict__ strips, int* __restrict__ n_strips,
                          unsigned long long* __restrict__ stats) {
     size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     size_t total = (size_t)d.n_batch * d.n_modes * 2;
@@ -60,7 +61,7 @@ __global__ void k_strips(FdemriDims d, const int* __restrict__ lmn, const double
     int m = lmn[3 * v + 1], n = lmn[3 * v + 2];
     const double s = sg ? -1.0 : 1.0;
     const double* R = rec + bv * (size_t)d.n_seg * R_DOUBLES;
-    int2* E = ent + id * (size_t)d.ent_max;
+    int4* E = ent + id * (size_t)d.ent_max;
     StripRaw* ST = strips + id * FDEMRI_MAX_STRIPS;
     const int64_t first_pos = fdemri_first_gt(d, 0.0);      // bins with f > 0 only (R13)
     int ne = 0, ns = 0;
@@ -104,7 +105,7 @@ __global__ void k_strips(FdemriDims d, const int* __restrict__ lmn, const double
                 if (dir) cur_hi = hi1 - 1; else cur_lo = lo;
             }
             if (ne < d.ent_max) {
-                E[ne++] = make_int2((int)lo, k | (br << 30));
+                E[ne++] = make_int4((int)lo, (int)(hi1 - 1), k | (br << 30), 0);
                 ++cur_n;
                 evals += (unsigned long long)(hi1 - lo);
             } else {
@@ -117,6 +118,7 @@ __global__ void k_strips(FdemriDims d, const int* __restrict__ lmn, const double
         else flags |= 2ull;
     }
     n_strips[id] = ns;
+    n_ent[id] = ne;
     if (ne) atomicAdd(stats + 0, (unsigned long long)ne);
     if (ns) atomicAdd(stats + 1, (unsigned long long)ns);
     if (evals) atomicAdd(stats + 2, evals);

@@ -29,7 +29,9 @@
 struct SumArgs {
     FdemriDims d;
     const double* rec;        // [B][V][S][R_DOUBLES]
-    const int2* ent;          // [B][V][2][ent_max]
+    const int4* ent;          // [B][V][2][ent_max] {first bin, last bin, seg | branchB << 30, 0}
+    const unsigned int* tile_off;   // [B * n_tiles + 1] first pair of every tile
+    const unsigned int* pairs;      // sorted keys (voice*2+sign)*ent_max + e of every tile
     const int4* dense;        // [B][dense_cap]
     const int* n_dense;       // [B]
     const int2* bin_range;    // [B] {first, last} bin covered by any strip
@@ -53,6 +55,9 @@ __constant__ double c_gim[6] = {-0.06944444444444445, 0.03799305912780064, -0.11
 __device__ __forceinline__ double fdemri_xorsign(double x, unsigned mask) {
     return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));
 }
+
+// high word of |x|: monotone in |x| for finite x, and larger than any finite threshold for NaN/Inf
+__device__ __forceinline__ int fdemri_hiabs(double x) { return __double2hiint(x) & 0x7fffffff; }
 
 // sin, cos of q quarter turns (|q| up to ~1e4; absolute error ~1e-14 + (pi/2) ulp(q))
 __device__ __forceinline__ void fdemri_sincos_quarter(double q, double& sn, double& cs) {
@@ -114,16 +119,19 @@ __device__ __forceinline__ void fdemri_mbar_init(uint64_t* bar, unsigned count) 
 __device__ __forceinline__ void fdemri_mbar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(fdemri_smem_addr(bar)) : "memory");
 }
-__device__ __forceinline__ void fdemri_mbar_wait(uint64_t* bar, unsigned parity) {
-    const unsigned addr = fdemri_smem_addr(bar);
+__device__ __forceinline__ bool fdemri_mbar_try(unsigned addr, unsigned parity) {
     unsigned done;
-    do {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(done)
-            : "r"(addr), "r"(parity)
-            : "memory");
-    } while (!done);
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(addr), "r"(parity)
+        : "memory");
+    return done != 0u;
+}
+// spin with a back-off of `ns` nanoseconds between polls (a polling warp takes issue slots from its SM sub-partition)
+__device__ __forceinline__ void fdemri_mbar_wait(uint64_t* bar, unsigned parity, unsigned ns) {
+    const unsigned addr = fdemri_smem_addr(bar);
+    while (!fdemri_mbar_try(addr, parity)) __nanosleep(ns);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -158,11 +166,11 @@ __device__ __forceinline__ bool fdemri_term_fast(const double* __restrict__ it, 
     y = fma(y, tq, y);                                 // |F'(tau)|^(-1/2) to first order in delta
     // accept: the neglected second-order terms are below rounding (|F'' delta / F'| <= 1e-6 and |delta| <= 3e-8 h)
     // and the iterate sits in the segment (the root does, by membership R6)
-    bool ok = (fabs(tq) <= 5e-7) && (fabs(delta) <= it[S_TOLH]) && (fabs(tau - it[S_HH]) <= it[S_HH1]);
-    // 1/X = 3 F''^2 / (2 pi F'^3)
+    // (compared on the high words: |v| <= T  <=>  hi(|v|) <= hi(T) up to 2^-20 relative; NaN fails)
     const double pq = Fh * r;
-    const double u = (pq * pq) * (r * it[S_CU]);
-    ok = ok && (fabs(u) <= 2.5e-3);
+    const double u = (pq * pq) * (r * it[S_CU]);       // 1/X = 3 F''^2 / (2 pi F'^3)
+    const bool ok = (fdemri_hiabs(tq) <= 0x3ea0c6f7) & (fdemri_hiabs(delta) <= __double2hiint(it[S_TOLH])) &
+                    (fdemri_hiabs(tau - it[S_HH]) <= __double2hiint(it[S_HH1])) & (fdemri_hiabs(u) <= 0x3f647ae1);
     const double u2 = u * u;
     const double dq = u * fma(u2, FDEMRI_G_DQ3, FDEMRI_G_DQ1);
     const double yr = y * fma(u2, fma(u2, FDEMRI_G_R4, FDEMRI_G_R2), 1.0);
@@ -348,7 +356,8 @@ __device__ __forceinline__ void fdemri_stage_item(double* dst, const double* __r
     d2[15] = make_double2(-w.y, s * w.y);
 }
 
-__device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ring, int lane) {
+// Fallback producer (the pair lists did not fit the work space): scans the strips of the batch item.
+__device__ __noinline__ void fdemri_producer_scan(const SumArgs& a, FdemriRing* ring, int lane) {
     const FdemriDims& d = a.d;
     const int V = d.n_modes;
     int stage = 0;
@@ -359,7 +368,7 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
         gt = __shfl_sync(0xffffffffu, gt, 0);
         const bool done = gt >= a.total_tiles;
         // a fresh stage for this tile
-        fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u);
+        fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, 256u);
         if (done) {
             if (lane == 0) {
                 ring->st[stage].hdr[0] = -1; ring->st[stage].hdr[1] = 0; ring->st[stage].hdr[2] = 1;
@@ -381,7 +390,7 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
             // ---- candidate strip of this lane ----
             const int c = base + lane;
             int remaining = 0, e_next = 0, ne = 0, dir = 0, vs = 0, s_lo = 0, s_hi = 0;
-            const int2* E = nullptr;
+            const int4* E = nullptr;
             if (c < nd) {
                 const int4 s = dense_b[c];
                 if (s.x <= tile_hi && s.y >= tile_lo) {
@@ -412,9 +421,9 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
                     remaining = eb - ea + 1;
                 }
             }
-            // ---- rounds: every candidate emits up to 2 items per round, in candidate order ----
+            // ---- rounds: every candidate emits one item per round, in candidate order ----
             for (;;) {
-                const int n_emit = min(remaining, 2);
+                const int n_emit = min(remaining, 1);
                 int incl = n_emit;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
@@ -431,23 +440,20 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
                         fdemri_mbar_arrive(&ring->full[stage]);
                     }
                     if (++stage == FDEMRI_STAGES) { stage = 0; phase ^= 1u; }
-                    fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u);
+                    fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, 256u);
                     fill = 0;
                 }
                 const int off = fill + incl - n_emit;
                 for (int i = 0; i < n_emit; ++i) {
                     const int e = e_next + i;
-                    const int2 en = E[e];
-                    int lo_e = en.x, hi_e;
-                    if (dir) hi_e = (e + 1 < ne) ? E[e + 1].x - 1 : s_hi;
-                    else hi_e = (e > 0) ? E[e - 1].x - 1 : s_hi;
-                    lo_e = max(max(lo_e, s_lo), tile_lo) - tile_lo;
-                    hi_e = min(min(hi_e, s_hi), tile_hi) - tile_lo;
-                    const int seg = en.y & 0x3fffffff;
+                    const int4 en = E[e];
+                    const int lo_e = max(max(en.x, s_lo), tile_lo) - tile_lo;
+                    const int hi_e = min(min(en.y, s_hi), tile_hi) - tile_lo;
+                    const int seg = en.z & 0x3fffffff;
                     const int v = vs >> 1;
                     fdemri_stage_item(ring->st[stage].items[off + i],
                                       a.rec + (rbase + (size_t)v * d.n_seg + seg) * R_DOUBLES, a.wts[wbase + v], lo_e, hi_e,
-                                      (unsigned)(vs & 1), (unsigned)((en.y >> 30) & 1));
+                                      (unsigned)(vs & 1), (unsigned)((en.z >> 30) & 1));
                 }
                 fill += total;
                 e_next += n_emit;
@@ -464,6 +470,59 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
     }
 }
 
+// Producer: walks the sorted pair list of every tile it draws (S2c, fdemri_pairs.cuh), one ring stage per
+// 32 keys: key -> entry (bin interval, segment, branch) -> record + weights -> staged item.
+__device__ __forceinline__ void fdemri_producer_lists(const SumArgs& a, FdemriRing* ring, int lane) {
+    const FdemriDims& d = a.d;
+    const int V = d.n_modes;
+    int stage = 0;
+    unsigned phase = 0;
+    for (;;) {
+        int gt = 0;
+        if (lane == 0) gt = (int)atomicAdd(a.tile_counter, 1u);
+        gt = __shfl_sync(0xffffffffu, gt, 0);
+        if (gt >= a.total_tiles) break;
+        const int b = gt / d.n_tiles, tile = gt - b * d.n_tiles;
+        const int64_t bin0 = (int64_t)tile * FDEMRI_TILE;
+        const int tile_lo = (int)bin0;
+        const int tile_hi = (int)min(bin0 + FDEMRI_TILE - 1, d.n_freq - 1);
+        const unsigned int off = a.tile_off[gt];
+        const int n = (int)(a.tile_off[gt + 1] - off);
+        const int wbase = (a.n_angles > 1 ? b : 0) * V;
+        const size_t rbase = (size_t)b * V * d.n_seg;
+        const int4* ent_b = a.ent + (size_t)b * 2 * V * d.ent_max;
+        int base = 0;
+        do {
+            const int cnt = min(n - base, FDEMRI_CHUNK);
+            fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, 256u);
+            if (lane < cnt) {
+                const unsigned int key = a.pairs[off + base + lane];
+                const int4 en = ent_b[key];                              // key = (voice*2+sign)*ent_max + e
+                const int vs = (int)(key / (unsigned)d.ent_max);
+                const int lo_e = max(en.x, tile_lo) - tile_lo;
+                const int hi_e = min(en.y, tile_hi) - tile_lo;
+                const int seg = en.z & 0x3fffffff;
+                const int v = vs >> 1;
+                fdemri_stage_item(ring->st[stage].items[lane], a.rec + (rbase + (size_t)v * d.n_seg + seg) * R_DOUBLES,
+                                  a.wts[wbase + v], lo_e, hi_e, (unsigned)(vs & 1), (unsigned)((en.z >> 30) & 1));
+            }
+            base += FDEMRI_CHUNK;
+            __syncwarp();
+            if (lane == 0) {
+                ring->st[stage].hdr[0] = gt; ring->st[stage].hdr[1] = cnt; ring->st[stage].hdr[2] = (base >= n);
+                fdemri_mbar_arrive(&ring->full[stage]);
+            }
+            if (++stage == FDEMRI_STAGES) { stage = 0; phase ^= 1u; }
+        } while (base < n);
+    }
+    // no more work
+    fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, 256u);
+    if (lane == 0) {
+        ring->st[stage].hdr[0] = -1; ring->st[stage].hdr[1] = 0; ring->st[stage].hdr[2] = 1;
+        fdemri_mbar_arrive(&ring->full[stage]);
+    }
+}
+
 __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ring, int cw, int lane) {
     const FdemriDims& d = a.d;
     int stage = 0;
@@ -477,7 +536,7 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
     const int wb = cw * 32 * FDEMRI_BPL;          // first tile-relative bin of this warp
     const int rel0 = wb + lane, rel1 = rel0 + 32;
     for (;;) {
-        fdemri_mbar_wait(&ring->full[stage], phase);
+        fdemri_mbar_wait(&ring->full[stage], phase, 64u);
         const FdemriStage* S = &ring->st[stage];
         const int gt = S->hdr[0], cnt = S->hdr[1], last = S->hdr[2];
         if (gt < 0) break;
@@ -555,10 +614,11 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
     }
 }
 
-#ifndef FDEMRI_MINBLOCKS
-#define FDEMRI_MINBLOCKS 2
+// Registers: the two interleaved evaluations of a consumer lane need ~128 registers without spilling
+#ifndef FDEMRI_MAXNREG
+#define FDEMRI_MAXNREG 128
 #endif
-__global__ void __launch_bounds__(FDEMRI_SUM_THREADS, FDEMRI_MINBLOCKS) k_tile_sum(SumArgs a) {
+__global__ void __maxnreg__(FDEMRI_MAXNREG) k_tile_sum(SumArgs a) {
     extern __shared__ __align__(16) unsigned char fdemri_smem[];
     FdemriRing* ring = reinterpret_cast<FdemriRing*>(fdemri_smem);
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -569,6 +629,10 @@ __global__ void __launch_bounds__(FDEMRI_SUM_THREADS, FDEMRI_MINBLOCKS) k_tile_s
         }
     }
     __syncthreads();
-    if (wid == FDEMRI_CWARPS) fdemri_producer(a, ring, lane);
+    if (wid == FDEMRI_CWARPS) {
+        const bool lists = !(*(volatile const unsigned long long*)(a.stats + 5) & FDEMRI_BAD_LIST_OVERFLOW_BIT);
+        if (lists) fdemri_producer_lists(a, ring, lane);
+        else fdemri_producer_scan(a, ring, lane);
+    }
     else fdemri_consumer(a, ring, wid, lane);
 }
