@@ -31,7 +31,7 @@ extern "C" {
 enum {
     FDEMRI_OK = 0,
     FDEMRI_ERR_INVALID_ARG = 1, /* bad size, NULL pointer, l<2, m<0, m>l, unsorted knots ...            */
-    FDEMRI_ERR_WORKSPACE = 2,   /* work space missing or too small                                        */
+    FDEMRI_ERR_WORKSPACE = 2,   /* work space missing or too small (fdemri_stats.n_pairs: work-list entries needed) */
     FDEMRI_ERR_CUDA = 3,        /* a CUDA runtime call or kernel failed                                   */
     FDEMRI_ERR_NOT_BUILT = 4,   /* fdemri_sum / get_coeffs before fdemri_build_splines                    */
     FDEMRI_ERR_UNSUPPORTED = 5  /* input violates an assumption of the method (see fdemri_stats.flags)    */
@@ -47,19 +47,18 @@ enum {
 /* bits of fdemri_stats.flags (device-side validation, read back by fdemri_get_stats) */
 enum {
     FDEMRI_BAD_TWO_EXTREMA = 1,   /* a segment cubic has two interior extrema (paper assumes <= 1, L105)   */
-    FDEMRI_BAD_STRIP_OVERFLOW = 2,/* a voice has more monotone branches than the map holds                 */
     FDEMRI_BAD_NONFINITE = 4,     /* NaN/Inf met in the inputs or spline coefficients                      */
     FDEMRI_BAD_NEWTON = 8,        /* a root iteration hit its iteration cap                                */
-    FDEMRI_BAD_LIST_OVERFLOW = 16 /* not an error: the per-tile work list did not fit the work space (n_pairs
-                                     entries of 4 bytes needed) or a tile held too many items; fdemri_sum then
-                                     scans the map inside the kernel instead (same results, slower)           */
+    FDEMRI_BAD_LIST_OVERFLOW = 16 /* the per-tile work list did not fit the work space: fdemri_sum fills its outputs
+                                     with NaN and fdemri_get_stats returns FDEMRI_ERR_WORKSPACE; give
+                                     fdemri_set_workspace at least 4 * n_pairs more bytes and build again      */
 };
 
 typedef struct fdemri_plan_s* fdemri_plan_t;
 
 typedef struct {
-    uint64_t n_items;        /* non-empty (voice, sign, segment-branch) items of the last sum (S2)            */
-    uint64_t n_strips;       /* monotone branches ("strips") those items form                               */
+    uint64_t n_items;        /* non-empty (voice, sign, segment-branch) entries of the last build (S2)        */
+    uint64_t reserved;
     uint64_t n_evals;        /* accumulated (voice, sign, root, bin) terms = "mode-bin evaluations" (P9)      */
     uint64_t n_turnover;     /* segments with an interior extremum of F (Fdot = 0, L92, L105)                 */
     uint64_t n_airy;         /* evaluations that took the small-|X| (Airy) path                              */
@@ -88,7 +87,8 @@ int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, int n_
  * The work space holds the spline records, the segment->bin map and the per-tile work list; it must stay valid
  * and untouched between build_splines and the last sum.  The size returned includes a default capacity for the
  * work list (4 bytes per (item, tile) pair); whatever the caller gives beyond the fixed part is used for it, and
- * fdemri_stats.n_pairs reports what the last build needed (see FDEMRI_BAD_LIST_OVERFLOW). */
+ * fdemri_stats.n_pairs reports what the last build needed (see FDEMRI_BAD_LIST_OVERFLOW).  fdemri_set_workspace
+ * may be called again with a larger buffer; fdemri_build_splines must then be repeated. */
 size_t fdemri_workspace_bytes(fdemri_plan_t plan);
 int fdemri_set_workspace(fdemri_plan_t plan, void* dev_ptr, size_t bytes);
 

@@ -24,7 +24,7 @@ EXPORTS = ["fdemri_plan", "fdemri_workspace_bytes", "fdemri_set_workspace", "fde
 
 
 class FdemriStats(C.Structure):
-    _fields_ = [("n_items", C.c_uint64), ("n_strips", C.c_uint64), ("n_evals", C.c_uint64),
+    _fields_ = [("n_items", C.c_uint64), ("reserved", C.c_uint64), ("n_evals", C.c_uint64),
                 ("n_turnover", C.c_uint64), ("n_airy", C.c_uint64), ("flags", C.c_uint64), ("n_slow", C.c_uint64), ("n_pairs", C.c_uint64)]
 
 

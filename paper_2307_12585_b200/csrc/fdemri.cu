@@ -15,7 +15,6 @@
 #include "fdemri_common.cuh"
 #include "fdemri_map.cuh"
 #include "fdemri_splines.cuh"
-#include "fdemri_strips.cuh"
 #include "fdemri_pairs.cuh"
 #include "fdemri_sum.cuh"
 
@@ -30,17 +29,10 @@ struct fdemri_plan_s {
     SplineFac* fac;
     double *sh_hi, *sh_lo, *rec;
     int4* ent;
-    int* n_ent;
     int* tile_cnt;                 // [B * n_tiles] pairs per tile, then [B * n_tiles] fill cursors
     unsigned int* tile_off;        // [B * n_tiles + 1]
     unsigned int* pairs;           // [pair_cap]
     unsigned long long pair_cap;
-    StripRaw* strips;
-    int* n_strips;
-    int4* dense;
-    int* n_dense;
-    int2* bin_range;
-    int dense_cap;
     double4* wts;
     double* angles;
     unsigned long long* stats;     // [0..5], [7], [8] = fdemri_stats, [6] = tile counter (low 32 bits); 16 slots
@@ -72,16 +64,9 @@ static size_t carve(fdemri_plan_s* p, char* base) {
     p->sh_lo = (double*)take(B * 4 * S * 4 * sizeof(double));
     p->rec = (double*)take(B * V * S * R_DOUBLES * sizeof(double));
     p->ent = (int4*)take(B * V * 2 * (size_t)d.ent_max * sizeof(int4));
-    p->n_ent = (int*)take(B * V * 2 * sizeof(int));
     const size_t NT = B * (size_t)d.n_tiles;
     p->tile_cnt = (int*)take(2 * NT * sizeof(int));
     p->tile_off = (unsigned int*)take((NT + 1) * sizeof(unsigned int));
-    p->strips = (StripRaw*)take(B * V * 2 * FDEMRI_MAX_STRIPS * sizeof(StripRaw));
-    p->n_strips = (int*)take(B * V * 2 * sizeof(int));
-    p->dense_cap = (int)(2 * V * FDEMRI_MAX_STRIPS);
-    p->dense = (int4*)take(B * (size_t)p->dense_cap * sizeof(int4));
-    p->n_dense = (int*)take(B * sizeof(int));
-    p->bin_range = (int2*)take(B * sizeof(int2));
     p->wts = (double4*)take(B * V * sizeof(double4));
     p->angles = (double*)take(B * 2 * sizeof(double));
     p->stats = (unsigned long long*)take(16 * sizeof(unsigned long long));
@@ -112,7 +97,7 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
     p->d.n_batch = n_batch;
     p->d.n_knots = n_knots;
     p->d.n_seg = n_knots - 1;
-    p->d.ent_max = n_knots - 1 + FDEMRI_ENT_EXTRA;
+    p->d.ent_max = 2 * (n_knots - 1);                 /* slot = 2*segment + branch */
     p->d.n_freq = n_freq;
     p->d.n_tiles = (int)n_tiles;
     p->d.f0 = f0;
@@ -196,28 +181,17 @@ extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const 
     if (d.n_knots <= 128) launch_splines<128>(p, f_phi, f_r, Phi_phi, Phi_r, amp, st);
     else if (d.n_knots <= 256) launch_splines<256>(p, f_phi, f_r, Phi_phi, Phi_r, amp, st);
     else launch_splines<FDEMRI_MAX_KNOTS>(p, f_phi, f_r, Phi_phi, Phi_r, amp, st);
+    // S2: records, entries and tile counts; then the per-tile work lists (prefix sum, fill, sort)
+    const size_t NT = (size_t)d.n_batch * d.n_tiles;
+    if (cudaMemsetAsync(p->tile_cnt, 0, 2 * NT * sizeof(int), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
     size_t nrec = (size_t)d.n_batch * d.n_modes * d.n_seg;
-    k_records<<<(unsigned)((nrec + 127) / 128), 128, 0, st>>>(d, p->lmn_dev, p->t_knots_dev, p->sh_hi, p->sh_lo, p->rec,
-                                                              p->stats);
-    size_t nvs = (size_t)d.n_batch * d.n_modes * 2;
-    k_strips<<<(unsigned)((nvs + 63) / 64), 64, 0, st>>>(d, p->lmn_dev, f_phi, f_r, p->rec, p->ent, p->n_ent,
-                                                         p->strips, p->n_strips, p->stats);
-    k_strip_compact<<<d.n_batch, 1024, 0, st>>>(d.n_modes, p->dense_cap, p->strips, p->n_strips, p->dense, p->n_dense,
-                                                p->bin_range);
-    // S2c: per-tile pair lists (count, prefix sum, fill, sort)
-    {
-        const size_t NT = (size_t)d.n_batch * d.n_tiles;
-        if (cudaMemsetAsync(p->tile_cnt, 0, 2 * NT * sizeof(int), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
-        const size_t nslots = nvs * (size_t)d.ent_max;
-        const unsigned nb = (unsigned)((nslots + 255) / 256);
-        k_pair_pass<0><<<nb, 256, 0, st>>>(d, p->ent, p->n_ent, p->tile_cnt, p->tile_off, p->tile_cnt + NT, p->pairs,
-                                          p->pair_cap, p->stats);
-        k_pair_scan<<<1, 1024, 0, st>>>(NT, p->tile_cnt, p->tile_off, p->pair_cap, p->stats);
-        k_pair_pass<1><<<nb, 256, 0, st>>>(d, p->ent, p->n_ent, p->tile_cnt, p->tile_off, p->tile_cnt + NT, p->pairs,
-                                          p->pair_cap, p->stats);
-        k_pair_sort<<<(unsigned)NT, 256, FDEMRI_SORT_MAX * sizeof(unsigned int), st>>>(NT, p->tile_off, p->pairs,
-                                                                                     p->pair_cap, p->stats);
-    }
+    k_records<<<(unsigned)((nrec + 127) / 128), 128, 0, st>>>(d, p->lmn_dev, p->t_knots_dev, p->sh_hi, p->sh_lo, f_phi, f_r,
+                                                              p->rec, p->ent, p->tile_cnt, p->stats);
+    k_pair_scan<<<1, 1024, 0, st>>>(NT, p->tile_cnt, p->tile_off, p->pair_cap, p->stats);
+    const size_t nslots = (size_t)d.n_batch * d.n_modes * 2 * d.ent_max;
+    k_pair_fill<<<(unsigned)((nslots + 255) / 256), 256, 0, st>>>(d, p->ent, p->tile_off, p->tile_cnt + NT, p->pairs,
+                                                                  p->pair_cap);
+    k_pair_sort<<<(unsigned)NT, 256, FDEMRI_SORT_MAX * sizeof(unsigned int), st>>>(NT, p->tile_off, p->pairs, p->pair_cap);
     if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
     p->built = true;
     return FDEMRI_OK;
@@ -253,10 +227,6 @@ extern "C" int fdemri_sum(fdemri_plan_t p, int n_angles, const double* theta_hos
     a.ent = p->ent;
     a.tile_off = p->tile_off;
     a.pairs = p->pairs;
-    a.dense = p->dense;
-    a.n_dense = p->n_dense;
-    a.bin_range = p->bin_range;
-    a.dense_cap = p->dense_cap;
     a.wts = p->wts;
     a.n_angles = n_angles;
     a.hp = hplus_dev;
@@ -298,14 +268,14 @@ extern "C" int fdemri_get_stats(fdemri_plan_t p, fdemri_stats* out) {
     if (cudaStreamSynchronize(p->last_stream) != cudaSuccess) return FDEMRI_ERR_CUDA;
     if (cudaMemcpy(h, p->stats, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess) return FDEMRI_ERR_CUDA;
     out->n_items = h[0];
-    out->n_strips = h[1];
     out->n_evals = h[2];
     out->n_turnover = h[3];
     out->n_airy = h[4];
     out->flags = h[5];
     out->n_slow = h[7];
     out->n_pairs = h[8];
-    if (h[5] & (FDEMRI_BAD_TWO_EXTREMA | FDEMRI_BAD_STRIP_OVERFLOW)) return FDEMRI_ERR_UNSUPPORTED;
+    if (h[5] & FDEMRI_BAD_LIST_OVERFLOW) return FDEMRI_ERR_WORKSPACE;
+    if (h[5] & FDEMRI_BAD_TWO_EXTREMA) return FDEMRI_ERR_UNSUPPORTED;
     if (h[5] & FDEMRI_BAD_NONFINITE) return FDEMRI_ERR_INVALID_ARG;
     return FDEMRI_OK;
 }

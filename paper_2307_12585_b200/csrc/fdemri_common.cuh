@@ -5,8 +5,6 @@
 #include <stdint.h>
 
 #define FDEMRI_MAX_KNOTS 512
-#define FDEMRI_MAX_STRIPS 8          // monotone branches kept per (voice, sign)
-#define FDEMRI_ENT_EXTRA 8           // entries per (voice, sign) = (n_knots-1) + FDEMRI_ENT_EXTRA
 #ifndef FDEMRI_CWARPS
 #define FDEMRI_CWARPS 12             // consumer (evaluating) warps per CTA of the sum kernel
 #endif
@@ -80,7 +78,7 @@ enum {
 
 struct FdemriDims {
     int n_modes, n_batch, n_knots, n_seg;   // n_seg = n_knots - 1
-    int ent_max;                            // entries per (voice, sign)
+    int ent_max;                            // entry slots per (voice, sign) = 2 * n_seg (segment, branch)
     int64_t n_freq;
     int n_tiles;                            // tiles per batch item
     double f0, df;

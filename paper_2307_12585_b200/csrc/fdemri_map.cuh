@@ -3,9 +3,17 @@
 // S2 follows PAPER.md L103 (A..D = mode-number-weighted sums of the fundamental-frequency spline
 // coefficients) and L105 ("the spline segment in which each value of f falls is predetermined before the
 // summation").  The map is inverted with respect to the paper: instead of a segment index per (f, voice) it
-// stores, per (voice, sign, segment-branch), the contiguous interval of bins the branch covers.  Along a
-// monotone run of branches these intervals are adjacent, so runs are kept as "strips" [lo, hi] and a bin
-// finds its segment inside a strip by a short search over the branch start bins.
+// stores, per (voice, sign, segment-branch), the contiguous interval of bins the branch covers ("entry"), and
+// counts, per tile of FDEMRI_TILE bins, the entries that intersect it (fdemri_pairs.cuh turns the counts into
+// the per-tile work lists).
+//
+// Membership (R6-R8), decided on doubles only: the knot values F_k (fdemri_knotF), the extremum
+// value F_e of a turnover segment (record slot R_Q2) and the bin frequencies f_i.
+//   branch from value Va (start, in time) to Vb (end):
+//     normal segment        : Va = F_k included, Vb = F_{k+1} excluded          (half-open in time, R6)
+//     turnover, 1st branch  : Va = F_k included, Vb = F_e included               (R7)
+//     turnover, 2nd branch  : Va = F_e excluded, Vb = F_{k+1} excluded
+//   a bin f_i > 0 belongs to the branch for sign s when s*f_i lies between Va and Vb under those rules.
 #pragma once
 #include "fdemri_common.cuh"
 
@@ -93,9 +101,41 @@ __device__ double fdemri_root_build(double FB, double FC, double FD, double x, d
     return t;
 }
 
+// first bin index with f_i >= x  (n_freq if none)
+__device__ int64_t fdemri_first_ge(const FdemriDims& d, double x) {
+    int64_t n = d.n_freq;
+    if (d.freq) {
+        int64_t lo = 0, hi = n;
+        while (lo < hi) { int64_t mid = (lo + hi) >> 1; if (__ldg(d.freq + mid) < x) lo = mid + 1; else hi = mid; }
+        return lo;
+    }
+    double g = ceil((x - d.f0) / d.df);
+    int64_t i = (g <= 0.0) ? 0 : (g >= (double)n ? n : (int64_t)g);
+    while (i > 0 && fdemri_freq(d, i - 1) >= x) --i;
+    while (i < n && fdemri_freq(d, i) < x) ++i;
+    return i;
+}
+// first bin index with f_i > x
+__device__ int64_t fdemri_first_gt(const FdemriDims& d, double x) {
+    int64_t n = d.n_freq;
+    if (d.freq) {
+        int64_t lo = 0, hi = n;
+        while (lo < hi) { int64_t mid = (lo + hi) >> 1; if (__ldg(d.freq + mid) <= x) lo = mid + 1; else hi = mid; }
+        return lo;
+    }
+    double g = floor((x - d.f0) / d.df) + 1.0;
+    int64_t i = (g <= 0.0) ? 0 : (g >= (double)n ? n : (int64_t)g);
+    while (i > 0 && fdemri_freq(d, i - 1) > x) --i;
+    while (i < n && fdemri_freq(d, i) <= x) ++i;
+    return i;
+}
+
+// ent: [B][V][2][ent_max] int4 {first bin, last bin, seg | branchB << 30, 1}, slot = 2*seg + branch (time order);
+// empty slots have w = 0.  tile_cnt: [B][n_tiles] entries intersecting every tile.
 __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ t_knots,
                           const double* __restrict__ sh_hi, const double* __restrict__ sh_lo,
-                          double* __restrict__ rec, unsigned long long* __restrict__ stats) {
+                          const double* __restrict__ f_phi, const double* __restrict__ f_r, double* __restrict__ rec,
+                          int4* __restrict__ ent, int* __restrict__ tile_cnt, unsigned long long* __restrict__ stats) {
     size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     size_t total = (size_t)d.n_batch * d.n_modes * d.n_seg;
     if (id >= total) return;
@@ -177,4 +217,46 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
         atomicOr(stats + 5, 1ull);                           // FDEMRI_BAD_TWO_EXTREMA
     }
     if (bad) atomicOr(stats + 5, 4ull);
+    // ---- bin intervals of the branches of this segment, for both signs (L105) ----
+    const int type = (int)R[R_TYPE];
+    const double Fk = FA;
+    const double Fk1 = (k + 1 < d.n_seg) ? fdemri_knotF(m, n, hi[4], hi[per + 4])
+                                         : fdemri_knotF(m, n, f_phi[(size_t)b * d.n_knots + d.n_knots - 1],
+                                                        f_r[(size_t)b * d.n_knots + d.n_knots - 1]);
+    const int64_t first_pos = fdemri_first_gt(d, 0.0);      // bins with f > 0 only (R13)
+    unsigned long long evals = 0, items = 0;
+    for (int sg = 0; sg < 2; ++sg) {
+        int4* E = ent + ((bv * 2 + sg) * (size_t)d.ent_max) + 2 * k;
+        for (int br = 0; br < 2; ++br) {
+            int4 e4 = make_int4(0, -1, k | (br << 30), 0);
+            if (type != 2 && (br == 0 || type == 1)) {
+                double Va, Vb; bool a_incl, b_incl;
+                if (type == 0) { Va = Fk; Vb = Fk1; a_incl = true; b_incl = false; }
+                else if (br == 0) { Va = Fk; Vb = R[R_Q2]; a_incl = true; b_incl = true; }
+                else { Va = R[R_Q2]; Vb = Fk1; a_incl = false; b_incl = false; }
+                if (Va != Vb) {
+                    const double lo_v = fmin(Va, Vb), hi_v = fmax(Va, Vb);
+                    const bool lo_incl = (Va < Vb) ? a_incl : b_incl;
+                    const bool hi_incl = (Va < Vb) ? b_incl : a_incl;
+                    const double flo = sg ? -hi_v : lo_v, fhi = sg ? -lo_v : hi_v;
+                    const bool flo_incl = sg ? hi_incl : lo_incl, fhi_incl = sg ? lo_incl : hi_incl;
+                    if (fhi > 0.0) {
+                        int64_t lo_b = flo_incl ? fdemri_first_ge(d, flo) : fdemri_first_gt(d, flo);
+                        const int64_t hi1 = fhi_incl ? fdemri_first_gt(d, fhi) : fdemri_first_ge(d, fhi);
+                        if (lo_b < first_pos) lo_b = first_pos;
+                        if (lo_b < hi1) {
+                            e4.x = (int)lo_b; e4.y = (int)(hi1 - 1); e4.w = 1;
+                            evals += (unsigned long long)(hi1 - lo_b);
+                            ++items;
+                            const int t0 = e4.x / FDEMRI_TILE, t1 = e4.y / FDEMRI_TILE;
+                            for (int t = t0; t <= t1; ++t) atomicAdd(tile_cnt + (size_t)b * d.n_tiles + t, 1);
+                        }
+                    }
+                }
+            }
+            E[br] = e4;
+        }
+    }
+    if (items) atomicAdd(stats + 0, items);
+    if (evals) atomicAdd(stats + 2, evals);
 }

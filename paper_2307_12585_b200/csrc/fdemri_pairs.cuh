@@ -6,37 +6,29 @@
 // the order inside a tile is arbitrary until k_pair_sort puts the keys (unique, = entry index) in ascending
 // order: the sum kernel then walks every tile in a data-determined order (bitwise reproducible results).
 //   key = (voice*2 + sign) * ent_max + e                (32 bits; the batch item is implied by the tile)
-// If the pair list does not fit the work space, or a tile holds more keys than the sorter takes, the flag
-// FDEMRI_BAD_LIST_OVERFLOW is raised and fdemri_sum falls back to scanning the strips inside the kernel.
+// If the pair list does not fit the work space the flag FDEMRI_BAD_LIST_OVERFLOW is raised: fdemri_sum then fills
+// its outputs with NaN and fdemri_get_stats returns FDEMRI_ERR_WORKSPACE with the number of pairs needed.
 #pragma once
 #include "fdemri_common.cuh"
 
 #define FDEMRI_SORT_MAX 8192         // keys per tile the shared-memory sorter takes
 
-// One thread per (batch item, voice, sign, entry slot).  mode 0: count per tile;  mode 1: fill.
-template <int MODE>
-__global__ void k_pair_pass(FdemriDims d, const int4* __restrict__ ent, const int* __restrict__ n_ent,
-                            int* __restrict__ tile_cnt, const unsigned int* __restrict__ tile_off,
-                            int* __restrict__ tile_cur, unsigned int* __restrict__ pairs, unsigned long long cap,
-                            unsigned long long* __restrict__ stats) {
+// Fill: one thread per (batch item, voice, sign, entry slot); the counts come from k_records.
+__global__ void k_pair_fill(FdemriDims d, const int4* __restrict__ ent, const unsigned int* __restrict__ tile_off,
+                            int* __restrict__ tile_cur, unsigned int* __restrict__ pairs, unsigned long long cap) {
     const size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const size_t total = (size_t)d.n_batch * d.n_modes * 2 * d.ent_max;
     if (id >= total) return;
-    const int e = (int)(id % d.ent_max);
-    const size_t bvs = id / d.ent_max;                 // (batch item, voice, sign)
-    if (e >= n_ent[bvs]) return;
     const int4 en = ent[id];
-    const int b = (int)(bvs / ((size_t)2 * d.n_modes));
-    const unsigned key = (unsigned)((bvs - (size_t)b * 2 * d.n_modes) * d.ent_max + e);
+    if (!en.w) return;
+    const size_t per_item = (size_t)2 * d.n_modes * d.ent_max;
+    const int b = (int)(id / per_item);
+    const unsigned key = (unsigned)(id - (size_t)b * per_item);
     const int t0 = en.x / FDEMRI_TILE, t1 = en.y / FDEMRI_TILE;
     for (int t = t0; t <= t1; ++t) {
         const size_t gt = (size_t)b * d.n_tiles + t;
-        if (MODE == 0) {
-            atomicAdd(tile_cnt + gt, 1);
-        } else {
-            const unsigned long long pos = (unsigned long long)tile_off[gt] + (unsigned)atomicAdd(tile_cur + gt, 1);
-            if (pos < cap) pairs[pos] = key;
-        }
+        const unsigned long long pos = (unsigned long long)tile_off[gt] + (unsigned)atomicAdd(tile_cur + gt, 1);
+        if (pos < cap) pairs[pos] = key;
     }
 }
 
@@ -93,10 +85,29 @@ __global__ void __launch_bounds__(1024) k_pair_scan(size_t n, const int* __restr
     }
 }
 
-// One CTA per tile: ascending bitonic sort of the tile's keys in shared memory.
+// One CTA per tile: ascending bitonic sort of the tile's keys, in shared memory when they fit and in place in
+// global memory otherwise.  Network for arbitrary n: every merge starts with a "flip" step (partner i ^ (2k-1))
+// followed by "shift" steps (partner i ^ j), all ascending, so keys past the end act as +infinity and are skipped.
+__device__ __forceinline__ void fdemri_bitonic(unsigned int* buf, unsigned int n) {
+    unsigned int np = 2;
+    while (np < n) np <<= 1;
+    for (unsigned int k = 1; k < np; k <<= 1) {                     // merge sorted runs of length k into runs of 2k
+        for (unsigned int j = k; j > 0; j >>= 1) {
+            for (unsigned int i = threadIdx.x; i < (np >> 1); i += blockDim.x) {
+                const unsigned int a = ((i & ~(j - 1)) << 1) | (i & (j - 1));       // bit j clear
+                const unsigned int bb = (j == k) ? (a ^ ((j << 1) - 1)) : (a + j);    // flip : shift
+                if (bb < n) {
+                    const unsigned int x = buf[a], y = buf[bb];
+                    if (x > y) { buf[a] = y; buf[bb] = x; }
+                }
+            }
+            __syncthreads();
+        }
+    }
+}
+
 __global__ void __launch_bounds__(256) k_pair_sort(size_t n_tiles_total, const unsigned int* __restrict__ tile_off,
-                                                   unsigned int* __restrict__ pairs, unsigned long long cap,
-                                                   unsigned long long* __restrict__ stats) {
+                                                   unsigned int* __restrict__ pairs, unsigned long long cap) {
     extern __shared__ unsigned int s_key[];
     const size_t gt = blockIdx.x;
     if (gt >= n_tiles_total) return;
@@ -104,25 +115,11 @@ __global__ void __launch_bounds__(256) k_pair_sort(size_t n_tiles_total, const u
     const unsigned int n = o1 - o0;
     if (n < 2u || (unsigned long long)o1 > cap) return;
     if (n > FDEMRI_SORT_MAX) {
-        if (threadIdx.x == 0) atomicOr(stats + 5, (unsigned long long)FDEMRI_BAD_LIST_OVERFLOW_BIT);
+        fdemri_bitonic(pairs + o0, n);
         return;
     }
-    unsigned int np = 2;
-    while (np < n) np <<= 1;
-    for (unsigned int i = threadIdx.x; i < np; i += blockDim.x) s_key[i] = (i < n) ? pairs[o0 + i] : 0xffffffffu;
+    for (unsigned int i = threadIdx.x; i < n; i += blockDim.x) s_key[i] = pairs[o0 + i];
     __syncthreads();
-    for (unsigned int k = 2; k <= np; k <<= 1) {
-        for (unsigned int j = k >> 1; j > 0; j >>= 1) {
-            for (unsigned int i = threadIdx.x; i < (np >> 1); i += blockDim.x) {
-                // i-th compare-exchange of this stage: partner indices a < b = a + j
-                const unsigned int a = ((i & ~(j - 1)) << 1) | (i & (j - 1));
-                const unsigned int bb = a + j;
-                const bool up = (a & k) == 0;
-                const unsigned int x = s_key[a], y = s_key[bb];
-                if ((x > y) == up) { s_key[a] = y; s_key[bb] = x; }
-            }
-            __syncthreads();
-        }
-    }
+    fdemri_bitonic(s_key, n);
     for (unsigned int i = threadIdx.x; i < n; i += blockDim.x) pairs[o0 + i] = s_key[i];
 }

@@ -2,11 +2,10 @@
 //
 // A CTA owns a tile of FDEMRI_TILE consecutive bins of one batch item at a time (tiles are handed out by an
 // atomic counter).  It is warp-specialised:
-//   * one PRODUCER warp scans the item's strips in their fixed (voice, sign, time) order, turns every strip that
-//     intersects the tile into "items" -- (voice, sign, segment-branch) with the sub-range of the tile they
-//     cover -- reads their records and weights from global memory, folds everything that does not depend on
-//     the bin into a 256-byte staged item, and pushes chunks of staged items through a shared-memory ring
-//     (full/empty mbarriers);
+//   * one PRODUCER warp walks the tile's work list (fdemri_pairs.cuh: the entries -- (voice, sign, segment-branch)
+//     -- that intersect the tile, in the fixed order (voice, sign, time)), reads their records and weights
+//     from global memory, folds everything that does not depend on the bin into a 256-byte staged item, and
+//     pushes chunks of staged items through a shared-memory ring (full/empty mbarriers);
 //   * FDEMRI_CWARPS CONSUMER warps each own 64 consecutive bins of the tile, two per lane (lane, lane + 32),
 //     with the eight accumulators in registers.  For every staged item that overlaps its bins a consumer warp
 //     evaluates the term of Eq. 9 for both of its bins at once (two independent
@@ -29,13 +28,9 @@
 struct SumArgs {
     FdemriDims d;
     const double* rec;        // [B][V][S][R_DOUBLES]
-    const int4* ent;          // [B][V][2][ent_max] {first bin, last bin, seg | branchB << 30, 0}
+    const int4* ent;          // [B][V][2][ent_max] {first bin, last bin, seg | branchB << 30, valid}
     const unsigned int* tile_off;   // [B * n_tiles + 1] first pair of every tile
     const unsigned int* pairs;      // sorted keys (voice*2+sign)*ent_max + e of every tile
-    const int4* dense;        // [B][dense_cap]
-    const int* n_dense;       // [B]
-    const int2* bin_range;    // [B] {first, last} bin covered by any strip
-    int dense_cap;
     const double4* wts;       // [n_angles][V]
     int n_angles;
     double* hp;               // [B][n_freq][2]
@@ -356,123 +351,9 @@ __device__ __forceinline__ void fdemri_stage_item(double* dst, const double* __r
     d2[15] = make_double2(-w.y, s * w.y);
 }
 
-// Fallback producer (the pair lists did not fit the work space): scans the strips of the batch item.
-__device__ __noinline__ void fdemri_producer_scan(const SumArgs& a, FdemriRing* ring, int lane) {
-    const FdemriDims& d = a.d;
-    const int V = d.n_modes;
-    int stage = 0;
-    unsigned phase = 0;
-    for (;;) {
-        int gt = 0;
-        if (lane == 0) gt = (int)atomicAdd(a.tile_counter, 1u);
-        gt = __shfl_sync(0xffffffffu, gt, 0);
-        const bool done = gt >= a.total_tiles;
-        // a fresh stage for this tile
-        fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, 256u);
-        if (done) {
-            if (lane == 0) {
-                ring->st[stage].hdr[0] = -1; ring->st[stage].hdr[1] = 0; ring->st[stage].hdr[2] = 1;
-                fdemri_mbar_arrive(&ring->full[stage]);
-            }
-            return;
-        }
-        int fill = 0;
-        const int b = gt / d.n_tiles, tile = gt - b * d.n_tiles;
-        const int64_t bin0 = (int64_t)tile * FDEMRI_TILE;
-        const int tile_lo = (int)bin0;
-        const int tile_hi = (int)min(bin0 + FDEMRI_TILE - 1, d.n_freq - 1);
-        const int2 br = a.bin_range[b];
-        const int nd = (br.y < tile_lo || br.x > tile_hi) ? 0 : a.n_dense[b];
-        const int4* dense_b = a.dense + (size_t)b * a.dense_cap;
-        const int wbase = (a.n_angles > 1 ? b : 0) * V;
-        const size_t rbase = (size_t)b * V * d.n_seg;
-        for (int base = 0; base < nd; base += 32) {
-            // ---- candidate strip of this lane ----
-            const int c = base + lane;
-            int remaining = 0, e_next = 0, ne = 0, dir = 0, vs = 0, s_lo = 0, s_hi = 0;
-            const int4* E = nullptr;
-            if (c < nd) {
-                const int4 s = dense_b[c];
-                if (s.x <= tile_hi && s.y >= tile_lo) {
-                    vs = s.z >> 1; dir = s.z & 1;
-                    const int e0 = s.w & 0xffff;
-                    ne = s.w >> 16;
-                    s_lo = s.x; s_hi = s.y;
-                    E = a.ent + ((size_t)b * 2 * V + vs) * d.ent_max + e0;
-                    const int clo = max(s.x, tile_lo), chi = min(s.y, tile_hi);
-                    // entry holding bin x: dir=1: last e with E[e].x <= x;  dir=0: first e with E[e].x <= x
-                    int ea, eb;
-                    if (dir) {
-                        int lo = 0, hi = ne - 1;
-                        while (lo < hi) { int mid = (lo + hi + 1) >> 1; if (E[mid].x <= clo) lo = mid; else hi = mid - 1; }
-                        ea = lo;
-                        hi = ne - 1;
-                        while (lo < hi) { int mid = (lo + hi + 1) >> 1; if (E[mid].x <= chi) lo = mid; else hi = mid - 1; }
-                        eb = lo;
-                    } else {
-                        int lo = 0, hi = ne - 1;
-                        while (lo < hi) { int mid = (lo + hi) >> 1; if (E[mid].x <= chi) hi = mid; else lo = mid + 1; }
-                        ea = lo;
-                        hi = ne - 1;
-                        while (lo < hi) { int mid = (lo + hi) >> 1; if (E[mid].x <= clo) hi = mid; else lo = mid + 1; }
-                        eb = lo;
-                    }
-                    e_next = ea;
-                    remaining = eb - ea + 1;
-                }
-            }
-            // ---- rounds: every candidate emits one item per round, in candidate order ----
-            for (;;) {
-                const int n_emit = min(remaining, 1);
-                int incl = n_emit;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    int t = __shfl_up_sync(0xffffffffu, incl, o);
-                    if (lane >= o) incl += t;
-                }
-                const int total = __shfl_sync(0xffffffffu, incl, 31);
-                if (total == 0) break;
-                if (fill + total > FDEMRI_CHUNK) {
-                    // publish the chunk and take the next stage
-                    __syncwarp();
-                    if (lane == 0) {
-                        ring->st[stage].hdr[0] = gt; ring->st[stage].hdr[1] = fill; ring->st[stage].hdr[2] = 0;
-                        fdemri_mbar_arrive(&ring->full[stage]);
-                    }
-                    if (++stage == FDEMRI_STAGES) { stage = 0; phase ^= 1u; }
-                    fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, 256u);
-                    fill = 0;
-                }
-                const int off = fill + incl - n_emit;
-                for (int i = 0; i < n_emit; ++i) {
-                    const int e = e_next + i;
-                    const int4 en = E[e];
-                    const int lo_e = max(max(en.x, s_lo), tile_lo) - tile_lo;
-                    const int hi_e = min(min(en.y, s_hi), tile_hi) - tile_lo;
-                    const int seg = en.z & 0x3fffffff;
-                    const int v = vs >> 1;
-                    fdemri_stage_item(ring->st[stage].items[off + i],
-                                      a.rec + (rbase + (size_t)v * d.n_seg + seg) * R_DOUBLES, a.wts[wbase + v], lo_e, hi_e,
-                                      (unsigned)(vs & 1), (unsigned)((en.z >> 30) & 1));
-                }
-                fill += total;
-                e_next += n_emit;
-                remaining -= n_emit;
-            }
-        }
-        // last chunk of the tile (possibly empty)
-        __syncwarp();
-        if (lane == 0) {
-            ring->st[stage].hdr[0] = gt; ring->st[stage].hdr[1] = fill; ring->st[stage].hdr[2] = 1;
-            fdemri_mbar_arrive(&ring->full[stage]);
-        }
-        if (++stage == FDEMRI_STAGES) { stage = 0; phase ^= 1u; }
-    }
-}
-
 // Producer: walks the sorted pair list of every tile it draws (S2c, fdemri_pairs.cuh), one ring stage per
 // 32 keys: key -> entry (bin interval, segment, branch) -> record + weights -> staged item.
-__device__ __forceinline__ void fdemri_producer_lists(const SumArgs& a, FdemriRing* ring, int lane) {
+__device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ring, int lane) {
     const FdemriDims& d = a.d;
     const int V = d.n_modes;
     int stage = 0;
@@ -629,10 +510,16 @@ __global__ void __maxnreg__(FDEMRI_MAXNREG) k_tile_sum(SumArgs a) {
         }
     }
     __syncthreads();
-    if (wid == FDEMRI_CWARPS) {
-        const bool lists = !(*(volatile const unsigned long long*)(a.stats + 5) & FDEMRI_BAD_LIST_OVERFLOW_BIT);
-        if (lists) fdemri_producer_lists(a, ring, lane);
-        else fdemri_producer_scan(a, ring, lane);
+    if (*(volatile const unsigned long long*)(a.stats + 5) & FDEMRI_BAD_LIST_OVERFLOW_BIT) {
+        // the work list did not fit the work space: fail loudly (NaN everywhere; see fdemri_get_stats)
+        const size_t n = (size_t)a.d.n_batch * a.d.n_freq * 2;
+        const double nan = __longlong_as_double(0x7ff8000000000000ll);
+        for (size_t i = (size_t)blockIdx.x * blockDim.x + tid; i < n; i += (size_t)gridDim.x * blockDim.x) {
+            a.hp[i] = nan;
+            a.hx[i] = nan;
+        }
+        return;
     }
+    if (wid == FDEMRI_CWARPS) fdemri_producer(a, ring, lane);
     else fdemri_consumer(a, ring, wid, lane);
 }
