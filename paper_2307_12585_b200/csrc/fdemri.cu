@@ -26,7 +26,6 @@ struct fdemri_plan_s {
     void* ws;
     size_t ws_bytes;
     int* lmn_dev;
-    SplineFac* fac;
     double *sh_hi, *sh_lo, *rec;
     int4* ent;
     int* tile_cnt;                 // [B * n_tiles] pairs per tile, then [B * n_tiles] fill cursors
@@ -40,6 +39,7 @@ struct fdemri_plan_s {
     bool built;
     cudaStream_t last_stream;
     int sm_count;
+    bool spline_attr_set;
     int sum_blocks_per_sm;         // resident CTAs of k_tile_sum per SM (0: not queried yet)
     uint32_t flags;
     cudaEvent_t ev0, ev1;
@@ -59,7 +59,6 @@ static size_t carve(fdemri_plan_s* p, char* base) {
         return ptr;
     };
     p->lmn_dev = (int*)take(V * 3 * sizeof(int));
-    p->fac = (SplineFac*)take(B * N * sizeof(SplineFac));
     p->sh_hi = (double*)take(B * 4 * S * 4 * sizeof(double));
     p->sh_lo = (double*)take(B * 4 * S * 4 * sizeof(double));
     p->rec = (double*)take(B * V * S * R_DOUBLES * sizeof(double));
@@ -117,6 +116,7 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
     }
     p->sm_count = prop.multiProcessorCount;
     p->sum_blocks_per_sm = 0;
+    p->spline_attr_set = false;
     p->flags = flags;
     p->ev_valid = false;
     p->ev0 = p->ev1 = nullptr;
@@ -157,18 +157,6 @@ extern "C" int fdemri_set_workspace(fdemri_plan_t p, void* dev_ptr, size_t bytes
     return FDEMRI_OK;
 }
 
-template <int MAXN>
-static void launch_splines(fdemri_plan_s* p, const double* f_phi, const double* f_r, const double* Phi_phi,
-                           const double* Phi_r, const double* amp, cudaStream_t st) {
-    const FdemriDims& d = p->d;
-    int nb = (d.n_batch * 4 + 63) / 64;
-    k_spline_shared<MAXN><<<nb, 64, 0, st>>>(d.n_batch, d.n_knots, f_phi, f_r, Phi_phi, Phi_r, p->fac, p->sh_hi,
-                                             p->sh_lo, p->stats + 5);
-    size_t nt = (size_t)d.n_batch * d.n_modes * 2;
-    k_spline_amp<MAXN><<<(unsigned)((nt + 127) / 128), 128, 0, st>>>(d.n_batch, d.n_modes, d.n_knots, amp, p->fac,
-                                                                      p->rec, p->stats + 5);
-}
-
 extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const double* f_r, const double* Phi_phi,
                                     const double* Phi_r, const double* amp, void* cuda_stream) {
     if (!p || !f_phi || !f_r || !Phi_phi || !Phi_r || !amp) return FDEMRI_ERR_INVALID_ARG;
@@ -177,10 +165,25 @@ extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const 
     const FdemriDims& d = p->d;
     p->last_stream = st;
     if (cudaMemsetAsync(p->stats, 0, 16 * sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
-    k_spline_factor<<<(d.n_batch + 63) / 64, 64, 0, st>>>(d.n_batch, d.n_knots, p->t_knots_dev, p->fac, p->stats + 5);
-    if (d.n_knots <= 128) launch_splines<128>(p, f_phi, f_r, Phi_phi, Phi_r, amp, st);
-    else if (d.n_knots <= 256) launch_splines<256>(p, f_phi, f_r, Phi_phi, Phi_r, amp, st);
-    else launch_splines<FDEMRI_MAX_KNOTS>(p, f_phi, f_r, Phi_phi, Phi_r, amp, st);
+    // S1: parallel cyclic reduction, one thread per knot
+    {
+        const int N = d.n_knots;
+        const int threads = (N + 31) & ~31;
+        const size_t sm_sh = (size_t)(2 * N * FDEMRI_SH_ROW + 5 * N) * sizeof(double2);
+        const size_t sm_am = ((size_t)2 * N * FDEMRI_AMP_ROW + N + (N & 1)) * sizeof(double) +
+                             (size_t)2 * FDEMRI_AMP_VOICES * N * sizeof(double2);
+        if (!p->spline_attr_set) {
+            if (cudaFuncSetAttribute(k_spline_shared, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_sh) != cudaSuccess ||
+                cudaFuncSetAttribute(k_spline_amp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_am) != cudaSuccess)
+                return FDEMRI_ERR_CUDA;
+            p->spline_attr_set = true;
+        }
+        k_spline_shared<<<d.n_batch, threads, sm_sh, st>>>(N, p->t_knots_dev, f_phi, f_r, Phi_phi, Phi_r, p->sh_hi, p->sh_lo,
+                                                          p->stats + 5);
+        const int groups = (d.n_modes + FDEMRI_AMP_VOICES - 1) / FDEMRI_AMP_VOICES;
+        k_spline_amp<<<(unsigned)((size_t)d.n_batch * groups), threads, sm_am, st>>>(d.n_modes, N, p->t_knots_dev, amp, p->rec,
+                                                                                  p->stats + 5);
+    }
     // S2: records, entries and tile counts; then the per-tile work lists (prefix sum, fill, sort)
     const size_t NT = (size_t)d.n_batch * d.n_tiles;
     if (cudaMemsetAsync(p->tile_cnt, 0, 2 * NT * sizeof(int), st) != cudaSuccess) return FDEMRI_ERR_CUDA;

@@ -257,6 +257,16 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
             E[br] = e4;
         }
     }
-    if (items) atomicAdd(stats + 0, items);
-    if (evals) atomicAdd(stats + 2, evals);
+    // counters: one atomic per warp (every thread of a warp adding to the same word serialises in L2)
+    {
+        const unsigned mask = __activemask();
+        const unsigned it_w = __reduce_add_sync(mask, (unsigned)items);
+        const unsigned lo_w = __reduce_add_sync(mask, (unsigned)(evals & 0xffffu));
+        const unsigned hi_w = __reduce_add_sync(mask, (unsigned)(evals >> 16));
+        if ((threadIdx.x & 31) == __ffs(mask) - 1) {
+            if (it_w) atomicAdd(stats + 0, (unsigned long long)it_w);
+            const unsigned long long ev = ((unsigned long long)hi_w << 16) + lo_w;
+            if (ev) atomicAdd(stats + 2, ev);
+        }
+    }
 }
