@@ -48,7 +48,7 @@ enum {
 // ------------------------------------------------------------------------------------------------
 enum {
     S_META = 0, // int2 {lo | hi << 16 (tile-relative bins), type | branchB << 1 | sign << 2}
-    S_HSF = 1,  // 0.5 * sign of dF/dtau on this branch (folded into S_PC4; the slow path adds it back)
+    S_F32A = 1, // float2 {FB, FC}: single-precision copies for the first iterate of the inversion
     S_NFA = 2,  // -FA
     S_FB = 3,
     S_FC = 4,
@@ -56,17 +56,18 @@ enum {
     S_Q1 = 6,
     S_Q2 = 7,
     S_Q3 = 8,
-    S_TOLH = 9, // acceptance threshold of the last Newton correction, 3e-8 h
+    S_TOLH = 9, // acceptance threshold of the last Newton correction, 2e-7 h
     S_HH = 10,  // h/2
-    S_HH1 = 11, // h/2 (1 + 1e-9)
+    S_F32B = 11,// float2 {FD, Q1}
     S_CU = 12,  // 1/X = CU * (F''/2)^2 / |F'|^3,  CU = sign(F') 6/pi
     S_TK4 = 13, // 4 t_k
     S_NBH4 = 14,// -4 b'_hi
     S_NBL4 = 15,// -4 b'_lo
     S_NC4 = 16, // 4 (-c_Phi/2pi)
     S_ND4 = 17, // 4 (-d_Phi/2pi)
-    S_PC4 = 18, // 4 (PC + m phi/2pi) - 0.5 sign(F')     (the e^{-+i pi/4} of the standard SPA, L119)
-    S_SPARE = 19,
+    S_PC4 = 18, // 4 (PC + m phi/2pi) - 0.5 sign(F')     (the e^{-+i pi/4} of the standard SPA, L119; the slow
+                // path takes the fold out again with the sign of S_CU)
+    S_F32C = 19,// float2 {Q2, Q3}
     S_AR = 20,  // 20..23
     S_AI = 24,  // 24..27
     S_WP = 28,  // w+

@@ -16,9 +16,11 @@
 // on the data, never on scheduling: results are bitwise reproducible.
 // The paper's own layout -- one block per (voice, segment), atomicAdd into global memory (L121) -- is prior art.
 //
-// Fast path (monotone segment, |X| >= 400, > 99 % of the evaluations): division-free inversion of the segment
-// cubic -- stored inverse-cubic seed, one Halley step, one Newton correction whose size is the acceptance test --
-// then the polar form of the asymptotic g(X) series and a polynomial sincos of the phase in quarter turns.
+// Fast path (monotone segment, |X| >= 400, ~99 % of the evaluations): division-free inversion of the segment
+// cubic -- stored inverse-cubic seed and one Halley step in SINGLE precision (FMA pipe), then one FP64 Newton
+// correction whose size is the acceptance test -- then the polar form of the asymptotic g(X) series and a
+// polynomial sincos of the phase in quarter turns.  The FP64 pipe is the bound (a DFMA with three distinct
+// register operands issues every 3 cycles, not 2: see profiles/), so everything that tolerates it runs elsewhere.
 // Everything else (turnover segments, small |X|, rejected iterations) goes to fdemri_term_slow.
 #pragma once
 #include "fdemri_common.cuh"
@@ -100,9 +102,11 @@ __device__ __forceinline__ double4 fdemri_ld4(const double4* p) {
     return v;
 }
 
-__device__ __forceinline__ double fdemri_rsqrt_seed(double a) {      // ~21 good bits (MUFU.RSQ64H)
+// ~21 good bits of |a|^(-1/2) (MUFU.RSQ64H reads the high word only; the sign is cleared with an integer op)
+__device__ __forceinline__ double fdemri_rsqrt_seed_abs(double a) {
     double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    const double aa = __hiloint2double(__double2hiint(a) & 0x7fffffff, 0);
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(aa));
     return y;
 }
 
@@ -136,36 +140,50 @@ __device__ __forceinline__ void fdemri_mbar_wait(uint64_t* bar, unsigned parity,
 __device__ __forceinline__ bool fdemri_term_fast(const double* __restrict__ it, double sf, double& Tre, double& Tim) {
     const double FB = it[S_FB], FC = it[S_FC], FD = it[S_FD];
     const double x = sf + it[S_NFA];
-    double tau = x * fma(x, fma(x, it[S_Q3], it[S_Q2]), it[S_Q1]);          // seed: stored inverse cubic
-    // Halley step:  tau <- tau - d (1 + d F''/(2 F')),  d = G/F',  1/F' from the 64-bit rsqrt seed squared
-    double b2 = fma(tau, FD, FC), b1 = fma(tau, b2, FB), G = fma(tau, b1, -x);
-    double c2 = fma(tau, FD, b2), dG = fma(tau, c2, b1), Fh = fma(tau, FD, c2);   // Fh = F''/2
-    double y = fdemri_rsqrt_seed(fabs(dG));
-    double r = copysign(y * y, dG);
-    const double d0 = G * r;
-    tau = fma(-d0, d0 * (Fh * r), tau - d0);
+    // First iterate in SINGLE precision (FMA pipe, not the FP64 pipe): stored inverse-cubic seed, then a Halley
+    // step  tau <- tau - d (1 + d F''/(2 F')),  d = G/F'.  It only has to land within ~1e-7 h of the root.
+    double tau;
+    {
+        const float2 c0 = *reinterpret_cast<const float2*>(it + S_F32A);      // FB, FC
+        const float2 c1 = *reinterpret_cast<const float2*>(it + S_F32B);      // FD, Q1
+        const float2 c2f = *reinterpret_cast<const float2*>(it + S_F32C);     // Q2, Q3
+        const float xf = (float)x;
+        float tf = xf * fmaf(xf, fmaf(xf, c2f.y, c2f.x), c1.y);
+        const float b2 = fmaf(tf, c1.x, c0.y), b1 = fmaf(tf, b2, c0.x), G = fmaf(tf, b1, -xf);
+        const float c2 = fmaf(tf, c1.x, b2), dG = fmaf(tf, c2, b1), Fh = fmaf(tf, c1.x, c2);
+        float r;
+        asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(dG));
+        const float d0 = G * r;
+        tf = fmaf(-d0, d0 * (Fh * r), tf - d0);
+        tau = (double)tf;
+    }
     // Newton correction at the new point; its size is the acceptance test
-    b2 = fma(tau, FD, FC); b1 = fma(tau, b2, FB); G = fma(tau, b1, -x);
-    c2 = fma(tau, FD, b2); dG = fma(tau, c2, b1); Fh = fma(tau, FD, c2);
-    y = fdemri_rsqrt_seed(fabs(dG));
+    const double b2 = fma(tau, FD, FC), b1 = fma(tau, b2, FB), G = fma(tau, b1, -x);
+    const double c2 = fma(tau, FD, b2), dG = fma(tau, c2, b1), Fh = fma(tau, FD, c2);   // Fh = F''/2
+    double y = fdemri_rsqrt_seed_abs(dG);
     {   // third-order refinement of y ~ |F'|^(-1/2): relative error 2^-22 -> < 1e-17
         const double t = fabs(dG) * y;
         const double e = fma(-t, y, 1.0);
         y = fma(y, e * fma(e, 0.375, 0.5), y);
     }
-    r = y * y;                                         // 1/|F'|
+    const double r = y * y;                            // 1/|F'|
     const double rs = copysign(r, dG);
     const double delta = G * rs;
     tau -= delta;
-    const double tq = (delta * Fh) * rs;               // relative change of F' over the correction, halved
-    y = fma(y, tq, y);                                 // |F'(tau)|^(-1/2) to first order in delta
-    // accept: the neglected second-order terms are below rounding (|F'' delta / F'| <= 1e-6 and |delta| <= 3e-8 h)
+    // values at the corrected point, to first order in delta (second order is below 1e-13):
+    //   F''/2 -> Fh - 3 FD delta,   F' -> F' (1 - 2 tq),  tq = delta (Fh - 1.5 FD delta) / F',   |F'|^(-1/2) -> y (1 + tq)
+    const double t3 = delta * FD;
+    const double Fhc = fma(t3, -3.0, Fh);
+    const double tq = (delta * fma(t3, -1.5, Fh)) * rs;
+    y = fma(y, tq, y);
+    // accept: the neglected second-order terms are below rounding (|F'' delta / F'| <= 5e-7 and |delta| <= 2e-7 h)
     // and the iterate sits in the segment (the root does, by membership R6)
     // (compared on the high words: |v| <= T  <=>  hi(|v|) <= hi(T) up to 2^-20 relative; NaN fails)
-    const double pq = Fh * r;
-    const double u = (pq * pq) * (r * it[S_CU]);       // 1/X = 3 F''^2 / (2 pi F'^3)
-    const bool ok = (fdemri_hiabs(tq) <= 0x3ea0c6f7) & (fdemri_hiabs(delta) <= __double2hiint(it[S_TOLH])) &
-                    (fdemri_hiabs(tau - it[S_HH]) <= __double2hiint(it[S_HH1])) & (fdemri_hiabs(u) <= 0x3f647ae1);
+    const double rc = y * y;                           // 1/|F'| at the corrected point
+    const double pq = Fhc * rc;
+    const double u = (pq * pq) * (rc * it[S_CU]);      // 1/X = 3 F''^2 / (2 pi F'^3), needed to 1e-9 relative
+    const bool ok = (fdemri_hiabs(tq) <= 0x3e90c6f7) & (fdemri_hiabs(delta) <= __double2hiint(it[S_TOLH])) &
+                    (fdemri_hiabs(tau - it[S_HH]) <= __double2hiint(it[S_HH])) & (fdemri_hiabs(u) <= 0x3f647ae1);
     const double u2 = u * u;
     const double dq = u * fma(u2, FDEMRI_G_DQ3, FDEMRI_G_DQ1);
     const double yr = y * fma(u2, fma(u2, FDEMRI_G_R4, FDEMRI_G_R2), 1.0);
@@ -179,8 +197,8 @@ __device__ __forceinline__ bool fdemri_term_fast(const double* __restrict__ it, 
     const double big4 = 27021597764222976.0;           // 1.5 * 2^54: adding it rounds to a multiple of 4
     const double pr = P - ((P + big4) - big4);
     const double wv = fma(sf, 4.0, it[S_NBH4]) + it[S_NBL4];
-    const double loc = tau * fma(tau, fma(tau, it[S_ND4], it[S_NC4]), wv);
-    const double q = ((pr + e) + it[S_PC4]) + (loc + dq);
+    const double loc = fma(tau, fma(tau, fma(tau, it[S_ND4], it[S_NC4]), wv), it[S_PC4]);
+    const double q = (pr + e) + (loc + dq);
     double sn, cs;
     fdemri_sincos_quarter(q, sn, cs);
     const double Er = yr * cs, Ei = yr * sn;
@@ -264,7 +282,7 @@ __device__ __noinline__ FdemriSlowOut fdemri_term_slow(const double* it, double 
     const double pr = P - ((P + big4) - big4);
     const double wv = fma(sf, 4.0, it[S_NBH4]) + it[S_NBL4];
     const double loc = tau * fma(tau, fma(tau, it[S_ND4], it[S_NC4]), wv);
-    double q = ((pr + e) + (it[S_PC4] + it[S_HSF])) + loc;
+    double q = ((pr + e) + (it[S_PC4] + copysign(0.5, it[S_CU]))) + loc;
     double Sre, Sim;
     if (series) {
         const double y = rsqrt(aFd);
@@ -333,16 +351,19 @@ __device__ __forceinline__ void fdemri_stage_item(double* dst, const double* __r
     const double h = r1.w;
     double2* d2 = reinterpret_cast<double2*>(dst);
     int2 meta = make_int2(lo | (hi << 16), (int)((type & 1u) | (brB << 1) | (sg << 2)));
-    d2[0] = make_double2(__hiloint2double(meta.y, meta.x), 0.5 * sF);
+    const float2 f32a = make_float2((float)r0.y, (float)r0.z);               // FB, FC
+    const float2 f32b = make_float2((float)r0.w, (float)r1.x);               // FD, Q1
+    const float2 f32c = make_float2((float)r1.y, (float)r1.z);               // Q2, Q3
+    d2[0] = make_double2(__hiloint2double(meta.y, meta.x), *reinterpret_cast<const double*>(&f32a));
     d2[1] = make_double2(-r0.x, r0.y);
     d2[2] = make_double2(r0.z, r0.w);
     d2[3] = make_double2(r1.x, r1.y);
-    d2[4] = make_double2(r1.z, 3e-8 * h);
-    d2[5] = make_double2(0.5 * h, 0.5 * h * 1.000000001);
+    d2[4] = make_double2(r1.z, 2e-7 * h);
+    d2[5] = make_double2(0.5 * h, *reinterpret_cast<const double*>(&f32b));
     d2[6] = make_double2(sF * 1.9098593171027440, 4.0 * r5.y);
     d2[7] = make_double2(-4.0 * r4.y, -4.0 * r4.z);
     d2[8] = make_double2(4.0 * r4.w, 4.0 * r5.x);
-    d2[9] = make_double2(fma(4.0, r4.x + w.z, -0.5 * sF), 0.0);
+    d2[9] = make_double2(fma(4.0, r4.x + w.z, -0.5 * sF), *reinterpret_cast<const double*>(&f32c));
     d2[10] = make_double2(r2.x, r2.y);
     d2[11] = make_double2(r2.z, r2.w);
     d2[12] = make_double2(r3.x, r3.y);
@@ -430,11 +451,23 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
             f1 = (bin_a + 32 < d.n_freq) ? fdemri_freq(d, bin_a + 32) : 0.0;
             a00 = a01 = a02 = a03 = a10 = a11 = a12 = a13 = 0.0;
         }
-        for (int j = 0; j < cnt; ++j) {
+        // items of the chunk that overlap this warp's bins: lane j looks at item j, one ballot, then the set
+        // bits are walked in ascending (= list) order
+        unsigned todo;
+        {
+            bool mine = false;
+            if (lane < cnt) {
+                const int mx = *reinterpret_cast<const int*>(S->items[lane]);       // lo | hi << 16
+                mine = !((mx >> 16) < wb || (mx & 0xffff) > wb + 32 * FDEMRI_BPL - 1);
+            }
+            todo = __ballot_sync(0xffffffffu, mine);
+        }
+        while (todo) {
+            const int j = __ffs(todo) - 1;
+            todo &= todo - 1;
             const double* it = S->items[j];
             const int2 meta = *reinterpret_cast<const int2*>(it);        // {lo | hi << 16, flags}
             const int lo = meta.x & 0xffff, hi = meta.x >> 16;
-            if (hi < wb || lo > wb + 32 * FDEMRI_BPL - 1) continue;      // warp-uniform
             const unsigned flags = (unsigned)meta.y;
             const unsigned sbit = (flags & 4u) << 29;
             const bool act0 = rel0 >= lo && rel0 <= hi;
