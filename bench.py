@@ -27,7 +27,7 @@ sys.path.insert(0, ROOT)
 
 METRIC = "waveforms/s, 3843-mode 2-yr FD sum (FP64)"
 FLOP_PER_EVAL = 200.0          # SURVEY.md 8(d) / DESIGN.md: algorithmic FP64 flop per mode-bin evaluation
-KERNELS_PER_STEP = 8           # factor, shared, amp, records, strips, compact | weights, tile_sum
+KERNELS_PER_STEP = 8           # spline_shared, spline_amp, records, pair_scan, pair_fill, pair_sort | weights, tile_sum
 
 
 def load_workload(idx):
@@ -132,6 +132,71 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_batched(args, fd, fdist, torch, dev, rank, world, local, barrier):
+    """BASELINE config 4: many parameter sets, evaluated chunk by chunk in one launch sequence.  A "step" is one
+    pass over this rank's share of the items (S1-S4 for every chunk, inputs resident in HBM)."""
+    from paper_2307_12585_b200 import synth
+    mine = fdist.shard_range(args.items, world, rank)
+    chunk = args.chunk
+    chunks = [list(mine)[i:i + chunk] for i in range(0, len(mine), chunk)]
+    # generate and upload all chunks first (untimed), keep every output resident
+    loads = []
+    for ids in chunks:
+        w = synth.config4(items=ids)
+        wf = fd.Waveform(w.lmn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df, device=dev, flags=1)
+        dev_in = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
+                  for a in (w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)]
+        wf._inputs = tuple(dev_in)
+        fd.fdemri_build_splines(wf.plan, *dev_in)
+        wf.ensure_capacity()                               # grows the work space if the default list capacity is short
+        loads.append((w, wf, dev_in))
+    stream = torch.cuda.current_stream()
+
+    def one_pass():
+        for w, wf, dev_in in loads:
+            fd.fdemri_build_splines(wf.plan, *dev_in)
+            fd.fdemri_sum(wf.plan, w.theta, w.phi, wf.hplus, wf.hcross)
+
+    for _ in range(max(1, args.warmup)):
+        one_pass()
+    torch.cuda.synchronize()
+    evals = sum(wf.stats()["n_evals"] for _, wf, _ in loads)
+    peak_tf = fd.fdemri_measure_fp64_peak(1 << 16)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    kern_ms = 0.0
+    for _ in range(args.steps):
+        one_pass()
+    e1.record(stream)
+    e1.synchronize()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = fdist.max_over_ranks(e0.elapsed_time(e1), device=dev)
+    all_items = fdist.sum_over_ranks(len(mine), device=dev)
+    all_evals = fdist.sum_over_ranks(evals, device=dev)
+    if rank == 0:
+        secs = total_ms * 1e-3 / args.steps
+        achieved = all_evals * FLOP_PER_EVAL / secs * 1e-12 / world
+        line = {"metric": "waveforms/s, batched 3843-mode 1-yr FD sums (FP64)", "value": all_items / secs,
+                "unit": "waveforms/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": f"BASELINE config 4: first {args.items} of the 1024 seeded parameter sets (M log-uniform "
+                                       f"1e5..1e7, e0 0..0.5, T = 1 yr, 100 knots, 3843 modes, 1577909 bins), chunks of {chunk}",
+                           "step": "fdemri_build_splines + fdemri_sum per chunk, one launch sequence",
+                           "l2": "inputs and outputs of a pass exceed L2", "parallelism": "items sharded over ranks, no collective"},
+                "evals_per_step": all_evals, "evals_per_s": all_evals / secs,
+                "gpu_launches": KERNELS_PER_STEP * args.steps * len(chunks),
+                "roofline": {"bound": "alu", "kernel": "whole pass (k_tile_sum dominates)", "achieved": achieved, "peak": peak_tf,
+                             "unit": "TFLOP/s", "frac": achieved / peak_tf, "traffic": None, "flop_per_eval": FLOP_PER_EVAL},
+                "clocks": clocks}
+        print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -141,6 +206,8 @@ def main():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--items", type=int, default=64, help="config 4: parameter sets (of the 1024) to evaluate")
+    ap.add_argument("--chunk", type=int, default=16, help="config 4: parameter sets per plan / launch sequence")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
@@ -150,9 +217,8 @@ def main():
     import torch.distributed as dist
     import paper_2307_12585_b200 as fd
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2307_12585_b200 import dist as fdist
+    rank, world, local = fdist.env_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; there is no CPU fallback (use --impl reference for the oracle)")
     torch.cuda.set_device(local)
@@ -161,9 +227,11 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device(dev))
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        fdist.barrier()
         torch.cuda.synchronize()
+
+    if args.config == 4:
+        return run_batched(args, fd, fdist, torch, dev, rank, world, local, barrier)
 
     w = load_workload(args.config)
     FLAG_TIMING = 1
@@ -184,6 +252,7 @@ def main():
     st = wf.stats()
     n_evals = st["n_evals"]
     peak_tf = fd.fdemri_measure_fp64_peak(1 << 16)
+    peak3_tf = fd.fdemri_measure_fp64_peak_3reg(1 << 16)
 
     # ---- timed: K steps, L2 flushed between steps, CUDA events on the launching stream ----
     sampler = ClockSampler(local)
@@ -205,11 +274,7 @@ def main():
         kern_ms.append(fd.fdemri_get_kernel_ms(wf.plan))
     barrier()
     clocks = sampler.stop() if rank == 0 else None
-    total_ms = float(sum(step_ms))
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = fdist.max_over_ranks(float(sum(step_ms)), device=dev)
 
     # ---- end to end through host buffers (pinned H2D of inputs, D2H of both polarisations) ----
     e2e = None
@@ -240,10 +305,7 @@ def main():
             b.synchronize()
             ems += a.elapsed_time(b)
         barrier()
-        if world > 1:
-            t = torch.tensor([ems], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ems = float(t.item())
+        ems = fdist.max_over_ranks(ems, device=dev)
         e2e = {"value": world * args.steps / (ems * 1e-3), "unit": "waveforms/s", "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "ms_per_step": ems / args.steps}
 
@@ -267,7 +329,10 @@ def main():
                          "frac": achieved / peak_tf, "traffic": None, "kernel_ms": k_ms,
                          "flop_per_eval": FLOP_PER_EVAL,
                          "peak_source": "FP64 DFMA loop measured live (fdemri_measure_fp64_peak); nominal 148 SM x 64 "
-                                        "lanes x 2 x 1.965 GHz = 37.2 TFLOP/s; MEASURED_PEAKS.json has no FP64 entry"},
+                                        "lanes x 2 x 1.965 GHz = 37.2 TFLOP/s; MEASURED_PEAKS.json has no FP64 entry",
+                         "peak_3reg": peak3_tf, "frac_of_peak_3reg": achieved / peak3_tf,
+                         "peak_3reg_note": "the same loop with three distinct register operands per DFMA (the form "
+                                           "of most DFMAs here): register-file read bandwidth caps it at ~2/3"},
             "clocks": clocks, "stats": st,
         }
         if e2e:

@@ -90,6 +90,8 @@ int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, int n_
  * fdemri_stats.n_pairs reports what the last build needed (see FDEMRI_BAD_LIST_OVERFLOW).  fdemri_set_workspace
  * may be called again with a larger buffer; fdemri_build_splines must then be repeated. */
 size_t fdemri_workspace_bytes(fdemri_plan_t plan);
+/* The fixed part alone (no room for a work list worth the name): the least fdemri_set_workspace accepts. */
+size_t fdemri_workspace_bytes_min(fdemri_plan_t plan);
 int fdemri_set_workspace(fdemri_plan_t plan, void* dev_ptr, size_t bytes);
 
 /* S1.  All inputs are device pointers, borrowed until the enqueued kernels have run.
@@ -123,6 +125,9 @@ int fdemri_get_kernel_ms(fdemri_plan_t plan, float* ms_out);
 /* FP64 FMA peak of the current device measured with a register-resident DFMA loop (the roofline denominator
  * of the ALU-bound tile kernel): writes TFLOP/s (2 flop per DFMA).  Synchronous; n_iters ~ 1<<16. */
 int fdemri_measure_fp64_peak(int n_iters, double* tflops_out);
+/* The same loop with three distinct, changing register operands per DFMA (a_i <- a_i*b_i + b_j): the rate a
+ * general FP64 kernel can reach; on B200 about 2/3 of the figure above (register-file read bandwidth). */
+int fdemri_measure_fp64_peak_3reg(int n_iters, double* tflops_out);
 
 int fdemri_destroy(fdemri_plan_t plan);
 const char* fdemri_strerror(int status);

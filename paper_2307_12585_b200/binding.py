@@ -19,8 +19,8 @@ FDEMRI_OK = 0
 STATUS = {0: "FDEMRI_OK", 1: "FDEMRI_ERR_INVALID_ARG", 2: "FDEMRI_ERR_WORKSPACE", 3: "FDEMRI_ERR_CUDA",
           4: "FDEMRI_ERR_NOT_BUILT", 5: "FDEMRI_ERR_UNSUPPORTED"}
 
-EXPORTS = ["fdemri_plan", "fdemri_workspace_bytes", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum",
-           "fdemri_get_stats", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
+EXPORTS = ["fdemri_plan", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum",
+           "fdemri_get_stats", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_measure_fp64_peak_3reg", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
 
 
 class FdemriStats(C.Structure):
@@ -51,6 +51,8 @@ def lib() -> C.CDLL:
                                   C.c_double, C.c_uint32]
         L.fdemri_workspace_bytes.restype = C.c_size_t
         L.fdemri_workspace_bytes.argtypes = [vp]
+        L.fdemri_workspace_bytes_min.restype = C.c_size_t
+        L.fdemri_workspace_bytes_min.argtypes = [vp]
         L.fdemri_set_workspace.restype = C.c_int
         L.fdemri_set_workspace.argtypes = [vp, vp, C.c_size_t]
         L.fdemri_build_splines.restype = C.c_int
@@ -65,6 +67,8 @@ def lib() -> C.CDLL:
         L.fdemri_get_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
         L.fdemri_measure_fp64_peak.restype = C.c_int
         L.fdemri_measure_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
+        L.fdemri_measure_fp64_peak_3reg.restype = C.c_int
+        L.fdemri_measure_fp64_peak_3reg.argtypes = [C.c_int, C.POINTER(C.c_double)]
         L.fdemri_destroy.restype = C.c_int
         L.fdemri_destroy.argtypes = [vp]
         L.fdemri_strerror.restype = C.c_char_p
@@ -108,6 +112,10 @@ def fdemri_plan(lmn, n_batch, n_knots, t_knots, n_freq, freq=None, f0=0.0, df=0.
 
 def fdemri_workspace_bytes(plan) -> int:
     return int(lib().fdemri_workspace_bytes(plan))
+
+
+def fdemri_workspace_bytes_min(plan) -> int:
+    return int(lib().fdemri_workspace_bytes_min(plan))
 
 
 def fdemri_set_workspace(plan, ws):
@@ -154,6 +162,12 @@ def fdemri_measure_fp64_peak(n_iters=1 << 16) -> float:
     return float(tf.value)
 
 
+def fdemri_measure_fp64_peak_3reg(n_iters=1 << 16) -> float:
+    tf = C.c_double()
+    _chk("fdemri_measure_fp64_peak_3reg", lib().fdemri_measure_fp64_peak_3reg(int(n_iters), C.byref(tf)))
+    return float(tf.value)
+
+
 def fdemri_destroy(plan):
     _chk("fdemri_destroy", lib().fdemri_destroy(plan))
 
@@ -178,14 +192,35 @@ class Waveform:
         self.t_knots = torch.from_numpy(t_knots).to(self.dev)
         self.freqs = None if freqs is None else torch.from_numpy(np.ascontiguousarray(freqs, dtype=np.float64)).to(self.dev)
         self.plan = fdemri_plan(self.lmn, self.n_batch, self.n_knots, self.t_knots, self.n_freq, self.freqs, f0, df, flags)
-        nbytes = fdemri_workspace_bytes(self.plan)
-        self.ws = torch.empty((nbytes + 255) // 8 + 32, dtype=torch.float64, device=self.dev)
-        off = (-self.ws.data_ptr()) % 256
-        self.ws_view = self.ws.view(torch.uint8)[off:off + nbytes]
-        fdemri_set_workspace(self.plan, self.ws_view)
+        self._alloc_workspace(fdemri_workspace_bytes(self.plan))
         self.hplus = torch.empty((self.n_batch, self.n_freq, 2), dtype=torch.float64, device=self.dev)
         self.hcross = torch.empty_like(self.hplus)
         self._inputs = None
+
+    def _alloc_workspace(self, nbytes):
+        torch = self.torch
+        self.ws = None                                      # release the old buffer first
+        self.ws = torch.empty((nbytes + 255) // 8 + 32, dtype=torch.float64, device=self.dev)
+        off = (-self.ws.data_ptr()) % 256
+        self.ws_view = self.ws.view(torch.uint8)[off:off + nbytes]
+        self.ws_bytes = nbytes
+        fdemri_set_workspace(self.plan, self.ws_view)
+
+    def ensure_capacity(self, stream=None) -> bool:
+        """Synchronises.  If the last build reported FDEMRI_BAD_LIST_OVERFLOW (the per-tile work list did not fit),
+        allocates a work space with room for fdemri_stats.n_pairs entries and builds again.  Returns True if it
+        had to.  (Marshalling only: the C library never allocates.)"""
+        st = fdemri_get_stats(self.plan, check=False)
+        if not (st["flags"] & 16):
+            return False
+        extra = 4 * int(st["n_pairs"] * 1.1) + 4096
+        self._alloc_workspace(fdemri_workspace_bytes(self.plan) + extra)
+        assert self._inputs is not None
+        fdemri_build_splines(self.plan, *self._inputs, stream=stream)
+        st = fdemri_get_stats(self.plan, check=False)
+        if st["flags"] & 16:
+            raise FdemriError("fdemri_build_splines (work list still does not fit)", 2)
+        return True
 
     def build_splines(self, f_phi, f_r, Phi_phi, Phi_r, amp, stream=None):
         """Arguments: CUDA tensors, or numpy arrays (copied to the device first)."""
@@ -233,4 +268,5 @@ class Waveform:
 def waveform_from_workload(w, device="cuda:0", flags=0) -> Waveform:
     wf = Waveform(w.lmn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df, device=device, flags=flags)
     wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)
+    wf.ensure_capacity()
     return wf

@@ -139,6 +139,12 @@ extern "C" size_t fdemri_workspace_bytes(fdemri_plan_t p) {
     return carve(&tmp, nullptr) + align_up(pairs * sizeof(unsigned int));
 }
 
+extern "C" size_t fdemri_workspace_bytes_min(fdemri_plan_t p) {
+    if (!p) return 0;
+    fdemri_plan_s tmp = *p;
+    return carve(&tmp, nullptr) + 256;
+}
+
 extern "C" int fdemri_set_workspace(fdemri_plan_t p, void* dev_ptr, size_t bytes) {
     if (!p || !dev_ptr) return FDEMRI_ERR_INVALID_ARG;
     if (((uintptr_t)dev_ptr & 255) != 0) return FDEMRI_ERR_INVALID_ARG;
@@ -323,20 +329,28 @@ extern "C" int fdemri_get_kernel_ms(fdemri_plan_t p, float* ms_out) {
     return FDEMRI_OK;
 }
 
-// 8 independent DFMA chains per thread, all in registers
+// 8 independent DFMA chains per thread, all in registers.  REG3 = false: a <- a*m + c with loop-invariant m, c (one
+// fresh register operand per instruction: the classic peak loop).  REG3 = true: a_i <- a_i*b_i + b_j with three
+// distinct, changing register operands -- the form of most DFMAs of a real kernel; on B200 this issues every
+// three cycles per SM sub-partition instead of every two (register-file read bandwidth).
+template <bool REG3>
 __global__ void __launch_bounds__(512) k_dfma_peak(int n_iters, double seed, double* sink) {
-    double a0 = seed + threadIdx.x, a1 = a0 + 1.0, a2 = a0 + 2.0, a3 = a0 + 3.0, a4 = a0 + 4.0, a5 = a0 + 5.0,
-           a6 = a0 + 6.0, a7 = a0 + 7.0;
+    double a[8], b[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { a[i] = seed + threadIdx.x + i; b[i] = 0.999999 + 1e-9 * (threadIdx.x + i); }
     const double m = 0.999999, c = 1e-9;
-    for (int i = 0; i < n_iters; ++i) {
-        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
-        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    for (int it = 0; it < n_iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) a[i] = REG3 ? fma(a[i], b[i], b[(i + 3) & 7]) : fma(a[i], m, c);
     }
-    double r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+    double r = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) r += a[i];
     if (r == 12345.678) sink[0] = r;     // never true; keeps the chains alive
 }
 
-extern "C" int fdemri_measure_fp64_peak(int n_iters, double* tflops_out) {
+template <bool REG3>
+static int measure_peak(int n_iters, double* tflops_out) {
     if (!tflops_out || n_iters < 1) return FDEMRI_ERR_INVALID_ARG;
     int dev = 0;
     cudaDeviceProp prop;
@@ -347,11 +361,11 @@ extern "C" int fdemri_measure_fp64_peak(int n_iters, double* tflops_out) {
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
     const int threads = 512, blocks = prop.multiProcessorCount * 4;
-    k_dfma_peak<<<blocks, threads>>>(n_iters / 8 + 1, 1.0, sink);    // warm-up
+    k_dfma_peak<REG3><<<blocks, threads>>>(n_iters / 8 + 1, 1.0, sink);    // warm-up
     float best = 1e30f;
     for (int rep = 0; rep < 3; ++rep) {
         cudaEventRecord(e0);
-        k_dfma_peak<<<blocks, threads>>>(n_iters, 1.0, sink);
+        k_dfma_peak<REG3><<<blocks, threads>>>(n_iters, 1.0, sink);
         cudaEventRecord(e1);
         cudaEventSynchronize(e1);
         float ms = 0.f;
@@ -366,6 +380,9 @@ extern "C" int fdemri_measure_fp64_peak(int n_iters, double* tflops_out) {
     *tflops_out = flops / (best * 1e-3) * 1e-12;
     return FDEMRI_OK;
 }
+
+extern "C" int fdemri_measure_fp64_peak(int n_iters, double* tflops_out) { return measure_peak<false>(n_iters, tflops_out); }
+extern "C" int fdemri_measure_fp64_peak_3reg(int n_iters, double* tflops_out) { return measure_peak<true>(n_iters, tflops_out); }
 
 extern "C" int fdemri_destroy(fdemri_plan_t p) {
     if (!p) return FDEMRI_ERR_INVALID_ARG;

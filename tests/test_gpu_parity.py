@@ -229,3 +229,46 @@ def test_edge_cases(fd, orc):
         fd.fdemri_sum(p, 0.1, 0.2, out, out)                                               # no work space
     assert ei.value.status == 2
     fd.fdemri_destroy(p)
+
+
+def test_work_list_overflow_is_loud_then_recovers(fd, orc):
+    """A work space with no room for the per-tile work list: fdemri_sum must fill NaN and get_stats must say
+    FDEMRI_ERR_WORKSPACE with the number of pairs needed; Waveform.ensure_capacity then makes it work."""
+    import torch
+    w = workload(0)
+    wf = fd.Waveform(w.lmn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df)
+    nmin = fd.fdemri_workspace_bytes_min(wf.plan)
+    assert nmin < fd.fdemri_workspace_bytes(wf.plan)
+    wf._alloc_workspace(nmin)                                    # capacity: 64 pairs
+    wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)
+    wf.sum(w.theta, w.phi)
+    hp, hx = wf.result()
+    st = wf.stats(check=False)
+    assert st["status"] == 2 and (st["flags"] & 16) and st["n_pairs"] > 64
+    assert np.all(np.isnan(hp.view(np.float64))) and np.all(np.isnan(hx.view(np.float64)))
+    assert wf.ensure_capacity() is True
+    wf.sum(w.theta, w.phi)
+    hp, hx = wf.result()
+    ref = oracle_c(orc, w, w.freq_array())
+    check(hp[0], hx[0], ref, "config0 after growing the work space")
+    assert wf.stats()["n_evals"] == ref["n_evals"]
+    wf.close()
+
+
+def test_many_voices_in_one_tile(fd, orc):
+    """More entries in a tile than the shared-memory sorter takes (FDEMRI_SORT_MAX = 8192): the in-place global
+    sort must give the same fixed order.  9000 voices (l = 2, m = 2, n = 0) all cover the same bins."""
+    from paper_2307_12585_b200 import synth
+    base = synth.small_case(seed=3, n_knots=6, n_freq=3000, modes=((2, 2, 0),), turnover=False)
+    nv = 9000
+    base.lmn = np.repeat(base.lmn, nv, axis=0)
+    rng = np.random.Generator(np.random.PCG64(7))
+    scale = rng.uniform(0.5, 1.5, (1, nv, 1, 1))
+    base.amp = np.ascontiguousarray(np.repeat(base.amp, nv, axis=1) * scale)
+    wf, hp, hx, st = run_gpu(fd, base)
+    ref = oracle_c(orc, base, base.freq_array())
+    check(hp[0], hx[0], ref, "9000 voices in one tile")
+    assert st["n_evals"] == ref["n_evals"]
+    wf2, hp2, hx2, _ = run_gpu(fd, base)                         # and it is reproducible bit for bit
+    assert np.array_equal(hp, hp2) and np.array_equal(hx, hx2)
+    wf.close(); wf2.close()
