@@ -27,7 +27,15 @@ sys.path.insert(0, ROOT)
 
 METRIC = "waveforms/s, 3843-mode 2-yr FD sum (FP64)"
 FLOP_PER_EVAL = 200.0          # SURVEY.md 8(d) / DESIGN.md: algorithmic FP64 flop per mode-bin evaluation
+TILE_SUM_DRAM_BYTES = 174.7e6    # ncu capture of config 2, profiles/r1f_tile_v3.md
 KERNELS_PER_STEP = 8           # spline_shared, spline_amp, records, pair_scan, pair_fill, pair_sort | weights, tile_sum
+
+
+def workload_name(idx, w):
+    if idx == 2:
+        return (f"BASELINE config 2: 3843 modes l=2..10,n=-30..30; M=2e6, e0=0.4, 2 yr, 150 knots; uniform grid "
+                f"{w.n_freq} bins (dt=10 s)")
+    return f"BASELINE config {idx}"
 
 
 def load_workload(idx):
@@ -124,7 +132,7 @@ def run_reference(args):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / max(1, args.steps),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f80 (x87 long double)",
             "data": "synthetic",
-            "config": {"workload": f"BASELINE config {args.config} (3843 modes, 2 yr, dt=10 s), 30000-bin samples"},
+            "config": {"workload": workload_name(args.config, w), "sample": "30000 random bins of the covered band per step"},
             "cpu_baseline": {"value": val, "unit": "waveforms/s", "cores": orc.num_threads, "kind": "oracle",
                              "sample": "each step: 30000 random bins of the covered band incl. spline build, scaled by "
                                        "evaluation count (3.299e8 per waveform)"},
@@ -140,28 +148,56 @@ def run_batched(args, fd, fdist, torch, dev, rank, world, local, barrier):
     mine = fdist.shard_range(args.items, world, rank)
     chunk = args.chunk
     chunks = [list(mine)[i:i + chunk] for i in range(0, len(mine), chunk)]
-    # generate and upload all chunks first (untimed), keep every output resident
+    # generate and upload all chunks first (untimed); every input and output stays resident in HBM, the work
+    # space is ONE buffer shared by the plans of all chunks (a chunk's sum is enqueued right after its build)
     loads = []
+    ws = None
+    ws_bytes = 0
+
+    def give_workspace(plan, need):
+        nonlocal ws, ws_bytes
+        if need > ws_bytes:
+            ws = None
+            ws_bytes = int(need * 1.25) + (1 << 20)
+            ws = torch.empty(ws_bytes // 8 + 64, dtype=torch.float64, device=dev)
+            for ld in loads:                                # re-point the plans made so far
+                fd.fdemri_set_workspace(ld["plan"], ws_view())
+        fd.fdemri_set_workspace(plan, ws_view())
+
+    def ws_view():
+        off = (-ws.data_ptr()) % 256
+        return ws.view(torch.uint8)[off:off + ws_bytes]
+
     for ids in chunks:
         w = synth.config4(items=ids)
-        wf = fd.Waveform(w.lmn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df, device=dev, flags=1)
+        t_knots = torch.from_numpy(np.ascontiguousarray(w.t_knots)).to(dev)
+        plan = fd.fdemri_plan(w.lmn, w.n_batch, w.n_knots, t_knots, w.n_freq, None, w.f0, w.df, 0)
         dev_in = [torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
                   for a in (w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)]
-        wf._inputs = tuple(dev_in)
-        fd.fdemri_build_splines(wf.plan, *dev_in)
-        wf.ensure_capacity()                               # grows the work space if the default list capacity is short
-        loads.append((w, wf, dev_in))
+        hp = torch.empty((w.n_batch, w.n_freq, 2), dtype=torch.float64, device=dev)
+        hx = torch.empty_like(hp)
+        ld = dict(plan=plan, t_knots=t_knots, dev_in=dev_in, hp=hp, hx=hx, theta=w.theta, phi=w.phi)
+        give_workspace(plan, fd.fdemri_workspace_bytes(plan))
+        fd.fdemri_build_splines(plan, *dev_in)
+        st = fd.fdemri_get_stats(plan, check=False)
+        if st["flags"] & 16:                                # work list larger than the default capacity: grow
+            give_workspace(plan, fd.fdemri_workspace_bytes(plan) + 4 * int(st["n_pairs"] * 1.1))
+            fd.fdemri_build_splines(plan, *dev_in)
+            st = fd.fdemri_get_stats(plan, check=True)
+        ld["n_evals"] = st["n_evals"]
+        loads.append(ld)
+        del w
     stream = torch.cuda.current_stream()
 
     def one_pass():
-        for w, wf, dev_in in loads:
-            fd.fdemri_build_splines(wf.plan, *dev_in)
-            fd.fdemri_sum(wf.plan, w.theta, w.phi, wf.hplus, wf.hcross)
+        for ld in loads:
+            fd.fdemri_build_splines(ld["plan"], *ld["dev_in"])
+            fd.fdemri_sum(ld["plan"], ld["theta"], ld["phi"], ld["hp"], ld["hx"])
 
     for _ in range(max(1, args.warmup)):
         one_pass()
     torch.cuda.synchronize()
-    evals = sum(wf.stats()["n_evals"] for _, wf, _ in loads)
+    evals = sum(ld["n_evals"] for ld in loads)
     peak_tf = fd.fdemri_measure_fp64_peak(1 << 16)
     sampler = ClockSampler(local)
     if rank == 0:
@@ -336,9 +372,7 @@ def main():
             "metric": METRIC, "value": world * args.steps / (total_ms * 1e-3), "unit": "waveforms/s",
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"BASELINE config {args.config}: 3843 modes l=2..10,n=-30..30; M=2e6, e0=0.4, 2 yr, "
-                                   f"150 knots; uniform grid {w.n_freq} bins (dt=10 s)" if args.config == 2 else
-                                   f"BASELINE config {args.config}",
+            "config": {"workload": workload_name(args.config, w),
                        "step": "fdemri_build_splines + fdemri_sum (S0-S4)", "l2": "flushed between steps (512 MB fill)",
                        "parallelism": "replicas, one waveform per GPU, no collective"},
             "ms_per_waveform": total_ms / args.steps, "evals_per_waveform": n_evals,
@@ -346,7 +380,10 @@ def main():
             "ms_build_splines": float(np.mean(step_ms) - np.mean(sum_ms)), "ms_sum": float(np.mean(sum_ms)),
             "gpu_launches": KERNELS_PER_STEP * args.steps,
             "roofline": {"bound": "alu", "kernel": "k_tile_sum", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
-                         "frac": achieved / peak_tf, "traffic": None, "kernel_ms": k_ms,
+                         "frac": achieved / peak_tf, "traffic": TILE_SUM_DRAM_BYTES if args.config == 2 else None,
+                         "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of one k_tile_sum launch, ncu --set full "
+                                         "(profiles/r1f_tile_v3.md); bytes, for context: the bound is the FP64 pipe",
+                         "kernel_ms": k_ms,
                          "flop_per_eval": FLOP_PER_EVAL,
                          "peak_source": "FP64 DFMA loop measured live (fdemri_measure_fp64_peak); nominal 148 SM x 64 "
                                         "lanes x 2 x 1.965 GHz = 37.2 TFLOP/s; MEASURED_PEAKS.json has no FP64 entry",

@@ -164,11 +164,8 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
     dd bq = dd_mul(Pb, inv2pi);
     double tk = t_knots[(size_t)b * d.n_knots + k];
     double h = __dadd_rn(t_knots[(size_t)b * d.n_knots + k + 1], -tk);
-    R[R_FA] = FA; R[R_FB] = FB; R[R_FC] = FC; R[R_FD] = FD;
-    R[R_PC] = pc; R[R_BH] = bq.hi; R[R_BL] = bq.lo;
-    R[R_NC] = -dd_mul(Pc, inv2pi).hi;
-    R[R_ND] = -dd_mul(Pd, inv2pi).hi;
-    R[R_TK] = tk; R[R_H] = h;
+    // the record is written as four 32-byte stores at the end (slots 8..15 belong to k_spline_amp)
+    double rQ1, rQ2, rQ3, rTYPE, rSF;
     // interior extrema of F on (0, h): roots of FB + 2 FC t + 3 FD t^2
     double ext[2]; int ne = 0;
     {
@@ -202,23 +199,30 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
             double idF = 1.0 / dF;
             q1 = alp * idF; q2 = bet * idF * idF; q3 = gam * idF * idF * idF;
         }
-        R[R_Q1] = q1; R[R_Q2] = q2; R[R_Q3] = q3; R[R_TYPE] = 0.0;
-        R[R_SF] = (dF < 0.0) ? -1.0 : 1.0;
+        rQ1 = q1; rQ2 = q2; rQ3 = q3; rTYPE = 0.0;
+        rSF = (dF < 0.0) ? -1.0 : 1.0;
     } else if (ne == 1) {
         double te = ext[0];
-        R[R_Q1] = te;
-        R[R_Q2] = FA + te * (FB + te * (FC + te * FD));     // F_e (R7)
-        R[R_Q3] = FC + 3.0 * FD * te;                        // F(t) - F_e = z^2 (Q3 + FD z), z = t - te
-        R[R_TYPE] = 1.0;
-        R[R_SF] = (R[R_Q2] < FA) ? -1.0 : 1.0;               // first branch runs from F_k to F_e
+        rQ1 = te;
+        rQ2 = FA + te * (FB + te * (FC + te * FD));          // F_e (R7)
+        rQ3 = FC + 3.0 * FD * te;                            // F(t) - F_e = z^2 (Q3 + FD z), z = t - te
+        rTYPE = 1.0;
+        rSF = (rQ2 < FA) ? -1.0 : 1.0;                       // first branch runs from F_k to F_e
         atomicAdd(stats + 3, 1ull);
     } else {
-        R[R_Q1] = 0.0; R[R_Q2] = 0.0; R[R_Q3] = 0.0; R[R_TYPE] = 2.0; R[R_SF] = 1.0;
+        rQ1 = 0.0; rQ2 = 0.0; rQ3 = 0.0; rTYPE = 2.0; rSF = 1.0;
         atomicOr(stats + 5, 1ull);                           // FDEMRI_BAD_TWO_EXTREMA
     }
     if (bad) atomicOr(stats + 5, 4ull);
     // ---- bin intervals of the branches of this segment, for both signs (L105) ----
-    const int type = (int)R[R_TYPE];
+    {
+        double4* R4 = reinterpret_cast<double4*>(R);        // rec is 256-byte aligned, records are 192 bytes
+        R4[0] = make_double4(FA, FB, FC, FD);
+        R4[1] = make_double4(rQ1, rQ2, rQ3, h);
+        R4[4] = make_double4(pc, bq.hi, bq.lo, -dd_mul(Pc, inv2pi).hi);
+        R4[5] = make_double4(-dd_mul(Pd, inv2pi).hi, tk, rTYPE, rSF);
+    }
+    const int type = (int)rTYPE;
     const double Fk = FA;
     const double Fk1 = (k + 1 < d.n_seg) ? fdemri_knotF(m, n, hi[4], hi[per + 4])
                                          : fdemri_knotF(m, n, f_phi[(size_t)b * d.n_knots + d.n_knots - 1],
@@ -232,8 +236,8 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
             if (type != 2 && (br == 0 || type == 1)) {
                 double Va, Vb; bool a_incl, b_incl;
                 if (type == 0) { Va = Fk; Vb = Fk1; a_incl = true; b_incl = false; }
-                else if (br == 0) { Va = Fk; Vb = R[R_Q2]; a_incl = true; b_incl = true; }
-                else { Va = R[R_Q2]; Vb = Fk1; a_incl = false; b_incl = false; }
+                else if (br == 0) { Va = Fk; Vb = rQ2; a_incl = true; b_incl = true; }
+                else { Va = rQ2; Vb = Fk1; a_incl = false; b_incl = false; }
                 if (Va != Vb) {
                     const double lo_v = fmin(Va, Vb), hi_v = fmax(Va, Vb);
                     const bool lo_incl = (Va < Vb) ? a_incl : b_incl;

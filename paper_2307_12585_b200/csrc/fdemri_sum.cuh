@@ -476,8 +476,16 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
             double T0r = 0.0, T0i = 0.0, T1r = 0.0, T1i = 0.0;
             bool ok0 = false, ok1 = false;
             if (!(flags & 1u)) {
-                ok0 = fdemri_term_fast(it, sf0, T0r, T0i);
-                ok1 = fdemri_term_fast(it, sf1, T1r, T1i);
+                // an item that ends inside this warp's 64 bins may leave one of the two slots without any lane
+                const bool any0 = lo <= wb + 31, any1 = hi >= wb + 32;       // warp-uniform
+                if (any0 && any1) {
+                    ok0 = fdemri_term_fast(it, sf0, T0r, T0i);
+                    ok1 = fdemri_term_fast(it, sf1, T1r, T1i);
+                } else if (any0) {
+                    ok0 = fdemri_term_fast(it, sf0, T0r, T0i);
+                } else {
+                    ok1 = fdemri_term_fast(it, sf1, T1r, T1i);
+                }
             }
             if (act0 && !ok0) {
                 const FdemriSlowOut o = fdemri_term_slow(it, sf0, flags);

@@ -260,6 +260,7 @@ def test_many_voices_in_one_tile(fd, orc):
     sort must give the same fixed order.  9000 voices (l = 2, m = 2, n = 0) all cover the same bins."""
     from paper_2307_12585_b200 import synth
     base = synth.small_case(seed=3, n_knots=6, n_freq=3000, modes=((2, 2, 0),), turnover=False)
+    base.f0 = 4.0e-3                                             # F = 2 f_phi sweeps 4.0 .. 5.8 mHz
     nv = 9000
     base.lmn = np.repeat(base.lmn, nv, axis=0)
     rng = np.random.Generator(np.random.PCG64(7))
@@ -268,7 +269,7 @@ def test_many_voices_in_one_tile(fd, orc):
     wf, hp, hx, st = run_gpu(fd, base)
     ref = oracle_c(orc, base, base.freq_array())
     check(hp[0], hx[0], ref, "9000 voices in one tile")
-    assert st["n_evals"] == ref["n_evals"]
+    assert st["n_evals"] == ref["n_evals"] and st["n_evals"] >= 2 * nv * 2000 and st["n_pairs"] >= 3 * nv
     wf2, hp2, hx2, _ = run_gpu(fd, base)                         # and it is reproducible bit for bit
     assert np.array_equal(hp, hp2) and np.array_equal(hx, hx2)
     wf.close(); wf2.close()
