@@ -150,6 +150,25 @@ class Oracle:
                     n_evals=int(ne.value), nterms=nterms, ambiguous=amb, max_roots=int(mr.value))
 
 
+    def inner(self, hplus, hcross, dplus=None, dcross=None, w=None):
+        """Eq. 12 as a sum over the grid: (<h|h>, <d|h>) with <a|b> = sum_k w_k (a+ conj b+ + ax conj bx)."""
+        hp = np.ascontiguousarray(hplus, dtype=np.complex128)
+        hx = np.ascontiguousarray(hcross, dtype=np.complex128)
+        n = hp.shape[0]
+        args = [C.c_int64(n), None, hp.view(np.float64).ctypes.data_as(_dp), hx.view(np.float64).ctypes.data_as(_dp), None, None]
+        keep = []
+        if w is not None:
+            wa, wp = _d(w); keep.append(wa); args[1] = wp
+        if dplus is not None:
+            dp = np.ascontiguousarray(dplus, dtype=np.complex128); dx = np.ascontiguousarray(dcross, dtype=np.complex128)
+            keep += [dp, dx]
+            args[4] = dp.view(np.float64).ctypes.data_as(_dp); args[5] = dx.view(np.float64).ctypes.data_as(_dp)
+        out = np.zeros(3)
+        if self.lib.fdemri_oracle_inner(*args, out.ctypes.data_as(_dp)):
+            raise ValueError("fdemri_oracle_inner")
+        return float(out[0]), complex(out[1], out[2])
+
+
 _ORACLE = None
 
 

@@ -313,6 +313,29 @@ static ld solve_piece(const ld* c, ld x, ld ta, ld tb) {
 static int g_explicit_voices = 0;
 extern "C" void fdemri_oracle_set_explicit(int on) { g_explicit_voices = on; }
 
+/* Eq. 12, both polarisations, as the plain sum it is on a frequency grid:
+ *   <a|b> = sum_k w_k [ a+(f_k) conj b+(f_k) + ax(f_k) conj bx(f_k) ],   w_k = 4 df / S_n(f_k)  (w = 1 if NULL).
+ * The paper's inner product is the real part; the imaginary part is returned as well.  long double sums in index
+ * order.  out = {<h|h>, Re<d|h>, Im<d|h>};  d may be NULL (then only out[0] is set). */
+extern "C" int fdemri_oracle_inner(int64_t n_freq, const double* w, const double* hplus, const double* hcross,
+                                   const double* dplus, const double* dcross, double* out) {
+    if (n_freq < 0 || !hplus || !hcross || !out) return 1;
+    long double hh = 0.0L, dr = 0.0L, di = 0.0L;
+    for (int64_t k = 0; k < n_freq; ++k) {
+        const long double wk = w ? (long double)w[k] : 1.0L;
+        const long double pr = hplus[2 * k], pi = hplus[2 * k + 1], xr = hcross[2 * k], xi = hcross[2 * k + 1];
+        hh += wk * (pr * pr + pi * pi + xr * xr + xi * xi);
+        if (dplus && dcross) {
+            const long double ar = dplus[2 * k], ai = dplus[2 * k + 1], br = dcross[2 * k], bi = dcross[2 * k + 1];
+            /* d conj(h) = (ar + i ai)(pr - i pi) */
+            dr += wk * (ar * pr + ai * pi + br * xr + bi * xi);
+            di += wk * (ai * pr - ar * pi + bi * xr - br * xi);
+        }
+    }
+    out[0] = (double)hh; out[1] = (double)dr; out[2] = (double)di;
+    return 0;
+}
+
 static int sum_impl(int n_modes, const int32_t* lmn, int N, const double* t,
                     const double* fphi_k, const double* fr_k,
                     const ld* sh,      // [4][N-1][4]

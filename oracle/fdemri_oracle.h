@@ -71,6 +71,11 @@ int fdemri_oracle_waveform(int n_modes, const int32_t* lmn, int n_knots, const d
                            int64_t* n_evals, int32_t* nterms, uint8_t* ambiguous, int32_t* max_roots,
                            int n_threads);
 
+/* Eq. 12 (L134-141) on a frequency grid, both polarisations: <a|b> = sum_k w_k [a+ conj b+ + ax conj bx],
+ * w_k = 4 df / S_n(f_k) (NULL: w = 1).  hplus, hcross, dplus, dcross: [n_freq][2].  out = {<h|h>, Re<d|h>, Im<d|h>}. */
+int fdemri_oracle_inner(int64_t n_freq, const double* w, const double* hplus, const double* hcross,
+                        const double* dplus, const double* dcross, double* out);
+
 int fdemri_oracle_num_threads(void);
 /* Test switch for pin P7: list voices stand for themselves only (m of either sign, no implied partner). */
 void fdemri_oracle_set_explicit(int on);

@@ -178,3 +178,22 @@ def test_regular_form_at_zero_slope(orc):
         y = (3 * X / 2) ** (mp.mpf(2) / 3)
         ref = mp.e ** (-1j * X) * mp.pi * (mp.pi * abs(Fdd)) ** (-mp.mpf(1) / 3) * (mp.airyai(-y) - 1j * mp.airybi(-y))
         assert abs(a - complex(ref)) < 1e-13 * abs(ref)
+
+
+def test_inner_product_is_the_weighted_dot_product(orc):
+    """Pin of fdemri_oracle_inner (Eq. 12): equals numpy's vdot on random arrays (library
+    routine); <h|h> = sum |h|^2 for w = 1; Hermitian: <d|h> = conj <h|d>; linear in w."""
+    rng = np.random.default_rng(5)
+    n = 1000
+    hp, hx, dp, dx = (rng.standard_normal(n) + 1j * rng.standard_normal(n) for _ in range(4))
+    w = rng.uniform(0.1, 2.0, n)
+    hh, dh = orc.inner(hp, hx, dp, dx, w)
+    want_hh = np.sum(w * (np.abs(hp) ** 2 + np.abs(hx) ** 2))
+    want_dh = np.vdot(hp, w * dp) + np.vdot(hx, w * dx)            # vdot conjugates its first argument
+    assert abs(hh - want_hh) <= 1e-12 * want_hh and abs(dh - want_dh) <= 1e-12 * abs(want_dh)
+    hh1, _ = orc.inner(hp, hx)
+    assert abs(hh1 - (np.vdot(hp, hp) + np.vdot(hx, hx)).real) <= 1e-12 * hh1
+    _, hd = orc.inner(dp, dx, hp, hx, w)
+    assert abs(hd - np.conj(dh)) <= 1e-12 * abs(dh)
+    hh2, dh2 = orc.inner(hp, hx, dp, dx, 3.0 * w)
+    assert abs(hh2 - 3.0 * hh) <= 1e-12 * hh2 and abs(dh2 - 3.0 * dh) <= 1e-12 * abs(dh2)
