@@ -109,6 +109,20 @@ int fdemri_build_splines(fdemri_plan_t plan, const double* f_phi, const double* 
 int fdemri_sum(fdemri_plan_t plan, int n_angles, const double* theta_host, const double* phi_host,
                double* hplus_dev, double* hcross_dev, void* cuda_stream);
 
+/* S0 + S3 + S4 with the noise-weighted inner products of Eq. 12 (the likelihood of Eq. 13,
+ * L151-153) accumulated on the fly, so that the waveform need not be written to memory:
+ *     <a|b> = sum_k w_k [ a+(f_k) conj b+(f_k) + ax(f_k) conj bx(f_k) ]
+ * (the paper's inner product is the real part with w_k = 4 df / S_n(f_k); ln L = -(<d|d> - 2 Re<d|h> + <h|h>)/2).
+ *  weight_dev     [n_freq] w_k >= 0, shared by the batch; NULL: w = 1
+ *  data_plus_dev, data_cross_dev  [n_freq][2] (re, im) data of the two polarisations, shared by the batch; both
+ *                 NULL: only <h|h> is formed
+ *  hplus_dev, hcross_dev  as in fdemri_sum, or both NULL: nothing but the inner products leaves the kernel
+ *  inner_out_dev  [n_batch][4] = {<h|h>, Re<d|h>, Im<d|h>, 0}, device memory; sums are formed in a fixed order
+ *                 (bitwise reproducible) */
+int fdemri_sum_inner(fdemri_plan_t plan, int n_angles, const double* theta_host, const double* phi_host,
+                     const double* weight_dev, const double* data_plus_dev, const double* data_cross_dev,
+                     double* hplus_dev, double* hcross_dev, double* inner_out_dev, void* cuda_stream);
+
 /* Counters of the last fdemri_sum (synchronises the stream used by that call). */
 int fdemri_get_stats(fdemri_plan_t plan, fdemri_stats* out);
 

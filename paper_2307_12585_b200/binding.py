@@ -19,7 +19,7 @@ FDEMRI_OK = 0
 STATUS = {0: "FDEMRI_OK", 1: "FDEMRI_ERR_INVALID_ARG", 2: "FDEMRI_ERR_WORKSPACE", 3: "FDEMRI_ERR_CUDA",
           4: "FDEMRI_ERR_NOT_BUILT", 5: "FDEMRI_ERR_UNSUPPORTED"}
 
-EXPORTS = ["fdemri_plan", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum",
+EXPORTS = ["fdemri_plan", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum", "fdemri_sum_inner",
            "fdemri_get_stats", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_measure_fp64_peak_3reg", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
 
 
@@ -59,6 +59,8 @@ def lib() -> C.CDLL:
         L.fdemri_build_splines.argtypes = [vp, dp, dp, dp, dp, dp, vp]
         L.fdemri_sum.restype = C.c_int
         L.fdemri_sum.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), dp, dp, vp]
+        L.fdemri_sum_inner.restype = C.c_int
+        L.fdemri_sum_inner.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), dp, dp, dp, dp, dp, dp, vp]
         L.fdemri_get_stats.restype = C.c_int
         L.fdemri_get_stats.argtypes = [vp, C.POINTER(FdemriStats)]
         L.fdemri_get_coeffs.restype = C.c_int
@@ -134,6 +136,17 @@ def fdemri_sum(plan, theta, phi, hplus, hcross, stream=None):
     dp = C.POINTER(C.c_double)
     _chk("fdemri_sum", lib().fdemri_sum(plan, th.shape[0], th.ctypes.data_as(dp), ph.ctypes.data_as(dp), _ptr(hplus),
                                         _ptr(hcross), _stream_ptr(stream)))
+
+
+def fdemri_sum_inner(plan, theta, phi, inner_out, weight=None, data_plus=None, data_cross=None, hplus=None, hcross=None,
+                     stream=None):
+    th = np.atleast_1d(np.asarray(theta, dtype=np.float64))
+    ph = np.atleast_1d(np.asarray(phi, dtype=np.float64))
+    assert th.shape == ph.shape
+    dp = C.POINTER(C.c_double)
+    _chk("fdemri_sum_inner", lib().fdemri_sum_inner(plan, th.shape[0], th.ctypes.data_as(dp), ph.ctypes.data_as(dp),
+                                                    _ptr(weight), _ptr(data_plus), _ptr(data_cross), _ptr(hplus),
+                                                    _ptr(hcross), _ptr(inner_out), _stream_ptr(stream)))
 
 
 def fdemri_get_stats(plan, check=True) -> dict:

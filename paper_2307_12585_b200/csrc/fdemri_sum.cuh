@@ -40,6 +40,11 @@ struct SumArgs {
     unsigned int* tile_counter;
     unsigned long long* stats;
     int total_tiles;
+    // fused inner products (Eq. 12): all NULL for a plain sum
+    const double* weight;     // [n_freq] w_k = 4 df / S_n(f_k), or NULL for w = 1
+    const double* dplus;      // [n_freq][2] data, + polarisation (NULL: only <h|h>)
+    const double* dcross;     // [n_freq][2]
+    double* inner_part;       // [total_tiles][FDEMRI_CWARPS][4] partial sums {<h|h>, Re<d|h>, Im<d|h>, 0}
 };
 
 // asymptotic series of g(X) e^{+i pi/4 sgn X} = sum_k i^k a_k u^k, u = 1/X, a_k = prod_j (4/9-(2j-1)^2)/(k! 8^k)
@@ -507,15 +512,51 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
             }
         }
         if (last) {
-            if (bin_a < d.n_freq) {
-                const size_t o = ((size_t)b * d.n_freq + bin_a) * 2;
-                *reinterpret_cast<double2*>(a.hp + o) = make_double2(a00, a01);
-                *reinterpret_cast<double2*>(a.hx + o) = make_double2(a02, a03);
+            const bool v0 = bin_a < d.n_freq, v1 = bin_a + 32 < d.n_freq;
+            if (a.hp) {
+                if (v0) {
+                    const size_t o = ((size_t)b * d.n_freq + bin_a) * 2;
+                    *reinterpret_cast<double2*>(a.hp + o) = make_double2(a00, a01);
+                    *reinterpret_cast<double2*>(a.hx + o) = make_double2(a02, a03);
+                }
+                if (v1) {
+                    const size_t o = ((size_t)b * d.n_freq + bin_a + 32) * 2;
+                    *reinterpret_cast<double2*>(a.hp + o) = make_double2(a10, a11);
+                    *reinterpret_cast<double2*>(a.hx + o) = make_double2(a12, a13);
+                }
             }
-            if (bin_a + 32 < d.n_freq) {
-                const size_t o = ((size_t)b * d.n_freq + bin_a + 32) * 2;
-                *reinterpret_cast<double2*>(a.hp + o) = make_double2(a10, a11);
-                *reinterpret_cast<double2*>(a.hx + o) = make_double2(a12, a13);
+            if (a.inner_part) {
+                // Eq. 12 on the fly: this warp's share of sum_k w_k (|h+|^2 + |hx|^2) and sum_k w_k (d+ conj h+ + dx conj hx),
+                // reduced over the lanes in a fixed butterfly; k_inner_reduce adds the warps in a fixed order
+                double hh = 0.0, dr = 0.0, di = 0.0;
+                if (v0) {
+                    const double w0 = a.weight ? __ldg(a.weight + bin_a) : 1.0;
+                    hh = w0 * (a00 * a00 + a01 * a01 + a02 * a02 + a03 * a03);
+                    if (a.dplus) {
+                        const double2 dp = *reinterpret_cast<const double2*>(a.dplus + 2 * bin_a);
+                        const double2 dx = *reinterpret_cast<const double2*>(a.dcross + 2 * bin_a);
+                        dr = w0 * (dp.x * a00 + dp.y * a01 + dx.x * a02 + dx.y * a03);
+                        di = w0 * (dp.y * a00 - dp.x * a01 + dx.y * a02 - dx.x * a03);
+                    }
+                }
+                if (v1) {
+                    const double w1 = a.weight ? __ldg(a.weight + bin_a + 32) : 1.0;
+                    hh += w1 * (a10 * a10 + a11 * a11 + a12 * a12 + a13 * a13);
+                    if (a.dplus) {
+                        const double2 dp = *reinterpret_cast<const double2*>(a.dplus + 2 * (bin_a + 32));
+                        const double2 dx = *reinterpret_cast<const double2*>(a.dcross + 2 * (bin_a + 32));
+                        dr += w1 * (dp.x * a10 + dp.y * a11 + dx.x * a12 + dx.y * a13);
+                        di += w1 * (dp.y * a10 - dp.x * a11 + dx.y * a12 - dx.x * a13);
+                    }
+                }
+#pragma unroll
+                for (int o = 16; o; o >>= 1) {
+                    hh += __shfl_xor_sync(0xffffffffu, hh, o);
+                    dr += __shfl_xor_sync(0xffffffffu, dr, o);
+                    di += __shfl_xor_sync(0xffffffffu, di, o);
+                }
+                if (lane == 0)
+                    *reinterpret_cast<double4*>(a.inner_part + ((size_t)gt * FDEMRI_CWARPS + cw) * 4) = make_double4(hh, dr, di, 0.0);
             }
         }
         // release the stage
@@ -555,12 +596,41 @@ __global__ void __maxnreg__(FDEMRI_MAXNREG) k_tile_sum(SumArgs a) {
         // the work list did not fit the work space: fail loudly (NaN everywhere; see fdemri_get_stats)
         const size_t n = (size_t)a.d.n_batch * a.d.n_freq * 2;
         const double nan = __longlong_as_double(0x7ff8000000000000ll);
-        for (size_t i = (size_t)blockIdx.x * blockDim.x + tid; i < n; i += (size_t)gridDim.x * blockDim.x) {
-            a.hp[i] = nan;
-            a.hx[i] = nan;
+        if (a.hp) {
+            for (size_t i = (size_t)blockIdx.x * blockDim.x + tid; i < n; i += (size_t)gridDim.x * blockDim.x) {
+                a.hp[i] = nan;
+                a.hx[i] = nan;
+            }
+        }
+        if (a.inner_part) {
+            const size_t m = (size_t)a.total_tiles * FDEMRI_CWARPS * 4;
+            for (size_t i = (size_t)blockIdx.x * blockDim.x + tid; i < m; i += (size_t)gridDim.x * blockDim.x) a.inner_part[i] = nan;
         }
         return;
     }
     if (wid == FDEMRI_CWARPS) fdemri_producer(a, ring, lane);
     else fdemri_consumer(a, ring, wid, lane);
+}
+
+// Fixed-order sum of the per-(tile, warp) partial inner products of one batch item.  One CTA per item.
+// out: [B][4] = {<h|h>, Re<d|h>, Im<d|h>, 0}
+__global__ void __launch_bounds__(256) k_inner_reduce(int n_tiles, const double* __restrict__ part, double* __restrict__ out) {
+    __shared__ double s_r[3][256];
+    const int b = blockIdx.x, tid = threadIdx.x;
+    const size_t n = (size_t)n_tiles * FDEMRI_CWARPS;
+    const double4* p = reinterpret_cast<const double4*>(part) + (size_t)b * n;
+    double hh = 0.0, dr = 0.0, di = 0.0;
+    for (size_t i = tid; i < n; i += 256) {
+        const double4 v = p[i];
+        hh += v.x; dr += v.y; di += v.z;
+    }
+    s_r[0][tid] = hh; s_r[1][tid] = dr; s_r[2][tid] = di;
+    __syncthreads();
+    for (int o = 128; o; o >>= 1) {
+        if (tid < o) {
+            s_r[0][tid] += s_r[0][tid + o]; s_r[1][tid] += s_r[1][tid + o]; s_r[2][tid] += s_r[2][tid + o];
+        }
+        __syncthreads();
+    }
+    if (tid == 0) *reinterpret_cast<double4*>(out + 4 * (size_t)b) = make_double4(s_r[0][0], s_r[1][0], s_r[2][0], 0.0);
 }

@@ -273,3 +273,49 @@ def test_many_voices_in_one_tile(fd, orc):
     wf2, hp2, hx2, _ = run_gpu(fd, base)                         # and it is reproducible bit for bit
     assert np.array_equal(hp, hp2) and np.array_equal(hx, hx2)
     wf.close(); wf2.close()
+
+
+def test_fused_inner_products_eq12(fd, orc):
+    """fdemri_sum_inner (Eq. 12) against the oracle: the oracle's own waveform, its own inner product.
+    Data = the oracle-independent seeded noise + a scaled copy of a *different* small waveform; weights random.
+    Checked with and without writing the waveform, and bit-for-bit reproducible."""
+    import torch
+    w = workload(1)
+    freq = w.freq_array()
+    ref = oracle_c(orc, w, freq)
+    rng = np.random.default_rng(11)
+    n = w.n_freq
+    scale = np.abs(ref["hplus"]).max()
+    dplus = scale * (rng.standard_normal(n) + 1j * rng.standard_normal(n))
+    dcross = scale * (rng.standard_normal(n) + 1j * rng.standard_normal(n))
+    weight = rng.uniform(0.2, 3.0, n)
+    want_hh, want_dh = orc.inner(ref["hplus"], ref["hcross"], dplus, dcross, weight)
+    want_hh1, _ = orc.inner(ref["hplus"], ref["hcross"])
+    wf = fd.waveform_from_workload(w)
+    dev = wf.dev
+    t_w = torch.from_numpy(weight).to(dev)
+    t_dp = torch.from_numpy(np.ascontiguousarray(dplus).view(np.float64).reshape(n, 2)).to(dev)
+    t_dx = torch.from_numpy(np.ascontiguousarray(dcross).view(np.float64).reshape(n, 2)).to(dev)
+    out = torch.zeros((1, 4), dtype=torch.float64, device=dev)
+    # (1) inner products only: no waveform leaves the kernel
+    fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, out, weight=t_w, data_plus=t_dp, data_cross=t_dx)
+    torch.cuda.synchronize()
+    o1 = out.cpu().numpy()[0].copy()
+    assert abs(o1[0] - want_hh) <= 1e-10 * want_hh
+    assert abs(complex(o1[1], o1[2]) - want_dh) <= 1e-10 * np.sqrt(want_hh * orc.inner(dplus, dcross, w=weight)[0])
+    # (2) with the waveform written as well: same numbers bit for bit, waveform as in fdemri_sum
+    out2 = torch.zeros_like(out)
+    fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, out2, weight=t_w, data_plus=t_dp, data_cross=t_dx, hplus=wf.hplus,
+                        hcross=wf.hcross)
+    hp, hx = wf.result()
+    assert np.array_equal(out2.cpu().numpy()[0], o1)
+    check(hp[0], hx[0], ref, "config1 via fdemri_sum_inner")
+    # (3) w = 1, no data: <h|h> = sum |h|^2
+    out3 = torch.zeros_like(out)
+    fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, out3)
+    torch.cuda.synchronize()
+    o3 = out3.cpu().numpy()[0]
+    assert abs(o3[0] - want_hh1) <= 1e-10 * want_hh1 and o3[1] == 0.0 and o3[2] == 0.0
+    print(f"[parity] fused inner products: <h|h> rel {abs(o1[0] - want_hh) / want_hh:.2e}, "
+          f"<d|h> rel {abs(complex(o1[1], o1[2]) - want_dh) / abs(want_dh):.2e}")
+    wf.close()
