@@ -277,6 +277,12 @@ def main():
     dev_in = [torch.from_numpy(a).to(dev) for a in host]
     flush = torch.empty(512 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)     # 512 MB > 126 MB L2
     stream = torch.cuda.current_stream()
+    # fused Eq. 12 inner products against seeded synthetic data (timed separately below: `fused_inner`)
+    gen = torch.Generator(device=dev); gen.manual_seed(230712585)
+    inner_w = torch.rand(w.n_freq, dtype=torch.float64, device=dev, generator=gen) + 0.5
+    inner_dp = torch.randn((w.n_freq, 2), dtype=torch.float64, device=dev, generator=gen)
+    inner_dx = torch.randn((w.n_freq, 2), dtype=torch.float64, device=dev, generator=gen)
+    inner_out = torch.zeros((w.n_batch, 4), dtype=torch.float64, device=dev)
 
     def step_device():
         fd.fdemri_build_splines(wf.plan, *dev_in)
@@ -311,6 +317,21 @@ def main():
         kern_ms.append(fd.fdemri_get_kernel_ms(wf.plan))
     barrier()
     total_ms = fdist.max_over_ranks(float(sum(step_ms)), device=dev)
+    # the same step with the inner products of Eq. 12 formed on the fly and no waveform written
+    inner_ms = []
+    for i in range(3 + args.steps):
+        flush.fill_(1.0)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        fd.fdemri_build_splines(wf.plan, *dev_in)
+        fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, inner_out, weight=inner_w, data_plus=inner_dp, data_cross=inner_dx)
+        e1.record(stream)
+        e1.synchronize()
+        if i >= 3:
+            inner_ms.append(e0.elapsed_time(e1))
+    fused_inner = {"ms_per_step": float(np.mean(inner_ms)), "waveforms_per_s": 1e3 / float(np.mean(inner_ms)),
+                   "what": "fdemri_build_splines + fdemri_sum_inner: <h|h> and <d|h> of Eq. 12 per waveform, no waveform "
+                           "written (32 B leave the GPU)", "inner": inner_out.cpu().numpy()[0, :3].tolist()}
 
     # ---- end to end through host buffers (pinned H2D of inputs, D2H of both polarisations) ----
     e2e = None
@@ -390,7 +411,7 @@ def main():
                          "peak_3reg": peak3_tf, "frac_of_peak_3reg": achieved / peak3_tf,
                          "peak_3reg_note": "the same loop with three distinct register operands per DFMA (the form "
                                            "of most DFMAs here): register-file read bandwidth caps it at ~2/3"},
-            "clocks": clocks, "stats": st,
+            "clocks": clocks, "stats": st, "fused_inner": fused_inner,
         }
         if e2e:
             line["e2e"] = e2e
