@@ -150,7 +150,7 @@ class Oracle:
                     n_evals=int(ne.value), nterms=nterms, ambiguous=amb, max_roots=int(mr.value))
 
 
-    def inner(self, hplus, hcross, dplus=None, dcross=None, w=None):
+    def inner(self, hplus, hcross, dplus=None, dcross=None, w=None, hann=False):
         """Eq. 12 as a sum over the grid: (<h|h>, <d|h>) with <a|b> = sum_k w_k (a+ conj b+ + ax conj bx)."""
         hp = np.ascontiguousarray(hplus, dtype=np.complex128)
         hx = np.ascontiguousarray(hcross, dtype=np.complex128)
@@ -164,7 +164,7 @@ class Oracle:
             keep += [dp, dx]
             args[4] = dp.view(np.float64).ctypes.data_as(_dp); args[5] = dx.view(np.float64).ctypes.data_as(_dp)
         out = np.zeros(3)
-        if self.lib.fdemri_oracle_inner(*args, out.ctypes.data_as(_dp)):
+        if self.lib.fdemri_oracle_inner(*args, C.c_int(1 if hann else 0), out.ctypes.data_as(_dp)):
             raise ValueError("fdemri_oracle_inner")
         return float(out[0]), complex(out[1], out[2])
 

@@ -316,14 +316,23 @@ extern "C" void fdemri_oracle_set_explicit(int on) { g_explicit_voices = on; }
 /* Eq. 12, both polarisations, as the plain sum it is on a frequency grid:
  *   <a|b> = sum_k w_k [ a+(f_k) conj b+(f_k) + ax(f_k) conj bx(f_k) ],   w_k = 4 df / S_n(f_k)  (w = 1 if NULL).
  * The paper's inner product is the real part; the imaginary part is returned as well.  long double sums in index
- * order.  out = {<h|h>, Re<d|h>, Im<d|h>};  d may be NULL (then only out[0] is set). */
+ * order.  out = {<h|h>, Re<d|h>, Im<d|h>};  d may be NULL (then only out[0] is set).
+ * hann != 0: h is first replaced by its convolution with the DFT of the Hann window (L145):
+ *   h_k <- h_k/2 - h_{k-1}/4 - h_{k+1}/4,  bins outside the grid counting as zero. */
 extern "C" int fdemri_oracle_inner(int64_t n_freq, const double* w, const double* hplus, const double* hcross,
-                                   const double* dplus, const double* dcross, double* out) {
+                                   const double* dplus, const double* dcross, int hann, double* out) {
     if (n_freq < 0 || !hplus || !hcross || !out) return 1;
     long double hh = 0.0L, dr = 0.0L, di = 0.0L;
+    auto at = [&](const double* h, int64_t k, int c) -> long double {
+        return (k < 0 || k >= n_freq) ? 0.0L : (long double)h[2 * k + c];
+    };
+    auto val = [&](const double* h, int64_t k, int c) -> long double {
+        if (!hann) return at(h, k, c);
+        return 0.5L * at(h, k, c) - 0.25L * at(h, k - 1, c) - 0.25L * at(h, k + 1, c);
+    };
     for (int64_t k = 0; k < n_freq; ++k) {
         const long double wk = w ? (long double)w[k] : 1.0L;
-        const long double pr = hplus[2 * k], pi = hplus[2 * k + 1], xr = hcross[2 * k], xi = hcross[2 * k + 1];
+        const long double pr = val(hplus, k, 0), pi = val(hplus, k, 1), xr = val(hcross, k, 0), xi = val(hcross, k, 1);
         hh += wk * (pr * pr + pi * pi + xr * xr + xi * xi);
         if (dplus && dcross) {
             const long double ar = dplus[2 * k], ai = dplus[2 * k + 1], br = dcross[2 * k], bi = dcross[2 * k + 1];

@@ -72,9 +72,10 @@ int fdemri_oracle_waveform(int n_modes, const int32_t* lmn, int n_knots, const d
                            int n_threads);
 
 /* Eq. 12 (L134-141) on a frequency grid, both polarisations: <a|b> = sum_k w_k [a+ conj b+ + ax conj bx],
- * w_k = 4 df / S_n(f_k) (NULL: w = 1).  hplus, hcross, dplus, dcross: [n_freq][2].  out = {<h|h>, Re<d|h>, Im<d|h>}. */
+ * w_k = 4 df / S_n(f_k) (NULL: w = 1).  hplus, hcross, dplus, dcross: [n_freq][2].  out = {<h|h>, Re<d|h>, Im<d|h>}.
+ * hann != 0: h is first convolved with the DFT of the Hann window, h_k/2 - h_{k-1}/4 - h_{k+1}/4 (L145). */
 int fdemri_oracle_inner(int64_t n_freq, const double* w, const double* hplus, const double* hcross,
-                        const double* dplus, const double* dcross, double* out);
+                        const double* dplus, const double* dcross, int hann, double* out);
 
 int fdemri_oracle_num_threads(void);
 /* Test switch for pin P7: list voices stand for themselves only (m of either sign, no implied partner). */

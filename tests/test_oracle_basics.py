@@ -197,3 +197,25 @@ def test_inner_product_is_the_weighted_dot_product(orc):
     assert abs(hd - np.conj(dh)) <= 1e-12 * abs(dh)
     hh2, dh2 = orc.inner(hp, hx, dp, dx, 3.0 * w)
     assert abs(hh2 - 3.0 * hh) <= 1e-12 * hh2 and abs(dh2 - 3.0 * dh) <= 1e-12 * abs(dh2)
+
+
+def test_hann_filter_is_the_dft_of_the_windowed_series(orc):
+    """Pin of the 3-point filter (the Hann window on the time series is a convolution of the
+    frequency-domain waveform with the window's DFT): for a series whose spectrum vanishes at both ends of the
+    grid, DFT(hann * x)_k = X_k/2 - X_{k-1}/4 - X_{k+1}/4 exactly, so the oracle's filtered <h|h> must equal the
+    sum over the FFT of the windowed series."""
+    rng = np.random.default_rng(9)
+    N = 512
+    X = np.zeros(N, dtype=complex)
+    X[3:200] = rng.standard_normal(197) + 1j * rng.standard_normal(197)      # zero at the grid ends: no wrap-around
+    x = np.fft.ifft(X)
+    n = np.arange(N)
+    win = 0.5 * (1.0 - np.cos(2.0 * np.pi * n / N))
+    Xw = np.fft.fft(win * x)
+    want = np.sum(np.abs(Xw[:256]) ** 2)
+    zeros = np.zeros(256, dtype=complex)
+    got, _ = orc.inner(X[:256], zeros, hann=True)
+    assert abs(got - want) <= 1e-12 * want
+    d = rng.standard_normal(256) + 1j * rng.standard_normal(256)
+    _, dh = orc.inner(X[:256], zeros, d, zeros, hann=True)
+    assert abs(dh - np.vdot(Xw[:256], d)) <= 1e-12 * abs(dh)
