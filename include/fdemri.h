@@ -116,11 +116,14 @@ int fdemri_sum(fdemri_plan_t plan, int n_angles, const double* theta_host, const
  *  weight_dev     [n_freq] w_k >= 0, shared by the batch; NULL: w = 1
  *  data_plus_dev, data_cross_dev  [n_freq][2] (re, im) data of the two polarisations, shared by the batch; both
  *                 NULL: only <h|h> is formed
+ *  hann           != 0: the waveform entering the inner products is first convolved with the DFT of the Hann
+ *                 window, h_k/2 - h_{k-1}/4 - h_{k+1}/4 with bins outside the grid counting as zero (L145: the
+ *                 window the paper applies to the time series); the waveform written to hplus/hcross is not filtered
  *  hplus_dev, hcross_dev  as in fdemri_sum, or both NULL: nothing but the inner products leaves the kernel
  *  inner_out_dev  [n_batch][4] = {<h|h>, Re<d|h>, Im<d|h>, 0}, device memory; sums are formed in a fixed order
  *                 (bitwise reproducible) */
 int fdemri_sum_inner(fdemri_plan_t plan, int n_angles, const double* theta_host, const double* phi_host,
-                     const double* weight_dev, const double* data_plus_dev, const double* data_cross_dev,
+                     const double* weight_dev, const double* data_plus_dev, const double* data_cross_dev, int hann,
                      double* hplus_dev, double* hcross_dev, double* inner_out_dev, void* cuda_stream);
 
 /* Counters of the last fdemri_sum (synchronises the stream used by that call). */

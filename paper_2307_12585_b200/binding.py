@@ -60,7 +60,8 @@ def lib() -> C.CDLL:
         L.fdemri_sum.restype = C.c_int
         L.fdemri_sum.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), dp, dp, vp]
         L.fdemri_sum_inner.restype = C.c_int
-        L.fdemri_sum_inner.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), dp, dp, dp, dp, dp, dp, vp]
+        L.fdemri_sum_inner.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), dp, dp, dp, C.c_int, dp, dp, dp,
+                                       vp]
         L.fdemri_get_stats.restype = C.c_int
         L.fdemri_get_stats.argtypes = [vp, C.POINTER(FdemriStats)]
         L.fdemri_get_coeffs.restype = C.c_int
@@ -138,15 +139,15 @@ def fdemri_sum(plan, theta, phi, hplus, hcross, stream=None):
                                         _ptr(hcross), _stream_ptr(stream)))
 
 
-def fdemri_sum_inner(plan, theta, phi, inner_out, weight=None, data_plus=None, data_cross=None, hplus=None, hcross=None,
-                     stream=None):
+def fdemri_sum_inner(plan, theta, phi, inner_out, weight=None, data_plus=None, data_cross=None, hann=False, hplus=None,
+                     hcross=None, stream=None):
     th = np.atleast_1d(np.asarray(theta, dtype=np.float64))
     ph = np.atleast_1d(np.asarray(phi, dtype=np.float64))
     assert th.shape == ph.shape
     dp = C.POINTER(C.c_double)
     _chk("fdemri_sum_inner", lib().fdemri_sum_inner(plan, th.shape[0], th.ctypes.data_as(dp), ph.ctypes.data_as(dp),
-                                                    _ptr(weight), _ptr(data_plus), _ptr(data_cross), _ptr(hplus),
-                                                    _ptr(hcross), _ptr(inner_out), _stream_ptr(stream)))
+                                                    _ptr(weight), _ptr(data_plus), _ptr(data_cross), int(bool(hann)),
+                                                    _ptr(hplus), _ptr(hcross), _ptr(inner_out), _stream_ptr(stream)))
 
 
 def fdemri_get_stats(plan, check=True) -> dict:

@@ -32,6 +32,7 @@ struct fdemri_plan_s {
     unsigned int* tile_off;        // [B * n_tiles + 1]
     unsigned int* pairs;           // [pair_cap]
     double* inner_part;            // [B * n_tiles][FDEMRI_CWARPS][4] partial inner products
+    double* inner_edge;            // [B * n_tiles][FDEMRI_CWARPS][4][4] edge bins for the Hann filter
     unsigned long long pair_cap;
     double4* wts;
     double* angles;
@@ -71,6 +72,7 @@ static size_t carve(fdemri_plan_s* p, char* base) {
     p->angles = (double*)take(B * 2 * sizeof(double));
     p->stats = (unsigned long long*)take(16 * sizeof(unsigned long long));
     p->inner_part = (double*)take(NT * FDEMRI_CWARPS * 4 * sizeof(double));
+    p->inner_edge = (double*)take(NT * FDEMRI_CWARPS * 16 * sizeof(double));
     // the pair list takes what is left of the work space (default: see fdemri_workspace_bytes)
     p->pairs = (unsigned int*)take(0);
     return off;
@@ -211,7 +213,7 @@ extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const 
 // S0 + S3 + S4 (+ the fused inner products when inner_out_dev is given)
 static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, const double* phi_host, double* hplus_dev,
                        double* hcross_dev, const double* weight_dev, const double* dplus_dev, const double* dcross_dev,
-                       double* inner_out_dev, void* cuda_stream) {
+                       int hann, double* inner_out_dev, void* cuda_stream) {
     if (!p || !theta_host || !phi_host) return FDEMRI_ERR_INVALID_ARG;
     if ((hplus_dev == nullptr) != (hcross_dev == nullptr)) return FDEMRI_ERR_INVALID_ARG;
     if (!hplus_dev && !inner_out_dev) return FDEMRI_ERR_INVALID_ARG;
@@ -254,6 +256,7 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
     a.dplus = dplus_dev;
     a.dcross = dcross_dev;
     a.inner_part = inner_out_dev ? p->inner_part : nullptr;
+    a.inner_edge = (inner_out_dev && hann) ? p->inner_edge : nullptr;
     const size_t smem = sizeof(FdemriRing);
     if (p->sum_blocks_per_sm == 0) {
         if (cudaFuncSetAttribute(k_tile_sum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
@@ -279,7 +282,8 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
         }
     }
     if (inner_out_dev) {
-        k_inner_reduce<<<d.n_batch, 256, 0, st>>>(d.n_tiles, p->inner_part, inner_out_dev);
+        k_inner_reduce<<<d.n_batch, 256, 0, st>>>(d.n_tiles, d.n_freq, p->inner_part, a.inner_edge, weight_dev, dplus_dev,
+                                                  dcross_dev, inner_out_dev);
         if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
     }
     return FDEMRI_OK;
@@ -288,15 +292,15 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
 extern "C" int fdemri_sum(fdemri_plan_t p, int n_angles, const double* theta_host, const double* phi_host,
                           double* hplus_dev, double* hcross_dev, void* cuda_stream) {
     if (!hplus_dev || !hcross_dev) return FDEMRI_ERR_INVALID_ARG;
-    return enqueue_sum(p, n_angles, theta_host, phi_host, hplus_dev, hcross_dev, nullptr, nullptr, nullptr, nullptr, cuda_stream);
+    return enqueue_sum(p, n_angles, theta_host, phi_host, hplus_dev, hcross_dev, nullptr, nullptr, nullptr, 0, nullptr, cuda_stream);
 }
 
 extern "C" int fdemri_sum_inner(fdemri_plan_t p, int n_angles, const double* theta_host, const double* phi_host,
                                 const double* weight_dev, const double* data_plus_dev, const double* data_cross_dev,
-                                double* hplus_dev, double* hcross_dev, double* inner_out_dev, void* cuda_stream) {
+                                int hann, double* hplus_dev, double* hcross_dev, double* inner_out_dev, void* cuda_stream) {
     if (!inner_out_dev) return FDEMRI_ERR_INVALID_ARG;
     return enqueue_sum(p, n_angles, theta_host, phi_host, hplus_dev, hcross_dev, weight_dev, data_plus_dev, data_cross_dev,
-                       inner_out_dev, cuda_stream);
+                       hann, inner_out_dev, cuda_stream);
 }
 
 

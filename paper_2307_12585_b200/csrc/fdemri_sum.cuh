@@ -45,6 +45,8 @@ struct SumArgs {
     const double* dplus;      // [n_freq][2] data, + polarisation (NULL: only <h|h>)
     const double* dcross;     // [n_freq][2]
     double* inner_part;       // [total_tiles][FDEMRI_CWARPS][4] partial sums {<h|h>, Re<d|h>, Im<d|h>, 0}
+    double* inner_edge;       // Hann filter (L145): [total_tiles][FDEMRI_CWARPS][4][4] h at the first two and last two bins
+                              // of every warp range; NULL: no window
 };
 
 // asymptotic series of g(X) e^{+i pi/4 sgn X} = sum_k i^k a_k u^k, u = 1/X, a_k = prod_j (4/9-(2j-1)^2)/(k! 8^k)
@@ -528,25 +530,60 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
             if (a.inner_part) {
                 // Eq. 12 on the fly: this warp's share of sum_k w_k (|h+|^2 + |hx|^2) and sum_k w_k (d+ conj h+ + dx conj hx),
                 // reduced over the lanes in a fixed butterfly; k_inner_reduce adds the warps in a fixed order
+                double p0r = a00, p0i = a01, x0r = a02, x0i = a03, p1r = a10, p1i = a11, x1r = a12, x1i = a13;
+                bool use0 = v0, use1 = v1;
+                if (a.inner_edge) {
+                    // Hann window as the 3-point filter h_k/2 - h_{k-1}/4 - h_{k+1}/4 (L145).  Neighbours come from the
+                    // adjacent lanes; the first and the last bin of the warp's range need a bin of another warp and
+                    // are left to k_inner_reduce, which gets the two bins at either end of the range.
+                    if (lane < 2 || lane >= 30) {
+                        double* e = a.inner_edge + (((size_t)gt * FDEMRI_CWARPS + cw) * 4 + (lane < 2 ? lane : lane - 28)) * 4;
+                        if (lane < 2) *reinterpret_cast<double4*>(e) = make_double4(a00, a01, a02, a03);
+                        else *reinterpret_cast<double4*>(e) = make_double4(a10, a11, a12, a13);
+                    }
+                    const unsigned full = 0xffffffffu;
+                    // slot 0: left neighbour = lane - 1 of slot 0; right neighbour = lane + 1 of slot 0, or lane 0 of slot 1
+                    const double l0a = __shfl_up_sync(full, a00, 1), l0b = __shfl_up_sync(full, a01, 1);
+                    const double l0c = __shfl_up_sync(full, a02, 1), l0d = __shfl_up_sync(full, a03, 1);
+                    double r0a = __shfl_down_sync(full, a00, 1), r0b = __shfl_down_sync(full, a01, 1);
+                    double r0c = __shfl_down_sync(full, a02, 1), r0d = __shfl_down_sync(full, a03, 1);
+                    const double f1a = __shfl_sync(full, a10, 0), f1b = __shfl_sync(full, a11, 0);
+                    const double f1c = __shfl_sync(full, a12, 0), f1d = __shfl_sync(full, a13, 0);
+                    if (lane == 31) { r0a = f1a; r0b = f1b; r0c = f1c; r0d = f1d; }
+                    // slot 1: left neighbour = lane - 1 of slot 1, or lane 31 of slot 0; right neighbour = lane + 1 of slot 1
+                    double l1a = __shfl_up_sync(full, a10, 1), l1b = __shfl_up_sync(full, a11, 1);
+                    double l1c = __shfl_up_sync(full, a12, 1), l1d = __shfl_up_sync(full, a13, 1);
+                    const double g0a = __shfl_sync(full, a00, 31), g0b = __shfl_sync(full, a01, 31);
+                    const double g0c = __shfl_sync(full, a02, 31), g0d = __shfl_sync(full, a03, 31);
+                    if (lane == 0) { l1a = g0a; l1b = g0b; l1c = g0c; l1d = g0d; }
+                    const double r1a = __shfl_down_sync(full, a10, 1), r1b = __shfl_down_sync(full, a11, 1);
+                    const double r1c = __shfl_down_sync(full, a12, 1), r1d = __shfl_down_sync(full, a13, 1);
+                    p0r = 0.5 * a00 - 0.25 * (l0a + r0a); p0i = 0.5 * a01 - 0.25 * (l0b + r0b);
+                    x0r = 0.5 * a02 - 0.25 * (l0c + r0c); x0i = 0.5 * a03 - 0.25 * (l0d + r0d);
+                    p1r = 0.5 * a10 - 0.25 * (l1a + r1a); p1i = 0.5 * a11 - 0.25 * (l1b + r1b);
+                    x1r = 0.5 * a12 - 0.25 * (l1c + r1c); x1i = 0.5 * a13 - 0.25 * (l1d + r1d);
+                    use0 = v0 && lane != 0;
+                    use1 = v1 && lane != 31;
+                }
                 double hh = 0.0, dr = 0.0, di = 0.0;
-                if (v0) {
+                if (use0) {
                     const double w0 = a.weight ? __ldg(a.weight + bin_a) : 1.0;
-                    hh = w0 * (a00 * a00 + a01 * a01 + a02 * a02 + a03 * a03);
+                    hh = w0 * (p0r * p0r + p0i * p0i + x0r * x0r + x0i * x0i);
                     if (a.dplus) {
                         const double2 dp = *reinterpret_cast<const double2*>(a.dplus + 2 * bin_a);
                         const double2 dx = *reinterpret_cast<const double2*>(a.dcross + 2 * bin_a);
-                        dr = w0 * (dp.x * a00 + dp.y * a01 + dx.x * a02 + dx.y * a03);
-                        di = w0 * (dp.y * a00 - dp.x * a01 + dx.y * a02 - dx.x * a03);
+                        dr = w0 * (dp.x * p0r + dp.y * p0i + dx.x * x0r + dx.y * x0i);
+                        di = w0 * (dp.y * p0r - dp.x * p0i + dx.y * x0r - dx.x * x0i);
                     }
                 }
-                if (v1) {
+                if (use1) {
                     const double w1 = a.weight ? __ldg(a.weight + bin_a + 32) : 1.0;
-                    hh += w1 * (a10 * a10 + a11 * a11 + a12 * a12 + a13 * a13);
+                    hh += w1 * (p1r * p1r + p1i * p1i + x1r * x1r + x1i * x1i);
                     if (a.dplus) {
                         const double2 dp = *reinterpret_cast<const double2*>(a.dplus + 2 * (bin_a + 32));
                         const double2 dx = *reinterpret_cast<const double2*>(a.dcross + 2 * (bin_a + 32));
-                        dr += w1 * (dp.x * a10 + dp.y * a11 + dx.x * a12 + dx.y * a13);
-                        di += w1 * (dp.y * a10 - dp.x * a11 + dx.y * a12 - dx.x * a13);
+                        dr += w1 * (dp.x * p1r + dp.y * p1i + dx.x * x1r + dx.y * x1i);
+                        di += w1 * (dp.y * p1r - dp.x * p1i + dx.y * x1r - dx.x * x1i);
                     }
                 }
 #pragma unroll
@@ -605,6 +642,8 @@ __global__ void __maxnreg__(FDEMRI_MAXNREG) k_tile_sum(SumArgs a) {
         if (a.inner_part) {
             const size_t m = (size_t)a.total_tiles * FDEMRI_CWARPS * 4;
             for (size_t i = (size_t)blockIdx.x * blockDim.x + tid; i < m; i += (size_t)gridDim.x * blockDim.x) a.inner_part[i] = nan;
+            if (a.inner_edge)
+                for (size_t i = (size_t)blockIdx.x * blockDim.x + tid; i < 4 * m; i += (size_t)gridDim.x * blockDim.x) a.inner_edge[i] = nan;
         }
         return;
     }
@@ -613,16 +652,51 @@ __global__ void __maxnreg__(FDEMRI_MAXNREG) k_tile_sum(SumArgs a) {
 }
 
 // Fixed-order sum of the per-(tile, warp) partial inner products of one batch item.  One CTA per item.
+// With the Hann filter (edge != NULL) it also adds the first and the last bin of every warp range, whose filtered
+// values need a bin of the neighbouring range: range i covers bins 64 i .. 64 i + 63 of the item.
 // out: [B][4] = {<h|h>, Re<d|h>, Im<d|h>, 0}
-__global__ void __launch_bounds__(256) k_inner_reduce(int n_tiles, const double* __restrict__ part, double* __restrict__ out) {
+__device__ __forceinline__ void fdemri_inner_bin(const double4 h, int64_t k, const double* __restrict__ weight,
+                                                 const double* __restrict__ dplus, const double* __restrict__ dcross,
+                                                 double& hh, double& dr, double& di) {
+    const double w = weight ? weight[k] : 1.0;
+    hh += w * (h.x * h.x + h.y * h.y + h.z * h.z + h.w * h.w);
+    if (dplus) {
+        const double2 dp = *reinterpret_cast<const double2*>(dplus + 2 * k);
+        const double2 dx = *reinterpret_cast<const double2*>(dcross + 2 * k);
+        dr += w * (dp.x * h.x + dp.y * h.y + dx.x * h.z + dx.y * h.w);
+        di += w * (dp.y * h.x - dp.x * h.y + dx.y * h.z - dx.x * h.w);
+    }
+}
+__device__ __forceinline__ double4 fdemri_hann3(const double4 l, const double4 c, const double4 r) {
+    return make_double4(0.5 * c.x - 0.25 * (l.x + r.x), 0.5 * c.y - 0.25 * (l.y + r.y), 0.5 * c.z - 0.25 * (l.z + r.z),
+                        0.5 * c.w - 0.25 * (l.w + r.w));
+}
+
+__global__ void __launch_bounds__(256) k_inner_reduce(int n_tiles, int64_t n_freq, const double* __restrict__ part,
+                                                      const double* __restrict__ edge, const double* __restrict__ weight,
+                                                      const double* __restrict__ dplus, const double* __restrict__ dcross,
+                                                      double* __restrict__ out) {
     __shared__ double s_r[3][256];
     const int b = blockIdx.x, tid = threadIdx.x;
     const size_t n = (size_t)n_tiles * FDEMRI_CWARPS;
     const double4* p = reinterpret_cast<const double4*>(part) + (size_t)b * n;
+    const double4* e = edge ? reinterpret_cast<const double4*>(edge) + (size_t)b * n * 4 : nullptr;
+    const double4 zero = make_double4(0.0, 0.0, 0.0, 0.0);
     double hh = 0.0, dr = 0.0, di = 0.0;
     for (size_t i = tid; i < n; i += 256) {
         const double4 v = p[i];
         hh += v.x; dr += v.y; di += v.z;
+        if (e) {
+            const int64_t k0 = (int64_t)i * 64, k1 = k0 + 63;
+            if (k0 < n_freq) {
+                const double4 left = (i > 0) ? e[(i - 1) * 4 + 3] : zero;
+                fdemri_inner_bin(fdemri_hann3(left, e[i * 4 + 0], e[i * 4 + 1]), k0, weight, dplus, dcross, hh, dr, di);
+            }
+            if (k1 < n_freq) {
+                const double4 right = (i + 1 < n) ? e[(i + 1) * 4 + 0] : zero;
+                fdemri_inner_bin(fdemri_hann3(e[i * 4 + 2], e[i * 4 + 3], right), k1, weight, dplus, dcross, hh, dr, di);
+            }
+        }
     }
     s_r[0][tid] = hh; s_r[1][tid] = dr; s_r[2][tid] = di;
     __syncthreads();

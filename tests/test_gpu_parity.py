@@ -316,6 +316,37 @@ def test_fused_inner_products_eq12(fd, orc):
     torch.cuda.synchronize()
     o3 = out3.cpu().numpy()[0]
     assert abs(o3[0] - want_hh1) <= 1e-10 * want_hh1 and o3[1] == 0.0 and o3[2] == 0.0
+    # (4) Hann window as the 3-point frequency-domain filter (L145), including the bins at warp and tile borders
+    want_hh4, want_dh4 = orc.inner(ref["hplus"], ref["hcross"], dplus, dcross, weight, hann=True)
+    out4 = torch.zeros_like(out)
+    fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, out4, weight=t_w, data_plus=t_dp, data_cross=t_dx, hann=True)
+    torch.cuda.synchronize()
+    o4 = out4.cpu().numpy()[0]
+    assert abs(o4[0] - want_hh4) <= 1e-10 * want_hh4 and abs(want_hh4 - want_hh) > 1e-3 * want_hh
+    assert abs(complex(o4[1], o4[2]) - want_dh4) <= 1e-10 * np.sqrt(want_hh4 * orc.inner(dplus, dcross, w=weight)[0])
+    print(f"[parity] fused inner products, Hann filter: <h|h> rel {abs(o4[0] - want_hh4) / want_hh4:.2e}, "
+          f"<d|h> rel {abs(complex(o4[1], o4[2]) - want_dh4) / abs(want_dh4):.2e}")
     print(f"[parity] fused inner products: <h|h> rel {abs(o1[0] - want_hh) / want_hh:.2e}, "
           f"<d|h> rel {abs(complex(o1[1], o1[2]) - want_dh) / abs(want_dh):.2e}")
+    wf.close()
+
+
+def test_fused_inner_ragged_grid_with_hann(fd, orc):
+    """Ragged grid (20001 bins: the last warp range and the last tile are partial) with the Hann filter and w = 1."""
+    import torch
+    from paper_2307_12585_b200 import synth
+    w = synth.small_case(seed=7, n_knots=5, n_freq=20001)
+    ref = oracle_c(orc, w, w.freq_array())
+    rng = np.random.default_rng(3)
+    d = np.abs(ref["hplus"]).max() * (rng.standard_normal((2, w.n_freq)) + 1j * rng.standard_normal((2, w.n_freq)))
+    wf = fd.waveform_from_workload(w)
+    t_d = [torch.from_numpy(np.ascontiguousarray(x).view(np.float64).reshape(-1, 2)).to(wf.dev) for x in d]
+    out = torch.zeros((1, 4), dtype=torch.float64, device=wf.dev)
+    for hann in (False, True):
+        want_hh, want_dh = orc.inner(ref["hplus"], ref["hcross"], d[0], d[1], hann=hann)
+        fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, out, data_plus=t_d[0], data_cross=t_d[1], hann=hann)
+        torch.cuda.synchronize()
+        o = out.cpu().numpy()[0]
+        assert abs(o[0] - want_hh) <= 1e-10 * want_hh
+        assert abs(complex(o[1], o[2]) - want_dh) <= 1e-10 * np.sqrt(want_hh * orc.inner(d[0], d[1])[0])
     wf.close()
