@@ -12,7 +12,9 @@
 #define FDEMRI_TILE (FDEMRI_CWARPS * 32 * FDEMRI_BPL)     // bins per tile (512)
 #define FDEMRI_SUM_THREADS ((FDEMRI_CWARPS + 1) * 32)     // + one producer warp
 #define FDEMRI_CHUNK 32              // staged items per ring stage (one per producer lane)
+#ifndef FDEMRI_STAGES
 #define FDEMRI_STAGES 8              // ring depth
+#endif
 #define FDEMRI_BAD_LIST_OVERFLOW_BIT 16ull   // = FDEMRI_BAD_LIST_OVERFLOW of fdemri.h
 
 // ------------------------------------------------------------------------------------------------
