@@ -123,7 +123,7 @@ def run_reference(args):
     total_evals = 3.299e8 if args.config == 2 else None
     times, evals = [], 0
     for i in range(args.warmup + args.steps):
-        r = cpu_oracle_sample(w, total_evals or 1.0, n_bins=30000, seed=i)
+        r = cpu_oracle_sample(w, total_evals or 1.0, n_bins=200000, seed=i)
         if i >= args.warmup:
             times.append(r["seconds"]); evals += r["evals_per_s"] * r["seconds"]
     tot = sum(times)
@@ -132,9 +132,9 @@ def run_reference(args):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / max(1, args.steps),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f80 (x87 long double)",
             "data": "synthetic",
-            "config": {"workload": workload_name(args.config, w), "sample": "30000 random bins of the covered band per step"},
+            "config": {"workload": workload_name(args.config, w), "sample": "200000 random bins of the covered band per step"},
             "cpu_baseline": {"value": val, "unit": "waveforms/s", "cores": orc.num_threads, "kind": "oracle",
-                             "sample": "each step: 30000 random bins of the covered band incl. spline build, scaled by "
+                             "sample": "each step: 200000 random bins of the covered band incl. spline build, scaled by "
                                        "evaluation count (3.299e8 per waveform)"},
             "e2e": {"value": val, "unit": "waveforms/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "evals_per_s": evals / tot}
