@@ -94,6 +94,7 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
     int64_t n_tiles = (n_freq + FDEMRI_TILE - 1) / FDEMRI_TILE;
     if (n_tiles * (int64_t)n_batch >= ((int64_t)1 << 31)) return FDEMRI_ERR_INVALID_ARG;
     if ((int64_t)n_batch * n_modes * (n_knots - 1) >= ((int64_t)1 << 31)) return FDEMRI_ERR_INVALID_ARG;   /* 32-bit record index */
+    if ((int64_t)n_modes * 4 * (n_knots - 1) >= ((int64_t)1 << 32)) return FDEMRI_ERR_INVALID_ARG;          /* 32-bit work-list key */
     fdemri_plan_s* p = new (std::nothrow) fdemri_plan_s();
     if (!p) return FDEMRI_ERR_INVALID_ARG;
     p->d.n_modes = n_modes;

@@ -63,8 +63,8 @@ enum {
     S_F32B = 11,// float2 {FD, Q1}
     S_CU = 12,  // 1/X = CU * (F''/2)^2 / |F'|^3,  CU = sign(F') 6/pi
     S_TK4 = 13, // 4 t_k
-    S_NBH4 = 14,// -4 b'_hi
-    S_NBL4 = 15,// -4 b'_lo
+    S_WC = 14,  // 4 (F_k - b'), b' = b_Phi/2pi (hi + lo): the linear phase coefficient is 4 (s f - b') = 4 x + WC
+    S_FREE = 15,
     S_NC4 = 16, // 4 (-c_Phi/2pi)
     S_ND4 = 17, // 4 (-d_Phi/2pi)
     S_PC4 = 18, // 4 (PC + m phi/2pi) - 0.5 sign(F')     (the e^{-+i pi/4} of the standard SPA, L119; the slow

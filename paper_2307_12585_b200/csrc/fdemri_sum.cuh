@@ -203,7 +203,7 @@ __device__ __forceinline__ bool fdemri_term_fast(const double* __restrict__ it, 
     const double e = __fma_rn(sf, TK4, -P);
     const double big4 = 27021597764222976.0;           // 1.5 * 2^54: adding it rounds to a multiple of 4
     const double pr = P - ((P + big4) - big4);
-    const double wv = fma(sf, 4.0, it[S_NBH4]) + it[S_NBL4];
+    const double wv = fma(x, 4.0, it[S_WC]);           // 4 (s f - b'), b' = Phi'(t_k)/2pi, through x = s f - F_k
     const double loc = fma(tau, fma(tau, fma(tau, it[S_ND4], it[S_NC4]), wv), it[S_PC4]);
     const double q = (pr + e) + (loc + dq);
     double sn, cs;
@@ -287,7 +287,7 @@ __device__ __noinline__ FdemriSlowOut fdemri_term_slow(const double* it, double 
     const double e = __fma_rn(sf, TK4, -P);
     const double big4 = 27021597764222976.0;
     const double pr = P - ((P + big4) - big4);
-    const double wv = fma(sf, 4.0, it[S_NBH4]) + it[S_NBL4];
+    const double wv = fma(sf + it[S_NFA], 4.0, it[S_WC]);
     const double loc = tau * fma(tau, fma(tau, it[S_ND4], it[S_NC4]), wv);
     double q = ((pr + e) + (it[S_PC4] + copysign(0.5, it[S_CU]))) + loc;
     double Sre, Sim;
@@ -368,7 +368,7 @@ __device__ __forceinline__ void fdemri_stage_item(double* dst, const double* __r
     d2[4] = make_double2(r1.z, 2e-7 * h);
     d2[5] = make_double2(0.5 * h, *reinterpret_cast<const double*>(&f32b));
     d2[6] = make_double2(sF * 1.9098593171027440, 4.0 * r5.y);
-    d2[7] = make_double2(-4.0 * r4.y, -4.0 * r4.z);
+    d2[7] = make_double2(4.0 * ((r0.x - r4.y) - r4.z), 0.0);      // F_k and b' nearly cancel: the difference is exact
     d2[8] = make_double2(4.0 * r4.w, 4.0 * r5.x);
     d2[9] = make_double2(fma(4.0, r4.x + w.z, -0.5 * sF), *reinterpret_cast<const double*>(&f32c));
     d2[10] = make_double2(r2.x, r2.y);
