@@ -350,3 +350,50 @@ def test_fused_inner_ragged_grid_with_hann(fd, orc):
         assert abs(o[0] - want_hh) <= 1e-10 * want_hh
         assert abs(complex(o[1], o[2]) - want_dh) <= 1e-10 * np.sqrt(want_hh * orc.inner(d[0], d[1])[0])
     wf.close()
+
+
+def test_random_small_cases_sweep(fd, orc):
+    """Twenty seeded small cases with random knot counts, mode sets (m = 0, negative n, high l), grids (offset f0,
+    ragged sizes), angles and with/without a turnover: per-bin parity, evaluation counts (P9) and exact zeros outside
+    the support (P8) on every one of them."""
+    from paper_2307_12585_b200 import synth
+    rng = np.random.default_rng(20230712)
+    worst, skipped = 0.0, 0
+    for case in range(20):
+        n_knots = int(rng.integers(4, 40))
+        n_modes = int(rng.integers(1, 9))
+        modes = []
+        for _ in range(n_modes):
+            l = int(rng.integers(2, 11))
+            modes.append((l, int(rng.integers(0, l + 1)), int(rng.integers(-6, 7))))
+        n_freq = int(rng.integers(500, 40000))
+        w = synth.small_case(seed=100 + case, n_knots=n_knots, n_freq=n_freq, modes=tuple(modes),
+                             turnover=bool(case & 1))
+        if case % 3 == 0:
+            w.f0 = float(rng.uniform(0.0, 2e-3))
+        w.theta, w.phi = float(rng.uniform(0.05, 3.0)), float(rng.uniform(-3.0, 3.0))
+        wf = fd.waveform_from_workload(w)
+        wf.sum(w.theta, w.phi)
+        hp, hx = wf.result()
+        st = wf.stats(check=False)
+        if st["status"] == 5:                      # a segment cubic with two interior extrema (R5): flagged, not summed
+            assert st["flags"] & 1
+            skipped += 1
+            wf.close()
+            continue
+        assert st["status"] == 0
+        ref = oracle_c(orc, w, w.freq_array())
+        assert st["n_evals"] == ref["n_evals"], (case, modes)
+        if ref["n_evals"] == 0:
+            assert not hp.any() and not hx.any()
+        else:
+            keep = ref["ambiguous"] == 0
+            assert (~keep).sum() <= 2
+            err = max_rel_err(hp[0], hx[0], ref["hplus"], ref["hcross"], mask=keep)
+            zero = (ref["nterms"] == 0) & keep
+            assert np.all(hp[0][zero] == 0) and np.all(hx[0][zero] == 0)
+            assert err <= TOL_BIN, (case, modes, err)
+            worst = max(worst, err)
+        wf.close()
+    assert skipped <= 5
+    print(f"[parity] 20 random small cases ({skipped} flagged unsupported): worst max|dh|/max|h| = {worst:.3e}")
