@@ -319,12 +319,18 @@ def main():
     total_ms = fdist.max_over_ranks(float(sum(step_ms)), device=dev)
     # the same step with the inner products of Eq. 12 formed on the fly and no waveform written
     inner_ms = []
+    inner_kw = {}
+    try:
+        fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, inner_out, weight=inner_w, data_plus=inner_dp, data_cross=inner_dx)
+    except fd.FdemriError:                                   # bin-major plan: the products come from the written waveform
+        inner_kw = dict(hplus=wf.hplus, hcross=wf.hcross)
     for i in range(3 + args.steps):
         flush.fill_(1.0)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         fd.fdemri_build_splines(wf.plan, *dev_in)
-        fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, inner_out, weight=inner_w, data_plus=inner_dp, data_cross=inner_dx)
+        fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, inner_out, weight=inner_w, data_plus=inner_dp, data_cross=inner_dx,
+                            **inner_kw)
         e1.record(stream)
         e1.synchronize()
         if i >= 3:

@@ -40,8 +40,13 @@ enum {
 /* plan flags */
 enum {
     FDEMRI_FLAG_NONE = 0,
-    FDEMRI_FLAG_TIMING = 1     /* record CUDA events around the S3 tile kernel of every fdemri_sum (see
+    FDEMRI_FLAG_TIMING = 1,    /* record CUDA events around the S3 sum kernel of every fdemri_sum (see
                                   fdemri_get_kernel_ms); costs two event records per call                  */
+    FDEMRI_FLAG_BIN_MAJOR = 2, /* force the bin-major sum kernel (one warp per frequency bin, lanes over the
+                                  entries that cover it): the right shape when a (voice, segment) covers only a
+                                  few bins -- sparse or down-sampled frequency arrays (section 3.3)  */
+    FDEMRI_FLAG_TILE_MAJOR = 4 /* force the tile-major sum kernel (a CTA owns 768 consecutive bins): dense grids.
+                                  Default: bin-major iff n_freq < 256 (n_knots - 1)                         */
 };
 
 /* bits of fdemri_stats.flags (device-side validation, read back by fdemri_get_stats) */
@@ -120,6 +125,8 @@ int fdemri_sum(fdemri_plan_t plan, int n_angles, const double* theta_host, const
  *                 window, h_k/2 - h_{k-1}/4 - h_{k+1}/4 with bins outside the grid counting as zero (L145: the
  *                 window the paper applies to the time series); the waveform written to hplus/hcross is not filtered
  *  hplus_dev, hcross_dev  as in fdemri_sum, or both NULL: nothing but the inner products leaves the kernel
+ *                 (tile-major plans only: a bin-major plan forms the products from the waveform it writes and
+ *                 returns FDEMRI_ERR_UNSUPPORTED without these buffers)
  *  inner_out_dev  [n_batch][4] = {<h|h>, Re<d|h>, Im<d|h>, 0}, device memory; sums are formed in a fixed order
  *                 (bitwise reproducible) */
 int fdemri_sum_inner(fdemri_plan_t plan, int n_angles, const double* theta_host, const double* phi_host,

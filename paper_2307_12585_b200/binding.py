@@ -16,6 +16,7 @@ from . import build as _build
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
 FDEMRI_OK = 0
+FDEMRI_FLAG_TIMING, FDEMRI_FLAG_BIN_MAJOR, FDEMRI_FLAG_TILE_MAJOR = 1, 2, 4
 STATUS = {0: "FDEMRI_OK", 1: "FDEMRI_ERR_INVALID_ARG", 2: "FDEMRI_ERR_WORKSPACE", 3: "FDEMRI_ERR_CUDA",
           4: "FDEMRI_ERR_NOT_BUILT", 5: "FDEMRI_ERR_UNSUPPORTED"}
 

@@ -71,8 +71,10 @@ static size_t carve(fdemri_plan_s* p, char* base) {
     p->wts = (double4*)take(B * V * sizeof(double4));
     p->angles = (double*)take(B * 2 * sizeof(double));
     p->stats = (unsigned long long*)take(16 * sizeof(unsigned long long));
-    p->inner_part = (double*)take(NT * FDEMRI_CWARPS * 4 * sizeof(double));
-    p->inner_edge = (double*)take(NT * FDEMRI_CWARPS * 16 * sizeof(double));
+    // partial inner products of the tile-major kernel (the bin-major mode forms them from the waveform in memory)
+    const size_t NI = (d.tile_bins == 1) ? 0 : NT;
+    p->inner_part = (double*)take(NI * FDEMRI_CWARPS * 4 * sizeof(double));
+    p->inner_edge = (double*)take(NI * FDEMRI_CWARPS * 16 * sizeof(double));
     // the pair list takes what is left of the work space (default: see fdemri_workspace_bytes)
     p->pairs = (unsigned int*)take(0);
     return off;
@@ -91,7 +93,14 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
         int l = lmn_host[3 * v], m = lmn_host[3 * v + 1], n = lmn_host[3 * v + 2];
         if (l < 2 || l > 60 || m < 0 || m > l || n < -100000 || n > 100000) return FDEMRI_ERR_INVALID_ARG;
     }
-    int64_t n_tiles = (n_freq + FDEMRI_TILE - 1) / FDEMRI_TILE;
+    /* Which sum kernel: tile-major when the entries are wide in bins (dense grids), bin-major
+       when a bin interval holds only a few bins (sparse grids, section 3.3).  The entries of a voice split its
+       band into n_seg pieces, so n_freq / n_seg bounds the bins per entry. */
+    if ((flags & FDEMRI_FLAG_BIN_MAJOR) && (flags & FDEMRI_FLAG_TILE_MAJOR)) return FDEMRI_ERR_INVALID_ARG;
+    const bool bin_major = (flags & FDEMRI_FLAG_BIN_MAJOR) ||
+                           (!(flags & FDEMRI_FLAG_TILE_MAJOR) && n_freq < (int64_t)256 * (n_knots - 1));
+    const int tile_bins = bin_major ? 1 : FDEMRI_TILE;
+    int64_t n_tiles = (n_freq + tile_bins - 1) / tile_bins;
     if (n_tiles * (int64_t)n_batch >= ((int64_t)1 << 31)) return FDEMRI_ERR_INVALID_ARG;
     if ((int64_t)n_batch * n_modes * (n_knots - 1) >= ((int64_t)1 << 31)) return FDEMRI_ERR_INVALID_ARG;   /* 32-bit record index */
     if ((int64_t)n_modes * 4 * (n_knots - 1) >= ((int64_t)1 << 32)) return FDEMRI_ERR_INVALID_ARG;          /* 32-bit work-list key */
@@ -103,6 +112,7 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
     p->d.n_seg = n_knots - 1;
     p->d.ent_max = 2 * (n_knots - 1);                 /* slot = 2*segment + branch */
     p->d.n_freq = n_freq;
+    p->d.tile_bins = tile_bins;
     p->d.n_tiles = (int)n_tiles;
     p->d.f0 = f0;
     p->d.df = df;
@@ -258,22 +268,29 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
     a.dcross = dcross_dev;
     a.inner_part = inner_out_dev ? p->inner_part : nullptr;
     a.inner_edge = (inner_out_dev && hann) ? p->inner_edge : nullptr;
-    const size_t smem = sizeof(FdemriRing);
+    const bool bin_major = d.tile_bins == 1;
+    if (bin_major && !hplus_dev) return FDEMRI_ERR_UNSUPPORTED;      /* bin-major: inner products come from the waveform */
+    if (bin_major) a.inner_part = a.inner_edge = nullptr;
+    const size_t smem = bin_major ? (size_t)FDEMRI_BIN_WARPS * 32 * FDEMRI_BIN_STRIDE * sizeof(double) : sizeof(FdemriRing);
+    const int threads = bin_major ? FDEMRI_BIN_WARPS * 32 : FDEMRI_SUM_THREADS;
     if (p->sum_blocks_per_sm == 0) {
-        if (cudaFuncSetAttribute(k_tile_sum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        const void* fn = bin_major ? (const void*)k_bin_sum : (const void*)k_tile_sum;
+        if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
             return FDEMRI_ERR_CUDA;
         int per_sm = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_tile_sum, FDEMRI_SUM_THREADS, smem) != cudaSuccess ||
-            per_sm < 1)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, smem) != cudaSuccess || per_sm < 1)
             per_sm = 1;
         p->sum_blocks_per_sm = per_sm;
         if (getenv("FDEMRI_DEBUG"))
-            fprintf(stderr, "[fdemri] k_tile_sum: %d threads, %zu B smem, %d CTAs/SM\n", FDEMRI_SUM_THREADS, smem, per_sm);
+            fprintf(stderr, "[fdemri] %s: %d threads, %zu B smem, %d CTAs/SM\n", bin_major ? "k_bin_sum" : "k_tile_sum", threads,
+                    smem, per_sm);
     }
     long long grid = (long long)p->sm_count * p->sum_blocks_per_sm;
-    if (grid > a.total_tiles) grid = a.total_tiles;
+    const long long units = bin_major ? (a.total_tiles + FDEMRI_BIN_WARPS - 1) / FDEMRI_BIN_WARPS : a.total_tiles;
+    if (grid > units) grid = units;
     if (p->ev0) cudaEventRecord(p->ev0, st);
-    k_tile_sum<<<(unsigned)grid, FDEMRI_SUM_THREADS, smem, st>>>(a);
+    if (bin_major) k_bin_sum<<<(unsigned)grid, threads, smem, st>>>(a);
+    else k_tile_sum<<<(unsigned)grid, threads, smem, st>>>(a);
     if (p->ev1) { cudaEventRecord(p->ev1, st); p->ev_valid = true; }
     {
         const cudaError_t err = cudaGetLastError();
@@ -281,6 +298,11 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
             if (getenv("FDEMRI_DEBUG")) fprintf(stderr, "[fdemri] fdemri_sum: %s\n", cudaGetErrorString(err));
             return FDEMRI_ERR_CUDA;
         }
+    }
+    if (inner_out_dev && bin_major) {
+        k_inner_dense<<<d.n_batch, 1024, 0, st>>>(d.n_freq, hplus_dev, hcross_dev, weight_dev, dplus_dev, dcross_dev, hann,
+                                                  inner_out_dev);
+        return cudaGetLastError() == cudaSuccess ? FDEMRI_OK : FDEMRI_ERR_CUDA;
     }
     if (inner_out_dev) {
         k_inner_reduce<<<d.n_batch, 256, 0, st>>>(d.n_tiles, d.n_freq, p->inner_part, a.inner_edge, weight_dev, dplus_dev,

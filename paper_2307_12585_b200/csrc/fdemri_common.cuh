@@ -83,7 +83,8 @@ struct FdemriDims {
     int n_modes, n_batch, n_knots, n_seg;   // n_seg = n_knots - 1
     int ent_max;                            // entry slots per (voice, sign) = 2 * n_seg (segment, branch)
     int64_t n_freq;
-    int n_tiles;                            // tiles per batch item
+    int tile_bins;                          // bins per work-list tile: FDEMRI_TILE (tile-major sum) or 1 (bin-major sum)
+    int n_tiles;                            // tiles per batch item = ceil(n_freq / tile_bins)
     double f0, df;
     const double* freq;                     // NULL => uniform grid
 };

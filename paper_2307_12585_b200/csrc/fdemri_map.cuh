@@ -4,7 +4,7 @@
 // coefficients) and L105 ("the spline segment in which each value of f falls is predetermined before the
 // summation").  The map is inverted with respect to the paper: instead of a segment index per (f, voice) it
 // stores, per (voice, sign, segment-branch), the contiguous interval of bins the branch covers ("entry"), and
-// counts, per tile of FDEMRI_TILE bins, the entries that intersect it (fdemri_pairs.cuh turns the counts into
+// counts, per tile of d.tile_bins bins (FDEMRI_TILE, or 1 for the bin-major sum), the entries that intersect it (fdemri_pairs.cuh turns the counts into
 // the per-tile work lists).
 //
 // Membership (R6-R8), decided on doubles only: the knot values F_k (fdemri_knotF), the extremum
@@ -252,7 +252,7 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
                             e4.x = (int)lo_b; e4.y = (int)(hi1 - 1); e4.w = 1;
                             evals += (unsigned long long)(hi1 - lo_b);
                             ++items;
-                            const int t0 = e4.x / FDEMRI_TILE, t1 = e4.y / FDEMRI_TILE;
+                            const int t0 = e4.x / d.tile_bins, t1 = e4.y / d.tile_bins;
                             for (int t = t0; t <= t1; ++t) atomicAdd(tile_cnt + (size_t)b * d.n_tiles + t, 1);
                         }
                     }

@@ -1,4 +1,5 @@
-// fdemri_pairs.cuh -- S2c: the balanced work list.  For every tile of FDEMRI_TILE bins, the list of entries
+// fdemri_pairs.cuh -- S2c: the balanced work list.  For every tile of d.tile_bins bins (FDEMRI_TILE for the
+// tile-major sum kernel, 1 for the bin-major one), the list of entries
 // (voice, sign, segment-branch) whose bin interval intersects it, in the fixed order (voice, sign, time).
 //
 // "the spline segment in which each value of f falls is predetermined before the summation";
@@ -24,7 +25,7 @@ __global__ void k_pair_fill(FdemriDims d, const int4* __restrict__ ent, const un
     const size_t per_item = (size_t)2 * d.n_modes * d.ent_max;
     const int b = (int)(id / per_item);
     const unsigned key = (unsigned)(id - (size_t)b * per_item);
-    const int t0 = en.x / FDEMRI_TILE, t1 = en.y / FDEMRI_TILE;
+    const int t0 = en.x / d.tile_bins, t1 = en.y / d.tile_bins;
     for (int t = t0; t <= t1; ++t) {
         const size_t gt = (size_t)b * d.n_tiles + t;
         const unsigned long long pos = (unsigned long long)tile_off[gt] + (unsigned)atomicAdd(tile_cur + gt, 1);

@@ -708,3 +708,126 @@ __global__ void __launch_bounds__(256) k_inner_reduce(int n_tiles, int64_t n_fre
     }
     if (tid == 0) *reinterpret_cast<double4*>(out + 4 * (size_t)b) = make_double4(s_r[0][0], s_r[1][0], s_r[2][0], 0.0);
 }
+
+// ---------------------------------------------------------------------------------------------------------
+// Bin-major sum (sparse or down-sampled frequency arrays, section 3.3 / L218-242): when a (voice,
+// segment) covers only a few bins, a tile of bins would run every item for a handful of lanes.  Here the work
+// lists are per BIN (d.tile_bins = 1): one warp per bin, the lanes take the entries that cover it 32 at a time,
+// each lane stages its own item (same 256-byte layout, a 272-byte lane stride keeps 128-bit shared accesses
+// conflict-free), evaluates the same fast / slow term functions, and a fixed butterfly adds the lanes: every bin is
+// still written once, with no atomics, in a data-determined order.  This is the paper's own map -- the segment of
+// every (f, voice) predetermined (L105) -- with the threads over the voices of a frequency instead of over the
+// frequencies of a voice.
+// ---------------------------------------------------------------------------------------------------------
+#define FDEMRI_BIN_WARPS 8
+#define FDEMRI_BIN_STRIDE 34         // doubles per lane slot
+
+__device__ __forceinline__ bool fdemri_overflow_poison(const SumArgs& a) {
+    if (!(*(volatile const unsigned long long*)(a.stats + 5) & FDEMRI_BAD_LIST_OVERFLOW_BIT)) return false;
+    // the work list did not fit the work space: fail loudly (NaN everywhere; see fdemri_get_stats)
+    const size_t n = (size_t)a.d.n_batch * a.d.n_freq * 2;
+    const double nan = __longlong_as_double(0x7ff8000000000000ll);
+    const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nt = (size_t)gridDim.x * blockDim.x;
+    if (a.hp) {
+        for (size_t i = tid; i < n; i += nt) {
+            a.hp[i] = nan;
+            a.hx[i] = nan;
+        }
+    }
+    return true;
+}
+
+__global__ void __launch_bounds__(FDEMRI_BIN_WARPS * 32, 2) k_bin_sum(SumArgs a) {
+    extern __shared__ __align__(16) double fdemri_bin_smem[];
+    if (fdemri_overflow_poison(a)) return;
+    const FdemriDims& d = a.d;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    double* it = fdemri_bin_smem + ((size_t)wid * 32 + lane) * FDEMRI_BIN_STRIDE;
+    const int V = d.n_modes;
+    unsigned n_airy = 0, n_slow = 0, errs = 0;
+    for (;;) {
+        int gb = 0;
+        if (lane == 0) gb = (int)atomicAdd(a.tile_counter, 1u);
+        gb = __shfl_sync(0xffffffffu, gb, 0);
+        if (gb >= a.total_tiles) break;
+        const int b = gb / d.n_tiles, bin = gb - b * d.n_tiles;           // n_tiles = n_freq in this mode
+        const double f = fdemri_freq(d, bin);
+        const unsigned int off = a.tile_off[gb];
+        const int n = (int)(a.tile_off[gb + 1] - off);
+        const int wbase = (a.n_angles > 1 ? b : 0) * V;
+        const size_t rbase = (size_t)b * V * d.n_seg;
+        const int4* ent_b = a.ent + (size_t)b * 2 * V * d.ent_max;
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+        for (int base = 0; base < n; base += 32) {
+            if (base + lane < n) {
+                const unsigned int key = a.pairs[off + base + lane];
+                const int4 en = ent_b[key];
+                const int vs = (int)(key / (unsigned)d.ent_max);
+                const int v = vs >> 1;
+                const unsigned flags_in = (unsigned)((en.z >> 30) & 1);
+                fdemri_stage_item(it, a.rec + (rbase + (size_t)v * d.n_seg + (en.z & 0x3fffffff)) * R_DOUBLES, a.wts[wbase + v],
+                                  0, 0, (unsigned)(vs & 1), flags_in);
+                const unsigned flags = (unsigned)(*reinterpret_cast<const int2*>(it)).y;
+                const double sf = fdemri_xorsign(f, (flags & 4u) << 29);
+                double Tr = 0.0, Ti = 0.0;
+                bool ok = false;
+                if (!(flags & 1u)) ok = fdemri_term_fast(it, sf, Tr, Ti);
+                if (!ok) {
+                    const FdemriSlowOut o = fdemri_term_slow(it, sf, flags);
+                    Tr = o.tre; Ti = o.tim;
+                    n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                }
+                a0 = fma(it[S_WP], Tr, a0); a1 = fma(it[S_SWP], Ti, a1); a2 = fma(it[S_NWX], Ti, a2); a3 = fma(it[S_SWX], Tr, a3);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+            a0 += __shfl_xor_sync(0xffffffffu, a0, o); a1 += __shfl_xor_sync(0xffffffffu, a1, o);
+            a2 += __shfl_xor_sync(0xffffffffu, a2, o); a3 += __shfl_xor_sync(0xffffffffu, a3, o);
+        }
+        if (lane == 0) {
+            const size_t o = ((size_t)b * d.n_freq + bin) * 2;
+            *reinterpret_cast<double2*>(a.hp + o) = make_double2(a0, a1);
+            *reinterpret_cast<double2*>(a.hx + o) = make_double2(a2, a3);
+        }
+    }
+    for (int o = 16; o; o >>= 1) {
+        n_airy += __shfl_xor_sync(0xffffffffu, n_airy, o);
+        n_slow += __shfl_xor_sync(0xffffffffu, n_slow, o);
+        errs |= __shfl_xor_sync(0xffffffffu, errs, o);
+    }
+    if (lane == 0) {
+        if (n_airy) atomicAdd(a.stats + 4, (unsigned long long)n_airy);
+        if (n_slow) atomicAdd(a.stats + 7, (unsigned long long)n_slow);
+        if (errs) atomicOr(a.stats + 5, (unsigned long long)errs);
+    }
+}
+
+// Inner products of Eq. 12 from a waveform in memory (bin-major mode): one CTA per batch item, fixed order.
+__global__ void __launch_bounds__(1024) k_inner_dense(int64_t n_freq, const double* __restrict__ hp, const double* __restrict__ hx,
+                                                       const double* __restrict__ weight, const double* __restrict__ dplus,
+                                                       const double* __restrict__ dcross, int hann, double* __restrict__ out) {
+    __shared__ double s_r[3][1024];
+    const int b = blockIdx.x, tid = threadIdx.x;
+    const double4 zero = make_double4(0.0, 0.0, 0.0, 0.0);
+    const double* p = hp + (size_t)b * n_freq * 2;
+    const double* x = hx + (size_t)b * n_freq * 2;
+    auto at = [&](int64_t k) {
+        if (k < 0 || k >= n_freq) return zero;
+        return make_double4(p[2 * k], p[2 * k + 1], x[2 * k], x[2 * k + 1]);
+    };
+    double hh = 0.0, dr = 0.0, di = 0.0;
+    for (int64_t k = tid; k < n_freq; k += 1024) {
+        const double4 h = hann ? fdemri_hann3(at(k - 1), at(k), at(k + 1)) : at(k);
+        fdemri_inner_bin(h, k, weight, dplus, dcross, hh, dr, di);
+    }
+    s_r[0][tid] = hh; s_r[1][tid] = dr; s_r[2][tid] = di;
+    __syncthreads();
+    for (int o = 512; o; o >>= 1) {
+        if (tid < o) {
+            s_r[0][tid] += s_r[0][tid + o]; s_r[1][tid] += s_r[1][tid + o]; s_r[2][tid] += s_r[2][tid + o];
+        }
+        __syncthreads();
+    }
+    if (tid == 0) *reinterpret_cast<double4*>(out + 4 * (size_t)b) = make_double4(s_r[0][0], s_r[1][0], s_r[2][0], 0.0);
+}

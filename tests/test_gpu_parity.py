@@ -397,3 +397,43 @@ def test_random_small_cases_sweep(fd, orc):
         wf.close()
     assert skipped <= 5
     print(f"[parity] 20 random small cases ({skipped} flagged unsupported): worst max|dh|/max|h| = {worst:.3e}")
+
+
+@pytest.mark.parametrize("mode", ["bin", "tile"])
+def test_both_sum_kernels_on_the_same_inputs(fd, orc, mode):
+    """The bin-major kernel (sparse grids, section 3.3) and the tile-major kernel forced on the same inputs:
+    a small turnover case, and config 3 (the 10^4 log-spaced frequencies) -- each against the oracle."""
+    from paper_2307_12585_b200 import synth
+    flag = fd.FDEMRI_FLAG_BIN_MAJOR if mode == "bin" else fd.FDEMRI_FLAG_TILE_MAJOR
+    for label, w in (("small", synth.small_case(seed=2, n_knots=14)), ("config3", workload(3))):
+        wf = fd.waveform_from_workload(w, flags=flag)
+        wf.sum(w.theta, w.phi)
+        hp, hx = wf.result()
+        st = wf.stats()
+        ref = oracle_c(orc, w, w.freq_array())
+        check(hp[0], hx[0], ref, f"{label}, {mode}-major")
+        assert st["n_evals"] == ref["n_evals"]
+        if mode == "bin":
+            assert st["n_pairs"] == ref["n_evals"]            # one work-list entry per (entry, bin)
+        wf.close()
+
+
+def test_bin_major_grows_its_work_list_and_fused_inner(fd, orc):
+    """Config 1 forced through the bin-major kernel: 4.9e7 work-list entries do not fit the default capacity, so the
+    binding has to grow the work space; then parity, and the Eq. 12 inner products formed from the written waveform."""
+    import torch
+    w = workload(1)
+    wf = fd.waveform_from_workload(w, flags=fd.FDEMRI_FLAG_BIN_MAJOR)
+    ref = oracle_c(orc, w, w.freq_array())
+    out = torch.zeros((1, 4), dtype=torch.float64, device=wf.dev)
+    fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, out, hann=True, hplus=wf.hplus, hcross=wf.hcross)
+    hp, hx = wf.result()
+    check(hp[0], hx[0], ref, "config1, bin-major")
+    st = wf.stats()
+    assert st["n_pairs"] == ref["n_evals"] == st["n_evals"]
+    want_hh, _ = orc.inner(ref["hplus"], ref["hcross"], hann=True)
+    assert abs(out.cpu().numpy()[0, 0] - want_hh) <= 1e-10 * want_hh
+    with pytest.raises(fd.FdemriError) as ei:                    # no waveform buffers: unsupported in this mode
+        fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, out)
+    assert ei.value.status == 5
+    wf.close()
