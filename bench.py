@@ -28,7 +28,7 @@ sys.path.insert(0, ROOT)
 METRIC = "waveforms/s, 3843-mode 2-yr FD sum (FP64)"
 FLOP_PER_EVAL = 200.0          # SURVEY.md 8(d) / DESIGN.md: algorithmic FP64 flop per mode-bin evaluation
 TILE_SUM_DRAM_BYTES = 175.3e6    # ncu capture of config 2, profiles/r1g_final.md
-KERNELS_PER_STEP = 8           # spline_shared, spline_amp, records, pair_scan, pair_fill, pair_sort | weights, tile_sum
+KERNELS_PER_STEP = 8           # spline_shared, spline_amp, records, pair_scan, pair_pass<1>, pair_sort | weights, sum (+ pair_pass<0> in bin-major mode)
 
 
 def workload_name(idx, w):

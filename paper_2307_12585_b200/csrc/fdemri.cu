@@ -210,12 +210,16 @@ extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const 
     if (cudaMemsetAsync(p->tile_cnt, 0, 2 * NT * sizeof(int), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
     size_t nrec = (size_t)d.n_batch * d.n_modes * d.n_seg;
     k_records<<<(unsigned)((nrec + 127) / 128), 128, 0, st>>>(d, p->lmn_dev, p->t_knots_dev, p->sh_hi, p->sh_lo, f_phi, f_r,
-                                                              p->rec, p->ent, p->tile_cnt, p->stats);
-    k_pair_scan<<<1, 1024, 0, st>>>(NT, p->tile_cnt, p->tile_off, p->pair_cap, p->stats);
+                                                              p->rec, p->ent, d.tile_bins == 1 ? nullptr : p->tile_cnt, p->stats);
     const size_t nslots = (size_t)d.n_batch * d.n_modes * 2 * d.ent_max;
-    k_pair_fill<<<(unsigned)((nslots + 255) / 256), 256, 0, st>>>(d, p->ent, p->tile_off, p->tile_cnt + NT, p->pairs,
-                                                                  p->pair_cap);
-    k_pair_sort<<<(unsigned)NT, 256, FDEMRI_SORT_MAX * sizeof(unsigned int), st>>>(NT, p->tile_off, p->pairs, p->pair_cap);
+    const unsigned nb = (unsigned)((nslots + 255) / 256);
+    if (d.tile_bins == 1)
+        k_pair_pass<0><<<nb, 256, 0, st>>>(d, p->ent, p->tile_cnt, p->tile_off, p->tile_cnt + NT, p->pairs, p->pair_cap);
+    k_pair_scan<<<1, 1024, 0, st>>>(NT, p->tile_cnt, p->tile_off, p->pair_cap, p->stats);
+    k_pair_pass<1><<<nb, 256, 0, st>>>(d, p->ent, p->tile_cnt, p->tile_off, p->tile_cnt + NT, p->pairs, p->pair_cap);
+    // per-bin lists are short (a few hundred keys): smaller CTAs, more of them resident
+    k_pair_sort<<<(unsigned)NT, d.tile_bins == 1 ? 64 : 256, FDEMRI_SORT_MAX * sizeof(unsigned int), st>>>(NT, p->tile_off, p->pairs,
+                                                                                                       p->pair_cap);
     if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
     p->built = true;
     return FDEMRI_OK;

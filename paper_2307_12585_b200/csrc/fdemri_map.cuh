@@ -3,9 +3,8 @@
 // S2 follows PAPER.md L103 (A..D = mode-number-weighted sums of the fundamental-frequency spline
 // coefficients) and L105 ("the spline segment in which each value of f falls is predetermined before the
 // summation").  The map is inverted with respect to the paper: instead of a segment index per (f, voice) it
-// stores, per (voice, sign, segment-branch), the contiguous interval of bins the branch covers ("entry"), and
-// counts, per tile of d.tile_bins bins (FDEMRI_TILE, or 1 for the bin-major sum), the entries that intersect it (fdemri_pairs.cuh turns the counts into
-// the per-tile work lists).
+// stores, per (voice, sign, segment-branch), the contiguous interval of bins the branch covers ("entry");
+// fdemri_pairs.cuh turns the entries into per-tile work lists.
 //
 // Membership (R6-R8), decided on doubles only: the knot values F_k (fdemri_knotF), the extremum
 // value F_e of a turnover segment (record slot R_Q2) and the bin frequencies f_i.
@@ -131,7 +130,8 @@ __device__ int64_t fdemri_first_gt(const FdemriDims& d, double x) {
 }
 
 // ent: [B][V][2][ent_max] int4 {first bin, last bin, seg | branchB << 30, 1}, slot = 2*seg + branch (time order);
-// empty slots have w = 0.  tile_cnt: [B][n_tiles] entries intersecting every tile.
+// empty slots have w = 0.  tile_cnt: [B][n_tiles] entries per tile, counted here for the tile-major lists (NULL: the
+// per-bin lists of the bin-major mode are counted by k_pair_pass<0>, which shares wide entries among the lanes).
 __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ t_knots,
                           const double* __restrict__ sh_hi, const double* __restrict__ sh_lo,
                           const double* __restrict__ f_phi, const double* __restrict__ f_r, double* __restrict__ rec,
@@ -252,8 +252,10 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
                             e4.x = (int)lo_b; e4.y = (int)(hi1 - 1); e4.w = 1;
                             evals += (unsigned long long)(hi1 - lo_b);
                             ++items;
-                            const int t0 = e4.x / d.tile_bins, t1 = e4.y / d.tile_bins;
-                            for (int t = t0; t <= t1; ++t) atomicAdd(tile_cnt + (size_t)b * d.n_tiles + t, 1);
+                            if (tile_cnt) {                 // tile-major lists: an entry meets a handful of tiles
+                                const int t0 = e4.x / d.tile_bins, t1 = e4.y / d.tile_bins;
+                                for (int t = t0; t <= t1; ++t) atomicAdd(tile_cnt + (size_t)b * d.n_tiles + t, 1);
+                            }
                         }
                     }
                 }

@@ -3,7 +3,8 @@
 // (voice, sign, segment-branch) whose bin interval intersects it, in the fixed order (voice, sign, time).
 //
 // "the spline segment in which each value of f falls is predetermined before the summation";
-// here the predetermined map is per tile: count -> prefix sum -> fill -> sort.  The fill uses atomic cursors, so
+// here the predetermined map is per tile: count -> prefix sum -> fill -> sort (k_pair_pass<0>, k_pair_scan,
+// k_pair_pass<1>, k_pair_sort).  The fill uses atomic cursors, so
 // the order inside a tile is arbitrary until k_pair_sort puts the keys (unique, = entry index) in ascending
 // order: the sum kernel then walks every tile in a data-determined order (bitwise reproducible results).
 //   key = (voice*2 + sign) * ent_max + e                (32 bits; the batch item is implied by the tile)
@@ -14,23 +15,52 @@
 
 #define FDEMRI_SORT_MAX 8192         // keys per tile the shared-memory sorter takes
 
-// Fill: one thread per (batch item, voice, sign, entry slot); the counts come from k_records.
-__global__ void k_pair_fill(FdemriDims d, const int4* __restrict__ ent, const unsigned int* __restrict__ tile_off,
-                            int* __restrict__ tile_cur, unsigned int* __restrict__ pairs, unsigned long long cap) {
+// Tiles t0..t1 of one entry, for every lane of a warp: narrow ranges (the rule) are walked by their own lane, wide
+// ones -- an entry of a slowly sweeping voice can cover thousands of bins of a sparse grid -- by the whole warp, so
+// that no lane holds the others up.  op(key, tile_base, tile) is called once per (entry, tile) pair, with the
+// entry's key and tile base (batch item * n_tiles).  All 32 lanes must call this (has = false: no entry).
+template <class Op>
+__device__ __forceinline__ void fdemri_for_tiles(bool has, int t0, int t1, unsigned key, unsigned long long tile_base, Op op) {
+    const int lane = threadIdx.x & 31;
+    const bool wide = has && (t1 - t0) >= 16;
+    if (has && !wide)
+        for (int t = t0; t <= t1; ++t) op(key, tile_base, t);
+    __syncwarp();
+    unsigned todo = __ballot_sync(0xffffffffu, wide);
+    while (todo) {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const int a0 = __shfl_sync(0xffffffffu, t0, src), a1 = __shfl_sync(0xffffffffu, t1, src);
+        const unsigned k = __shfl_sync(0xffffffffu, key, src);
+        const unsigned long long tb = __shfl_sync(0xffffffffu, tile_base, src);
+        for (int t = a0 + lane; t <= a1; t += 32) op(k, tb, t);
+    }
+}
+
+// One thread per (batch item, voice, sign, entry slot).  MODE 0: count the entries of every tile;  MODE 1: fill the
+// lists through atomic cursors (k_pair_sort then fixes the order).  blockDim.x % 32 == 0.
+template <int MODE>
+__global__ void k_pair_pass(FdemriDims d, const int4* __restrict__ ent, int* __restrict__ tile_cnt,
+                            const unsigned int* __restrict__ tile_off, int* __restrict__ tile_cur,
+                            unsigned int* __restrict__ pairs, unsigned long long cap) {
     const size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const size_t total = (size_t)d.n_batch * d.n_modes * 2 * d.ent_max;
-    if (id >= total) return;
-    const int4 en = ent[id];
-    if (!en.w) return;
     const size_t per_item = (size_t)2 * d.n_modes * d.ent_max;
-    const int b = (int)(id / per_item);
-    const unsigned key = (unsigned)(id - (size_t)b * per_item);
-    const int t0 = en.x / d.tile_bins, t1 = en.y / d.tile_bins;
-    for (int t = t0; t <= t1; ++t) {
-        const size_t gt = (size_t)b * d.n_tiles + t;
-        const unsigned long long pos = (unsigned long long)tile_off[gt] + (unsigned)atomicAdd(tile_cur + gt, 1);
-        if (pos < cap) pairs[pos] = key;
-    }
+    int4 en = make_int4(0, -1, 0, 0);
+    if (id < total) en = ent[id];
+    const size_t idc = id < total ? id : total - 1;
+    const int b = (int)(idc / per_item);
+    const unsigned key = (unsigned)(idc - (size_t)b * per_item);
+    fdemri_for_tiles(en.w != 0, en.x / d.tile_bins, en.y / d.tile_bins, key, (unsigned long long)b * d.n_tiles,
+                     [&](unsigned k, unsigned long long tb, int t) {
+                         const size_t gt = (size_t)tb + t;
+                         if (MODE == 0) {
+                             atomicAdd(tile_cnt + gt, 1);
+                         } else {
+                             const unsigned long long pos = (unsigned long long)tile_off[gt] + (unsigned)atomicAdd(tile_cur + gt, 1);
+                             if (pos < cap) pairs[pos] = k;
+                         }
+                     });
 }
 
 // Exclusive prefix sum of cnt[0..n) into off[0..n], off[n] = total.  One CTA (n is a few thousand per waveform).
