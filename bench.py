@@ -105,7 +105,15 @@ def cpu_oracle_sample(w, total_evals, n_bins=500000, seed=0):
                      w.theta, w.phi, extra=False)
     dt = time.perf_counter() - t0
     frac = r["n_evals"] / float(total_evals) if total_evals else float("nan")
-    return {"value": frac / dt, "unit": "waveforms/s", "cores": orc.num_threads, "kind": "oracle",
+    # one thread, on a smaller sample (single-thread time beside the all-cores one)
+    idx1 = idx[:: max(1, len(idx) // 12000)]
+    t1 = time.perf_counter()
+    r1 = orc.waveform(w.lmn, w.t_knots[0], w.f_phi[0], w.f_r[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0], w.freq_array()[idx1],
+                      w.theta, w.phi, extra=False, n_threads=1)
+    dt1 = time.perf_counter() - t1
+    single = {"evals_per_s": r1["n_evals"] / dt1, "waveforms_per_s": (r1["n_evals"] / float(total_evals)) / dt1 if total_evals else None,
+              "seconds": dt1, "bins": int(len(idx1))}
+    return {"single_thread": single, "value": frac / dt, "unit": "waveforms/s", "cores": orc.num_threads, "kind": "oracle",
             "sample": f"{len(idx)} random bins of the covered band ({r['n_evals']} of {int(total_evals)} mode-bin "
                       f"evaluations) incl. the oracle's spline build, {dt:.2f} s wall; scaled by evaluation count",
             "evals_per_s": r["n_evals"] / dt, "seconds": dt}

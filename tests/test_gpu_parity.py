@@ -437,3 +437,14 @@ def test_bin_major_grows_its_work_list_and_fused_inner(fd, orc):
         fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, out)
     assert ei.value.status == 5
     wf.close()
+
+
+def test_config2_every_bin(fd, orc):
+    """BASELINE config 2 element by element over all 3 155 816 bins (the oracle needs ~20 s on the box's host cores):
+    per-bin parity, mismatch, evaluation count (P9), exact zeros wherever the oracle has no term (P8)."""
+    w = workload(2)
+    wf, hp, hx, st = run_gpu(fd, w)
+    ref = oracle_c(orc, w, w.freq_array())
+    check(hp[0], hx[0], ref, "config2, every bin")
+    assert st["n_evals"] == ref["n_evals"] and ref["max_roots"] == 2
+    wf.close()
