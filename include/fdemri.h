@@ -35,7 +35,8 @@ enum {
     FDEMRI_ERR_WORKSPACE = 2,   /* work space missing or too small (fdemri_stats.n_pairs: work-list entries needed) */
     FDEMRI_ERR_CUDA = 3,        /* a CUDA runtime call or kernel failed                                   */
     FDEMRI_ERR_NOT_BUILT = 4,   /* fdemri_sum / get_coeffs before fdemri_build_splines                    */
-    FDEMRI_ERR_UNSUPPORTED = 5  /* input violates an assumption of the method (see fdemri_stats.flags)    */
+    FDEMRI_ERR_UNSUPPORTED = 5  /* the call is not available in this configuration (fdemri_sum_inner without
+                                   waveform buffers on a bin-major plan)                                    */
 };
 
 /* plan flags */
@@ -52,7 +53,8 @@ enum {
 
 /* bits of fdemri_stats.flags (device-side validation, read back by fdemri_get_stats) */
 enum {
-    FDEMRI_BAD_TWO_EXTREMA = 1,   /* a segment cubic has two interior extrema (paper assumes <= 1, L105)   */
+    FDEMRI_BAD_TWO_EXTREMA = 1,   /* (not raised any more: a segment cubic with two interior extrema -- the paper
+                                     assumes at most one, L105 -- is split into its three monotone branches)   */
     FDEMRI_BAD_NONFINITE = 4,     /* NaN/Inf met in the inputs or spline coefficients                      */
     FDEMRI_BAD_NEWTON = 8,        /* a root iteration hit its iteration cap                                */
     FDEMRI_BAD_LIST_OVERFLOW = 16 /* the per-tile work list did not fit the work space: fdemri_sum fills its outputs

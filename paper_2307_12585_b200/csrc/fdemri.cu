@@ -103,14 +103,14 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
     int64_t n_tiles = (n_freq + tile_bins - 1) / tile_bins;
     if (n_tiles * (int64_t)n_batch >= ((int64_t)1 << 31)) return FDEMRI_ERR_INVALID_ARG;
     if ((int64_t)n_batch * n_modes * (n_knots - 1) >= ((int64_t)1 << 31)) return FDEMRI_ERR_INVALID_ARG;   /* 32-bit record index */
-    if ((int64_t)n_modes * 4 * (n_knots - 1) >= ((int64_t)1 << 32)) return FDEMRI_ERR_INVALID_ARG;          /* 32-bit work-list key */
+    if ((int64_t)n_modes * 6 * (n_knots - 1) >= ((int64_t)1 << 32)) return FDEMRI_ERR_INVALID_ARG;          /* 32-bit work-list key */
     fdemri_plan_s* p = new (std::nothrow) fdemri_plan_s();
     if (!p) return FDEMRI_ERR_INVALID_ARG;
     p->d.n_modes = n_modes;
     p->d.n_batch = n_batch;
     p->d.n_knots = n_knots;
     p->d.n_seg = n_knots - 1;
-    p->d.ent_max = 2 * (n_knots - 1);                 /* slot = 2*segment + branch */
+    p->d.ent_max = 3 * (n_knots - 1);                 /* slot = 3*segment + branch */
     p->d.n_freq = n_freq;
     p->d.tile_bins = tile_bins;
     p->d.n_tiles = (int)n_tiles;
@@ -345,7 +345,6 @@ extern "C" int fdemri_get_stats(fdemri_plan_t p, fdemri_stats* out) {
     out->n_slow = h[7];
     out->n_pairs = h[8];
     if (h[5] & FDEMRI_BAD_LIST_OVERFLOW) return FDEMRI_ERR_WORKSPACE;
-    if (h[5] & FDEMRI_BAD_TWO_EXTREMA) return FDEMRI_ERR_UNSUPPORTED;
     if (h[5] & FDEMRI_BAD_NONFINITE) return FDEMRI_ERR_INVALID_ARG;
     return FDEMRI_OK;
 }

@@ -27,7 +27,7 @@ enum {
     R_FC = 2,
     R_FD = 3,
     R_Q1 = 4,   // normal segment: seed tau0 = x (Q1 + x (Q2 + x Q3)), x = s f - FA
-    R_Q2 = 5,   // turnover segment: Q1 = tau_e, Q2 = F_e, Q3 = C + 3 D tau_e
+    R_Q2 = 5,   // one interior extremum: Q1 = tau_e, Q2 = F_e;  two (R5): Q1 = tau_e1, Q2 = F_e1, Q3 = tau_e2, SF = F_e2
     R_Q3 = 6,
     R_H = 7,    // segment length h_k
     R_AR = 8,   // Re A coefficients a,b,c,d  (8..11)   (32-byte aligned: written as one double4)
@@ -38,8 +38,8 @@ enum {
     R_NC = 19,  // -c_Phi/2pi
     R_ND = 20,  // -d_Phi/2pi
     R_TK = 21,  // t_k
-    R_TYPE = 22,// 0.0 normal, 1.0 turnover (one interior extremum), 2.0 unsupported (two)
-    R_SF = 23,  // sign (+-1.0) of dF/dtau on the segment (turnover: on its first branch)
+    R_TYPE = 22,// number of interior extrema of F on the segment: 0.0, 1.0 or 2.0
+    R_SF = 23,  // type 0: sign (+-1.0) of dF/dtau on the segment;  type 2: F_e2
     R_DOUBLES = 24
 };
 
@@ -49,15 +49,16 @@ enum {
 // 32 doubles = 256 B; consumers read it with broadcast LDS.
 // ------------------------------------------------------------------------------------------------
 enum {
-    S_META = 0, // int2 {lo | hi << 16 (tile-relative bins), type | branchB << 1 | sign << 2}
+    S_META = 0, // int2 {lo | hi << 16 (tile-relative bins), flags: 1 = branch of a segment with extrema (slow path),
+                // 2 = a second extremum bounds the branch, 4 = sign s}
     S_F32A = 1, // float2 {FB, FC}: single-precision copies for the first iterate of the inversion
     S_NFA = 2,  // -FA
     S_FB = 3,
     S_FC = 4,
     S_FD = 5,
-    S_Q1 = 6,
-    S_Q2 = 7,
-    S_Q3 = 8,
+    S_Q1 = 6,   // monotone segment: seed of the inverse (Q1..Q3).  Branch of a segment with extrema: the extremum it
+    S_Q2 = 7,   // starts or ends at, {tau_e, F_e, c2 = C + 3 D tau_e}: F - F_e = z^2 (c2 + D z), z = tau - tau_e; its time
+    S_Q3 = 8,   // bracket [ta, tb] in S_F32A, S_F32B; a second extremum {tau_e, F_e, c2} in S_F32C, S_FREE, S_TOLH
     S_TOLH = 9, // acceptance threshold of the last Newton correction, 2e-7 h
     S_HH = 10,  // h/2
     S_F32B = 11,// float2 {FD, Q1}
@@ -81,7 +82,7 @@ enum {
 
 struct FdemriDims {
     int n_modes, n_batch, n_knots, n_seg;   // n_seg = n_knots - 1
-    int ent_max;                            // entry slots per (voice, sign) = 2 * n_seg (segment, branch)
+    int ent_max;                            // entry slots per (voice, sign) = 3 * n_seg (segment, branch)
     int64_t n_freq;
     int tile_bins;                          // bins per work-list tile: FDEMRI_TILE (tile-major sum) or 1 (bin-major sum)
     int n_tiles;                            // tiles per batch item = ceil(n_freq / tile_bins)

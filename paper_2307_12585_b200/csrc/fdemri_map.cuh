@@ -11,7 +11,8 @@
 //   branch from value Va (start, in time) to Vb (end):
 //     normal segment        : Va = F_k included, Vb = F_{k+1} excluded          (half-open in time, R6)
 //     turnover, 1st branch  : Va = F_k included, Vb = F_e included               (R7)
-//     turnover, 2nd branch  : Va = F_e excluded, Vb = F_{k+1} excluded
+//     turnover, last branch : Va = F_e excluded, Vb = F_{k+1} excluded
+//     two extrema (R5), middle branch: Va = F_e1 excluded, Vb = F_e2 included
 //   a bin f_i > 0 belongs to the branch for sign s when s*f_i lies between Va and Vb under those rules.
 #pragma once
 #include "fdemri_common.cuh"
@@ -129,7 +130,7 @@ __device__ int64_t fdemri_first_gt(const FdemriDims& d, double x) {
     return i;
 }
 
-// ent: [B][V][2][ent_max] int4 {first bin, last bin, seg | branchB << 30, 1}, slot = 2*seg + branch (time order);
+// ent: [B][V][2][ent_max] int4 {first bin, last bin, seg | branch << 30, 1}, slot = 3*seg + branch (time order);
 // empty slots have w = 0.  tile_cnt: [B][n_tiles] entries per tile, counted here for the tile-major lists (NULL: the
 // per-bin lists of the bin-major mode are counted by k_pair_pass<0>, which shares wide entries among the lanes).
 __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ t_knots,
@@ -205,13 +206,19 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
         double te = ext[0];
         rQ1 = te;
         rQ2 = FA + te * (FB + te * (FC + te * FD));          // F_e (R7)
-        rQ3 = FC + 3.0 * FD * te;                            // F(t) - F_e = z^2 (Q3 + FD z), z = t - te
+        rQ3 = 0.0;
         rTYPE = 1.0;
-        rSF = (rQ2 < FA) ? -1.0 : 1.0;                       // first branch runs from F_k to F_e
+        rSF = 0.0;
         atomicAdd(stats + 3, 1ull);
     } else {
-        rQ1 = 0.0; rQ2 = 0.0; rQ3 = 0.0; rTYPE = 2.0; rSF = 1.0;
-        atomicOr(stats + 5, 1ull);                           // FDEMRI_BAD_TWO_EXTREMA
+        // two interior extrema (the paper assumes at most one, L105; R5): three monotone branches
+        const double t1 = ext[0], t2 = ext[1];
+        rQ1 = t1;
+        rQ2 = FA + t1 * (FB + t1 * (FC + t1 * FD));          // F_e1
+        rQ3 = t2;
+        rTYPE = 2.0;
+        rSF = FA + t2 * (FB + t2 * (FC + t2 * FD));          // F_e2 (the slot of the sign, which type 0 alone needs)
+        atomicAdd(stats + 3, 1ull);
     }
     if (bad) atomicOr(stats + 5, 4ull);
     // ---- bin intervals of the branches of this segment, for both signs (L105) ----
@@ -229,15 +236,17 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
                                                         f_r[(size_t)b * d.n_knots + d.n_knots - 1]);
     const int64_t first_pos = fdemri_first_gt(d, 0.0);      // bins with f > 0 only (R13)
     unsigned long long evals = 0, items = 0;
+    // branch j of the segment runs from V[j] to V[j+1]: knot value, extremum values, next knot value; a branch includes
+    // its start iff that is the knot and its end iff that is an extremum (R6, R7)
+    const double Vv[4] = {Fk, type >= 1 ? rQ2 : Fk1, type == 2 ? rSF : Fk1, Fk1};
+    const int nbr = type + 1;
     for (int sg = 0; sg < 2; ++sg) {
-        int4* E = ent + ((bv * 2 + sg) * (size_t)d.ent_max) + 2 * k;
-        for (int br = 0; br < 2; ++br) {
+        int4* E = ent + ((bv * 2 + sg) * (size_t)d.ent_max) + 3 * k;
+        for (int br = 0; br < 3; ++br) {
             int4 e4 = make_int4(0, -1, k | (br << 30), 0);
-            if (type != 2 && (br == 0 || type == 1)) {
-                double Va, Vb; bool a_incl, b_incl;
-                if (type == 0) { Va = Fk; Vb = Fk1; a_incl = true; b_incl = false; }
-                else if (br == 0) { Va = Fk; Vb = rQ2; a_incl = true; b_incl = true; }
-                else { Va = rQ2; Vb = Fk1; a_incl = false; b_incl = false; }
+            if (br < nbr) {
+                const double Va = Vv[br], Vb = Vv[br + 1];
+                const bool a_incl = (br == 0), b_incl = (br + 1 < nbr);
                 if (Va != Vb) {
                     const double lo_v = fmin(Va, Vb), hi_v = fmax(Va, Vb);
                     const bool lo_incl = (Va < Vb) ? a_incl : b_incl;

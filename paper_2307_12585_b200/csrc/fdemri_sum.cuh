@@ -253,12 +253,14 @@ __device__ __noinline__ FdemriSlowOut fdemri_term_slow(const double* it, double 
         Fdd = 2.0 * fma(tau, FD, c2);
         out.info |= 2u;
     } else {
-        // turnover segment: F(tau) - F_e = z^2 (c2 + FD z), z = tau - tau_e; branch A: z < 0, branch B: z > 0
-        const double te = it[S_Q1], Fe = it[S_Q2], c2 = it[S_Q3];
-        const bool brB = flags & 2u;
+        // branch of a segment with extrema, bracket [ta, tb]: around the extremum it hangs on (the nearer one in value
+        // when it hangs between two)  F(tau) - F_e = z^2 (c2 + FD z),  z = tau - tau_e
+        const double ta = it[S_F32A], tb = it[S_F32B];
+        double te = it[S_Q1], Fe = it[S_Q2], c2 = it[S_Q3];
+        if ((flags & 2u) && fabs(sf - it[S_FREE]) < fabs(sf - Fe)) { te = it[S_F32C]; Fe = it[S_FREE]; c2 = it[S_TOLH]; }
         const double Delta = sf - Fe;
         double z = sqrt(fmax(Delta / c2, 0.0));
-        if (!brB) z = -z;
+        if (0.5 * (ta + tb) < te) z = -z;
         const double tol = 1e-14 * h;
         int n = 0;
         for (; n < 40; ++n) {
@@ -270,8 +272,8 @@ __device__ __noinline__ FdemriSlowOut fdemri_term_slow(const double* it, double 
             if (fabs(delta) <= tol) break;
         }
         if (n == 40) out.info |= (8u << 4);
-        z = brB ? fmin(fmax(z, 0.0), h - te) : fmax(fmin(z, 0.0), -te);
-        tau = te + z;
+        tau = fmin(fmax(te + z, ta), tb);
+        z = tau - te;
         Fd = z * fma(3.0 * FD, z, 2.0 * c2);          // exact factorisation, no cancellation near Fdot = 0
         Fdd = fma(6.0 * FD, tau, 2.0 * FC);
     }
@@ -344,7 +346,7 @@ struct FdemriRing {
 
 // Producer lane: folds record + weights + sign into the staged item `dst` (shared memory)
 __device__ __forceinline__ void fdemri_stage_item(double* dst, const double* __restrict__ R, const double4 w, int lo,
-                                                  int hi, unsigned sg, unsigned brB) {
+                                                  int hi, unsigned sg, unsigned br) {
     const double4* R4 = reinterpret_cast<const double4*>(R);
     const double4 r0 = fdemri_ld4(R4 + 0);       // FA FB FC FD
     const double4 r1 = fdemri_ld4(R4 + 1);       // Q1 Q2 Q3 H
@@ -352,25 +354,48 @@ __device__ __forceinline__ void fdemri_stage_item(double* dst, const double* __r
     const double4 r3 = fdemri_ld4(R4 + 3);       // Im A
     const double4 r4 = fdemri_ld4(R4 + 4);       // PC BH BL NC
     const double4 r5 = fdemri_ld4(R4 + 5);       // ND TK TYPE SF
-    const unsigned type = (unsigned)r5.z;
+    const unsigned type = (unsigned)r5.z;        // interior extrema of F on the segment: 0, 1, 2
     const double s = sg ? -1.0 : 1.0;
-    const double sF = (type == 1u && brB) ? -r5.w : r5.w;
     const double h = r1.w;
     double2* d2 = reinterpret_cast<double2*>(dst);
-    int2 meta = make_int2(lo | (hi << 16), (int)((type & 1u) | (brB << 1) | (sg << 2)));
-    const float2 f32a = make_float2((float)r0.y, (float)r0.z);               // FB, FC
-    const float2 f32b = make_float2((float)r0.w, (float)r1.x);               // FD, Q1
-    const float2 f32c = make_float2((float)r1.y, (float)r1.z);               // Q2, Q3
-    d2[0] = make_double2(__hiloint2double(meta.y, meta.x), *reinterpret_cast<const double*>(&f32a));
+    double sF, q1 = r1.x, q2 = r1.y, q3 = r1.z, x9, x11, x15 = 0.0, x19, x1;
+    unsigned fl = sg << 2;
+    if (type == 0u) {
+        sF = r5.w;
+        const float2 f32a = make_float2((float)r0.y, (float)r0.z);           // FB, FC
+        const float2 f32b = make_float2((float)r0.w, (float)r1.x);           // FD, Q1
+        const float2 f32c = make_float2((float)r1.y, (float)r1.z);           // Q2, Q3
+        x1 = *reinterpret_cast<const double*>(&f32a);
+        x11 = *reinterpret_cast<const double*>(&f32b);
+        x19 = *reinterpret_cast<const double*>(&f32c);
+        x9 = 2e-7 * h;
+    } else {
+        // branch `br` of a segment with extrema at te1 (< te2): [0, te1], (te1, te2 or h], (te2, h); F' alternates in sign
+        const double te1 = r1.x, Fe1 = r1.y, te2 = r1.z, Fe2 = r5.w;
+        const double s0 = (Fe1 < r0.x) ? -1.0 : 1.0;                        // first branch runs from F_k to F_e1
+        sF = (br == 1u) ? -s0 : s0;
+        const bool two = type == 2u;
+        const double ta = (br == 0u) ? 0.0 : (br == 1u ? te1 : te2);
+        const double tb = (br == 0u) ? te1 : (br == 1u && two ? te2 : h);
+        const bool useB = br == 2u;                                          // the extremum the branch hangs on
+        q1 = useB ? te2 : te1;
+        q2 = useB ? Fe2 : Fe1;
+        q3 = fma(3.0 * r0.w, q1, r0.z);                                      // c2 = C + 3 D tau_e
+        x1 = ta; x11 = tb;
+        x19 = te2; x15 = Fe2; x9 = fma(3.0 * r0.w, te2, r0.z);              // the second one (middle branch only)
+        fl |= 1u | ((br == 1u && two) ? 2u : 0u);
+    }
+    int2 meta = make_int2(lo | (hi << 16), (int)fl);
+    d2[0] = make_double2(__hiloint2double(meta.y, meta.x), x1);
     d2[1] = make_double2(-r0.x, r0.y);
     d2[2] = make_double2(r0.z, r0.w);
-    d2[3] = make_double2(r1.x, r1.y);
-    d2[4] = make_double2(r1.z, 2e-7 * h);
-    d2[5] = make_double2(0.5 * h, *reinterpret_cast<const double*>(&f32b));
+    d2[3] = make_double2(q1, q2);
+    d2[4] = make_double2(q3, x9);
+    d2[5] = make_double2(0.5 * h, x11);
     d2[6] = make_double2(sF * 1.9098593171027440, 4.0 * r5.y);
-    d2[7] = make_double2(4.0 * ((r0.x - r4.y) - r4.z), 0.0);      // F_k and b' nearly cancel: the difference is exact
+    d2[7] = make_double2(4.0 * ((r0.x - r4.y) - r4.z), x15);      // F_k and b' nearly cancel: the difference is exact
     d2[8] = make_double2(4.0 * r4.w, 4.0 * r5.x);
-    d2[9] = make_double2(fma(4.0, r4.x + w.z, -0.5 * sF), *reinterpret_cast<const double*>(&f32c));
+    d2[9] = make_double2(fma(4.0, r4.x + w.z, -0.5 * sF), x19);
     d2[10] = make_double2(r2.x, r2.y);
     d2[11] = make_double2(r2.z, r2.w);
     d2[12] = make_double2(r3.x, r3.y);
@@ -413,7 +438,7 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
                 const int seg = en.z & 0x3fffffff;
                 const int v = vs >> 1;
                 fdemri_stage_item(ring->st[stage].items[lane], a.rec + (rbase + (size_t)v * d.n_seg + seg) * R_DOUBLES,
-                                  a.wts[wbase + v], lo_e, hi_e, (unsigned)(vs & 1), (unsigned)((en.z >> 30) & 1));
+                                  a.wts[wbase + v], lo_e, hi_e, (unsigned)(vs & 1), (unsigned)((en.z >> 30) & 3));
             }
             base += FDEMRI_CHUNK;
             __syncwarp();
@@ -764,7 +789,7 @@ __global__ void __launch_bounds__(FDEMRI_BIN_WARPS * 32, 2) k_bin_sum(SumArgs a)
                 const int4 en = ent_b[key];
                 const int vs = (int)(key / (unsigned)d.ent_max);
                 const int v = vs >> 1;
-                const unsigned flags_in = (unsigned)((en.z >> 30) & 1);
+                const unsigned flags_in = (unsigned)((en.z >> 30) & 3);
                 fdemri_stage_item(it, a.rec + (rbase + (size_t)v * d.n_seg + (en.z & 0x3fffffff)) * R_DOUBLES, a.wts[wbase + v],
                                   0, 0, (unsigned)(vs & 1), flags_in);
                 const unsigned flags = (unsigned)(*reinterpret_cast<const int2*>(it)).y;
