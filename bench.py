@@ -350,26 +350,33 @@ def main():
     # ---- end to end through host buffers (pinned H2D of inputs, D2H of both polarisations) ----
     e2e = None
     if not args.no_e2e:
-        # Throughput pipeline over two sets of buffers: the compute stream uploads the inputs of step i (pinned H2D)
-        # and runs S0-S4 while the copy stream downloads the polarisations of step i-1 (pinned D2H, ~101 MB: the
-        # PCIe link, not the kernels, would otherwise set the pace).  Every byte in and out crosses inside the
-        # timed region; the region ends when the last download has landed.
+        # Throughput pipeline over two sets of buffers and three streams: the upload stream brings the inputs of step
+        # i+1 (pinned H2D, 9 MB), the compute stream runs S0-S4 of step i, the download stream takes the polarisations
+        # of step i-1 home (pinned D2H, 101 MB: the PCIe link, not the kernels, would otherwise set the pace).  Every
+        # byte in and out crosses inside the timed region; the region ends when the last download has landed.
         pin_in = [torch.from_numpy(a).pin_memory() for a in host]
+        ins = [dev_in, [torch.empty_like(t) for t in dev_in]]
         outs = [(wf.hplus, wf.hcross), (torch.empty_like(wf.hplus), torch.empty_like(wf.hcross))]
         pin_out = [[torch.empty(wf.hplus.shape, dtype=torch.float64).pin_memory() for _ in range(2)] for _ in range(2)]
         h2d = sum(a.numel() * 8 for a in pin_in)
         d2h = sum(a.numel() * 8 for a in pin_out[0])
         copy_stream = torch.cuda.Stream(device=dev)
+        up_stream = torch.cuda.Stream(device=dev)
+        in_ready = [torch.cuda.Event() for _ in range(2)]
         comp_done = [torch.cuda.Event() for _ in range(2)]
         copy_done = [torch.cuda.Event() for _ in range(2)]
 
         def run_e2e(n):
             for i in range(n):
                 k = i & 1
-                stream.wait_event(copy_done[k])             # buffer k free again (its last download landed)
-                for d, p in zip(dev_in, pin_in):
-                    d.copy_(p, non_blocking=True)
-                fd.fdemri_build_splines(wf.plan, *dev_in)
+                with torch.cuda.stream(up_stream):
+                    up_stream.wait_event(comp_done[k])      # the splines of step i-2 have consumed input buffer k
+                    for d, p in zip(ins[k], pin_in):
+                        d.copy_(p, non_blocking=True)
+                    in_ready[k].record(up_stream)
+                stream.wait_event(in_ready[k])
+                stream.wait_event(copy_done[k])             # output buffer k free again (its last download landed)
+                fd.fdemri_build_splines(wf.plan, *ins[k])
                 fd.fdemri_sum(wf.plan, w.theta, w.phi, outs[k][0], outs[k][1])
                 comp_done[k].record(stream)
                 with torch.cuda.stream(copy_stream):
@@ -378,6 +385,8 @@ def main():
                     pin_out[k][1].copy_(outs[k][1], non_blocking=True)
                     copy_done[k].record(copy_stream)
 
+        for ev in comp_done:
+            ev.record(stream)
         for ev in copy_done:
             ev.record(copy_stream)
         run_e2e(3)
@@ -396,8 +405,8 @@ def main():
         assert np.array_equal(pin_out[(args.steps - 1) & 1][0].numpy(), outs[(args.steps - 1) & 1][0].cpu().numpy())
         e2e = {"value": world * args.steps / (ems * 1e-3), "unit": "waveforms/s", "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "ms_per_step": ems / args.steps,
-               "how": "two-deep pipeline: pinned H2D + S0-S4 on one stream, pinned D2H of the previous step on another; "
-                      "inputs (9 MB) exceed nothing, outputs (101 MB per step) stream through L2"}
+               "how": "two-deep pipeline on three streams: pinned H2D of the next step's inputs, S0-S4, pinned D2H of the "
+                      "previous step's polarisations (101 MB per step)"}
 
     clocks = sampler.stop() if rank == 0 else None          # sampled over both timed regions (device and e2e)
     if rank == 0:
