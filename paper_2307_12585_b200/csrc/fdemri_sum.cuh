@@ -30,7 +30,7 @@
 struct SumArgs {
     FdemriDims d;
     const double* rec;        // [B][V][S][R_DOUBLES]
-    const int4* ent;          // [B][V][2][ent_max] {first bin, last bin, seg | branchB << 30, valid}
+    const int4* ent;          // [B][V][2][ent_max] {first bin, last bin, seg | branch << 30, valid}
     const unsigned int* tile_off;   // [B * n_tiles + 1] first pair of every tile
     const unsigned int* pairs;      // sorted keys (voice*2+sign)*ent_max + e of every tile
     const double4* wts;       // [n_angles][V]
@@ -216,7 +216,8 @@ __device__ __forceinline__ bool fdemri_term_fast(const double* __restrict__ it, 
 
 // ---------------------------------------------------------------------------------------------------------
 // Slow path of one term: turnover segments, small |X| (long series or Airy form), rejected fast iterations.
-// flags: bit 0 type (1 = turnover), bit 1 second branch, bit 2 sign.  Returns T and counters in `info`:
+// flags: bit 0 branch of a segment with extrema, bit 1 it hangs between two extrema, bit 2 sign.  Returns T and
+// counters in `info`:
 // bit 0 Airy form used, bit 1 monotone fallback Newton, bits 4.. error bits (FDEMRI_BAD_NEWTON << 4).
 // ---------------------------------------------------------------------------------------------------------
 struct FdemriSlowOut {
