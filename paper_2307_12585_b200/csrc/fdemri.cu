@@ -8,8 +8,10 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <algorithm>
 #include <cstring>
 #include <new>
+#include <unordered_map>
 #include <vector>
 
 #include "fdemri_common.cuh"
@@ -26,6 +28,12 @@ struct fdemri_plan_s {
     void* ws;
     size_t ws_bytes;
     int* lmn_dev;
+    int* lm_index_dev;             // [V] index of the voice's (l, m) in the weight table
+    int4* wmeta_dev;               // [n_lm][2] {terms, p0, q0, offset} for +m and -m
+    double* wcoef_dev;             // Wigner-sum coefficients
+    std::vector<int> lm_index;
+    std::vector<int4> wmeta;
+    std::vector<double> wcoef;
     double *sh_hi, *sh_lo, *rec;
     int4* ent;
     int* tile_cnt;                 // [B * n_tiles] pairs per tile, then [B * n_tiles] fill cursors
@@ -61,6 +69,9 @@ static size_t carve(fdemri_plan_s* p, char* base) {
         return ptr;
     };
     p->lmn_dev = (int*)take(V * 3 * sizeof(int));
+    p->lm_index_dev = (int*)take(V * sizeof(int));
+    p->wmeta_dev = (int4*)take(p->wmeta.size() * sizeof(int4));
+    p->wcoef_dev = (double*)take(p->wcoef.size() * sizeof(double));
     p->sh_hi = (double*)take(B * 4 * S * 4 * sizeof(double));
     p->sh_lo = (double*)take(B * 4 * S * 4 * sizeof(double));
     p->rec = (double*)take(B * V * S * R_DOUBLES * sizeof(double));
@@ -78,6 +89,53 @@ static size_t carve(fdemri_plan_s* p, char* base) {
     // the pair list takes what is left of the work space (default: see fdemri_workspace_bytes)
     p->pairs = (unsigned int*)take(0);
     return off;
+}
+
+// S0 table: -2Y_lm(theta, 0) = sqrt((2l+1)/4pi) d^l_{m,2}(theta) with the Wigner small-d function
+//   d^l_{mp,2} = sum_k (-1)^{mp-2+k} sqrt((l+mp)!(l-mp)!(l+2)!(l-2)!) / [(l+2-k)! k! (mp-2+k)! (l-mp-k)!]
+//                      cos(theta/2)^{2l+2-mp-2k} sin(theta/2)^{mp-2+2k}
+// Everything but the powers depends on (l, mp) only: tabulated once per distinct (l, m) for mp = +m and mp = -m
+// (the latter with the (-1)^l of the partner voice folded in), in long double.
+static void build_weight_table(fdemri_plan_s* p) {
+    const int V = p->d.n_modes;
+    p->lm_index.assign(V, 0);
+    p->wmeta.clear();
+    p->wcoef.clear();
+    std::unordered_map<int, int> seen;           // l * 1024 + m -> table row
+    for (int v = 0; v < V; ++v) {
+        const int l = p->lmn[3 * v], m = p->lmn[3 * v + 1];
+        const int code = l * 1024 + m;
+        int row;
+        const auto hit = seen.find(code);
+        if (hit != seen.end()) {
+            row = hit->second;
+        } else {
+            row = (int)seen.size();
+            seen.emplace(code, row);
+            const long double norm = sqrtl((2.0L * l + 1.0L) / (4.0L * 3.14159265358979323846264338327950288L));
+            for (int which = 0; which < 2; ++which) {
+                const int mp = which ? -m : m;
+                const long double lpref = 0.5L * (lgammal(l + mp + 1.0L) + lgammal(l - mp + 1.0L) + lgammal(l + 3.0L) +
+                                                  lgammal(l - 1.0L));
+                const int k0 = std::max(0, 2 - mp), k1 = std::min(l + 2, l - mp);
+                int4 meta;
+                meta.x = std::max(0, k1 - k0 + 1);
+                meta.y = 2 * l + 2 - mp - 2 * k0;
+                meta.z = mp - 2 + 2 * k0;
+                meta.w = (int)p->wcoef.size();
+                for (int k = k0; k <= k1; ++k) {
+                    const long double lt = lpref - lgammal(l + 2 - k + 1.0L) - lgammal(k + 1.0L) - lgammal(mp - 2 + k + 1.0L) -
+                                           lgammal(l - mp - k + 1.0L);
+                    long double c = norm * expl(lt);
+                    if ((mp - 2 + k) & 1) c = -c;
+                    if (which && (l & 1)) c = -c;
+                    p->wcoef.push_back((double)c);
+                }
+                p->wmeta.push_back(meta);
+            }
+        }
+        p->lm_index[v] = row;
+    }
 }
 
 extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, int n_batch, int n_knots,
@@ -118,6 +176,7 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
     p->d.df = df;
     p->d.freq = freq_dev;
     p->lmn.assign(lmn_host, lmn_host + (size_t)3 * n_modes);
+    build_weight_table(p);
     p->t_knots_dev = t_knots_dev;
     p->ws = nullptr;
     p->ws_bytes = 0;
@@ -172,7 +231,10 @@ extern "C" int fdemri_set_workspace(fdemri_plan_t p, void* dev_ptr, size_t bytes
     p->pair_cap = (bytes - fixed) / sizeof(unsigned int);
     if (p->pair_cap > 0xffffffffull) p->pair_cap = 0xffffffffull;
     p->built = false;
-    if (cudaMemcpy(p->lmn_dev, p->lmn.data(), p->lmn.size() * sizeof(int32_t), cudaMemcpyHostToDevice) != cudaSuccess)
+    if (cudaMemcpy(p->lmn_dev, p->lmn.data(), p->lmn.size() * sizeof(int32_t), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(p->lm_index_dev, p->lm_index.data(), p->lm_index.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(p->wmeta_dev, p->wmeta.data(), p->wmeta.size() * sizeof(int4), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(p->wcoef_dev, p->wcoef.data(), p->wcoef.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess)
         return FDEMRI_ERR_CUDA;
     if (cudaMemset(p->stats, 0, 16 * sizeof(unsigned long long)) != cudaSuccess) return FDEMRI_ERR_CUDA;
     return FDEMRI_OK;
@@ -250,7 +312,8 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
         return FDEMRI_ERR_CUDA;
     // S0
     int nw = n_angles * d.n_modes;
-    k_weights<<<(nw + 127) / 128, 128, 0, st>>>(n_angles, d.n_modes, p->lmn_dev, p->angles, p->wts);
+    k_weights<<<(nw + 127) / 128, 128, 0, st>>>(n_angles, d.n_modes, p->lmn_dev, p->lm_index_dev, p->wmeta_dev, p->wcoef_dev,
+                                                p->angles, p->wts);
     // reset the per-sum counters: n_airy (slot 4) and the tile counter (slot 6)
     if (cudaMemsetAsync(p->stats + 4, 0, sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
     if (cudaMemsetAsync(p->stats + 6, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;

@@ -23,39 +23,43 @@
 //   y+- = -2Y_{l,+-m}(theta, 0);  m = 0: w+ = wx = y/2 (R1, R2).
 // The factor e^{i m phi} goes into the phase as m*phi/2pi cycles.
 // ------------------------------------------------------------------------------------------------
-__device__ double fdemri_wigner_d(int l, int mp, int m, double ch, double sh) {
-    // d^l_{mp,m} = sqrt((l+mp)!(l-mp)!(l+m)!(l-m)!) sum_k (-1)^{mp-m+k} ch^{2l+m-mp-2k} sh^{mp-m+2k}
-    //              / [(l+m-k)! k! (mp-m+k)! (l-mp-k)!]
-    double lf[4] = {lgamma((double)(l + mp + 1)), lgamma((double)(l - mp + 1)), lgamma((double)(l + m + 1)),
-                    lgamma((double)(l - m + 1))};
-    double lpref = 0.5 * (lf[0] + lf[1] + lf[2] + lf[3]);
+// The theta-independent coefficients of the Wigner sum are tabulated per distinct (l, m) on the host at plan time
+// (fdemri.cu: build_weight_table), so that a call only evaluates  sum_j C_j ch^(p0-2j) sh^(q0+2j).
+__device__ __forceinline__ double fdemri_ipow(double x, int n) {      // x^n, n >= 0, by squaring
+    double r = 1.0;
+    while (n) {
+        if (n & 1) r *= x;
+        x *= x;
+        n >>= 1;
+    }
+    return r;
+}
+__device__ __forceinline__ double fdemri_wigner_sum(const int4 meta, const double* __restrict__ coef, double ch, double sh) {
+    // meta = {number of terms, p0, q0, offset of the coefficients}
+    const double* c = coef + meta.w;
     double tot = 0.0;
-    for (int k = 0; k <= 2 * l; ++k) {
-        int a = l + m - k, b = mp - m + k, d = l - mp - k;
-        if (a < 0 || b < 0 || d < 0) continue;
-        double lt = lpref - lgamma((double)(a + 1)) - lgamma((double)(k + 1)) - lgamma((double)(b + 1)) -
-                    lgamma((double)(d + 1));
-        double term = exp(lt) * pow(ch, (double)(2 * l + m - mp - 2 * k)) * pow(sh, (double)(mp - m + 2 * k));
-        tot += ((mp - m + k) & 1) ? -term : term;
+    for (int j = 0; j < meta.x; ++j) {
+        // ch^(p0 - 2j) sh^(q0 + 2j) without dividing (ch or sh may vanish): both exponents stay >= 0
+        tot = fma(c[j], fdemri_ipow(ch, meta.y - 2 * j) * fdemri_ipow(sh, meta.z + 2 * j), tot);
     }
     return tot;
 }
 
 // wts: [n_angles][V] double4 {w+, wx, m*phi/2pi (cycles, reduced), 0}
-__global__ void k_weights(int n_angles, int V, const int* __restrict__ lmn, const double* __restrict__ angles,
-                          double4* __restrict__ wts) {
+__global__ void k_weights(int n_angles, int V, const int* __restrict__ lmn, const int* __restrict__ lm_index,
+                          const int4* __restrict__ wmeta, const double* __restrict__ wcoef,
+                          const double* __restrict__ angles, double4* __restrict__ wts) {
     int id = blockIdx.x * blockDim.x + threadIdx.x;
     if (id >= n_angles * V) return;
     int a = id / V, v = id - a * V;
-    int l = lmn[3 * v], m = lmn[3 * v + 1];
+    const int m = lmn[3 * v + 1];
+    const int lm = lm_index[v];
     double theta = angles[2 * a], phi = angles[2 * a + 1];
     double ch = cos(0.5 * theta), sh = sin(0.5 * theta);
-    double norm = sqrt((2.0 * l + 1.0) / (4.0 * 3.14159265358979323846));
-    double yp = norm * fdemri_wigner_d(l, m, 2, ch, sh);
+    const double yp = fdemri_wigner_sum(wmeta[2 * lm], wcoef, ch, sh);            // -2Y_{l,m}(theta, 0)
     double wp, wx;
     if (m > 0) {
-        double ym = norm * fdemri_wigner_d(l, -m, 2, ch, sh);
-        if (l & 1) ym = -ym;
+        const double ym = fdemri_wigner_sum(wmeta[2 * lm + 1], wcoef, ch, sh);    // (-1)^l -2Y_{l,-m}(theta, 0)
         wp = 0.5 * (yp + ym);
         wx = 0.5 * (yp - ym);
     } else {
