@@ -92,14 +92,14 @@ __device__ double fdemri_root_build(double FB, double FC, double FD, double x, d
     bool inc = Gh > -x;                      // G(h) > G(0)
     double t = (Gh != -x) ? h * (x / (Gh + x)) : 0.5 * h;   // secant seed
     t = fmin(fmax(t, 0.0), h);
-    for (int it = 0; it < 80; ++it) {
+    for (int it = 0; it < 40; ++it) {
         double G = t * (FB + t * (FC + t * FD)) - x;
         double dG = FB + t * (2.0 * FC + 3.0 * FD * t);
         if (G == 0.0) break;
         if ((G > 0.0) == inc) hi = t; else lo = t;
         double tn = t - G / dG;
         if (!(tn > lo && tn < hi)) tn = 0.5 * (lo + hi);
-        if (fabs(tn - t) <= 1e-15 * h) { t = tn; break; }
+        if (fabs(tn - t) <= 1e-9 * h) { t = tn; break; }          // the points only shape the seed of the inverse
         t = tn;
     }
     return t;
@@ -150,21 +150,24 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
     int b = (int)(bv / d.n_modes);
     int m = lmn[3 * v + 1], n = lmn[3 * v + 2];
     const size_t per = (size_t)d.n_seg * 4;
-    const double* hi = sh_hi + (size_t)b * 4 * per + (size_t)k * 4;
-    const double* lo = sh_lo + (size_t)b * 4 * per + (size_t)k * 4;
+    // coefficients (a, b, c, d) of f_phi, f_r, Phi_phi, Phi_r on this segment, hi and lo parts: eight 32-byte loads
+    const double4* H4 = reinterpret_cast<const double4*>(sh_hi + (size_t)b * 4 * per) + k;
+    const double4* L4 = reinterpret_cast<const double4*>(sh_lo + (size_t)b * 4 * per) + k;
+    const double4 h0 = H4[0], h1 = H4[d.n_seg], h2 = H4[2 * (size_t)d.n_seg], h3 = H4[3 * (size_t)d.n_seg];
+    const double4 l0 = L4[0], l1 = L4[d.n_seg], l2 = L4[2 * (size_t)d.n_seg], l3 = L4[3 * (size_t)d.n_seg];
     double* R = rec + id * R_DOUBLES;
     // F cubic (Eq. 6)
-    double FA = fdemri_knotF(m, n, hi[0], hi[per]);
-    dd FBd = fdemri_combine(m, n, hi[1], lo[1], hi[per + 1], lo[per + 1]);
-    dd FCd = fdemri_combine(m, n, hi[2], lo[2], hi[per + 2], lo[per + 2]);
-    dd FDd = fdemri_combine(m, n, hi[3], lo[3], hi[per + 3], lo[per + 3]);
+    double FA = fdemri_knotF(m, n, h0.x, h1.x);
+    dd FBd = fdemri_combine(m, n, h0.y, l0.y, h1.y, l1.y);
+    dd FCd = fdemri_combine(m, n, h0.z, l0.z, h1.z, l1.z);
+    dd FDd = fdemri_combine(m, n, h0.w, l0.w, h1.w, l1.w);
     double FB = FBd.hi, FC = FCd.hi, FD = FDd.hi;
     // phase spline of the voice, in cycles (R9)
     const dd inv2pi = dd{FDEMRI_INV2PI_HI, FDEMRI_INV2PI_LO};
-    dd Pa = dd_add(two_prod((double)m, hi[2 * per]), two_prod((double)n, hi[3 * per]));   // knot values: exact
-    dd Pb = fdemri_combine(m, n, hi[2 * per + 1], lo[2 * per + 1], hi[3 * per + 1], lo[3 * per + 1]);
-    dd Pc = fdemri_combine(m, n, hi[2 * per + 2], lo[2 * per + 2], hi[3 * per + 2], lo[3 * per + 2]);
-    dd Pd = fdemri_combine(m, n, hi[2 * per + 3], lo[2 * per + 3], hi[3 * per + 3], lo[3 * per + 3]);
+    dd Pa = dd_add(two_prod((double)m, h2.x), two_prod((double)n, h3.x));   // knot values: exact
+    dd Pb = fdemri_combine(m, n, h2.y, l2.y, h3.y, l3.y);
+    dd Pc = fdemri_combine(m, n, h2.z, l2.z, h3.z, l3.z);
+    dd Pd = fdemri_combine(m, n, h2.w, l2.w, h3.w, l3.w);
     double pc = -dd_frac(dd_mul(Pa, inv2pi));
     dd bq = dd_mul(Pb, inv2pi);
     double tk = t_knots[(size_t)b * d.n_knots + k];
@@ -235,7 +238,7 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
     }
     const int type = (int)rTYPE;
     const double Fk = FA;
-    const double Fk1 = (k + 1 < d.n_seg) ? fdemri_knotF(m, n, hi[4], hi[per + 4])
+    const double Fk1 = (k + 1 < d.n_seg) ? fdemri_knotF(m, n, H4[1].x, H4[d.n_seg + 1].x)
                                          : fdemri_knotF(m, n, f_phi[(size_t)b * d.n_knots + d.n_knots - 1],
                                                         f_r[(size_t)b * d.n_knots + d.n_knots - 1]);
     const int64_t first_pos = fdemri_first_gt(d, 0.0);      // bins with f > 0 only (R13)
