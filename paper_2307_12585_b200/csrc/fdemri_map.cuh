@@ -92,7 +92,7 @@ __device__ double fdemri_root_build(double FB, double FC, double FD, double x, d
     bool inc = Gh > -x;                      // G(h) > G(0)
     double t = (Gh != -x) ? h * (x / (Gh + x)) : 0.5 * h;   // secant seed
     t = fmin(fmax(t, 0.0), h);
-    for (int it = 0; it < 40; ++it) {
+    for (int it = 0; it < 8; ++it) {                               // a seed: a handful of safeguarded steps is plenty
         double G = t * (FB + t * (FC + t * FD)) - x;
         double dG = FB + t * (2.0 * FC + 3.0 * FD * t);
         if (G == 0.0) break;
