@@ -35,7 +35,7 @@ struct fdemri_plan_s {
     std::vector<int4> wmeta;
     std::vector<double> wcoef;
     double *sh_hi, *sh_lo, *rec;
-    int4* ent;
+    int2* ent;
     int* tile_cnt;                 // [B * n_tiles] pairs per tile, then [B * n_tiles] fill cursors
     unsigned int* tile_off;        // [B * n_tiles + 1]
     unsigned int* pairs;           // [pair_cap]
@@ -62,7 +62,7 @@ static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 static size_t carve(fdemri_plan_s* p, char* base) {
     const FdemriDims& d = p->d;
     size_t off = 0;
-    const size_t B = d.n_batch, V = d.n_modes, N = d.n_knots, S = d.n_seg;
+    const size_t B = d.n_batch, V = d.n_modes, S = d.n_seg;
     auto take = [&](size_t bytes) {
         char* ptr = base ? base + off : nullptr;
         off += align_up(bytes);
@@ -75,7 +75,7 @@ static size_t carve(fdemri_plan_s* p, char* base) {
     p->sh_hi = (double*)take(B * 4 * S * 4 * sizeof(double));
     p->sh_lo = (double*)take(B * 4 * S * 4 * sizeof(double));
     p->rec = (double*)take(B * V * S * R_DOUBLES * sizeof(double));
-    p->ent = (int4*)take(B * V * 2 * (size_t)d.ent_max * sizeof(int4));
+    p->ent = (int2*)take(B * V * 2 * (size_t)d.ent_max * sizeof(int2));
     const size_t NT = B * (size_t)d.n_tiles;
     p->tile_cnt = (int*)take(2 * NT * sizeof(int));
     p->tile_off = (unsigned int*)take((NT + 1) * sizeof(unsigned int));

@@ -134,13 +134,12 @@ __device__ int64_t fdemri_first_gt(const FdemriDims& d, double x) {
     return i;
 }
 
-// ent: [B][V][2][ent_max] int4 {first bin, last bin, seg | branch << 30, 1}, slot = 3*seg + branch (time order);
-// empty slots have w = 0.  tile_cnt: [B][n_tiles] entries per tile, counted here for the tile-major lists (NULL: the
+// ent: [B][V][2][ent_max] int2 {first bin, last bin}, slot = 3*seg + branch (time order); empty slots have last < first.  tile_cnt: [B][n_tiles] entries per tile, counted here for the tile-major lists (NULL: the
 // per-bin lists of the bin-major mode are counted by k_pair_pass<0>, which shares wide entries among the lanes).
 __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ t_knots,
                           const double* __restrict__ sh_hi, const double* __restrict__ sh_lo,
                           const double* __restrict__ f_phi, const double* __restrict__ f_r, double* __restrict__ rec,
-                          int4* __restrict__ ent, int* __restrict__ tile_cnt, unsigned long long* __restrict__ stats) {
+                          int2* __restrict__ ent, int* __restrict__ tile_cnt, unsigned long long* __restrict__ stats) {
     size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     size_t total = (size_t)d.n_batch * d.n_modes * d.n_seg;
     if (id >= total) return;
@@ -248,9 +247,9 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
     const double Vv[4] = {Fk, type >= 1 ? rQ2 : Fk1, type == 2 ? rSF : Fk1, Fk1};
     const int nbr = type + 1;
     for (int sg = 0; sg < 2; ++sg) {
-        int4* E = ent + ((bv * 2 + sg) * (size_t)d.ent_max) + 3 * k;
+        int2* E = ent + ((bv * 2 + sg) * (size_t)d.ent_max) + 3 * k;
         for (int br = 0; br < 3; ++br) {
-            int4 e4 = make_int4(0, -1, k | (br << 30), 0);
+            int2 e4 = make_int2(0, -1);                     // empty: last < first
             if (br < nbr) {
                 const double Va = Vv[br], Vb = Vv[br + 1];
                 const bool a_incl = (br == 0), b_incl = (br + 1 < nbr);
@@ -265,7 +264,7 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
                         const int64_t hi1 = fhi_incl ? fdemri_first_gt(d, fhi) : fdemri_first_ge(d, fhi);
                         if (lo_b < first_pos) lo_b = first_pos;
                         if (lo_b < hi1) {
-                            e4.x = (int)lo_b; e4.y = (int)(hi1 - 1); e4.w = 1;
+                            e4.x = (int)lo_b; e4.y = (int)(hi1 - 1);
                             evals += (unsigned long long)(hi1 - lo_b);
                             ++items;
                             if (tile_cnt) {                 // tile-major lists: an entry meets a handful of tiles

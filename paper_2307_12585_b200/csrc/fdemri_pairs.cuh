@@ -40,18 +40,18 @@ __device__ __forceinline__ void fdemri_for_tiles(bool has, int t0, int t1, unsig
 // One thread per (batch item, voice, sign, entry slot).  MODE 0: count the entries of every tile;  MODE 1: fill the
 // lists through atomic cursors (k_pair_sort then fixes the order).  blockDim.x % 32 == 0.
 template <int MODE>
-__global__ void k_pair_pass(FdemriDims d, const int4* __restrict__ ent, int* __restrict__ tile_cnt,
+__global__ void k_pair_pass(FdemriDims d, const int2* __restrict__ ent, int* __restrict__ tile_cnt,
                             const unsigned int* __restrict__ tile_off, int* __restrict__ tile_cur,
                             unsigned int* __restrict__ pairs, unsigned long long cap) {
     const size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const size_t total = (size_t)d.n_batch * d.n_modes * 2 * d.ent_max;
     const size_t per_item = (size_t)2 * d.n_modes * d.ent_max;
-    int4 en = make_int4(0, -1, 0, 0);
+    int2 en = make_int2(0, -1);
     if (id < total) en = ent[id];
     const size_t idc = id < total ? id : total - 1;
     const int b = (int)(idc / per_item);
     const unsigned key = (unsigned)(idc - (size_t)b * per_item);
-    fdemri_for_tiles(en.w != 0, en.x / d.tile_bins, en.y / d.tile_bins, key, (unsigned long long)b * d.n_tiles,
+    fdemri_for_tiles(en.y >= en.x, en.x / d.tile_bins, en.y / d.tile_bins, key, (unsigned long long)b * d.n_tiles,
                      [&](unsigned k, unsigned long long tb, int t) {
                          const size_t gt = (size_t)tb + t;
                          if (MODE == 0) {

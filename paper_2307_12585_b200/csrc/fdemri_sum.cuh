@@ -30,7 +30,7 @@
 struct SumArgs {
     FdemriDims d;
     const double* rec;        // [B][V][S][R_DOUBLES]
-    const int4* ent;          // [B][V][2][ent_max] {first bin, last bin, seg | branch << 30, valid}
+    const int2* ent;          // [B][V][2][ent_max] {first bin, last bin}; slot = 3*segment + branch
     const unsigned int* tile_off;   // [B * n_tiles + 1] first pair of every tile
     const unsigned int* pairs;      // sorted keys (voice*2+sign)*ent_max + e of every tile
     const double4* wts;       // [n_angles][V]
@@ -425,21 +425,22 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
         const int n = (int)(a.tile_off[gt + 1] - off);
         const int wbase = (a.n_angles > 1 ? b : 0) * V;
         const size_t rbase = (size_t)b * V * d.n_seg;
-        const int4* ent_b = a.ent + (size_t)b * 2 * V * d.ent_max;
+        const int2* ent_b = a.ent + (size_t)b * 2 * V * d.ent_max;
         int base = 0;
         do {
             const int cnt = min(n - base, FDEMRI_CHUNK);
             fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, 256u);
             if (lane < cnt) {
                 const unsigned int key = a.pairs[off + base + lane];
-                const int4 en = ent_b[key];                              // key = (voice*2+sign)*ent_max + e
+                const int2 en = ent_b[key];                              // key = (voice*2+sign)*ent_max + 3*segment + branch
                 const int vs = (int)(key / (unsigned)d.ent_max);
+                const int slot = (int)(key - (unsigned)vs * (unsigned)d.ent_max);
+                const int seg = slot / 3, br = slot - 3 * seg;
                 const int lo_e = max(en.x, tile_lo) - tile_lo;
                 const int hi_e = min(en.y, tile_hi) - tile_lo;
-                const int seg = en.z & 0x3fffffff;
                 const int v = vs >> 1;
                 fdemri_stage_item(ring->st[stage].items[lane], a.rec + (rbase + (size_t)v * d.n_seg + seg) * R_DOUBLES,
-                                  a.wts[wbase + v], lo_e, hi_e, (unsigned)(vs & 1), (unsigned)((en.z >> 30) & 3));
+                                  a.wts[wbase + v], lo_e, hi_e, (unsigned)(vs & 1), (unsigned)br);
             }
             base += FDEMRI_CHUNK;
             __syncwarp();
@@ -782,17 +783,16 @@ __global__ void __launch_bounds__(FDEMRI_BIN_WARPS * 32, 2) k_bin_sum(SumArgs a)
         const int n = (int)(a.tile_off[gb + 1] - off);
         const int wbase = (a.n_angles > 1 ? b : 0) * V;
         const size_t rbase = (size_t)b * V * d.n_seg;
-        const int4* ent_b = a.ent + (size_t)b * 2 * V * d.ent_max;
         double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
         for (int base = 0; base < n; base += 32) {
             if (base + lane < n) {
                 const unsigned int key = a.pairs[off + base + lane];
-                const int4 en = ent_b[key];
-                const int vs = (int)(key / (unsigned)d.ent_max);
+                const int vs = (int)(key / (unsigned)d.ent_max);              // key = (voice*2+sign)*ent_max + 3*segment + branch
+                const int slot = (int)(key - (unsigned)vs * (unsigned)d.ent_max);
+                const int seg = slot / 3, br = slot - 3 * seg;
                 const int v = vs >> 1;
-                const unsigned flags_in = (unsigned)((en.z >> 30) & 3);
-                fdemri_stage_item(it, a.rec + (rbase + (size_t)v * d.n_seg + (en.z & 0x3fffffff)) * R_DOUBLES, a.wts[wbase + v],
-                                  0, 0, (unsigned)(vs & 1), flags_in);
+                fdemri_stage_item(it, a.rec + (rbase + (size_t)v * d.n_seg + seg) * R_DOUBLES, a.wts[wbase + v], 0, 0,
+                                  (unsigned)(vs & 1), (unsigned)br);
                 const unsigned flags = (unsigned)(*reinterpret_cast<const int2*>(it)).y;
                 const double sf = fdemri_xorsign(f, (flags & 4u) << 29);
                 double Tr = 0.0, Ti = 0.0;
