@@ -17,6 +17,8 @@
  *     buffer, including the work space; the plan owns only small host metadata.
  *   - Nothing here allocates device memory, and build_splines / sum do not synchronise: they enqueue
  *     kernels on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ *     build_splines runs one of its kernels on a stream of the plan, forked from and joined back into
+ *     `cuda_stream` with events, so ordering on `cuda_stream` is all a caller needs.
  *   - Every function returns a status: 0 = FDEMRI_OK, >0 = error.  No exceptions, no printing (with the
  *     environment variable FDEMRI_DEBUG set, fdemri_sum reports its launch shape and CUDA error strings on stderr).
  *   - Asynchronous CUDA errors surface in the next call or in fdemri_get_stats (which synchronises).

@@ -53,6 +53,8 @@ struct fdemri_plan_s {
     int sum_blocks_per_sm;         // resident CTAs of k_tile_sum per SM (0: not queried yet)
     uint32_t flags;
     cudaEvent_t ev0, ev1;
+    cudaStream_t side;             // the amplitude splines run beside the shared ones (fork/join on two events)
+    cudaEvent_t ev_fork, ev_join;
     bool ev_valid;
 };
 
@@ -194,6 +196,14 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
     p->flags = flags;
     p->ev_valid = false;
     p->ev0 = p->ev1 = nullptr;
+    p->side = nullptr;
+    p->ev_fork = p->ev_join = nullptr;
+    if (cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        delete p;
+        return FDEMRI_ERR_CUDA;
+    }
     if (flags & FDEMRI_FLAG_TIMING) {
         if (cudaEventCreate(&p->ev0) != cudaSuccess || cudaEventCreate(&p->ev1) != cudaSuccess) {
             delete p;
@@ -261,11 +271,16 @@ extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const 
                 return FDEMRI_ERR_CUDA;
             p->spline_attr_set = true;
         }
+        // the two solves are independent: the amplitudes go to a side stream, joined before S2 reads them
+        const int groups = (d.n_modes + FDEMRI_AMP_VOICES - 1) / FDEMRI_AMP_VOICES;
+        if (cudaEventRecord(p->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(p->side, p->ev_fork, 0) != cudaSuccess)
+            return FDEMRI_ERR_CUDA;
+        k_spline_amp<<<(unsigned)((size_t)d.n_batch * groups), threads, sm_am, p->side>>>(d.n_modes, N, p->t_knots_dev, amp,
+                                                                                       p->rec, p->stats + 5);
         k_spline_shared<<<d.n_batch, threads, sm_sh, st>>>(N, p->t_knots_dev, f_phi, f_r, Phi_phi, Phi_r, p->sh_hi, p->sh_lo,
                                                           p->stats + 5);
-        const int groups = (d.n_modes + FDEMRI_AMP_VOICES - 1) / FDEMRI_AMP_VOICES;
-        k_spline_amp<<<(unsigned)((size_t)d.n_batch * groups), threads, sm_am, st>>>(d.n_modes, N, p->t_knots_dev, amp, p->rec,
-                                                                                  p->stats + 5);
+        if (cudaEventRecord(p->ev_join, p->side) != cudaSuccess || cudaStreamWaitEvent(st, p->ev_join, 0) != cudaSuccess)
+            return FDEMRI_ERR_CUDA;
     }
     // S2: records, entries and tile counts; then the per-tile work lists (prefix sum, fill, sort)
     const size_t NT = (size_t)d.n_batch * d.n_tiles;
@@ -509,6 +524,9 @@ extern "C" int fdemri_measure_fp64_peak_3reg(int n_iters, double* tflops_out) { 
 
 extern "C" int fdemri_destroy(fdemri_plan_t p) {
     if (!p) return FDEMRI_ERR_INVALID_ARG;
+    if (p->side) cudaStreamDestroy(p->side);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
     if (p->ev0) cudaEventDestroy(p->ev0);
     if (p->ev1) cudaEventDestroy(p->ev1);
     delete p;
