@@ -27,6 +27,10 @@
 #include "airy_tables.inc"
 #include "poly_tables.inc"
 
+#ifndef FDEMRI_CONS_BACKOFF
+#define FDEMRI_CONS_BACKOFF 64u     // ns between polls of a consumer warp waiting for a stage
+#endif
+
 struct SumArgs {
     FdemriDims d;
     const double* rec;        // [B][V][S][R_DOUBLES]
@@ -472,7 +476,7 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
     const int wb = cw * 32 * FDEMRI_BPL;          // first tile-relative bin of this warp
     const int rel0 = wb + lane, rel1 = rel0 + 32;
     for (;;) {
-        fdemri_mbar_wait(&ring->full[stage], phase, 64u);
+        fdemri_mbar_wait(&ring->full[stage], phase, FDEMRI_CONS_BACKOFF);
         const FdemriStage* S = &ring->st[stage];
         const int gt = S->hdr[0], cnt = S->hdr[1], last = S->hdr[2];
         if (gt < 0) break;
