@@ -169,6 +169,32 @@ class Oracle:
         return float(out[0]), complex(out[1], out[2])
 
 
+def select_modes(amp, eps):
+    """Mode selection of PAPER.md L60, word by word, in plain numpy (no compiled code): "Within each time step of the
+    sparse array, we take |A(t)|^2 and sort the individual modes in descending order and compute a cumulative
+    summation.  From this sorted array, we check whether the additional power contributed by an individual mode falls
+    below the threshold eps related to the total power emitted.  ...  The selected modes are given by the union of
+    all contributing modes across all time steps."
+    amp: [n_modes][n_knots][2] (re, im).  Returns (keep [n_modes] bool, total [n_knots]).
+    Reading (R15): a mode contributes at a time step iff its own power is at least eps times the total power
+    of all modes at that step; in the sorted array this is a prefix, found here by walking the sorted array."""
+    amp = np.asarray(amp, dtype=np.float64)
+    power = amp[..., 0] ** 2 + amp[..., 1] ** 2                 # [n_modes][n_knots]
+    n_modes, n_knots = power.shape
+    keep = np.zeros(n_modes, dtype=bool)
+    total = np.empty(n_knots)
+    for k in range(n_knots):
+        order = np.argsort(-power[:, k], kind="stable")          # descending
+        sorted_p = power[order, k]
+        cumulative = np.cumsum(sorted_p)
+        total[k] = cumulative[-1]
+        for i in range(n_modes):                                 # the additional power of mode i is sorted_p[i]
+            if sorted_p[i] < eps * total[k]:
+                break
+            keep[order[i]] = True
+    return keep, total
+
+
 _ORACLE = None
 
 

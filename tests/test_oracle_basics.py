@@ -219,3 +219,27 @@ def test_hann_filter_is_the_dft_of_the_windowed_series(orc):
     d = rng.standard_normal(256) + 1j * rng.standard_normal(256)
     _, dh = orc.inner(X[:256], zeros, d, zeros, hann=True)
     assert abs(dh - np.vdot(Xw[:256], d)) <= 1e-12 * abs(dh)
+
+
+def test_mode_selection_reading():
+    """Pins of oracle.select_modes: the sorted-array walk equals the direct threshold on every mode's
+    own power; eps = 0 keeps every mode, eps > 1 none; the kept set shrinks as eps grows; a mode that dominates at a
+    single time step only is kept (the union over time steps)."""
+    import oracle
+    rng = np.random.default_rng(4)
+    V, N = 60, 17
+    amp = rng.standard_normal((V, N, 2)) * np.exp(rng.uniform(-8, 0, (V, 1, 1)))
+    amp[7, :, :] = 1e-9
+    amp[7, 5, :] = 30.0                                          # dominant at one step only
+    power = amp[..., 0] ** 2 + amp[..., 1] ** 2
+    prev = None
+    for eps in (0.0, 1e-8, 1e-5, 1e-2, 0.3, 1.5):
+        keep, total = oracle.select_modes(amp, eps)
+        direct = np.any(power >= eps * power.sum(axis=0)[None, :], axis=1)
+        assert np.array_equal(keep, direct)
+        assert np.allclose(total, power.sum(axis=0), rtol=1e-14)
+        if prev is not None:
+            assert np.all(prev | ~keep)                          # monotone: kept at larger eps => kept at smaller
+        prev = keep
+    assert oracle.select_modes(amp, 0.0)[0].all() and not oracle.select_modes(amp, 1.5)[0].any()
+    assert oracle.select_modes(amp, 0.3)[0][7]
