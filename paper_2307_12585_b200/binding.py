@@ -20,7 +20,7 @@ FDEMRI_FLAG_TIMING, FDEMRI_FLAG_BIN_MAJOR, FDEMRI_FLAG_TILE_MAJOR = 1, 2, 4
 STATUS = {0: "FDEMRI_OK", 1: "FDEMRI_ERR_INVALID_ARG", 2: "FDEMRI_ERR_WORKSPACE", 3: "FDEMRI_ERR_CUDA",
           4: "FDEMRI_ERR_NOT_BUILT", 5: "FDEMRI_ERR_UNSUPPORTED"}
 
-EXPORTS = ["fdemri_plan", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum", "fdemri_sum_inner",
+EXPORTS = ["fdemri_plan", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum", "fdemri_sum_inner", "fdemri_select_modes", "fdemri_set_mode_mask",
            "fdemri_get_stats", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_measure_fp64_peak_3reg", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
 
 
@@ -63,6 +63,10 @@ def lib() -> C.CDLL:
         L.fdemri_sum_inner.restype = C.c_int
         L.fdemri_sum_inner.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), dp, dp, dp, C.c_int, dp, dp, dp,
                                        vp]
+        L.fdemri_select_modes.restype = C.c_int
+        L.fdemri_select_modes.argtypes = [vp, dp, C.c_double, vp, vp, vp]
+        L.fdemri_set_mode_mask.restype = C.c_int
+        L.fdemri_set_mode_mask.argtypes = [vp, vp]
         L.fdemri_get_stats.restype = C.c_int
         L.fdemri_get_stats.argtypes = [vp, C.POINTER(FdemriStats)]
         L.fdemri_get_coeffs.restype = C.c_int
@@ -149,6 +153,18 @@ def fdemri_sum_inner(plan, theta, phi, inner_out, weight=None, data_plus=None, d
     _chk("fdemri_sum_inner", lib().fdemri_sum_inner(plan, th.shape[0], th.ctypes.data_as(dp), ph.ctypes.data_as(dp),
                                                     _ptr(weight), _ptr(data_plus), _ptr(data_cross), int(bool(hann)),
                                                     _ptr(hplus), _ptr(hcross), _ptr(inner_out), _stream_ptr(stream)))
+
+
+def fdemri_select_modes(plan, amp, eps, keep, n_keep, stream=None):
+    """keep: uint8 CUDA tensor [n_batch][n_modes]; n_keep: int32 CUDA tensor [n_batch]."""
+    assert keep.is_cuda and keep.is_contiguous() and keep.element_size() == 1
+    assert n_keep.is_cuda and n_keep.is_contiguous() and n_keep.element_size() == 4
+    _chk("fdemri_select_modes", lib().fdemri_select_modes(plan, _ptr(amp), float(eps), C.c_void_p(keep.data_ptr()),
+                                                          C.c_void_p(n_keep.data_ptr()), _stream_ptr(stream)))
+
+
+def fdemri_set_mode_mask(plan, keep):
+    _chk("fdemri_set_mode_mask", lib().fdemri_set_mode_mask(plan, None if keep is None else C.c_void_p(keep.data_ptr())))
 
 
 def fdemri_get_stats(plan, check=True) -> dict:

@@ -18,6 +18,7 @@
 #include "fdemri_map.cuh"
 #include "fdemri_splines.cuh"
 #include "fdemri_pairs.cuh"
+#include "fdemri_select.cuh"
 #include "fdemri_sum.cuh"
 
 struct fdemri_plan_s {
@@ -41,6 +42,8 @@ struct fdemri_plan_s {
     unsigned int* pairs;           // [pair_cap]
     double* inner_part;            // [B * n_tiles][FDEMRI_CWARPS][4] partial inner products
     double* inner_edge;            // [B * n_tiles][FDEMRI_CWARPS][4][4] edge bins for the Hann filter
+    double* sel_total;             // [B][n_knots] total power per time step (mode selection)
+    const unsigned char* mode_mask;// [B][V] borrowed from the caller, or NULL: every mode is summed
     unsigned long long pair_cap;
     double4* wts;
     double* angles;
@@ -84,6 +87,7 @@ static size_t carve(fdemri_plan_s* p, char* base) {
     p->wts = (double4*)take(B * V * sizeof(double4));
     p->angles = (double*)take(B * 2 * sizeof(double));
     p->stats = (unsigned long long*)take(16 * sizeof(unsigned long long));
+    p->sel_total = (double*)take(B * (size_t)d.n_knots * sizeof(double));
     // partial inner products of the tile-major kernel (the bin-major mode forms them from the waveform in memory)
     const size_t NI = (d.tile_bins == 1) ? 0 : NT;
     p->inner_part = (double*)take(NI * FDEMRI_CWARPS * 4 * sizeof(double));
@@ -193,6 +197,7 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
     p->sm_count = prop.multiProcessorCount;
     p->sum_blocks_per_sm = 0;
     p->spline_attr_set = false;
+    p->mode_mask = nullptr;
     p->flags = flags;
     p->ev_valid = false;
     p->ev0 = p->ev1 = nullptr;
@@ -287,7 +292,7 @@ extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const 
     if (cudaMemsetAsync(p->tile_cnt, 0, 2 * NT * sizeof(int), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
     size_t nrec = (size_t)d.n_batch * d.n_modes * d.n_seg;
     k_records<<<(unsigned)((nrec + 127) / 128), 128, 0, st>>>(d, p->lmn_dev, p->t_knots_dev, p->sh_hi, p->sh_lo, f_phi, f_r,
-                                                              p->rec, p->ent, d.tile_bins == 1 ? nullptr : p->tile_cnt, p->stats);
+                                                              p->rec, p->ent, d.tile_bins == 1 ? nullptr : p->tile_cnt, p->mode_mask, p->stats);
     const size_t nslots = (size_t)d.n_batch * d.n_modes * 2 * d.ent_max;
     const unsigned nb = (unsigned)((nslots + 255) / 256);
     if (d.tile_bins == 1)
@@ -408,6 +413,27 @@ extern "C" int fdemri_sum_inner(fdemri_plan_t p, int n_angles, const double* the
                        hann, inner_out_dev, cuda_stream);
 }
 
+
+extern "C" int fdemri_select_modes(fdemri_plan_t p, const double* amp_dev, double eps, unsigned char* keep_dev,
+                                   int32_t* n_keep_dev, void* cuda_stream) {
+    if (!p || !amp_dev || !keep_dev || !n_keep_dev || !(eps >= 0.0)) return FDEMRI_ERR_INVALID_ARG;
+    if (!p->ws) return FDEMRI_ERR_WORKSPACE;
+    const FdemriDims& d = p->d;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (cudaMemsetAsync(n_keep_dev, 0, d.n_batch * sizeof(int32_t), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    k_select_total<<<d.n_batch * d.n_knots, 256, 0, st>>>(d.n_modes, d.n_knots, amp_dev, p->sel_total);
+    const size_t n = (size_t)d.n_batch * d.n_modes;
+    k_select_keep<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(d.n_batch, d.n_modes, d.n_knots, amp_dev, p->sel_total, eps, keep_dev,
+                                                               n_keep_dev);
+    return cudaGetLastError() == cudaSuccess ? FDEMRI_OK : FDEMRI_ERR_CUDA;
+}
+
+extern "C" int fdemri_set_mode_mask(fdemri_plan_t p, const unsigned char* keep_dev) {
+    if (!p) return FDEMRI_ERR_INVALID_ARG;
+    p->mode_mask = keep_dev;
+    p->built = false;
+    return FDEMRI_OK;
+}
 
 extern "C" int fdemri_get_stats(fdemri_plan_t p, fdemri_stats* out) {
     if (!p || !out) return FDEMRI_ERR_INVALID_ARG;

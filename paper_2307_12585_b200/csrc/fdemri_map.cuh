@@ -139,7 +139,8 @@ __device__ int64_t fdemri_first_gt(const FdemriDims& d, double x) {
 __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ t_knots,
                           const double* __restrict__ sh_hi, const double* __restrict__ sh_lo,
                           const double* __restrict__ f_phi, const double* __restrict__ f_r, double* __restrict__ rec,
-                          int2* __restrict__ ent, int* __restrict__ tile_cnt, unsigned long long* __restrict__ stats) {
+                          int2* __restrict__ ent, int* __restrict__ tile_cnt, const unsigned char* __restrict__ mode_mask,
+                          unsigned long long* __restrict__ stats) {
     size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     size_t total = (size_t)d.n_batch * d.n_modes * d.n_seg;
     if (id >= total) return;
@@ -245,7 +246,7 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
     // branch j of the segment runs from V[j] to V[j+1]: knot value, extremum values, next knot value; a branch includes
     // its start iff that is the knot and its end iff that is an extremum (R6, R7)
     const double Vv[4] = {Fk, type >= 1 ? rQ2 : Fk1, type == 2 ? rSF : Fk1, Fk1};
-    const int nbr = type + 1;
+    const int nbr = (mode_mask && !mode_mask[bv]) ? 0 : type + 1;        // a mode the selection dropped has no entries
     for (int sg = 0; sg < 2; ++sg) {
         int2* E = ent + ((bv * 2 + sg) * (size_t)d.ent_max) + 3 * k;
         for (int br = 0; br < 3; ++br) {

@@ -506,3 +506,43 @@ def test_table2_grid_4yr(fd, orc):
     assert err <= TOL_BIN and mm <= TOL_MISMATCH and st["flags"] == 0
     assert hp[0][0] == 0 and np.all(hp[0][int(0.5 * w.n_freq):] == 0) and np.all(np.isfinite(hp[0]))
     wf.close()
+
+
+def test_mode_selection_feeds_the_sum(fd, orc):
+    """fdemri_select_modes against oracle.select_modes (modes whose decision hinges
+    on the rounding of the total are left out of the comparison), then the masked sum against the oracle run on the
+    selected mode list only."""
+    import torch
+    import oracle
+    w = workload(1)
+    amp = w.amp[0]
+    wf = fd.Waveform(w.lmn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df)
+    d_amp = torch.from_numpy(np.ascontiguousarray(w.amp)).to(wf.dev)
+    keep = torch.zeros((1, w.lmn.shape[0]), dtype=torch.uint8, device=wf.dev)
+    n_keep = torch.zeros(1, dtype=torch.int32, device=wf.dev)
+    power = amp[..., 0] ** 2 + amp[..., 1] ** 2
+    for eps in (0.0, 1e-5, 1e-2):
+        fd.fdemri_select_modes(wf.plan, d_amp, eps, keep, n_keep)
+        torch.cuda.synchronize()
+        got = keep.cpu().numpy()[0].astype(bool)
+        want, total = oracle.select_modes(amp, eps)
+        margin = np.min(np.abs(power - eps * total[None, :]) / total[None, :], axis=1)     # distance from the threshold
+        sure = margin > 1e-12
+        assert np.array_equal(got[sure], want[sure]) and sure.sum() >= len(sure) - 2
+        assert int(n_keep.item()) == int(got.sum())
+        if eps == 0.0:
+            assert got.all()
+    assert 0 < got.sum() < len(got)                               # eps = 1e-2 drops some of the 252 modes
+    # the masked sum = the oracle on the selected modes alone
+    fd.fdemri_set_mode_mask(wf.plan, keep)
+    wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)
+    wf.sum(w.theta, w.phi)
+    hp, hx = wf.result()
+    st = wf.stats()
+    sel = np.flatnonzero(got)
+    ref = orc.waveform(w.lmn[sel], w.t_knots[0], w.f_phi[0], w.f_r[0], w.Phi_phi[0], w.Phi_r[0], amp[sel], w.freq_array(),
+                       w.theta, w.phi)
+    check(hp[0], hx[0], ref, f"config1 with mode selection eps = 1e-2 ({len(sel)} of {len(got)} modes)")
+    assert st["n_evals"] == ref["n_evals"]
+    fd.fdemri_set_mode_mask(wf.plan, None)
+    wf.close()
