@@ -546,3 +546,22 @@ def test_mode_selection_feeds_the_sum(fd, orc):
     assert st["n_evals"] == ref["n_evals"]
     fd.fdemri_set_mode_mask(wf.plan, None)
     wf.close()
+
+
+def test_many_knots(fd, orc):
+    """400 knots: the cyclic-reduction solvers run with 416 threads and more than 48 KB of shared memory (the plan limit
+    is 512 knots); level B of the splines (phase increments against the oracle's long-double build) and level C."""
+    from paper_2307_12585_b200 import synth
+    w = synth.small_case(seed=11, n_knots=400, n_freq=20000)
+    wf, hp, hx, st = run_gpu(fd, w)
+    ref = oracle_c(orc, w, w.freq_array())
+    check(hp[0], hx[0], ref, "400 knots")
+    assert st["n_evals"] == ref["n_evals"]
+    hi, lo, am = wf.coeffs()
+    ohi, olo = orc.build_splines(w.t_knots[0], np.stack([w.f_phi[0], w.f_r[0], w.Phi_phi[0], w.Phi_r[0]]))
+    h = np.diff(w.t_knots[0])
+    dco = (hi[0] - ohi) + (lo[0] - olo)
+    for c in (2, 3):
+        inc = np.abs(dco[c, :, 1] * h) + np.abs(dco[c, :, 2] * h ** 2) + np.abs(dco[c, :, 3] * h ** 3)
+        assert inc.max() < 1e-12, f"phase-increment deviation {inc.max()} rad"
+    wf.close()
