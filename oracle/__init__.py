@@ -116,6 +116,33 @@ class Oracle:
         return dict(hplus=hp.view(np.complex128)[:, 0], hcross=hx.view(np.complex128)[:, 0],
                     n_evals=int(ne.value), nterms=nterms, ambiguous=amb, max_roots=int(mr.value))
 
+    def waveform_kerr(self, lmkn, t, f_phi, f_theta, f_r, Phi_phi, Phi_theta, Phi_r, amp, freq, theta, phi,
+                      extra=True, n_threads=0):
+        """Level-C oracle for general voices (l, m, k, n) of Eq. 1 (L64): F = m f_phi + k f_theta + n f_r (R16)."""
+        lmkn = np.ascontiguousarray(lmkn, dtype=np.int32)
+        assert lmkn.ndim == 2 and lmkn.shape[1] == 4
+        t, tp = _d(t)
+        a1, p1 = _d(f_phi); a2, p2 = _d(f_theta); a3, p3 = _d(f_r)
+        a4, p4 = _d(Phi_phi); a5, p5 = _d(Phi_theta); a6, p6 = _d(Phi_r)
+        amp, ap = _d(amp)
+        freq, fp = _d(freq)
+        n_modes, N, n_freq = lmkn.shape[0], t.shape[0], freq.shape[0]
+        assert amp.shape == (n_modes, N, 2)
+        hp, hx, nterms, amb = self._outs(n_freq, extra)
+        ne = C.c_int64(0)
+        mr = C.c_int32(0)
+        rc = self.lib.fdemri_oracle_waveform_kerr(
+            C.c_int(n_modes), lmkn.ctypes.data_as(_ip), C.c_int(N), tp, p1, p2, p3, p4, p5, p6, ap,
+            C.c_int64(n_freq), fp, C.c_double(theta), C.c_double(phi),
+            hp.ctypes.data_as(_dp), hx.ctypes.data_as(_dp), C.byref(ne),
+            nterms.ctypes.data_as(_ip) if extra else None,
+            amb.ctypes.data_as(C.POINTER(C.c_uint8)) if extra else None,
+            C.byref(mr), C.c_int(n_threads))
+        if rc:
+            raise ValueError(f"fdemri_oracle_waveform_kerr -> {rc}")
+        return dict(hplus=hp.view(np.complex128)[:, 0], hcross=hx.view(np.complex128)[:, 0],
+                    n_evals=int(ne.value), nterms=nterms, ambiguous=amb, max_roots=int(mr.value))
+
     def sum(self, lmn, t, fphi_k, fr_k, sh_hi, sh_lo, am_hi, am_lo, freq, theta, phi, extra=True, n_threads=0):
         """Level-A oracle: sum from given spline coefficients (hi + optional lo parts)."""
         lmn = np.ascontiguousarray(lmn, dtype=np.int32)

@@ -263,7 +263,7 @@ struct Piece {            // one monotone piece of one segment of one voice (R6,
 };
 
 struct Voice {
-    int l, m, n;
+    int l, m, n, k;                    // k: polar harmonic of the general voice (l, m, k, n) of Eq. 1; 0 in Schwarzschild
     std::vector<ld> cF, cP, cRe, cIm;  // [N-1][4] coefficient-wise voice splines (L103)
     std::vector<Piece> pieces;
     cld Wp, Wx;
@@ -345,9 +345,11 @@ extern "C" int fdemri_oracle_inner(int64_t n_freq, const double* w, const double
     return 0;
 }
 
-static int sum_impl(int n_modes, const int32_t* lmn, int N, const double* t,
-                    const double* fphi_k, const double* fr_k,
-                    const ld* sh,      // [4][N-1][4]
+// kk, fth_k NULL: Schwarzschild voices (l, m, n).  Otherwise kk[v] is the polar harmonic k of voice v (Eq. 1:
+// phase m Phi_phi + k Phi_theta + n Phi_r), fth_k the knot values of f_theta, and sh holds six splines.
+static int sum_impl(int n_modes, const int32_t* lmn, const int32_t* kk, int N, const double* t,
+                    const double* fphi_k, const double* fth_k, const double* fr_k,
+                    const ld* sh,      // [4][N-1][4]: f_phi, f_r, Phi_phi, Phi_r  (+ f_theta, Phi_theta: [6][N-1][4])
                     const ld* am,      // [n_modes][2][N-1][4]
                     int64_t n_freq, const double* freq, double theta, double phi,
                     double* hplus, double* hcross,
@@ -364,12 +366,17 @@ static int sum_impl(int n_modes, const int32_t* lmn, int N, const double* t,
     for (int v = 0; v < n_modes; ++v) {
         Voice& V = voices[v];
         V.l = lmn[3 * v]; V.m = lmn[3 * v + 1]; V.n = lmn[3 * v + 2];
+        V.k = kk ? kk[v] : 0;
         if (V.l < 2 || (V.m < 0 && !g_explicit_voices) || V.m > V.l || V.m < -V.l) return 1;
         V.cF.resize(per); V.cP.resize(per); V.cRe.resize(per); V.cIm.resize(per);
         for (size_t i = 0; i < per; ++i) {
             // L103: A..D "given by the sum of the spline coefficients ... multiplied by their mode number"
             V.cF[i] = (ld)V.m * sh[0 * per + i] + (ld)V.n * sh[1 * per + i];
             V.cP[i] = (ld)V.m * sh[2 * per + i] + (ld)V.n * sh[3 * per + i];
+            if (kk) {
+                V.cF[i] += (ld)V.k * sh[4 * per + i];
+                V.cP[i] += (ld)V.k * sh[5 * per + i];
+            }
             V.cRe[i] = am[((size_t)v * 2 + 0) * per + i];
             V.cIm[i] = am[((size_t)v * 2 + 1) * per + i];
         }
@@ -377,7 +384,7 @@ static int sum_impl(int n_modes, const int32_t* lmn, int N, const double* t,
         cld Y = ylm_m2(V.l, V.m, theta, phi);
         if (V.m > 0 && !g_explicit_voices) {
             cld Ym = std::conj(ylm_m2(V.l, -V.m, theta, phi));
-            ld sg = (V.l & 1) ? -1.0L : 1.0L;
+            ld sg = ((V.l + V.k) & 1) ? -1.0L : 1.0L;     // (-1)^(l+k): partner (l,-m,-k,-n), R16
             V.Wp = 0.5L * (Y + sg * Ym);
             V.Wx = cld(0.0L, 0.5L) * (Y - sg * Ym);
         } else {
@@ -389,6 +396,10 @@ static int sum_impl(int n_modes, const int32_t* lmn, int N, const double* t,
         for (int k = 0; k < N; ++k) {
             double pm = (double)V.m * fphi_k[k];
             double pn = (double)V.n * fr_k[k];
+            if (kk) {                              // Eq. 1's order: (m f_phi + k f_theta) + n f_r, each step rounded
+                double pk = (double)V.k * fth_k[k];
+                pm = pm + pk;
+            }
             Fk[k] = pm + pn;
         }
         // pieces: split every segment at the interior extrema of its cubic (R5, R7)
@@ -541,7 +552,7 @@ extern "C" int fdemri_oracle_sum(int n_modes, const int32_t* lmn, int n_knots, c
     std::vector<ld> sh(4 * per), am((size_t)n_modes * 2 * per);
     for (size_t i = 0; i < sh.size(); ++i) sh[i] = (ld)sh_hi[i] + (sh_lo ? (ld)sh_lo[i] : 0.0L);
     for (size_t i = 0; i < am.size(); ++i) am[i] = (ld)am_hi[i] + (am_lo ? (ld)am_lo[i] : 0.0L);
-    return sum_impl(n_modes, lmn, n_knots, t, fphi_k, fr_k, sh.data(), am.data(), n_freq, freq, theta, phi,
+    return sum_impl(n_modes, lmn, NULL, n_knots, t, fphi_k, NULL, fr_k, sh.data(), am.data(), n_freq, freq, theta, phi,
                     hplus, hcross, n_evals, nterms, ambiguous, max_roots, n_threads);
 }
 
@@ -567,8 +578,44 @@ extern "C" int fdemri_oracle_waveform(int n_modes, const int32_t* lmn, int n_kno
             for (int k = 0; k < N; ++k) y[k] = amp[((size_t)v * N + k) * 2 + c];
             ks.solve(y.data(), &am[((size_t)v * 2 + c) * per]);
         }
-    return sum_impl(n_modes, lmn, N, t, f_phi, f_r, sh.data(), am.data(), n_freq, freq, theta, phi,
+    return sum_impl(n_modes, lmn, NULL, N, t, f_phi, NULL, f_r, sh.data(), am.data(), n_freq, freq, theta, phi,
                     hplus, hcross, n_evals, nterms, ambiguous, max_roots, n_threads);
+}
+
+extern "C" int fdemri_oracle_waveform_kerr(int n_modes, const int32_t* lmkn, int n_knots, const double* t,
+                                           const double* f_phi, const double* f_theta, const double* f_r,
+                                           const double* Phi_phi, const double* Phi_theta, const double* Phi_r,
+                                           const double* amp,
+                                           int64_t n_freq, const double* freq, double theta, double phi,
+                                           double* hplus, double* hcross,
+                                           int64_t* n_evals, int32_t* nterms, uint8_t* ambiguous, int32_t* max_roots,
+                                           int n_threads) {
+    if (!knots_ok(n_knots, t) || !lmkn || !f_phi || !f_theta || !f_r || !Phi_phi || !Phi_theta || !Phi_r || !amp ||
+        n_modes < 0)
+        return 1;
+    const int N = n_knots;
+    size_t per = (size_t)(N - 1) * 4;
+    KnotSystem ks(N, t);
+    std::vector<ld> sh(6 * per), am((size_t)n_modes * 2 * per);
+    ks.solve(f_phi, &sh[0 * per]);
+    ks.solve(f_r, &sh[1 * per]);
+    ks.solve(Phi_phi, &sh[2 * per]);
+    ks.solve(Phi_r, &sh[3 * per]);
+    ks.solve(f_theta, &sh[4 * per]);
+    ks.solve(Phi_theta, &sh[5 * per]);
+    std::vector<double> y(N);
+    for (int v = 0; v < n_modes; ++v)
+        for (int c = 0; c < 2; ++c) {
+            for (int k = 0; k < N; ++k) y[k] = amp[((size_t)v * N + k) * 2 + c];
+            ks.solve(y.data(), &am[((size_t)v * 2 + c) * per]);
+        }
+    std::vector<int32_t> lmn((size_t)n_modes * 3), kk(n_modes);
+    for (int v = 0; v < n_modes; ++v) {            // (l, m, k, n) in the order of Eq. 1's subscript
+        lmn[3 * v] = lmkn[4 * v]; lmn[3 * v + 1] = lmkn[4 * v + 1]; lmn[3 * v + 2] = lmkn[4 * v + 3];
+        kk[v] = lmkn[4 * v + 2];
+    }
+    return sum_impl(n_modes, lmn.data(), kk.data(), N, t, f_phi, f_theta, f_r, sh.data(), am.data(), n_freq, freq,
+                    theta, phi, hplus, hcross, n_evals, nterms, ambiguous, max_roots, n_threads);
 }
 
 extern "C" int fdemri_oracle_num_threads(void) {

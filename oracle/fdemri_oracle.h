@@ -71,6 +71,18 @@ int fdemri_oracle_waveform(int n_modes, const int32_t* lmn, int n_knots, const d
                            int64_t* n_evals, int32_t* nterms, uint8_t* ambiguous, int32_t* max_roots,
                            int n_threads);
 
+/* The same for general voices (l, m, k, n) of Eq. 1 (L64): F = m f_phi + k f_theta + n f_r, phase likewise, partner
+ * (l,-m,-k,-n) implied for m > 0 with amplitude (-1)^(l+k) conj A; spherical harmonics stand in for the spheroidal ones
+ * (L66: "Future work will describe how we handle this complication"; R16).  lmkn [n_modes][4]. */
+int fdemri_oracle_waveform_kerr(int n_modes, const int32_t* lmkn, int n_knots, const double* t,
+                                const double* f_phi, const double* f_theta, const double* f_r,
+                                const double* Phi_phi, const double* Phi_theta, const double* Phi_r,
+                                const double* amp,
+                                int64_t n_freq, const double* freq, double theta, double phi,
+                                double* hplus, double* hcross,
+                                int64_t* n_evals, int32_t* nterms, uint8_t* ambiguous, int32_t* max_roots,
+                                int n_threads);
+
 /* Eq. 12 (L134-141) on a frequency grid, both polarisations: <a|b> = sum_k w_k [a+ conj b+ + ax conj bx],
  * w_k = 4 df / S_n(f_k) (NULL: w = 1).  hplus, hcross, dplus, dcross: [n_freq][2].  out = {<h|h>, Re<d|h>, Im<d|h>}.
  * hann != 0: h is first convolved with the DFT of the Hann window, h_k/2 - h_{k-1}/4 - h_{k+1}/4 (L145). */

@@ -238,6 +238,10 @@ class Workload:
     theta: float
     phi: float
     meta: dict
+    # general voices (l, m, k, n) of Eq. 1 (L64); None for the Schwarzschild workloads
+    lmkn: np.ndarray | None = None        # [n_modes][4] int32; lmn then holds the columns (l, m, n) of the same rows
+    f_theta: np.ndarray | None = None     # [B][N] Hz
+    Phi_theta: np.ndarray | None = None   # [B][N] rad
 
     @property
     def n_batch(self):
@@ -268,7 +272,7 @@ def _single(name, idx, M, mu, e0, T_yr, n_knots, lmn, scale_rule, p0=None, unifo
     return Workload(name, lmn, t[None, :], tr["f_phi"], tr["f_r"], tr["Phi_phi"], tr["Phi_r"],
                     amp[None], n_freq, f0, df, None, THETA, PHI,
                     dict(M=M, mu=mu, p0=p0, e0=e0, T_s=T_s, dt=dt, p_end=float(tr["p"][0, -1]),
-                         e_end=float(tr["e"][0, -1])))
+                         e_end=float(tr["e"][0, -1]), scale_rule=scale_rule))
 
 
 def config0():
@@ -354,3 +358,41 @@ def small_case(seed=1, n_knots=12, n_freq=30000, modes=((2, 2, 0), (2, 1, -2), (
     df = 1.0 / T_s
     return Workload("small", lmn, t[None], f_phi[None], f_r[None], Phi_phi[None], Phi_r[None], amp[None],
                     n_freq, 0.0, df, None, THETA, PHI, dict(T_s=T_s))
+
+
+# G9: general voices (l, m, k, n) -------------------------------------------------------------------------
+KERR_MIX = (0.8137, 0.1542)     # f_theta = a f_phi + b f_r: between f_r and f_phi, as for prograde Kerr orbits
+
+
+def with_polar_voices(w: Workload, k_max: int, seed: int = 0, k_decay: float = 1.0) -> Workload:
+    """A workload of general voices (l, m, k, n), k = -k_max..k_max, on the trajectory of `w` (Eq. 1; the paper
+    has no Kerr inputs: L252 expects "an order of magnitude" more modes).  The polar frequency is the fixed mix
+    f_theta = a f_phi + b f_r (KERR_MIX), so that Phi_theta = a Phi_phi + b Phi_r is its exact integral; amplitudes are
+    drawn like G6 with an extra factor exp(-k_decay |k|).  Rows: every (l, m, n) row of w.lmn, k ascending inside."""
+    a, b = KERR_MIX
+    ks = np.arange(-k_max, k_max + 1, dtype=np.int32)
+    n0 = w.lmn.shape[0]
+    lmn = np.repeat(w.lmn, ks.shape[0], axis=0)
+    kk = np.tile(ks, n0)
+    lmkn = np.stack([lmn[:, 0], lmn[:, 1], kk, lmn[:, 2]], axis=1).astype(np.int32)
+    rng = np.random.Generator(np.random.PCG64(SEED0 + 900 + seed))
+    amp = np.empty((w.n_batch, lmn.shape[0], w.n_knots, 2))
+    rule = w.meta.get("scale_rule", "n2")
+    for i in range(w.n_batch):
+        amp[i] = amplitudes(rng, lmn, w.t_knots[i], rule) * np.exp(-k_decay * np.abs(kk))[:, None, None]
+    meta = dict(w.meta, k_max=k_max, mix=KERR_MIX)
+    return dataclasses.replace(w, name=w.name + "+k", lmn=lmn, amp=amp, meta=meta, lmkn=lmkn,
+                               f_theta=a * w.f_phi + b * w.f_r, Phi_theta=a * w.Phi_phi + b * w.Phi_r)
+
+
+def small_case_kerr(seed=1, n_knots=12, n_freq=30000,
+                    modes=((2, 2, 0, 0), (2, 1, 1, -2), (3, 0, -1, 1), (2, 2, 2, -3), (3, 2, -1, 0), (4, 3, 1, 1)),
+                    T_s=3.0e6):
+    """small_case with a polar frequency of its own (analytic quadratic, exact phase), voices (l, m, k, n)."""
+    modes = np.asarray(modes, dtype=np.int32)
+    w = small_case(seed=seed, n_knots=n_knots, n_freq=n_freq, modes=modes[:, [0, 1, 3]], T_s=T_s)
+    s = w.t_knots[0] / T_s
+    c0, c1, c2 = 1.7e-3, 4.1e-4, 1.0e-4
+    f_theta = c0 + c1 * s + c2 * s ** 2
+    Phi_theta = 2 * np.pi * T_s * (c0 * s + c1 * s ** 2 / 2 + c2 * s ** 3 / 3)
+    return dataclasses.replace(w, name="small+k", lmkn=modes, f_theta=f_theta[None], Phi_theta=Phi_theta[None])

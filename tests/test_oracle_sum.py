@@ -210,3 +210,101 @@ def test_zero_outside_support_and_root_count(orc):
     assert out["n_evals"] == int(out["nterms"].sum())
     inside = out["nterms"] > 0
     assert np.all(np.abs(out["hplus"][inside]) > 0)
+
+
+# ---- general voices (l, m, k, n) of Eq. 1 (L64; R16) ------------------------------------------------
+def _run_kerr(orc, w, freq=None, lmkn=None, amp=None):
+    freq = w.freq_array() if freq is None else freq
+    return orc.waveform_kerr(w.lmkn if lmkn is None else lmkn, w.t_knots[0], w.f_phi[0], w.f_theta[0], w.f_r[0],
+                             w.Phi_phi[0], w.Phi_theta[0], w.Phi_r[0], w.amp[0] if amp is None else amp, freq, TH, PH)
+
+
+def test_kerr_voices_with_k_zero_are_the_schwarzschild_sum(orc):
+    """k = 0 on every voice: bit for bit the (l, m, n) sum, whatever f_theta is."""
+    w = synth.small_case_kerr(seed=5)
+    lmkn = w.lmkn.copy()
+    lmkn[:, 2] = 0
+    a = _run_kerr(orc, w, lmkn=lmkn)
+    b = _run(orc, lmkn[:, [0, 1, 3]], w.t_knots[0], w.f_phi[0], w.f_r[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0], w.freq_array())
+    assert np.max(np.abs(b["hplus"])) > 0
+    assert np.array_equal(a["hplus"], b["hplus"]) and np.array_equal(a["hcross"], b["hcross"])
+    assert a["n_evals"] == b["n_evals"]
+
+
+def test_kerr_voices_polar_equal_radial(orc):
+    """f_theta = f_r, Phi_theta = Phi_r: the voice (l, m, k, n) has the frequency and phase of (l, m, n + k), and for
+    even k the same partner sign, so the two sums agree (up to the rounding of the knot values: bins whose membership
+    hinges on it are left out)."""
+    w = synth.small_case_kerr(seed=6, modes=((2, 2, 2, -1), (2, 1, -2, 0), (3, 0, 4, -3), (3, 3, 0, 1), (4, 2, -4, 2)))
+    w.f_theta, w.Phi_theta = w.f_r.copy(), w.Phi_r.copy()
+    a = _run_kerr(orc, w)
+    lmn = np.stack([w.lmkn[:, 0], w.lmkn[:, 1], w.lmkn[:, 3] + w.lmkn[:, 2]], axis=1)
+    b = _run(orc, lmn, w.t_knots[0], w.f_phi[0], w.f_r[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0], w.freq_array())
+    ok = (a["ambiguous"] == 0) & (b["ambiguous"] == 0)
+    assert ok.sum() > 0.99 * ok.size and np.array_equal(a["nterms"][ok], b["nterms"][ok])
+    scale = np.max(np.abs(b["hplus"]))
+    assert scale > 0
+    assert np.max(np.abs(a["hplus"][ok] - b["hplus"][ok])) < 1e-11 * scale
+    assert np.max(np.abs(a["hcross"][ok] - b["hcross"][ok])) < 1e-11 * scale
+    # odd k flips the partner's sign, (-1)^(l+k): the same comparison must then fail for an m > 0 voice
+    w2 = synth.small_case_kerr(seed=6, modes=((2, 2, 1, -1),))
+    w2.f_theta, w2.Phi_theta = w2.f_r.copy(), w2.Phi_r.copy()
+    a2 = _run_kerr(orc, w2)
+    b2 = _run(orc, np.asarray([(2, 2, 0)], np.int32), w2.t_knots[0], w2.f_phi[0], w2.f_r[0], w2.Phi_phi[0], w2.Phi_r[0],
+              w2.amp[0], w2.freq_array())
+    assert np.max(np.abs(a2["hplus"] - b2["hplus"])) > 1e-3 * np.max(np.abs(b2["hplus"]))
+
+
+def test_kerr_partner_symmetry(orc):
+    """The implied partner of (l, m, k, n) is (l, -m, -k, -n) with amplitude (-1)^(l+k) conj A (R16): listing it
+    explicitly gives the same sum."""
+    w = synth.small_case_kerr(seed=7)
+    a = _run_kerr(orc, w)
+    rows, amps = [], []
+    for v, (l, m, k, n) in enumerate(w.lmkn):
+        rows.append((l, m, k, n)); amps.append(w.amp[0, v])
+        if m > 0:
+            rows.append((l, -m, -k, -n))
+            p = w.amp[0, v].copy() * (-1) ** (l + k)
+            p[:, 1] *= -1
+            amps.append(p)
+    try:
+        orc.set_explicit(True)
+        b = _run_kerr(orc, w, lmkn=np.asarray(rows, np.int32), amp=np.asarray(amps))
+    finally:
+        orc.set_explicit(False)
+    scale = np.max(np.abs(a["hplus"]))
+    assert scale > 0 and b["n_evals"] > a["n_evals"]
+    assert np.max(np.abs(a["hplus"] - b["hplus"])) < 1e-13 * scale
+    assert np.max(np.abs(a["hcross"] - b["hcross"])) < 1e-13 * scale
+
+
+def test_kerr_brute_force_fft(orc):
+    """Eq. 1 with its k Phi_theta term, summed in the time domain over the list and the implied partners and
+    Fourier-transformed, against the stationary-phase sum of the same voices."""
+    N, dt = 2 ** 19, 10.0
+    modes = [(2, 2, 0, 0), (2, 1, 1, 1), (2, 2, -1, -2), (3, 0, 2, 2), (3, 3, 1, -1), (2, 1, -2, -4), (4, 2, 1, 1),
+             (2, 0, -1, -1), (3, 1, 3, -2)]
+    w = synth.small_case_kerr(seed=3, n_knots=24, n_freq=N // 2 + 1, modes=modes, T_s=N * dt)
+    out = _run_kerr(orc, w)
+    t = w.t_knots[0]
+    tj = np.arange(N) * dt
+    sp = lambda y: CubicSpline(t, y, bc_type="not-a-knot")(tj)
+    Pp, Pt, Pr = sp(w.Phi_phi[0]), sp(w.Phi_theta[0]), sp(w.Phi_r[0])
+    h = np.zeros(N, complex)
+    for v, (l, m, k, n) in enumerate(w.lmkn):
+        A = sp(w.amp[0, v, :, 0]) + 1j * sp(w.amp[0, v, :, 1])
+        Phi = m * Pp + k * Pt + n * Pr
+        h += A * orc.ylm(int(l), int(m), TH, PH) * np.exp(-1j * Phi)
+        if m > 0:
+            h += (-1) ** (l + k) * np.conj(A) * orc.ylm(int(l), -int(m), TH, PH) * np.exp(+1j * Phi)
+    hann = 0.5 * (1 - np.cos(2 * np.pi * np.arange(N) / N))
+    Hpw = (N * dt * np.fft.ifft(h.real * hann))[: N // 2 + 1]
+    Hxw = (N * dt * np.fft.ifft(-h.imag * hann))[: N // 2 + 1]
+    filt = lambda H: 0.5 * H[1:-1] - 0.25 * H[:-2] - 0.25 * H[2:]
+    m_win = one_minus_overlap(filt(out["hplus"]), filt(out["hcross"]), Hpw[1:-1], Hxw[1:-1])
+    assert m_win < 2e-3, m_win
+    # sensitivity: dropping the k Phi_theta term, or the (-1)^k of the partner, is seen
+    lm0 = w.lmkn.copy(); lm0[:, 2] = 0
+    bad = _run_kerr(orc, w, lmkn=lm0)
+    assert one_minus_overlap(filt(bad["hplus"]), filt(bad["hcross"]), Hpw[1:-1], Hxw[1:-1]) > 0.2
