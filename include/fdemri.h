@@ -112,6 +112,24 @@ int fdemri_set_workspace(fdemri_plan_t plan, void* dev_ptr, size_t bytes);
 int fdemri_build_splines(fdemri_plan_t plan, const double* f_phi, const double* f_r, const double* Phi_phi,
                          const double* Phi_r, const double* amp, void* cuda_stream);
 
+/* General voices (l, m, k, n) of Eq. 1 (phase m Phi_phi + k Phi_theta + n Phi_r; L60 "m, k, and n label
+ * the azimuthal, polar, and radial modes"; L252: the extension to Kerr the paper announces, "where the number of modes
+ * is expected to increase by an order of magnitude").  Same path with a third fundamental frequency:
+ *   F_v = m f_phi + k f_theta + n f_r  (knot values rounded in that order),  Phi_v likewise;
+ *   the partner (l,-m,-k,-n) of an m > 0 voice is implied with amplitude (-1)^(l+k) conj A  (R16);
+ *   the harmonics stay the spin-weighted SPHERICAL ones -- the time-dependent spheroidal harmonics of Kerr are what
+ *   the paper leaves to "future work" (L66) and are not part of this library.
+ *  lmkn_host   [n_modes][4] int32 (l, m, k, n), l >= 2, 0 <= m <= l; everything else as fdemri_plan.
+ * A plan made here is built with fdemri_build_splines_kerr (fdemri_build_splines returns FDEMRI_ERR_INVALID_ARG, and
+ * vice versa); every other call is shared.  With k = 0 on every voice the results equal fdemri_plan's bit for bit. */
+int fdemri_plan_kerr(fdemri_plan_t* out, int n_modes, const int32_t* lmkn_host, int n_batch, int n_knots,
+                     const double* t_knots_dev, int64_t n_freq, const double* freq_dev, double f0, double df,
+                     uint32_t flags);
+/*  f_theta, Phi_theta  [n_batch][n_knots]  polar fundamental frequency (Hz) and phase (rad) at the knots (L48, L56) */
+int fdemri_build_splines_kerr(fdemri_plan_t plan, const double* f_phi, const double* f_theta, const double* f_r,
+                              const double* Phi_phi, const double* Phi_theta, const double* Phi_r, const double* amp,
+                              void* cuda_stream);
+
 /* S0 + S2 + S3 + S4.
  *  theta_host, phi_host  source-frame viewing angles (L66), [n_angles] on the host, n_angles = 1 or n_batch
  *  hplus_dev, hcross_dev [n_batch][n_freq][2] (re, im) FP64, fully overwritten (zeros where no voice has

@@ -20,7 +20,7 @@ FDEMRI_FLAG_TIMING, FDEMRI_FLAG_BIN_MAJOR, FDEMRI_FLAG_TILE_MAJOR = 1, 2, 4
 STATUS = {0: "FDEMRI_OK", 1: "FDEMRI_ERR_INVALID_ARG", 2: "FDEMRI_ERR_WORKSPACE", 3: "FDEMRI_ERR_CUDA",
           4: "FDEMRI_ERR_NOT_BUILT", 5: "FDEMRI_ERR_UNSUPPORTED"}
 
-EXPORTS = ["fdemri_plan", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum", "fdemri_sum_inner", "fdemri_select_modes", "fdemri_set_mode_mask",
+EXPORTS = ["fdemri_plan", "fdemri_plan_kerr", "fdemri_build_splines_kerr", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum", "fdemri_sum_inner", "fdemri_select_modes", "fdemri_set_mode_mask",
            "fdemri_get_stats", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_measure_fp64_peak_3reg", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
 
 
@@ -58,6 +58,10 @@ def lib() -> C.CDLL:
         L.fdemri_set_workspace.argtypes = [vp, vp, C.c_size_t]
         L.fdemri_build_splines.restype = C.c_int
         L.fdemri_build_splines.argtypes = [vp, dp, dp, dp, dp, dp, vp]
+        L.fdemri_plan_kerr.restype = C.c_int
+        L.fdemri_plan_kerr.argtypes = L.fdemri_plan.argtypes
+        L.fdemri_build_splines_kerr.restype = C.c_int
+        L.fdemri_build_splines_kerr.argtypes = [vp, dp, dp, dp, dp, dp, dp, dp, vp]
         L.fdemri_sum.restype = C.c_int
         L.fdemri_sum.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), dp, dp, vp]
         L.fdemri_sum_inner.restype = C.c_int
@@ -115,6 +119,17 @@ def fdemri_plan(lmn, n_batch, n_knots, t_knots, n_freq, freq=None, f0=0.0, df=0.
     rc = lib().fdemri_plan(C.byref(h), lmn.shape[0], lmn.ctypes.data_as(C.POINTER(C.c_int32)), n_batch, n_knots,
                            _ptr(t_knots), int(n_freq), _ptr(freq), float(f0), float(df), int(flags))
     _chk("fdemri_plan", rc)
+    return h
+
+
+def fdemri_plan_kerr(lmkn, n_batch, n_knots, t_knots, n_freq, freq=None, f0=0.0, df=0.0, flags=0):
+    lmkn = np.ascontiguousarray(lmkn, dtype=np.int32)
+    assert lmkn.ndim == 2 and lmkn.shape[1] == 4
+    assert tuple(t_knots.shape) == (n_batch, n_knots)
+    h = C.c_void_p()
+    rc = lib().fdemri_plan_kerr(C.byref(h), lmkn.shape[0], lmkn.ctypes.data_as(C.POINTER(C.c_int32)), n_batch, n_knots,
+                                _ptr(t_knots), int(n_freq), _ptr(freq), float(f0), float(df), int(flags))
+    _chk("fdemri_plan_kerr", rc)
     return h
 
 
@@ -207,9 +222,16 @@ def fdemri_version() -> str:
     return lib().fdemri_version().decode()
 
 
+def fdemri_build_splines_kerr(plan, f_phi, f_theta, f_r, Phi_phi, Phi_theta, Phi_r, amp, stream=None):
+    _chk("fdemri_build_splines_kerr",
+         lib().fdemri_build_splines_kerr(plan, _ptr(f_phi), _ptr(f_theta), _ptr(f_r), _ptr(Phi_phi), _ptr(Phi_theta),
+                                         _ptr(Phi_r), _ptr(amp), _stream_ptr(stream)))
+
+
 # ---- convenience: one object owning the torch buffers ---------------------------------------------------
 class Waveform:
-    """Owns the device buffers of one plan.  `w` is a synth.Workload-like object (numpy, host)."""
+    """Owns the device buffers of one plan.  `lmn` with four columns (l, m, k, n) makes a plan of general voices
+    (fdemri_plan_kerr); build_splines then wants f_theta and Phi_theta too."""
 
     def __init__(self, lmn, t_knots, n_freq, freqs=None, f0=0.0, df=0.0, device="cuda:0", flags=0):
         import torch
@@ -222,7 +244,9 @@ class Waveform:
         self.n_modes = self.lmn.shape[0]
         self.t_knots = torch.from_numpy(t_knots).to(self.dev)
         self.freqs = None if freqs is None else torch.from_numpy(np.ascontiguousarray(freqs, dtype=np.float64)).to(self.dev)
-        self.plan = fdemri_plan(self.lmn, self.n_batch, self.n_knots, self.t_knots, self.n_freq, self.freqs, f0, df, flags)
+        self.polar = self.lmn.shape[1] == 4
+        make = fdemri_plan_kerr if self.polar else fdemri_plan
+        self.plan = make(self.lmn, self.n_batch, self.n_knots, self.t_knots, self.n_freq, self.freqs, f0, df, flags)
         self._alloc_workspace(fdemri_workspace_bytes(self.plan))
         self.hplus = torch.empty((self.n_batch, self.n_freq, 2), dtype=torch.float64, device=self.dev)
         self.hcross = torch.empty_like(self.hplus)
@@ -247,18 +271,29 @@ class Waveform:
         extra = 4 * int(st["n_pairs"] * 1.1) + 4096
         self._alloc_workspace(fdemri_workspace_bytes(self.plan) + extra)
         assert self._inputs is not None
-        fdemri_build_splines(self.plan, *self._inputs, stream=stream)
+        self._build(stream)
         st = fdemri_get_stats(self.plan, check=False)
         if st["flags"] & 16:
             raise FdemriError("fdemri_build_splines (work list still does not fit)", 2)
         return True
 
-    def build_splines(self, f_phi, f_r, Phi_phi, Phi_r, amp, stream=None):
+    def _build(self, stream):
+        if self.polar:
+            fp, fr, Pp, Pr, am, ft, Pt = self._inputs
+            fdemri_build_splines_kerr(self.plan, fp, ft, fr, Pp, Pt, Pr, am, stream=stream)
+        else:
+            fdemri_build_splines(self.plan, *self._inputs, stream=stream)
+
+    def build_splines(self, f_phi, f_r, Phi_phi, Phi_r, amp, stream=None, f_theta=None, Phi_theta=None):
         """Arguments: CUDA tensors, or numpy arrays (copied to the device first)."""
         torch = self.torch
         conv = lambda a: a if torch.is_tensor(a) else torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(self.dev)
-        self._inputs = tuple(conv(a) for a in (f_phi, f_r, Phi_phi, Phi_r, amp))
-        fdemri_build_splines(self.plan, *self._inputs, stream=stream)
+        ins = [f_phi, f_r, Phi_phi, Phi_r, amp]
+        if self.polar:
+            assert f_theta is not None and Phi_theta is not None
+            ins += [f_theta, Phi_theta]
+        self._inputs = tuple(conv(a) for a in ins)
+        self._build(stream)
 
     def sum(self, theta, phi, stream=None):
         fdemri_sum(self.plan, theta, phi, self.hplus, self.hcross, stream=stream)
@@ -297,7 +332,12 @@ class Waveform:
 
 
 def waveform_from_workload(w, device="cuda:0", flags=0) -> Waveform:
-    wf = Waveform(w.lmn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df, device=device, flags=flags)
-    wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)
+    polar = getattr(w, "lmkn", None) is not None
+    wf = Waveform(w.lmkn if polar else w.lmn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df, device=device,
+                  flags=flags)
+    if polar:
+        wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp, f_theta=w.f_theta, Phi_theta=w.Phi_theta)
+    else:
+        wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)
     wf.ensure_capacity()
     return wf

@@ -24,6 +24,9 @@
 struct fdemri_plan_s {
     FdemriDims d;
     std::vector<int32_t> lmn;
+    std::vector<int32_t> kk;       // polar harmonic k per voice (general voices, fdemri_plan_kerr); empty otherwise
+    int* k_dev;                    // NULL unless kk is in use
+    double *sh2_hi, *sh2_lo;       // splines of (f_theta, Phi_theta), same layout as sh_hi/sh_lo; NULL unless kk
     const double* t_knots_dev;
     // work space carve-up (device pointers)
     void* ws;
@@ -74,6 +77,10 @@ static size_t carve(fdemri_plan_s* p, char* base) {
         return ptr;
     };
     p->lmn_dev = (int*)take(V * 3 * sizeof(int));
+    const bool polar = !p->kk.empty();
+    p->k_dev = polar ? (int*)take(V * sizeof(int)) : nullptr;
+    p->sh2_hi = polar ? (double*)take(B * 4 * S * 4 * sizeof(double)) : nullptr;
+    p->sh2_lo = polar ? (double*)take(B * 4 * S * 4 * sizeof(double)) : nullptr;
     p->lm_index_dev = (int*)take(V * sizeof(int));
     p->wmeta_dev = (int4*)take(p->wmeta.size() * sizeof(int4));
     p->wcoef_dev = (double*)take(p->wcoef.size() * sizeof(double));
@@ -144,9 +151,9 @@ static void build_weight_table(fdemri_plan_s* p) {
     }
 }
 
-extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, int n_batch, int n_knots,
-                           const double* t_knots_dev, int64_t n_freq, const double* freq_dev, double f0, double df,
-                           uint32_t flags) {
+static int plan_impl(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, const int32_t* k_host, int n_batch,
+                     int n_knots, const double* t_knots_dev, int64_t n_freq, const double* freq_dev, double f0, double df,
+                     uint32_t flags) {
     if (!out) return FDEMRI_ERR_INVALID_ARG;
     *out = nullptr;
     if (n_modes < 1 || n_modes > (1 << 20) || !lmn_host || n_batch < 1 || n_knots < 4 || n_knots > FDEMRI_MAX_KNOTS ||
@@ -156,6 +163,7 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
     for (int v = 0; v < n_modes; ++v) {
         int l = lmn_host[3 * v], m = lmn_host[3 * v + 1], n = lmn_host[3 * v + 2];
         if (l < 2 || l > 60 || m < 0 || m > l || n < -100000 || n > 100000) return FDEMRI_ERR_INVALID_ARG;
+        if (k_host && (k_host[v] < -100000 || k_host[v] > 100000)) return FDEMRI_ERR_INVALID_ARG;
     }
     /* Which sum kernel: tile-major when the entries are wide in bins (dense grids), bin-major
        when a bin interval holds only a few bins (sparse grids, section 3.3).  The entries of a voice split its
@@ -182,6 +190,7 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
     p->d.df = df;
     p->d.freq = freq_dev;
     p->lmn.assign(lmn_host, lmn_host + (size_t)3 * n_modes);
+    if (k_host) p->kk.assign(k_host, k_host + n_modes);
     build_weight_table(p);
     p->t_knots_dev = t_knots_dev;
     p->ws = nullptr;
@@ -220,6 +229,27 @@ extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_h
     return FDEMRI_OK;
 }
 
+extern "C" int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, int n_batch, int n_knots,
+                           const double* t_knots_dev, int64_t n_freq, const double* freq_dev, double f0, double df,
+                           uint32_t flags) {
+    return plan_impl(out, n_modes, lmn_host, nullptr, n_batch, n_knots, t_knots_dev, n_freq, freq_dev, f0, df, flags);
+}
+
+extern "C" int fdemri_plan_kerr(fdemri_plan_t* out, int n_modes, const int32_t* lmkn_host, int n_batch, int n_knots,
+                                const double* t_knots_dev, int64_t n_freq, const double* freq_dev, double f0, double df,
+                                uint32_t flags) {
+    if (out) *out = nullptr;
+    if (!out || !lmkn_host || n_modes < 1 || n_modes > (1 << 20)) return FDEMRI_ERR_INVALID_ARG;
+    std::vector<int32_t> lmn((size_t)3 * n_modes), kk(n_modes);
+    for (int v = 0; v < n_modes; ++v) {              // (l, m, k, n): the order of Eq. 1's subscript
+        lmn[3 * v] = lmkn_host[4 * v];
+        lmn[3 * v + 1] = lmkn_host[4 * v + 1];
+        kk[v] = lmkn_host[4 * v + 2];
+        lmn[3 * v + 2] = lmkn_host[4 * v + 3];
+    }
+    return plan_impl(out, n_modes, lmn.data(), kk.data(), n_batch, n_knots, t_knots_dev, n_freq, freq_dev, f0, df, flags);
+}
+
 extern "C" size_t fdemri_workspace_bytes(fdemri_plan_t p) {
     if (!p) return 0;
     fdemri_plan_s tmp = *p;
@@ -251,13 +281,18 @@ extern "C" int fdemri_set_workspace(fdemri_plan_t p, void* dev_ptr, size_t bytes
         cudaMemcpy(p->wmeta_dev, p->wmeta.data(), p->wmeta.size() * sizeof(int4), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(p->wcoef_dev, p->wcoef.data(), p->wcoef.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess)
         return FDEMRI_ERR_CUDA;
+    if (p->k_dev && cudaMemcpy(p->k_dev, p->kk.data(), p->kk.size() * sizeof(int32_t), cudaMemcpyHostToDevice) != cudaSuccess)
+        return FDEMRI_ERR_CUDA;
     if (cudaMemset(p->stats, 0, 16 * sizeof(unsigned long long)) != cudaSuccess) return FDEMRI_ERR_CUDA;
     return FDEMRI_OK;
 }
 
-extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const double* f_r, const double* Phi_phi,
-                                    const double* Phi_r, const double* amp, void* cuda_stream) {
+static int build_impl(fdemri_plan_t p, const double* f_phi, const double* f_theta, const double* f_r,
+                      const double* Phi_phi, const double* Phi_theta, const double* Phi_r, const double* amp,
+                      void* cuda_stream) {
     if (!p || !f_phi || !f_r || !Phi_phi || !Phi_r || !amp) return FDEMRI_ERR_INVALID_ARG;
+    const bool polar = !p->kk.empty();
+    if (polar != (f_theta != nullptr) || polar != (Phi_theta != nullptr)) return FDEMRI_ERR_INVALID_ARG;
     if (!p->ws) return FDEMRI_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const FdemriDims& d = p->d;
@@ -282,8 +317,9 @@ extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const 
             return FDEMRI_ERR_CUDA;
         k_spline_amp<<<(unsigned)((size_t)d.n_batch * groups), threads, sm_am, p->side>>>(d.n_modes, N, p->t_knots_dev, amp,
                                                                                        p->rec, p->stats + 5);
-        k_spline_shared<<<d.n_batch, threads, sm_sh, st>>>(N, p->t_knots_dev, f_phi, f_r, Phi_phi, Phi_r, p->sh_hi, p->sh_lo,
-                                                          p->stats + 5);
+        k_spline_shared<<<dim3(d.n_batch, polar ? 2 : 1), threads, sm_sh, st>>>(N, p->t_knots_dev, f_phi, f_r, Phi_phi, Phi_r,
+                                                                               p->sh_hi, p->sh_lo, p->stats + 5, f_theta,
+                                                                               Phi_theta, p->sh2_hi, p->sh2_lo);
         if (cudaEventRecord(p->ev_join, p->side) != cudaSuccess || cudaStreamWaitEvent(st, p->ev_join, 0) != cudaSuccess)
             return FDEMRI_ERR_CUDA;
     }
@@ -292,7 +328,8 @@ extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const 
     if (cudaMemsetAsync(p->tile_cnt, 0, 2 * NT * sizeof(int), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
     size_t nrec = (size_t)d.n_batch * d.n_modes * d.n_seg;
     k_records<<<(unsigned)((nrec + 127) / 128), 128, 0, st>>>(d, p->lmn_dev, p->t_knots_dev, p->sh_hi, p->sh_lo, f_phi, f_r,
-                                                              p->rec, p->ent, d.tile_bins == 1 ? nullptr : p->tile_cnt, p->mode_mask, p->stats);
+                                                              p->rec, p->ent, d.tile_bins == 1 ? nullptr : p->tile_cnt, p->mode_mask, p->stats,
+                                                              p->k_dev, p->sh2_hi, p->sh2_lo, f_theta);
     const size_t nslots = (size_t)d.n_batch * d.n_modes * 2 * d.ent_max;
     const unsigned nb = (unsigned)((nslots + 255) / 256);
     if (d.tile_bins == 1)
@@ -305,6 +342,18 @@ extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const 
     if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
     p->built = true;
     return FDEMRI_OK;
+}
+
+extern "C" int fdemri_build_splines(fdemri_plan_t p, const double* f_phi, const double* f_r, const double* Phi_phi,
+                                    const double* Phi_r, const double* amp, void* cuda_stream) {
+    return build_impl(p, f_phi, nullptr, f_r, Phi_phi, nullptr, Phi_r, amp, cuda_stream);
+}
+
+extern "C" int fdemri_build_splines_kerr(fdemri_plan_t p, const double* f_phi, const double* f_theta, const double* f_r,
+                                         const double* Phi_phi, const double* Phi_theta, const double* Phi_r,
+                                         const double* amp, void* cuda_stream) {
+    if (!f_theta || !Phi_theta) return FDEMRI_ERR_INVALID_ARG;
+    return build_impl(p, f_phi, f_theta, f_r, Phi_phi, Phi_theta, Phi_r, amp, cuda_stream);
 }
 
 // S0 + S3 + S4 (+ the fused inner products when inner_out_dev is given)
@@ -332,7 +381,7 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
         return FDEMRI_ERR_CUDA;
     // S0
     int nw = n_angles * d.n_modes;
-    k_weights<<<(nw + 127) / 128, 128, 0, st>>>(n_angles, d.n_modes, p->lmn_dev, p->lm_index_dev, p->wmeta_dev, p->wcoef_dev,
+    k_weights<<<(nw + 127) / 128, 128, 0, st>>>(n_angles, d.n_modes, p->lmn_dev, p->k_dev, p->lm_index_dev, p->wmeta_dev, p->wcoef_dev,
                                                 p->angles, p->wts);
     // reset the per-sum counters: n_airy (slot 4) and the tile counter (slot 6)
     if (cudaMemsetAsync(p->stats + 4, 0, sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;

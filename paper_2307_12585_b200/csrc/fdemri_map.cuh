@@ -46,7 +46,9 @@ __device__ __forceinline__ double fdemri_wigner_sum(const int4 meta, const doubl
 }
 
 // wts: [n_angles][V] double4 {w+, wx, m*phi/2pi (cycles, reduced), 0}
-__global__ void k_weights(int n_angles, int V, const int* __restrict__ lmn, const int* __restrict__ lm_index,
+// kk: polar harmonic k of every voice (general voices, Eq. 1) or NULL: the partner (l,-m,-k,-n) carries (-1)^(l+k) (R16).
+__global__ void k_weights(int n_angles, int V, const int* __restrict__ lmn, const int* __restrict__ kk,
+                          const int* __restrict__ lm_index,
                           const int4* __restrict__ wmeta, const double* __restrict__ wcoef,
                           const double* __restrict__ angles, double4* __restrict__ wts) {
     int id = blockIdx.x * blockDim.x + threadIdx.x;
@@ -59,7 +61,8 @@ __global__ void k_weights(int n_angles, int V, const int* __restrict__ lmn, cons
     const double yp = fdemri_wigner_sum(wmeta[2 * lm], wcoef, ch, sh);            // -2Y_{l,m}(theta, 0)
     double wp, wx;
     if (m > 0) {
-        const double ym = fdemri_wigner_sum(wmeta[2 * lm + 1], wcoef, ch, sh);    // (-1)^l -2Y_{l,-m}(theta, 0)
+        double ym = fdemri_wigner_sum(wmeta[2 * lm + 1], wcoef, ch, sh);          // (-1)^l -2Y_{l,-m}(theta, 0)
+        if (kk && (kk[v] & 1)) ym = -ym;
         wp = 0.5 * (yp + ym);
         wx = 0.5 * (yp - ym);
     } else {
@@ -83,6 +86,11 @@ __device__ __forceinline__ dd fdemri_combine(int m, int n, double ahi, double al
     dd x = dd_mul_d(dd{ahi, alo}, (double)m);
     dd y = dd_mul_d(dd{bhi, blo}, (double)n);
     return dd_add(x, y);
+}
+// general voices (Eq. 1): F = m f_phi + k f_theta + n f_r; knot values rounded in that order, so that k = 0
+// gives the two-frequency value bit for bit
+__device__ __forceinline__ double fdemri_knotF3(int m, int k, int n, double fphi, double fth, double fr) {
+    return __dadd_rn(__dadd_rn(__dmul_rn((double)m, fphi), __dmul_rn((double)k, fth)), __dmul_rn((double)n, fr));
 }
 
 // root of the monotone cubic  FB t + FC t^2 + FD t^3 = x  on [0, h]  (safeguarded Newton; build time only)
@@ -136,11 +144,15 @@ __device__ int64_t fdemri_first_gt(const FdemriDims& d, double x) {
 
 // ent: [B][V][2][ent_max] int2 {first bin, last bin}, slot = 3*seg + branch (time order); empty slots have last < first.  tile_cnt: [B][n_tiles] entries per tile, counted here for the tile-major lists (NULL: the
 // per-bin lists of the bin-major mode are counted by k_pair_pass<0>, which shares wide entries among the lanes).
+// kk != NULL: general voices (l, m, k, n) -- kk[v] = k, sh2_hi/sh2_lo the splines of (f_theta, Phi_theta) (components
+// 0 and 1 of a second [B][4][n_seg][4] array), f_theta the knot values.
 __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ t_knots,
                           const double* __restrict__ sh_hi, const double* __restrict__ sh_lo,
                           const double* __restrict__ f_phi, const double* __restrict__ f_r, double* __restrict__ rec,
                           int2* __restrict__ ent, int* __restrict__ tile_cnt, const unsigned char* __restrict__ mode_mask,
-                          unsigned long long* __restrict__ stats) {
+                          unsigned long long* __restrict__ stats, const int* __restrict__ kk,
+                          const double* __restrict__ sh2_hi, const double* __restrict__ sh2_lo,
+                          const double* __restrict__ f_theta) {
     size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     size_t total = (size_t)d.n_batch * d.n_modes * d.n_seg;
     if (id >= total) return;
@@ -161,13 +173,30 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
     dd FBd = fdemri_combine(m, n, h0.y, l0.y, h1.y, l1.y);
     dd FCd = fdemri_combine(m, n, h0.z, l0.z, h1.z, l1.z);
     dd FDd = fdemri_combine(m, n, h0.w, l0.w, h1.w, l1.w);
-    double FB = FBd.hi, FC = FCd.hi, FD = FDd.hi;
     // phase spline of the voice, in cycles (R9)
     const dd inv2pi = dd{FDEMRI_INV2PI_HI, FDEMRI_INV2PI_LO};
     dd Pa = dd_add(two_prod((double)m, h2.x), two_prod((double)n, h3.x));   // knot values: exact
     dd Pb = fdemri_combine(m, n, h2.y, l2.y, h3.y, l3.y);
     dd Pc = fdemri_combine(m, n, h2.z, l2.z, h3.z, l3.z);
     dd Pd = fdemri_combine(m, n, h2.w, l2.w, h3.w, l3.w);
+    int kq = 0;
+    const double4* G4 = nullptr;
+    if (kk) {                                               // the polar terms k f_theta, k Phi_theta (Eq. 1)
+        kq = kk[v];
+        G4 = reinterpret_cast<const double4*>(sh2_hi + (size_t)b * 4 * per) + k;
+        const double4* GL = reinterpret_cast<const double4*>(sh2_lo + (size_t)b * 4 * per) + k;
+        const double4 g0 = G4[0], g1 = G4[d.n_seg], e0 = GL[0], e1 = GL[d.n_seg];
+        const double kd = (double)kq;
+        FA = fdemri_knotF3(m, kq, n, h0.x, g0.x, h1.x);
+        FBd = dd_add(FBd, dd_mul_d(dd{g0.y, e0.y}, kd));
+        FCd = dd_add(FCd, dd_mul_d(dd{g0.z, e0.z}, kd));
+        FDd = dd_add(FDd, dd_mul_d(dd{g0.w, e0.w}, kd));
+        Pa = dd_add(Pa, two_prod(kd, g1.x));
+        Pb = dd_add(Pb, dd_mul_d(dd{g1.y, e1.y}, kd));
+        Pc = dd_add(Pc, dd_mul_d(dd{g1.z, e1.z}, kd));
+        Pd = dd_add(Pd, dd_mul_d(dd{g1.w, e1.w}, kd));
+    }
+    double FB = FBd.hi, FC = FCd.hi, FD = FDd.hi;
     double pc = -dd_frac(dd_mul(Pa, inv2pi));
     dd bq = dd_mul(Pb, inv2pi);
     double tk = t_knots[(size_t)b * d.n_knots + k];
@@ -238,9 +267,12 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
     }
     const int type = (int)rTYPE;
     const double Fk = FA;
-    const double Fk1 = (k + 1 < d.n_seg) ? fdemri_knotF(m, n, H4[1].x, H4[d.n_seg + 1].x)
-                                         : fdemri_knotF(m, n, f_phi[(size_t)b * d.n_knots + d.n_knots - 1],
-                                                        f_r[(size_t)b * d.n_knots + d.n_knots - 1]);
+    const size_t last = (size_t)b * d.n_knots + d.n_knots - 1;
+    double Fk1;
+    if (kk) Fk1 = (k + 1 < d.n_seg) ? fdemri_knotF3(m, kq, n, H4[1].x, G4[1].x, H4[d.n_seg + 1].x)
+                                    : fdemri_knotF3(m, kq, n, f_phi[last], f_theta[last], f_r[last]);
+    else    Fk1 = (k + 1 < d.n_seg) ? fdemri_knotF(m, n, H4[1].x, H4[d.n_seg + 1].x)
+                                    : fdemri_knotF(m, n, f_phi[last], f_r[last]);
     const int64_t first_pos = fdemri_first_gt(d, 0.0);      // bins with f > 0 only (R13)
     unsigned long long evals = 0, items = 0;
     // branch j of the segment runs from V[j] to V[j+1]: knot value, extremum values, next knot value; a branch includes

@@ -31,12 +31,20 @@ __device__ __forceinline__ dd from2(double2 a) { return dd{a.x, a.y}; }
 // shared memory per row and buffer: a, b, c, d0..d3 as double2 (hi, lo) = 7 double2
 #define FDEMRI_SH_ROW 7
 // y: 4 pointers (f_phi, f_r, Phi_phi, Phi_r), each [B][N].  out_hi/out_lo: [B][4][N-1][4].  blockDim.x >= N.
+// gridDim.y == 2 (general voices, Eq. 1): the CTAs with blockIdx.y == 1 build the splines of the polar pair
+// (f_theta, Phi_theta) from z0, z1 into out2_hi/out2_lo, same layout (components 0 and 1 are read, 2 and 3 repeat them).
 __global__ void k_spline_shared(int N, const double* __restrict__ t, const double* __restrict__ y0,
                                 const double* __restrict__ y1, const double* __restrict__ y2,
                                 const double* __restrict__ y3, double* __restrict__ out_hi,
-                                double* __restrict__ out_lo, unsigned long long* __restrict__ flags) {
+                                double* __restrict__ out_lo, unsigned long long* __restrict__ flags,
+                                const double* __restrict__ z0, const double* __restrict__ z1,
+                                double* __restrict__ out2_hi, double* __restrict__ out2_lo) {
     extern __shared__ double2 s_sh[];                  // [2][N][FDEMRI_SH_ROW] rows, then h[N] and M[4][N]
     const int b = blockIdx.x, i = threadIdx.x;
+    if (blockIdx.y) {
+        y0 = z0; y1 = z1; y2 = z0; y3 = z1;
+        out_hi = out2_hi; out_lo = out2_lo;
+    }
     double2* buf0 = s_sh;
     double2* buf1 = s_sh + (size_t)N * FDEMRI_SH_ROW;
     double2* s_h = s_sh + (size_t)2 * N * FDEMRI_SH_ROW;          // h_k as dd, k = 0..N-2

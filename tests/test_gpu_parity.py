@@ -34,6 +34,9 @@ def workload(idx):
 
 
 def oracle_c(orc, w, freq, b=0):
+    if getattr(w, "lmkn", None) is not None:
+        return orc.waveform_kerr(w.lmkn, w.t_knots[b], w.f_phi[b], w.f_theta[b], w.f_r[b], w.Phi_phi[b], w.Phi_theta[b],
+                                 w.Phi_r[b], w.amp[b], freq, w.theta, w.phi)
     return orc.waveform(w.lmn, w.t_knots[b], w.f_phi[b], w.f_r[b], w.Phi_phi[b], w.Phi_r[b], w.amp[b], freq,
                         w.theta, w.phi)
 
@@ -564,4 +567,79 @@ def test_many_knots(fd, orc):
     for c in (2, 3):
         inc = np.abs(dco[c, :, 1] * h) + np.abs(dco[c, :, 2] * h ** 2) + np.abs(dco[c, :, 3] * h ** 3)
         assert inc.max() < 1e-12, f"phase-increment deviation {inc.max()} rad"
+    wf.close()
+
+
+# ---- general voices (l, m, k, n) of Eq. 1: fdemri_plan_kerr / fdemri_build_splines_kerr -----------
+def test_kerr_voices_small(fd, orc):
+    from paper_2307_12585_b200 import synth
+    w = synth.small_case_kerr(seed=2, n_knots=14)
+    wf, hp, hx, st = run_gpu(fd, w)
+    ref = oracle_c(orc, w, w.freq_array())
+    check(hp[0], hx[0], ref, "general voices, small")
+    assert st["n_evals"] == ref["n_evals"] and st["n_evals"] > 0
+    # the two build calls belong to their own kind of plan
+    with pytest.raises(fd.FdemriError):
+        fd.fdemri_build_splines(wf.plan, *wf._inputs[:5])
+    wf.close()
+    w0 = synth.small_case(seed=2, n_knots=14)
+    wf0 = fd.waveform_from_workload(w0)
+    with pytest.raises(fd.FdemriError):
+        fd.fdemri_build_splines_kerr(wf0.plan, wf0._inputs[0], wf0._inputs[0], wf0._inputs[1], wf0._inputs[2],
+                                     wf0._inputs[2], wf0._inputs[3], wf0._inputs[4])
+    wf0.close()
+
+
+def test_kerr_voices_k_zero_bitwise(fd):
+    """k = 0 on every voice: the same bits as the (l, m, n) plan, whatever f_theta holds."""
+    import dataclasses
+    from paper_2307_12585_b200 import synth
+    w = synth.small_case_kerr(seed=4, n_knots=20, n_freq=50000)
+    lmkn = w.lmkn.copy()
+    lmkn[:, 2] = 0
+    wk = dataclasses.replace(w, lmkn=lmkn)
+    w0 = dataclasses.replace(w, lmkn=None, f_theta=None, Phi_theta=None)
+    _, hpk, hxk, stk = run_gpu(fd, wk)
+    _, hp0, hx0, st0 = run_gpu(fd, w0)
+    assert np.max(np.abs(hp0)) > 0
+    assert np.array_equal(hpk, hp0) and np.array_equal(hxk, hx0)
+    assert stk["n_evals"] == st0["n_evals"]
+
+
+def test_kerr_voices_config1_scale(fd, orc):
+    """Config 1's trajectory and grid with eleven polar harmonics per (l, m, n), both sum kernels."""
+    from paper_2307_12585_b200 import synth
+    w = synth.with_polar_voices(synth.config1(), k_max=5)
+    assert w.lmkn.shape == (11 * synth.config1().lmn.shape[0], 4)
+    freq = w.freq_array()
+    ref = oracle_c(orc, w, freq)
+    assert ref["max_roots"] >= 1
+    for flags, label in ((0, "tile-major"), (fd.FDEMRI_FLAG_BIN_MAJOR, "bin-major")):
+        wf = fd.waveform_from_workload(w, flags=flags)
+        wf.sum(w.theta, w.phi)
+        hp, hx = wf.result()
+        st = wf.stats()
+        check(hp[0], hx[0], ref, f"general voices, config 1 x 11 k, {label}")
+        assert st["n_evals"] == ref["n_evals"]
+        wf.close()
+
+
+def test_kerr_voices_batch_and_odd_k_weights(fd, orc):
+    """Two batch items with different trajectories; voices with odd k and m > 0 (partner sign (-1)^(l+k))."""
+    import dataclasses
+    from paper_2307_12585_b200 import synth
+    modes = ((2, 2, 1, 0), (2, 1, -1, 1), (3, 2, 3, -2), (3, 3, -3, 1), (4, 1, 2, 0), (2, 0, 1, -1))
+    a = synth.small_case_kerr(seed=8, n_knots=16, modes=modes)
+    b = synth.small_case_kerr(seed=9, n_knots=16, modes=modes)
+    cat = lambda x, y: np.concatenate([x, y], axis=0)
+    w = dataclasses.replace(a, t_knots=cat(a.t_knots, b.t_knots), f_phi=cat(a.f_phi, b.f_phi), f_r=cat(a.f_r, b.f_r),
+                            Phi_phi=cat(a.Phi_phi, b.Phi_phi), Phi_r=cat(a.Phi_r, b.Phi_r), amp=cat(a.amp, b.amp),
+                            f_theta=cat(a.f_theta, b.f_theta), Phi_theta=cat(a.Phi_theta, b.Phi_theta))
+    wf, hp, hx, st = run_gpu(fd, w)
+    tot = 0
+    for i in range(2):
+        ref = oracle_c(orc, w, w.freq_array(), b=i)
+        check(hp[i], hx[i], ref, f"general voices, batch item {i}")
+        tot += ref["n_evals"]
+    assert st["n_evals"] == tot
     wf.close()
