@@ -35,7 +35,34 @@ def workload_name(idx, w):
     if idx == 2:
         return (f"BASELINE config 2: 3843 modes l=2..10,n=-30..30; M=2e6, e0=0.4, 2 yr, 150 knots; uniform grid "
                 f"{w.n_freq} bins (dt=10 s)")
+    if idx == 5:
+        return (f"general voices (l,m,k,n) of Eq. 1, not a BASELINE config: config 2's trajectory and grid ({w.n_freq} bins) "
+                f"with polar harmonics k=-5..5, {w.lmn.shape[0]} voices (SURVEY 8(f) rank 4)")
     return f"BASELINE config {idx}"
+
+
+def workload_inputs(w):
+    """Host arrays in the order the binding keeps them: f_phi, f_r, Phi_phi, Phi_r, amp (, f_theta, Phi_theta)."""
+    arrs = [w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp]
+    if w.lmkn is not None:
+        arrs += [w.f_theta, w.Phi_theta]
+    return [np.ascontiguousarray(a, dtype=np.float64) for a in arrs]
+
+
+def build_call(fd, wf, ins):
+    if wf.polar:
+        fp, fr, Pp, Pr, am, ft, Pt = ins
+        fd.fdemri_build_splines_kerr(wf.plan, fp, ft, fr, Pp, Pt, Pr, am)
+    else:
+        fd.fdemri_build_splines(wf.plan, *ins)
+
+
+def oracle_waveform(orc, w, freq, **kw):
+    if w.lmkn is not None:
+        return orc.waveform_kerr(w.lmkn, w.t_knots[0], w.f_phi[0], w.f_theta[0], w.f_r[0], w.Phi_phi[0], w.Phi_theta[0],
+                                 w.Phi_r[0], w.amp[0], freq, w.theta, w.phi, **kw)
+    return orc.waveform(w.lmn, w.t_knots[0], w.f_phi[0], w.f_r[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0], freq,
+                        w.theta, w.phi, **kw)
 
 
 def load_workload(idx):
@@ -101,15 +128,13 @@ def cpu_oracle_sample(w, total_evals, n_bins=500000, seed=0):
     idx = np.unique(rng.integers(1, int(w.n_freq * 0.36), size=n_bins))
     freq = w.freq_array()[idx]
     t0 = time.perf_counter()
-    r = orc.waveform(w.lmn, w.t_knots[0], w.f_phi[0], w.f_r[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0], freq,
-                     w.theta, w.phi, extra=False)
+    r = oracle_waveform(orc, w, freq, extra=False)
     dt = time.perf_counter() - t0
     frac = r["n_evals"] / float(total_evals) if total_evals else float("nan")
     # one thread, on a smaller sample (single-thread time beside the all-cores one)
     idx1 = idx[:: max(1, len(idx) // 12000)]
     t1 = time.perf_counter()
-    r1 = orc.waveform(w.lmn, w.t_knots[0], w.f_phi[0], w.f_r[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0], w.freq_array()[idx1],
-                      w.theta, w.phi, extra=False, n_threads=1)
+    r1 = oracle_waveform(orc, w, w.freq_array()[idx1], extra=False, n_threads=1)
     dt1 = time.perf_counter() - t1
     single = {"evals_per_s": r1["n_evals"] / dt1, "waveforms_per_s": (r1["n_evals"] / float(total_evals)) / dt1 if total_evals else None,
               "seconds": dt1, "bins": int(len(idx1))}
@@ -280,8 +305,9 @@ def main():
 
     w = load_workload(args.config)
     FLAG_TIMING = 1
-    wf = fd.Waveform(w.lmn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df, device=dev, flags=FLAG_TIMING)
-    host = [np.ascontiguousarray(a, dtype=np.float64) for a in (w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)]
+    wf = fd.Waveform(w.lmkn if w.lmkn is not None else w.lmn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df,
+                     device=dev, flags=FLAG_TIMING)
+    host = workload_inputs(w)
     dev_in = [torch.from_numpy(a).to(dev) for a in host]
     flush = torch.empty(512 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)     # 512 MB > 126 MB L2
     stream = torch.cuda.current_stream()
@@ -293,7 +319,7 @@ def main():
     inner_out = torch.zeros((w.n_batch, 4), dtype=torch.float64, device=dev)
 
     def step_device():
-        fd.fdemri_build_splines(wf.plan, *dev_in)
+        build_call(fd, wf, dev_in)
         fd.fdemri_sum(wf.plan, w.theta, w.phi, wf.hplus, wf.hcross)
 
     # ---- warm-up ----
@@ -315,7 +341,7 @@ def main():
         flush.fill_(1.0)
         e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
         e0.record(stream)
-        fd.fdemri_build_splines(wf.plan, *dev_in)
+        build_call(fd, wf, dev_in)
         e1.record(stream)
         fd.fdemri_sum(wf.plan, w.theta, w.phi, wf.hplus, wf.hcross)
         e2.record(stream)
@@ -336,7 +362,7 @@ def main():
         flush.fill_(1.0)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        fd.fdemri_build_splines(wf.plan, *dev_in)
+        build_call(fd, wf, dev_in)
         fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, inner_out, weight=inner_w, data_plus=inner_dp, data_cross=inner_dx,
                             **inner_kw)
         e1.record(stream)
@@ -376,7 +402,7 @@ def main():
                     in_ready[k].record(up_stream)
                 stream.wait_event(in_ready[k])
                 stream.wait_event(copy_done[k])             # output buffer k free again (its last download landed)
-                fd.fdemri_build_splines(wf.plan, *ins[k])
+                build_call(fd, wf, ins[k])
                 fd.fdemri_sum(wf.plan, w.theta, w.phi, outs[k][0], outs[k][1])
                 comp_done[k].record(stream)
                 with torch.cuda.stream(copy_stream):

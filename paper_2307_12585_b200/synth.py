@@ -396,3 +396,12 @@ def small_case_kerr(seed=1, n_knots=12, n_freq=30000,
     f_theta = c0 + c1 * s + c2 * s ** 2
     Phi_theta = 2 * np.pi * T_s * (c0 * s + c1 * s ** 2 / 2 + c2 * s ** 3 / 3)
     return dataclasses.replace(w, name="small+k", lmkn=modes, f_theta=f_theta[None], Phi_theta=Phi_theta[None])
+
+
+def config5():
+    """Not a BASELINE config: config 2's trajectory and grid with the polar harmonics k = -5..5 on every (l, m, n), the
+    "order of magnitude" more modes the paper expects of Kerr (L252): 42273 voices."""
+    return with_polar_voices(config2(), k_max=5)
+
+
+CONFIGS[5] = config5
