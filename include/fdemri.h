@@ -179,7 +179,8 @@ int fdemri_get_stats(fdemri_plan_t plan, fdemri_stats* out);
 /* Spline coefficients as built on the device, for parity level A (oracle fed the GPU's coefficients).
  *  shared_hi, shared_lo [n_batch][4][n_knots-1][4]  (a,b,c,d) of f_phi, f_r, Phi_phi, Phi_r as hi + lo doubles
  *  amp_coef             [n_batch][n_modes][2][n_knots-1][4]  (a,b,c,d) of Re A, Im A
- * Device pointers; any may be NULL.  Enqueued on the stream of the last build_splines. */
+ * Device pointers; any may be NULL.  Enqueued on the stream of the last build_splines.  (A plan of general voices
+ * returns the same four shared components; the splines of f_theta, Phi_theta stay in the work space.) */
 int fdemri_get_coeffs(fdemri_plan_t plan, double* shared_hi_dev, double* shared_lo_dev, double* amp_coef_dev);
 
 /* Device time in ms of the S3/S4 tile kernel of the last fdemri_sum, from CUDA events recorded on that call's

@@ -327,9 +327,10 @@ static int build_impl(fdemri_plan_t p, const double* f_phi, const double* f_thet
     const size_t NT = (size_t)d.n_batch * d.n_tiles;
     if (cudaMemsetAsync(p->tile_cnt, 0, 2 * NT * sizeof(int), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
     size_t nrec = (size_t)d.n_batch * d.n_modes * d.n_seg;
-    k_records<<<(unsigned)((nrec + 127) / 128), 128, 0, st>>>(d, p->lmn_dev, p->t_knots_dev, p->sh_hi, p->sh_lo, f_phi, f_r,
-                                                              p->rec, p->ent, d.tile_bins == 1 ? nullptr : p->tile_cnt, p->mode_mask, p->stats,
-                                                              p->k_dev, p->sh2_hi, p->sh2_lo, f_theta);
+    auto records = polar ? k_records<true> : k_records<false>;
+    records<<<(unsigned)((nrec + 127) / 128), 128, 0, st>>>(d, p->lmn_dev, p->t_knots_dev, p->sh_hi, p->sh_lo, f_phi, f_r,
+                                                            p->rec, p->ent, d.tile_bins == 1 ? nullptr : p->tile_cnt, p->mode_mask, p->stats,
+                                                            p->k_dev, p->sh2_hi, p->sh2_lo, f_theta);
     const size_t nslots = (size_t)d.n_batch * d.n_modes * 2 * d.ent_max;
     const unsigned nb = (unsigned)((nslots + 255) / 256);
     if (d.tile_bins == 1)

@@ -144,8 +144,9 @@ __device__ int64_t fdemri_first_gt(const FdemriDims& d, double x) {
 
 // ent: [B][V][2][ent_max] int2 {first bin, last bin}, slot = 3*seg + branch (time order); empty slots have last < first.  tile_cnt: [B][n_tiles] entries per tile, counted here for the tile-major lists (NULL: the
 // per-bin lists of the bin-major mode are counted by k_pair_pass<0>, which shares wide entries among the lanes).
-// kk != NULL: general voices (l, m, k, n) -- kk[v] = k, sh2_hi/sh2_lo the splines of (f_theta, Phi_theta) (components
+// POLAR: general voices (l, m, k, n) -- kk[v] = k, sh2_hi/sh2_lo the splines of (f_theta, Phi_theta) (components
 // 0 and 1 of a second [B][4][n_seg][4] array), f_theta the knot values.
+template <bool POLAR>
 __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ t_knots,
                           const double* __restrict__ sh_hi, const double* __restrict__ sh_lo,
                           const double* __restrict__ f_phi, const double* __restrict__ f_r, double* __restrict__ rec,
@@ -181,7 +182,7 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
     dd Pd = fdemri_combine(m, n, h2.w, l2.w, h3.w, l3.w);
     int kq = 0;
     const double4* G4 = nullptr;
-    if (kk) {                                               // the polar terms k f_theta, k Phi_theta (Eq. 1)
+    if (POLAR) {                                            // the polar terms k f_theta, k Phi_theta (Eq. 1)
         kq = kk[v];
         G4 = reinterpret_cast<const double4*>(sh2_hi + (size_t)b * 4 * per) + k;
         const double4* GL = reinterpret_cast<const double4*>(sh2_lo + (size_t)b * 4 * per) + k;
@@ -269,7 +270,7 @@ __global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const doubl
     const double Fk = FA;
     const size_t last = (size_t)b * d.n_knots + d.n_knots - 1;
     double Fk1;
-    if (kk) Fk1 = (k + 1 < d.n_seg) ? fdemri_knotF3(m, kq, n, H4[1].x, G4[1].x, H4[d.n_seg + 1].x)
+    if (POLAR) Fk1 = (k + 1 < d.n_seg) ? fdemri_knotF3(m, kq, n, H4[1].x, G4[1].x, H4[d.n_seg + 1].x)
                                     : fdemri_knotF3(m, kq, n, f_phi[last], f_theta[last], f_r[last]);
     else    Fk1 = (k + 1 < d.n_seg) ? fdemri_knotF(m, n, H4[1].x, H4[d.n_seg + 1].x)
                                     : fdemri_knotF(m, n, f_phi[last], f_r[last]);
