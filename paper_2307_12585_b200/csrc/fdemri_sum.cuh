@@ -350,15 +350,24 @@ struct FdemriRing {
 };
 
 // Producer lane: folds record + weights + sign into the staged item `dst` (shared memory)
-__device__ __forceinline__ void fdemri_stage_item(double* dst, const double* __restrict__ R, const double4 w, int lo,
-                                                  int hi, unsigned sg, unsigned br) {
+// a record in registers: six 32-byte loads, issued together (the producer issues them before it waits for a ring slot)
+struct FdemriRecRegs {
+    double4 r0, r1, r2, r3, r4, r5;
+};
+__device__ __forceinline__ FdemriRecRegs fdemri_load_rec(const double* __restrict__ R) {
     const double4* R4 = reinterpret_cast<const double4*>(R);
-    const double4 r0 = fdemri_ld4(R4 + 0);       // FA FB FC FD
-    const double4 r1 = fdemri_ld4(R4 + 1);       // Q1 Q2 Q3 H
-    const double4 r2 = fdemri_ld4(R4 + 2);       // Re A
-    const double4 r3 = fdemri_ld4(R4 + 3);       // Im A
-    const double4 r4 = fdemri_ld4(R4 + 4);       // PC BH BL NC
-    const double4 r5 = fdemri_ld4(R4 + 5);       // ND TK TYPE SF
+    FdemriRecRegs q;
+    q.r0 = fdemri_ld4(R4 + 0);       // FA FB FC FD
+    q.r1 = fdemri_ld4(R4 + 1);       // Q1 Q2 Q3 H
+    q.r2 = fdemri_ld4(R4 + 2);       // Re A
+    q.r3 = fdemri_ld4(R4 + 3);       // Im A
+    q.r4 = fdemri_ld4(R4 + 4);       // PC BH BL NC
+    q.r5 = fdemri_ld4(R4 + 5);       // ND TK TYPE SF
+    return q;
+}
+__device__ __forceinline__ void fdemri_stage_regs(double* dst, const FdemriRecRegs& q, const double4 w, int lo,
+                                                  int hi, unsigned sg, unsigned br) {
+    const double4 r0 = q.r0, r1 = q.r1, r2 = q.r2, r3 = q.r3, r4 = q.r4, r5 = q.r5;
     const unsigned type = (unsigned)r5.z;        // interior extrema of F on the segment: 0, 1, 2
     const double s = sg ? -1.0 : 1.0;
     const double h = r1.w;
@@ -409,6 +418,11 @@ __device__ __forceinline__ void fdemri_stage_item(double* dst, const double* __r
     d2[15] = make_double2(-w.y, s * w.y);
 }
 
+__device__ __forceinline__ void fdemri_stage_item(double* dst, const double* __restrict__ R, const double4 w, int lo,
+                                                  int hi, unsigned sg, unsigned br) {
+    fdemri_stage_regs(dst, fdemri_load_rec(R), w, lo, hi, sg, br);
+}
+
 // Producer: walks the sorted pair list of every tile it draws (S2c, fdemri_pairs.cuh), one ring stage per
 // 32 keys: key -> entry (bin interval, segment, branch) -> record + weights -> staged item.
 __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ring, int lane) {
@@ -431,21 +445,38 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
         const size_t rbase = (size_t)b * V * d.n_seg;
         const int2* ent_b = a.ent + (size_t)b * 2 * V * d.ent_max;
         int base = 0;
+        // The loads of a chunk form a chain key -> entry -> record (three trips to L2).  They run ahead of the ring:
+        // the keys two chunks ahead, the entries one chunk ahead, the records of this chunk before the wait for its slot.
+        unsigned int key0 = 0u, key1 = 0u;
+        int2 en0 = make_int2(0, -1);
+        if (lane < n) {
+            key0 = a.pairs[off + lane];
+            en0 = ent_b[key0];                                          // key = (voice*2+sign)*ent_max + 3*segment + branch
+        }
+        if (FDEMRI_CHUNK + lane < n) key1 = a.pairs[off + FDEMRI_CHUNK + lane];
         do {
             const int cnt = min(n - base, FDEMRI_CHUNK);
+            const int vs = (int)(key0 / (unsigned)d.ent_max);
+            const int slot = (int)(key0 - (unsigned)vs * (unsigned)d.ent_max);
+            const int seg = slot / 3, br = slot - 3 * seg;
+            const int v = vs >> 1;
+            FdemriRecRegs q;
+            double4 w4 = make_double4(0.0, 0.0, 0.0, 0.0);
+            if (lane < cnt) {
+                q = fdemri_load_rec(a.rec + (rbase + (size_t)v * d.n_seg + seg) * R_DOUBLES);
+                w4 = a.wts[wbase + v];
+            }
+            int2 en1 = make_int2(0, -1);
+            unsigned int key2 = 0u;
+            if (base + FDEMRI_CHUNK + lane < n) en1 = ent_b[key1];
+            if (base + 2 * FDEMRI_CHUNK + lane < n) key2 = a.pairs[off + base + 2 * FDEMRI_CHUNK + lane];
             fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, 256u);
             if (lane < cnt) {
-                const unsigned int key = a.pairs[off + base + lane];
-                const int2 en = ent_b[key];                              // key = (voice*2+sign)*ent_max + 3*segment + branch
-                const int vs = (int)(key / (unsigned)d.ent_max);
-                const int slot = (int)(key - (unsigned)vs * (unsigned)d.ent_max);
-                const int seg = slot / 3, br = slot - 3 * seg;
-                const int lo_e = max(en.x, tile_lo) - tile_lo;
-                const int hi_e = min(en.y, tile_hi) - tile_lo;
-                const int v = vs >> 1;
-                fdemri_stage_item(ring->st[stage].items[lane], a.rec + (rbase + (size_t)v * d.n_seg + seg) * R_DOUBLES,
-                                  a.wts[wbase + v], lo_e, hi_e, (unsigned)(vs & 1), (unsigned)br);
+                const int lo_e = max(en0.x, tile_lo) - tile_lo;
+                const int hi_e = min(en0.y, tile_hi) - tile_lo;
+                fdemri_stage_regs(ring->st[stage].items[lane], q, w4, lo_e, hi_e, (unsigned)(vs & 1), (unsigned)br);
             }
+            key0 = key1; en0 = en1; key1 = key2;
             base += FDEMRI_CHUNK;
             __syncwarp();
             if (lane == 0) {
