@@ -27,7 +27,7 @@ sys.path.insert(0, ROOT)
 
 METRIC = "waveforms/s, 3843-mode 2-yr FD sum (FP64)"
 FLOP_PER_EVAL = 200.0          # SURVEY.md 8(d) / DESIGN.md: algorithmic FP64 flop per mode-bin evaluation
-TILE_SUM_DRAM_BYTES = 175.3e6    # ncu capture of config 2, profiles/r1i_final.md
+TILE_SUM_DRAM_BYTES = 170.3e6    # ncu capture of config 2, profiles/r1k_tile.md
 KERNELS_PER_STEP = 8           # spline_shared, spline_amp, records, pair_scan, pair_pass<1>, pair_sort | weights, sum (+ pair_pass<0> in bin-major mode)
 
 
@@ -452,7 +452,7 @@ def main():
             "roofline": {"bound": "alu", "kernel": "k_tile_sum", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
                          "frac": achieved / peak_tf, "traffic": TILE_SUM_DRAM_BYTES if args.config == 2 else None,
                          "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of one k_tile_sum launch, ncu --set full "
-                                         "(profiles/r1i_final.md); bytes, for context: the bound is the FP64 pipe",
+                                         "(profiles/r1k_tile.md); bytes, for context: the bound is the FP64 pipe",
                          "kernel_ms": k_ms,
                          "flop_per_eval": FLOP_PER_EVAL,
                          "peak_source": "FP64 DFMA loop measured live (fdemri_measure_fp64_peak); nominal 148 SM x 64 "

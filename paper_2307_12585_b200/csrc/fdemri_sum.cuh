@@ -30,6 +30,9 @@
 #ifndef FDEMRI_CONS_BACKOFF
 #define FDEMRI_CONS_BACKOFF 64u     // ns between polls of a consumer warp waiting for a stage
 #endif
+#ifndef FDEMRI_PROD_BACKOFF
+#define FDEMRI_PROD_BACKOFF 256u    // ns between polls of the producer warp waiting for a free stage
+#endif
 
 struct SumArgs {
     FdemriDims d;
@@ -470,7 +473,7 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
             unsigned int key2 = 0u;
             if (base + FDEMRI_CHUNK + lane < n) en1 = ent_b[key1];
             if (base + 2 * FDEMRI_CHUNK + lane < n) key2 = a.pairs[off + base + 2 * FDEMRI_CHUNK + lane];
-            fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, 256u);
+            fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, FDEMRI_PROD_BACKOFF);
             if (lane < cnt) {
                 const int lo_e = max(en0.x, tile_lo) - tile_lo;
                 const int hi_e = min(en0.y, tile_hi) - tile_lo;
@@ -487,7 +490,7 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
         } while (base < n);
     }
     // no more work
-    fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, 256u);
+    fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, FDEMRI_PROD_BACKOFF);
     if (lane == 0) {
         ring->st[stage].hdr[0] = -1; ring->st[stage].hdr[1] = 0; ring->st[stage].hdr[2] = 1;
         fdemri_mbar_arrive(&ring->full[stage]);
