@@ -643,3 +643,45 @@ def test_kerr_voices_batch_and_odd_k_weights(fd, orc):
         tot += ref["n_evals"]
     assert st["n_evals"] == tot
     wf.close()
+
+
+def test_kerr_voices_selection_and_fused_inner(fd, orc):
+    """General voices through the rest of the path: mode selection (L60; in the paper's words over |A_lmkn|^2) feeding
+    the work list, then the Eq. 12 inner products with the Hann filter formed on the fly."""
+    import torch
+    import oracle
+    from paper_2307_12585_b200 import synth
+    w = synth.with_polar_voices(synth.small_case(seed=12, n_knots=18, n_freq=40000,
+                                                 modes=((2, 2, 0), (2, 1, -1), (3, 2, 1), (3, 0, 2), (4, 4, -2))), k_max=3)
+    amp = w.amp[0]
+    wf = fd.Waveform(w.lmkn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df)
+    d_amp = torch.from_numpy(np.ascontiguousarray(w.amp)).to(wf.dev)
+    keep = torch.zeros((1, w.lmkn.shape[0]), dtype=torch.uint8, device=wf.dev)
+    n_keep = torch.zeros(1, dtype=torch.int32, device=wf.dev)
+    eps = 3e-3
+    fd.fdemri_select_modes(wf.plan, d_amp, eps, keep, n_keep)
+    torch.cuda.synchronize()
+    got = keep.cpu().numpy()[0].astype(bool)
+    want, total = oracle.select_modes(amp, eps)
+    power = amp[..., 0] ** 2 + amp[..., 1] ** 2
+    sure = np.min(np.abs(power - eps * total[None, :]) / total[None, :], axis=1) > 1e-12
+    assert np.array_equal(got[sure], want[sure]) and 0 < got.sum() < len(got)
+    fd.fdemri_set_mode_mask(wf.plan, keep)
+    wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp, f_theta=w.f_theta, Phi_theta=w.Phi_theta)
+    sel = np.flatnonzero(got)
+    ref = orc.waveform_kerr(w.lmkn[sel], w.t_knots[0], w.f_phi[0], w.f_theta[0], w.f_r[0], w.Phi_phi[0], w.Phi_theta[0],
+                            w.Phi_r[0], amp[sel], w.freq_array(), w.theta, w.phi)
+    rng = np.random.default_rng(5)
+    d = np.abs(ref["hplus"]).max() * (rng.standard_normal((2, w.n_freq)) + 1j * rng.standard_normal((2, w.n_freq)))
+    t_d = [torch.from_numpy(np.ascontiguousarray(x).view(np.float64).reshape(-1, 2)).to(wf.dev) for x in d]
+    out = torch.zeros((1, 4), dtype=torch.float64, device=wf.dev)
+    fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, out, data_plus=t_d[0], data_cross=t_d[1], hann=True, hplus=wf.hplus,
+                        hcross=wf.hcross)
+    hp, hx = wf.result()
+    check(hp[0], hx[0], ref, f"general voices, {len(sel)} of {len(got)} selected")
+    assert wf.stats()["n_evals"] == ref["n_evals"]
+    want_hh, want_dh = orc.inner(ref["hplus"], ref["hcross"], d[0], d[1], hann=True)
+    o = out.cpu().numpy()[0]
+    assert abs(o[0] - want_hh) <= 1e-10 * want_hh
+    assert abs(complex(o[1], o[2]) - want_dh) <= 1e-10 * np.sqrt(want_hh * orc.inner(d[0], d[1])[0])
+    wf.close()
