@@ -338,8 +338,9 @@ static int build_impl(fdemri_plan_t p, const double* f_phi, const double* f_thet
     k_pair_scan<<<1, 1024, 0, st>>>(NT, p->tile_cnt, p->tile_off, p->pair_cap, p->stats);
     k_pair_pass<1><<<nb, 256, 0, st>>>(d, p->ent, p->tile_cnt, p->tile_off, p->tile_cnt + NT, p->pairs, p->pair_cap);
     // per-bin lists are short (a few hundred keys): smaller CTAs, more of them resident
-    k_pair_sort<<<(unsigned)NT, d.tile_bins == 1 ? 64 : 256, FDEMRI_SORT_MAX * sizeof(unsigned int), st>>>(NT, p->tile_off, p->pairs,
-                                                                                                       p->pair_cap);
+    const unsigned sort_keys = d.tile_bins == 1 ? FDEMRI_SORT_CAP_BIN : FDEMRI_SORT_CAP_TILE;
+    k_pair_sort<<<(unsigned)NT, d.tile_bins == 1 ? FDEMRI_SORT_THREADS_BIN : FDEMRI_SORT_THREADS_TILE,
+                  sort_keys * sizeof(unsigned int), st>>>(NT, p->tile_off, p->pairs, p->pair_cap, sort_keys);
     if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
     p->built = true;
     return FDEMRI_OK;

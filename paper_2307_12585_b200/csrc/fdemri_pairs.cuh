@@ -13,7 +13,21 @@
 #pragma once
 #include "fdemri_common.cuh"
 
-#define FDEMRI_SORT_MAX 8192         // keys per tile the shared-memory sorter takes
+// k_pair_sort: keys per list the shared-memory sorter takes (longer lists are sorted in place in global memory) and
+// threads per CTA, for the tile-major lists (hundreds of keys per 768-bin tile) and the per-bin lists of the bin-major
+// mode (as many lists as bins: small CTAs with little shared memory, so that many are resident)
+#ifndef FDEMRI_SORT_CAP_TILE
+#define FDEMRI_SORT_CAP_TILE 8192
+#endif
+#ifndef FDEMRI_SORT_THREADS_TILE
+#define FDEMRI_SORT_THREADS_TILE 256
+#endif
+#ifndef FDEMRI_SORT_CAP_BIN
+#define FDEMRI_SORT_CAP_BIN 2048
+#endif
+#ifndef FDEMRI_SORT_THREADS_BIN
+#define FDEMRI_SORT_THREADS_BIN 64
+#endif
 
 // Tiles t0..t1 of one entry, for every lane of a warp: narrow ranges (the rule) are walked by their own lane, wide
 // ones -- an entry of a slowly sweeping voice can cover thousands of bins of a sparse grid -- by the whole warp, so
@@ -138,14 +152,15 @@ __device__ __forceinline__ void fdemri_bitonic(unsigned int* buf, unsigned int n
 }
 
 __global__ void __launch_bounds__(256) k_pair_sort(size_t n_tiles_total, const unsigned int* __restrict__ tile_off,
-                                                   unsigned int* __restrict__ pairs, unsigned long long cap) {
+                                                   unsigned int* __restrict__ pairs, unsigned long long cap,
+                                                   unsigned int smem_keys) {
     extern __shared__ unsigned int s_key[];
     const size_t gt = blockIdx.x;
     if (gt >= n_tiles_total) return;
     const unsigned int o0 = tile_off[gt], o1 = tile_off[gt + 1];
     const unsigned int n = o1 - o0;
     if (n < 2u || (unsigned long long)o1 > cap) return;
-    if (n > FDEMRI_SORT_MAX) {
+    if (n > smem_keys) {
         fdemri_bitonic(pairs + o0, n);
         return;
     }

@@ -259,8 +259,9 @@ def test_work_list_overflow_is_loud_then_recovers(fd, orc):
 
 
 def test_many_voices_in_one_tile(fd, orc):
-    """More entries in a tile than the shared-memory sorter takes (FDEMRI_SORT_MAX = 8192): the in-place global
-    sort must give the same fixed order.  9000 voices (l = 2, m = 2, n = 0) all cover the same bins."""
+    """More entries in a tile than the shared-memory sorter takes (FDEMRI_SORT_CAP_TILE = 8192 keys per tile,
+    FDEMRI_SORT_CAP_BIN = 2048 per bin of the bin-major mode): the in-place global sort must give the same fixed
+    order.  9000 voices (l = 2, m = 2, n = 0) all cover the same bins."""
     from paper_2307_12585_b200 import synth
     base = synth.small_case(seed=3, n_knots=6, n_freq=3000, modes=((2, 2, 0),), turnover=False)
     base.f0 = 4.0e-3                                             # F = 2 f_phi sweeps 4.0 .. 5.8 mHz
@@ -276,6 +277,15 @@ def test_many_voices_in_one_tile(fd, orc):
     wf2, hp2, hx2, _ = run_gpu(fd, base)                         # and it is reproducible bit for bit
     assert np.array_equal(hp, hp2) and np.array_equal(hx, hx2)
     wf.close(); wf2.close()
+    hb = []
+    for _ in range(2):                                           # per-bin lists of 9000 keys, twice: same bits
+        wf3 = fd.waveform_from_workload(base, flags=fd.FDEMRI_FLAG_BIN_MAJOR)
+        wf3.sum(base.theta, base.phi)
+        hb.append(wf3.result())
+        assert wf3.stats()["n_evals"] == ref["n_evals"]
+        wf3.close()
+    check(hb[0][0][0], hb[0][1][0], ref, "9000 voices per bin, bin-major")
+    assert np.array_equal(hb[0][0], hb[1][0]) and np.array_equal(hb[0][1], hb[1][1])
 
 
 def test_fused_inner_products_eq12(fd, orc):
