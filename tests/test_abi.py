@@ -42,3 +42,33 @@ def test_sass_is_sm100a_fp64():
     sass = subprocess.run([cuobjdump, "-sass", build.build()], capture_output=True, text=True).stdout
     body = sass.split("Function : _Z10k_tile_sum7SumArgs")[1].split("Function : ")[0]
     assert body.count("DFMA") > 50
+
+
+def test_plan_argument_validation_without_gpu():
+    """fdemri_plan / fdemri_plan_kerr reject bad arguments before touching the device (host logic only)."""
+    import numpy as np
+    L = binding.lib()
+    h = ctypes.c_void_p()
+    ip = ctypes.POINTER(ctypes.c_int32)
+    fake = ctypes.c_void_p(256)                          # a non-NULL "device pointer": never dereferenced on these paths
+
+    def plan(fn, modes, n_batch=1, n_knots=10, n_freq=1000, df=1e-6, flags=0, t=fake):
+        a = np.ascontiguousarray(modes, dtype=np.int32)
+        return fn(ctypes.byref(h), a.shape[0], a.ctypes.data_as(ip), n_batch, n_knots, t, n_freq, None, 0.0, df, flags)
+
+    INVALID = 1
+    for fn, good, bads in (
+            (L.fdemri_plan, [(2, 2, 0)], [[(1, 0, 0)], [(2, 3, 0)], [(2, -1, 0)], [(2, 2, 200000)], [(61, 0, 0)]]),
+            (L.fdemri_plan_kerr, [(2, 2, 1, 0)], [[(1, 0, 0, 0)], [(2, 3, 0, 0)], [(2, -1, 0, 0)], [(2, 2, 200000, 0)],
+                                                  [(2, 2, 0, 200000)]])):
+        for bad in bads:
+            assert plan(fn, bad) == INVALID and not h.value, bad
+        assert plan(fn, good, n_knots=3) == INVALID            # fewer than 4 knots: no not-a-knot spline
+        assert plan(fn, good, n_knots=513) == INVALID
+        assert plan(fn, good, n_freq=0) == INVALID
+        assert plan(fn, good, df=0.0) == INVALID               # uniform grid needs df > 0
+        assert plan(fn, good, t=None) == INVALID
+        assert plan(fn, good, flags=2 | 4) == INVALID          # bin-major and tile-major at once
+    assert L.fdemri_plan_kerr(None, 1, None, 1, 10, fake, 1000, None, 0.0, 1e-6, 0) == INVALID
+    assert L.fdemri_build_splines_kerr(None, fake, fake, fake, fake, fake, fake, fake, None) == INVALID
+    assert L.fdemri_build_splines(None, fake, fake, fake, fake, fake, None) == INVALID
