@@ -695,3 +695,35 @@ def test_kerr_voices_selection_and_fused_inner(fd, orc):
     assert abs(o[0] - want_hh) <= 1e-10 * want_hh
     assert abs(complex(o[1], o[2]) - want_dh) <= 1e-10 * np.sqrt(want_hh * orc.inner(d[0], d[1])[0])
     wf.close()
+
+
+def test_step_is_capturable_in_a_cuda_graph(fd, orc):
+    """build_splines + sum enqueue only (kernels, memsets, one small copy, an event fork/join onto the plan's side
+    stream): the sequence captures into a CUDA graph, and a replay on fresh inputs gives the bits of the stream launch."""
+    import torch
+    from paper_2307_12585_b200 import synth
+    w = synth.small_case(seed=13, n_knots=20, n_freq=40000)
+    wf = fd.waveform_from_workload(w)
+    ins = wf._inputs
+    s = torch.cuda.Stream()
+
+    def step():
+        fd.fdemri_build_splines(wf.plan, *ins)
+        fd.fdemri_sum(wf.plan, w.theta, w.phi, wf.hplus, wf.hcross)
+
+    with torch.cuda.stream(s):
+        step()
+    hp0, hx0 = wf.result()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        step()
+    # new amplitudes in the captured input buffer: the replay must follow them
+    ins[4].mul_(-2.0)
+    wf.hplus.zero_(); wf.hcross.zero_()
+    g.replay()
+    hp1, hx1 = wf.result()
+    assert np.array_equal(hp1, -2.0 * hp0) and np.array_equal(hx1, -2.0 * hx0)
+    ref = oracle_c(orc, w, w.freq_array())
+    check(hp1[0] / -2.0, hx1[0] / -2.0, ref, "graph replay")
+    del g
+    wf.close()
