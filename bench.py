@@ -130,6 +130,7 @@ def cpu_oracle_sample(w, total_evals, n_bins=500000, seed=0):
     t0 = time.perf_counter()
     r = oracle_waveform(orc, w, freq, extra=False)
     dt = time.perf_counter() - t0
+    cores = orc.num_threads                                 # read before the one-thread pass below resets it
     frac = r["n_evals"] / float(total_evals) if total_evals else float("nan")
     # one thread, on a smaller sample (single-thread time beside the all-cores one)
     idx1 = idx[:: max(1, len(idx) // 12000)]
@@ -138,7 +139,7 @@ def cpu_oracle_sample(w, total_evals, n_bins=500000, seed=0):
     dt1 = time.perf_counter() - t1
     single = {"evals_per_s": r1["n_evals"] / dt1, "waveforms_per_s": (r1["n_evals"] / float(total_evals)) / dt1 if total_evals else None,
               "seconds": dt1, "bins": int(len(idx1))}
-    return {"single_thread": single, "value": frac / dt, "unit": "waveforms/s", "cores": orc.num_threads, "kind": "oracle",
+    return {"single_thread": single, "value": frac / dt, "unit": "waveforms/s", "cores": cores, "kind": "oracle",
             "sample": f"{len(idx)} random bins of the covered band ({r['n_evals']} of {int(total_evals)} mode-bin "
                       f"evaluations) incl. the oracle's spline build, {dt:.2f} s wall; scaled by evaluation count",
             "evals_per_s": r["n_evals"] / dt, "seconds": dt}
@@ -154,9 +155,10 @@ def run_reference(args):
     # evaluation count of the full workload from a coarse oracle pass is too slow; use the count of the sample and
     # the covered-band fraction: report evaluations/s and the waveforms/s it implies with SURVEY's count
     total_evals = 3.299e8 if args.config == 2 else None
-    times, evals = [], 0
+    times, evals, cores = [], 0, orc.num_threads
     for i in range(args.warmup + args.steps):
         r = cpu_oracle_sample(w, total_evals or 1.0, n_bins=200000, seed=i)
+        cores = r["cores"]
         if i >= args.warmup:
             times.append(r["seconds"]); evals += r["evals_per_s"] * r["seconds"]
     tot = sum(times)
@@ -166,7 +168,7 @@ def run_reference(args):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f80 (x87 long double)",
             "data": "synthetic",
             "config": {"workload": workload_name(args.config, w), "sample": "200000 random bins of the covered band per step"},
-            "cpu_baseline": {"value": val, "unit": "waveforms/s", "cores": orc.num_threads, "kind": "oracle",
+            "cpu_baseline": {"value": val, "unit": "waveforms/s", "cores": cores, "kind": "oracle",
                              "sample": "each step: 200000 random bins of the covered band incl. spline build, scaled by "
                                        "evaluation count (3.299e8 per waveform)"},
             "e2e": {"value": val, "unit": "waveforms/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
