@@ -27,7 +27,8 @@ sys.path.insert(0, ROOT)
 
 METRIC = "waveforms/s, 3843-mode 2-yr FD sum (FP64)"
 FLOP_PER_EVAL = 200.0          # SURVEY.md 8(d) / DESIGN.md: algorithmic FP64 flop per mode-bin evaluation
-TILE_SUM_DRAM_BYTES = 170.3e6    # ncu capture of config 2, profiles/r1k_tile.md
+TILE_SUM_DRAM_BYTES = 170.9e6    # ncu capture of config 2, profiles/r1l_final.md
+TILE_SUM_EXECUTED_FLOP_FRAC = 0.399   # same capture: (2 DFMA + DADD + DMUL) thread instructions per cycle / (148 x 64 x 2)
 KERNELS_PER_STEP = 8           # spline_shared, spline_amp, records, pair_scan, pair_pass<1>, pair_sort | weights, sum (+ pair_pass<0> in bin-major mode)
 
 
@@ -454,7 +455,10 @@ def main():
             "roofline": {"bound": "alu", "kernel": "k_tile_sum", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
                          "frac": achieved / peak_tf, "traffic": TILE_SUM_DRAM_BYTES if args.config == 2 else None,
                          "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of one k_tile_sum launch, ncu --set full "
-                                         "(profiles/r1k_tile.md); bytes, for context: the bound is the FP64 pipe",
+                                         "(profiles/r1l_final.md); bytes, for context: the bound is the FP64 pipe",
+                         "executed_flop_frac_ncu": TILE_SUM_EXECUTED_FLOP_FRAC if args.config == 2 else None,
+                         "executed_flop_frac_note": "frac counts SURVEY 8(d)'s 200 algorithmic flop per evaluation; the kernel "
+                                                    "executes ~125 (ncu, profiles/r1l_final.md): this is the executed-instruction fraction",
                          "kernel_ms": k_ms,
                          "flop_per_eval": FLOP_PER_EVAL,
                          "peak_source": "FP64 DFMA loop measured live (fdemri_measure_fp64_peak); nominal 148 SM x 64 "
