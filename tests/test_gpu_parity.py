@@ -431,6 +431,64 @@ def test_both_sum_kernels_on_the_same_inputs(fd, orc, mode):
         wf.close()
 
 
+@pytest.mark.parametrize("mode", ["bin", "tile"])
+def test_empty_work_list_every_mode_masked_out(fd, orc, mode):
+    """Degenerate case: the mode mask of L60 drops every mode, so the segment -> bin map has no entry and the work list
+    is empty.  Both sum kernels must still write every bin (exact zeros, buffers pre-filled with NaN), count no
+    evaluation, and the fused inner products of the empty waveform are exactly 0; with the mask removed the same plan
+    gives the oracle's waveform again."""
+    import torch
+    from paper_2307_12585_b200 import synth
+    w = synth.small_case(seed=2, n_knots=14)
+    flag = fd.FDEMRI_FLAG_BIN_MAJOR if mode == "bin" else fd.FDEMRI_FLAG_TILE_MAJOR
+    wf = fd.waveform_from_workload(w, flags=flag)
+    keep = torch.zeros((1, w.lmn.shape[0]), dtype=torch.uint8, device=wf.dev)
+    fd.fdemri_set_mode_mask(wf.plan, keep)
+    wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)
+    wf.hplus.fill_(float("nan")); wf.hcross.fill_(float("nan"))
+    wf.sum(w.theta, w.phi)
+    hp, hx = wf.result()
+    st = wf.stats()
+    assert st["n_evals"] == 0 and st["n_pairs"] == 0 and st["flags"] == 0
+    assert np.all(hp == 0) and np.all(hx == 0)
+    out = torch.full((1, 4), float("nan"), dtype=torch.float64, device=wf.dev)
+    fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, out, hann=True)
+    torch.cuda.synchronize()
+    assert np.all(out.cpu().numpy()[0, :3] == 0.0)
+    fd.fdemri_set_mode_mask(wf.plan, None)
+    wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)
+    wf.sum(w.theta, w.phi)
+    hp, hx = wf.result()
+    ref = oracle_c(orc, w, w.freq_array())
+    check(hp[0], hx[0], ref, f"small case after removing an all-zero mask, {mode}-major")
+    assert wf.stats()["n_evals"] == ref["n_evals"] > 0
+    wf.close()
+
+
+def test_degenerate_constant_frequencies_and_zero_amplitudes(fd, orc):
+    """Two degenerate inputs.  (a) f_phi and f_r constant in time: every segment of every voice has F_k = F_{k+1}, so
+    under R6 (half-open intervals decided on the knot doubles) no bin belongs to any segment -- no entry, no
+    evaluation, exact zeros on both sides (the delta-function limit is not SPA, R10).  (b) A = 0 at every knot: the
+    map and the evaluation count are those of the non-zero case, every term is exactly 0."""
+    import dataclasses
+    from paper_2307_12585_b200 import synth
+    w = synth.small_case(seed=2, n_knots=14)
+    t = w.t_knots
+    wc = dataclasses.replace(w, f_phi=np.full_like(w.f_phi, 2.0e-3), f_r=np.full_like(w.f_r, 1.2e-3),
+                             Phi_phi=2 * np.pi * 2.0e-3 * t, Phi_r=2 * np.pi * 1.2e-3 * t)
+    wf, hp, hx, st = run_gpu(fd, wc)
+    ref = oracle_c(orc, wc, wc.freq_array())
+    assert ref["n_evals"] == 0 and st["n_evals"] == 0 and st["flags"] == 0
+    assert np.all(hp == 0) and np.all(hx == 0) and np.all(ref["hplus"] == 0)
+    wf.close()
+    wz = dataclasses.replace(w, amp=np.zeros_like(w.amp))
+    wf, hp, hx, st = run_gpu(fd, wz)
+    ref = oracle_c(orc, wz, wz.freq_array())
+    assert st["n_evals"] == ref["n_evals"] > 0 and st["flags"] == 0
+    assert np.all(hp == 0) and np.all(hx == 0) and np.all(ref["hplus"] == 0) and np.all(ref["hcross"] == 0)
+    wf.close()
+
+
 def test_bin_major_grows_its_work_list_and_fused_inner(fd, orc):
     """Config 1 forced through the bin-major kernel: 4.9e7 work-list entries do not fit the default capacity, so the
     binding has to grow the work space; then parity, and the Eq. 12 inner products formed from the written waveform."""
