@@ -452,7 +452,9 @@ def test_empty_work_list_every_mode_masked_out(fd, orc, mode):
     assert st["n_evals"] == 0 and st["n_pairs"] == 0 and st["flags"] == 0
     assert np.all(hp == 0) and np.all(hx == 0)
     out = torch.full((1, 4), float("nan"), dtype=torch.float64, device=wf.dev)
-    fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, out, hann=True)
+    # (bin-major plans take the inner products from the written waveform: include/fdemri.h, FDEMRI_ERR_UNSUPPORTED)
+    bufs = dict(hplus=wf.hplus, hcross=wf.hcross) if mode == "bin" else {}
+    fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, out, hann=True, **bufs)
     torch.cuda.synchronize()
     assert np.all(out.cpu().numpy()[0, :3] == 0.0)
     fd.fdemri_set_mode_mask(wf.plan, None)
