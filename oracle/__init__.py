@@ -196,15 +196,22 @@ class Oracle:
         return float(out[0]), complex(out[1], out[2])
 
 
-def select_modes(amp, eps):
-    """Mode selection of PAPER.md L60, word by word, in plain numpy (no compiled code): "Within each time step of the
-    sparse array, we take |A(t)|^2 and sort the individual modes in descending order and compute a cumulative
-    summation.  From this sorted array, we check whether the additional power contributed by an individual mode falls
-    below the threshold eps related to the total power emitted.  ...  The selected modes are given by the union of
-    all contributing modes across all time steps."
-    amp: [n_modes][n_knots][2] (re, im).  Returns (keep [n_modes] bool, total [n_knots]).
-    Reading (R15): a mode contributes at a time step iff its own power is at least eps times the total power
-    of all modes at that step; in the sorted array this is a prefix, found here by walking the sorted array."""
+def select_modes(amp, eps, rule="own"):
+    """Mode selection of PAPER.md L60 in plain numpy (no compiled code).  The paper: "Within each time step of the sparse
+    array, we take |A(t)|^2 and sort the individual modes in descending order and compute a cumulative summation.  From
+    this sorted array, we check whether the additional power contributed by an individual mode falls below the threshold
+    eps related to the total power emitted. ... The selected modes are given by the union of all contributing modes
+    across all time steps."  The rule itself is not printed (L60 defers to Katz et al. 2021): **parity unpinned** against
+    FEW; both readings of DESIGN.md R15 are written out here, step by step in the paper's order.
+      rule="own":        a mode contributes at a time step iff its own ("additional") power is at least eps times the
+                         total power of all modes at that step; in the sorted array this is a prefix, found by walking it.
+      rule="cumulative": the contributing modes are the shortest prefix of the sorted array whose cumulative sum reaches
+                         (1 - eps) times the total, i.e. sorted mode i is kept iff the cumulative sum BEFORE it is still
+                         below (1 - eps) * total; the discarded power is then at most eps * total.
+    Sorting is stable (equal powers keep mode order); the cumulative sum is numpy's sequential sum.
+    amp: [n_modes][n_knots][2] (re, im).  Returns (keep [n_modes] bool, total [n_knots])."""
+    if rule not in ("own", "cumulative"):
+        raise ValueError(rule)
     amp = np.asarray(amp, dtype=np.float64)
     power = amp[..., 0] ** 2 + amp[..., 1] ** 2                 # [n_modes][n_knots]
     n_modes, n_knots = power.shape
@@ -215,10 +222,16 @@ def select_modes(amp, eps):
         sorted_p = power[order, k]
         cumulative = np.cumsum(sorted_p)
         total[k] = cumulative[-1]
-        for i in range(n_modes):                                 # the additional power of mode i is sorted_p[i]
-            if sorted_p[i] < eps * total[k]:
-                break
+        before = 0.0                                             # cumulative sum of the modes before sorted mode i
+        for i in range(n_modes):
+            if rule == "own":
+                if sorted_p[i] < eps * total[k]:                 # the additional power of mode i is sorted_p[i]
+                    break
+            else:
+                if not (before < (1.0 - eps) * total[k]):
+                    break
             keep[order[i]] = True
+            before = cumulative[i]
     return keep, total
 
 

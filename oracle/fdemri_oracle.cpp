@@ -308,6 +308,37 @@ static ld solve_piece(const ld* c, ld x, ld ta, ld tb) {
     return tau;
 }
 
+// Interior extrema of the segment cubic F(tau) = c0 + c1 tau + c2 tau^2 + c3 tau^3 on (0, h): the points where
+// F'(tau) = c1 + 2 c2 tau + 3 c3 tau^2 changes sign (R7: "interior extremum tau_e from F'(tau) = 0").
+// F' is a parabola: monotone on either side of its vertex, so every sign change of F' on [0, h] is bracketed by
+// consecutive points of {0, vertex (if inside), h} and found by bisection to the last bit of long double.
+// (A double root of F' -- an inflection with a horizontal tangent -- is not a sign change and gives no extremum.)
+static void interior_extrema(const ld* c, ld h, ld* ext, int* ne) {
+    auto dF = [&](ld tau) { return c[1] + tau * (2.0L * c[2] + tau * 3.0L * c[3]); };
+    ld pts[3]; int np = 0;
+    pts[np++] = 0.0L;
+    if (c[3] != 0.0L) {
+        const ld tv = -c[2] / (3.0L * c[3]);              // vertex of the parabola F'
+        if (tv > 0.0L && tv < h) pts[np++] = tv;
+    }
+    pts[np++] = h;
+    *ne = 0;
+    for (int j = 0; j + 1 < np; ++j) {
+        ld a = pts[j], b = pts[j + 1];
+        ld fa = dF(a), fb = dF(b);
+        if (!((fa < 0.0L && fb > 0.0L) || (fa > 0.0L && fb < 0.0L))) continue;   // no strict sign change
+        for (;;) {
+            const ld mid = a + 0.5L * (b - a);
+            if (!(mid > a && mid < b)) break;             // the bracket has collapsed to neighbouring numbers
+            const ld fm = dF(mid);
+            if (fm == 0.0L) { a = b = mid; break; }
+            if ((fm < 0.0L) == (fa < 0.0L)) { a = mid; fa = fm; } else { b = mid; }
+        }
+        const ld r = a + 0.5L * (b - a);
+        if (r > 0.0L && r < h && *ne < 2) ext[(*ne)++] = r;
+    }
+}
+
 // Test switch (pin P7): when set, every list voice (any sign of m) stands for itself only -- no implied
 // (l,-m,-n) partner -- and contributes S(f) Y_lm to h~(f), i.e. W+ = Y/2, Wx = iY/2.
 static int g_explicit_voices = 0;
@@ -407,20 +438,7 @@ static int sum_impl(int n_modes, const int32_t* lmn, const int32_t* kk, int N, c
             const ld* c = &V.cF[4 * k];
             ld h = (ld)t[k + 1] - (ld)t[k];
             ld ext[2]; int ne = 0;
-            ld qa = 3.0L * c[3], qb = 2.0L * c[2], qc = c[1];      // F' = qc + qb tau + qa tau^2
-            if (qa == 0.0L) {
-                if (qb != 0.0L) { ld r = -qc / qb; if (r > 0.0L && r < h) ext[ne++] = r; }
-            } else {
-                ld disc = qb * qb - 4.0L * qa * qc;
-                if (disc > 0.0L) {
-                    ld sq = sqrtl(disc);
-                    ld qq = -0.5L * (qb + (qb >= 0 ? sq : -sq));
-                    ld r1 = qq / qa, r2 = (qq != 0.0L) ? qc / qq : r1;
-                    if (r1 > r2) std::swap(r1, r2);
-                    if (r1 > 0.0L && r1 < h) ext[ne++] = r1;
-                    if (r2 > 0.0L && r2 < h && r2 != r1) ext[ne++] = r2;
-                }
-            }
+            interior_extrema(c, h, ext, &ne);
             ld brk[4]; double val[4]; int nb = 0;
             brk[nb] = 0.0L; val[nb++] = Fk[k];
             for (int e = 0; e < ne; ++e) { brk[nb] = ext[e]; val[nb++] = (double)horner3(c, ext[e]); }

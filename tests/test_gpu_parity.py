@@ -1,8 +1,8 @@
 """GPU parity: libfdemri (through the C ABI) against the CPU oracle, element by element.
 
 Bar (BASELINE.json north_star): per bin |delta h| <= 1e-10 max|h|, and 1 - overlap <= 1e-12 (flat noise,
-both polarisations).  Bins the oracle marks boundary-ambiguous (R8) are excluded from the per-bin
-check (expected count: 0).  Level C = independent spline builds; level A = oracle fed the GPU's coefficients.
+both polarisations).  Bins the oracle marks boundary-ambiguous (R8: within 16 ulp of an
+extremum value F_e) are excluded from the per-bin check (expected count: 0; MAX_AMBIGUOUS = 2 tolerated per waveform).  Level C = independent spline builds; level A = oracle fed the GPU's coefficients.
 """
 import functools
 import math
@@ -16,6 +16,7 @@ pytestmark = pytest.mark.gpu
 
 TOL_BIN = 1e-10
 TOL_MISMATCH = 1e-12
+MAX_AMBIGUOUS = 2          # DESIGN.md R8
 
 
 @pytest.fixture(scope="module")
@@ -43,7 +44,7 @@ def oracle_c(orc, w, freq, b=0):
 
 def check(gp, gx, ref, label):
     keep = ref["ambiguous"] == 0
-    assert (~keep).sum() <= 2, f"{label}: {(~keep).sum()} ambiguous bins"
+    assert (~keep).sum() <= MAX_AMBIGUOUS, f"{label}: {(~keep).sum()} ambiguous bins"
     err = max_rel_err(gp, gx, ref["hplus"], ref["hcross"], mask=keep)
     mm = one_minus_overlap(gp[keep], gx[keep], ref["hplus"][keep], ref["hcross"][keep])
     print(f"[parity] {label}: max|dh|/max|h| = {err:.3e}, 1-overlap = {mm:.3e}, bins = {keep.sum()}")
@@ -371,7 +372,7 @@ def test_random_small_cases_sweep(fd, orc):
     the support (P8) on every one of them."""
     from paper_2307_12585_b200 import synth
     rng = np.random.default_rng(20230712)
-    worst, skipped = 0.0, 0
+    worst = 0.0
     for case in range(20):
         n_knots = int(rng.integers(4, 40))
         n_modes = int(rng.integers(1, 9))
@@ -388,28 +389,22 @@ def test_random_small_cases_sweep(fd, orc):
         wf = fd.waveform_from_workload(w)
         wf.sum(w.theta, w.phi)
         hp, hx = wf.result()
-        st = wf.stats(check=False)
-        if st["status"] == 5:                      # a segment cubic with two interior extrema (R5): flagged, not summed
-            assert st["flags"] & 1
-            skipped += 1
-            wf.close()
-            continue
-        assert st["status"] == 0
+        st = wf.stats()
+        assert st["status"] == 0 and st["flags"] == 0
         ref = oracle_c(orc, w, w.freq_array())
         assert st["n_evals"] == ref["n_evals"], (case, modes)
         if ref["n_evals"] == 0:
             assert not hp.any() and not hx.any()
         else:
             keep = ref["ambiguous"] == 0
-            assert (~keep).sum() <= 2
+            assert (~keep).sum() <= MAX_AMBIGUOUS
             err = max_rel_err(hp[0], hx[0], ref["hplus"], ref["hcross"], mask=keep)
             zero = (ref["nterms"] == 0) & keep
             assert np.all(hp[0][zero] == 0) and np.all(hx[0][zero] == 0)
             assert err <= TOL_BIN, (case, modes, err)
             worst = max(worst, err)
         wf.close()
-    assert skipped <= 5
-    print(f"[parity] 20 random small cases ({skipped} flagged unsupported): worst max|dh|/max|h| = {worst:.3e}")
+    print(f"[parity] 20 random small cases: worst max|dh|/max|h| = {worst:.3e}")
 
 
 @pytest.mark.parametrize("mode", ["bin", "tile"])
@@ -527,28 +522,8 @@ def test_segment_with_two_interior_extrema(fd, orc):
     """R5: the paper assumes at most one turnover per spline segment (L105).  A zig-zag f_r through 8 random knots
     (seed 7: one segment's cubic has TWO interior extrema; checked with scipy below) must be summed all the same, on
     its three monotone branches, by both kernels."""
-    from scipy.interpolate import CubicSpline
-    from paper_2307_12585_b200 import synth
-    rng = np.random.default_rng(7)
-    N = int(rng.integers(5, 9))
-    T = 3.0e6
-    t = np.sort(np.concatenate([[0, T], rng.uniform(0.05, 0.95, N - 2) * T]))
-    f_r = 1.3e-3 + 3e-4 * rng.uniform(-1, 1, N)
-    cs = CubicSpline(t, f_r)
-    two = 0
-    for k in range(N - 1):
-        r = np.roots([3 * cs.c[0, k], 2 * cs.c[1, k], cs.c[2, k]])
-        r = r[np.isreal(r)].real
-        two += int(np.sum((r > 0) & (r < t[k + 1] - t[k])) == 2)
-    assert two >= 1
-    f_phi = 2.0e-3 + 4.0e-4 * (t / T)
-    Phi_r = 2 * np.pi * np.concatenate([[0.0], np.cumsum(0.5 * (f_r[1:] + f_r[:-1]) * np.diff(t))])
-    Phi_phi = 2 * np.pi * (2.0e-3 * t + 2.0e-4 * t ** 2 / T)
-    lmn = np.array([[2, 0, 1], [3, 1, -1], [2, 2, 2]], dtype=np.int32)
-    amp = synth.amplitudes(np.random.Generator(np.random.PCG64(3)), lmn, t, "n2")
-    n_freq = 24000
-    w = synth.Workload("two-extrema", lmn, t[None], f_phi[None], f_r[None], Phi_phi[None], Phi_r[None], amp[None],
-                       n_freq, 0.0, 1.0 / T, None, 1.1, -0.4, {})
+    from helpers import zigzag_case
+    w = zigzag_case()
     ref = oracle_c(orc, w, w.freq_array())
     assert ref["max_roots"] >= 3
     for flag in (fd.FDEMRI_FLAG_TILE_MAJOR, fd.FDEMRI_FLAG_BIN_MAJOR):
