@@ -29,7 +29,7 @@ METRIC = "waveforms/s, 3843-mode 2-yr FD sum (FP64)"
 FLOP_PER_EVAL = 200.0          # SURVEY.md 8(d) / DESIGN.md: algorithmic FP64 flop per mode-bin evaluation
 TILE_SUM_DRAM_BYTES = 170.9e6    # ncu capture of config 2, profiles/r1l_final.md
 TILE_SUM_EXECUTED_FLOP_FRAC = 0.399   # same capture: (2 DFMA + DADD + DMUL) thread instructions per cycle / (148 x 64 x 2)
-KERNELS_PER_STEP = 8           # spline_shared, spline_amp, records, pair_scan, pair_pass<1>, pair_sort | weights, sum (+ pair_pass<0> in bin-major mode)
+KERNELS_PER_STEP = 5           # k_spline_amp, k_spline_shared, k_records | k_weights, k_tile_sum (or k_bin_sum)
 
 
 def workload_name(idx, w):
@@ -215,11 +215,7 @@ def run_batched(args, fd, fdist, torch, dev, rank, world, local, barrier):
         ld = dict(plan=plan, t_knots=t_knots, dev_in=dev_in, hp=hp, hx=hx, theta=w.theta, phi=w.phi)
         give_workspace(plan, fd.fdemri_workspace_bytes(plan))
         fd.fdemri_build_splines(plan, *dev_in)
-        st = fd.fdemri_get_stats(plan, check=False)
-        if st["flags"] & 16:                                # work list larger than the default capacity: grow
-            give_workspace(plan, fd.fdemri_workspace_bytes(plan) + 4 * int(st["n_pairs"] * 1.1))
-            fd.fdemri_build_splines(plan, *dev_in)
-            st = fd.fdemri_get_stats(plan, check=True)
+        st = fd.fdemri_get_stats(plan, check=True)
         ld["n_evals"] = st["n_evals"]
         loads.append(ld)
         del w

@@ -5,7 +5,8 @@
  *   S1  not-a-knot cubic splines of f_phi, f_r, Phi_phi, Phi_r and of Re/Im A_lmn over the sparse
  *       trajectory;
  *   S2  per voice (l,m,n) and segment, the cubic  f = A + B tau + C tau^2 + D tau^3  (Eq. 6) and
- *       the contiguous range of frequency bins it covers, "predetermined before the summation" (L105);
+ *       the contiguous range of frequency bins it covers, "predetermined before the summation" (L105), with two
+ *       levels of bands over those ranges from which the sum kernels find the entries that meet a tile of bins;
  *   S3  per bin and root t_j(f) the term of Eq. 9 (L107-119):
  *         A(t) g(X)/sqrt|Fdot| exp{i[2 pi f t - Phi(t)]},  X = 2 pi Fdot^3 / (3 Fddot^2),
  *       summed over voices with the spin-weighted harmonics (Eq. 1) into h~+(f), h~x(f), the
@@ -15,7 +16,8 @@
  * Conventions
  *   - "dev" pointers are CUDA device pointers, "host" pointers are host pointers.  The caller owns every
  *     buffer, including the work space; the plan owns only small host metadata.
- *   - Nothing here allocates device memory, and build_splines / sum do not synchronise: they enqueue
+ *   - No call allocates device memory except the two fdemri_measure_* microbenchmarks (8 bytes, freed before they
+ *     return); a plan owns a small pinned host buffer.  build_splines / sum do not synchronise: they enqueue
  *     kernels on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default stream).
  *     build_splines runs one of its kernels on a stream of the plan, forked from and joined back into
  *     `cuda_stream` with events, so ordering on `cuda_stream` is all a caller needs.
@@ -34,11 +36,10 @@ extern "C" {
 enum {
     FDEMRI_OK = 0,
     FDEMRI_ERR_INVALID_ARG = 1, /* bad size, NULL pointer, l<2, m<0, m>l, unsorted knots ...            */
-    FDEMRI_ERR_WORKSPACE = 2,   /* work space missing or too small (fdemri_stats.n_pairs: work-list entries needed) */
+    FDEMRI_ERR_WORKSPACE = 2,   /* work space missing or smaller than fdemri_workspace_bytes                        */
     FDEMRI_ERR_CUDA = 3,        /* a CUDA runtime call or kernel failed                                   */
     FDEMRI_ERR_NOT_BUILT = 4,   /* fdemri_sum / get_coeffs before fdemri_build_splines                    */
-    FDEMRI_ERR_UNSUPPORTED = 5  /* the call is not available in this configuration (fdemri_sum_inner without
-                                   waveform buffers on a bin-major plan)                                    */
+    FDEMRI_ERR_UNSUPPORTED = 5  /* the call is not available in this configuration (not returned at present)   */
 };
 
 /* plan flags */
@@ -46,22 +47,20 @@ enum {
     FDEMRI_FLAG_NONE = 0,
     FDEMRI_FLAG_TIMING = 1,    /* record CUDA events around the S3 sum kernel of every fdemri_sum (see
                                   fdemri_get_kernel_ms); costs two event records per call                  */
-    FDEMRI_FLAG_BIN_MAJOR = 2, /* force the bin-major sum kernel (one warp per frequency bin, lanes over the
-                                  entries that cover it): the right shape when a (voice, segment) covers only a
-                                  few bins -- sparse or down-sampled frequency arrays (section 3.3)  */
+    FDEMRI_FLAG_BIN_MAJOR = 2, /* force the bin-major sum kernel (a CTA owns 32 consecutive bins, one warp per bin at a
+                                  time, lanes over the entries that cover it): the right shape when a (voice, segment)
+                                  covers only a few bins -- sparse or down-sampled frequency arrays (PAPER.md 3.3)   */
     FDEMRI_FLAG_TILE_MAJOR = 4 /* force the tile-major sum kernel (a CTA owns 768 consecutive bins): dense grids.
                                   Default: bin-major iff n_freq < 256 (n_knots - 1)                         */
 };
 
 /* bits of fdemri_stats.flags (device-side validation, read back by fdemri_get_stats) */
 enum {
-    FDEMRI_BAD_TWO_EXTREMA = 1,   /* (not raised any more: a segment cubic with two interior extrema -- the paper
-                                     assumes at most one, L105 -- is split into its three monotone branches)   */
+    FDEMRI_BAD_TWO_EXTREMA = 1,   /* (kept for ABI stability, never raised: a segment cubic with two interior extrema --
+                                     the paper assumes at most one, L105 -- is split into its three monotone branches) */
     FDEMRI_BAD_NONFINITE = 4,     /* NaN/Inf met in the inputs or spline coefficients                      */
-    FDEMRI_BAD_NEWTON = 8,        /* a root iteration hit its iteration cap                                */
-    FDEMRI_BAD_LIST_OVERFLOW = 16 /* the per-tile work list did not fit the work space: fdemri_sum fills its outputs
-                                     with NaN and fdemri_get_stats returns FDEMRI_ERR_WORKSPACE; give
-                                     fdemri_set_workspace at least 4 * n_pairs more bytes and build again      */
+    FDEMRI_BAD_NEWTON = 8,        /* a root iteration of the last fdemri_sum hit its iteration cap          */
+    FDEMRI_BAD_LIST_OVERFLOW = 16 /* (kept for ABI stability, never raised: there is no work list any more)  */
 };
 
 typedef struct fdemri_plan_s* fdemri_plan_t;
@@ -69,13 +68,17 @@ typedef struct fdemri_plan_s* fdemri_plan_t;
 typedef struct {
     uint64_t n_items;        /* non-empty (voice, sign, segment-branch) entries of the last build (S2)        */
     uint64_t reserved;
-    uint64_t n_evals;        /* accumulated (voice, sign, root, bin) terms = "mode-bin evaluations" (P9)      */
+    uint64_t n_evals;        /* "mode-bin evaluations": (voice, sign, root, bin) terms the MAP of the last build assigns,
+                                i.e. the sum of the widths of the entries' bin intervals (P9).  Counted in S2, not by
+                                the sum kernel: per-bin parity is what shows that every one of them was accumulated
+                                (bin-major plans also count the accumulated terms themselves, see n_pairs)           */
     uint64_t n_turnover;     /* segments with an interior extremum of F (Fdot = 0, L92, L105)                 */
     uint64_t n_airy;         /* evaluations that took the small-|X| (Airy) path                              */
     uint64_t flags;          /* OR of FDEMRI_BAD_*                                                            */
     uint64_t n_slow;         /* evaluations of monotone segments that left the fast path (small |X| or a
                                 rejected iteration) and took the safeguarded Newton with a division           */
-    uint64_t n_pairs;        /* (item, tile) pairs of the work list built by the last fdemri_build_splines    */
+    uint64_t n_pairs;        /* last fdemri_sum: tile-major plans: (entry, tile) pairs the producer warps staged;
+                                bin-major plans: terms accumulated (= n_evals)                                   */
 } fdemri_stats;
 
 /* Create a plan.
@@ -83,7 +86,8 @@ typedef struct {
  *              m > 0 voice is implied (L64-66 + symmetry); m = 0 voices stand for themselves.
  *  n_batch     number of independent parameter sets evaluated per call (>= 1)
  *  n_knots     points of the sparse trajectory (4..512), the same for every batch item (L58: ~100)
- *  t_knots_dev [n_batch][n_knots] seconds, strictly increasing; borrowed until fdemri_build_splines returns
+ *  t_knots_dev [n_batch][n_knots] seconds, strictly increasing; borrowed for the plan's life (every
+ *              fdemri_build_splines reads it again, from kernels that run after the call has returned)
  *  n_freq      number of frequency bins
  *  freq_dev    [n_freq] Hz, sorted ascending, >= 0, shared by the batch; borrowed for the plan's life.
  *              NULL selects the uniform grid  f_i = f0 + (double)i*df  (product rounded, then sum rounded) --
@@ -94,17 +98,18 @@ int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, int n_
                 uint32_t flags);
 
 /* Device work space the plan needs (bytes); the caller allocates it (256-byte aligned) and hands it over.
- * The work space holds the spline records, the segment->bin map and the per-tile work list; it must stay valid
- * and untouched between build_splines and the last sum.  The size returned includes a default capacity for the
- * work list (4 bytes per (item, tile) pair); whatever the caller gives beyond the fixed part is used for it, and
- * fdemri_stats.n_pairs reports what the last build needed (see FDEMRI_BAD_LIST_OVERFLOW).  fdemri_set_workspace
- * may be called again with a larger buffer; fdemri_build_splines must then be repeated. */
+ * The work space holds the spline records, the segment->bin map and its bands; it must stay valid and untouched
+ * between build_splines and the last sum.  fdemri_set_workspace returns FDEMRI_ERR_WORKSPACE for a smaller buffer;
+ * it may be called again with another buffer, fdemri_build_splines must then be repeated.
+ * One stream at a time: the per-call scratch (angles, weights, counters, partial inner products) lives in the work
+ * space, so two fdemri_sum calls on one plan must not run concurrently on different streams. */
 size_t fdemri_workspace_bytes(fdemri_plan_t plan);
-/* The fixed part alone (no room for a work list worth the name): the least fdemri_set_workspace accepts. */
+/* The same number (kept for ABI stability: there is no optional part any more). */
 size_t fdemri_workspace_bytes_min(fdemri_plan_t plan);
 int fdemri_set_workspace(fdemri_plan_t plan, void* dev_ptr, size_t bytes);
 
-/* S1.  All inputs are device pointers, borrowed until the enqueued kernels have run.
+/* S1 + S2 (splines, then the records and the segment->bin map).  All inputs are device pointers, borrowed until the
+ * enqueued kernels have run.
  *  f_phi, f_r      [n_batch][n_knots] Hz      fundamental frequencies Omega/(2 pi M) at the knots (L94)
  *  Phi_phi, Phi_r  [n_batch][n_knots] rad     fundamental phases at the knots (L56)
  *  amp             [n_batch][n_modes][n_knots][2] (re, im) mode amplitudes at the knots (L60), with mu/d_L of
@@ -130,8 +135,10 @@ int fdemri_build_splines_kerr(fdemri_plan_t plan, const double* f_phi, const dou
                               const double* Phi_phi, const double* Phi_theta, const double* Phi_r, const double* amp,
                               void* cuda_stream);
 
-/* S0 + S2 + S3 + S4.
- *  theta_host, phi_host  source-frame viewing angles (L66), [n_angles] on the host, n_angles = 1 or n_batch
+/* S0 + S3 + S4 (S2 is part of fdemri_build_splines).
+ *  theta_host, phi_host  source-frame viewing angles (L66), [n_angles] on the host, n_angles = 1 or n_batch; copied
+ *                        into a pinned buffer of the plan before the call returns.  (When the call is captured into a
+ *                        CUDA graph, a replay uses the angles of the most recent fdemri_sum call on the plan.)
  *  hplus_dev, hcross_dev [n_batch][n_freq][2] (re, im) FP64, fully overwritten (zeros where no voice has
  *                        support, L147; the bin f = 0 is always zero) */
 int fdemri_sum(fdemri_plan_t plan, int n_angles, const double* theta_host, const double* phi_host,
@@ -148,8 +155,7 @@ int fdemri_sum(fdemri_plan_t plan, int n_angles, const double* theta_host, const
  *                 window, h_k/2 - h_{k-1}/4 - h_{k+1}/4 with bins outside the grid counting as zero (L145: the
  *                 window the paper applies to the time series); the waveform written to hplus/hcross is not filtered
  *  hplus_dev, hcross_dev  as in fdemri_sum, or both NULL: nothing but the inner products leaves the kernel
- *                 (tile-major plans only: a bin-major plan forms the products from the waveform it writes and
- *                 returns FDEMRI_ERR_UNSUPPORTED without these buffers)
+ *                 (either sum kernel)
  *  inner_out_dev  [n_batch][4] = {<h|h>, Re<d|h>, Im<d|h>, 0}, device memory; sums are formed in a fixed order
  *                 (bitwise reproducible) */
 int fdemri_sum_inner(fdemri_plan_t plan, int n_angles, const double* theta_host, const double* phi_host,
@@ -169,12 +175,15 @@ int fdemri_sum_inner(fdemri_plan_t plan, int n_angles, const double* theta_host,
  * Needs the work space (a [n_batch][n_knots] scratch of total powers).  Enqueued on cuda_stream. */
 int fdemri_select_modes(fdemri_plan_t plan, const double* amp_dev, double eps, unsigned char* keep_dev,
                         int32_t* n_keep_dev, void* cuda_stream);
-/* Modes with keep_dev[b][v] == 0 get no entries in the next fdemri_build_splines and so never reach the sum
- * (keep_dev is borrowed until then; NULL: every mode of the list is summed).  The mode list of the plan is unchanged. */
+/* Modes with keep_dev[b][v] == 0 get no entries in the next fdemri_build_splines and so never reach the sum.
+ * keep_dev is borrowed until it is replaced or the plan is destroyed (every later build reads it, from a kernel that
+ * runs after the call has returned); NULL: every mode of the list is summed.  The mode list of the plan is unchanged. */
 int fdemri_set_mode_mask(fdemri_plan_t plan, const unsigned char* keep_dev);
 
-/* Counters of the last fdemri_sum (synchronises the stream used by that call). */
+/* Counters of the last fdemri_build_splines / fdemri_sum (synchronises the stream used by the last call). */
 int fdemri_get_stats(fdemri_plan_t plan, fdemri_stats* out);
+/* fdemri_stats.n_evals per batch item: out_host [n_batch] on the host.  Synchronises like fdemri_get_stats. */
+int fdemri_get_item_evals(fdemri_plan_t plan, uint64_t* out_host);
 
 /* Spline coefficients as built on the device, for parity level A (oracle fed the GPU's coefficients).
  *  shared_hi, shared_lo [n_batch][4][n_knots-1][4]  (a,b,c,d) of f_phi, f_r, Phi_phi, Phi_r as hi + lo doubles

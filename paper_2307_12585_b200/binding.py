@@ -21,7 +21,7 @@ STATUS = {0: "FDEMRI_OK", 1: "FDEMRI_ERR_INVALID_ARG", 2: "FDEMRI_ERR_WORKSPACE"
           4: "FDEMRI_ERR_NOT_BUILT", 5: "FDEMRI_ERR_UNSUPPORTED"}
 
 EXPORTS = ["fdemri_plan", "fdemri_plan_kerr", "fdemri_build_splines_kerr", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum", "fdemri_sum_inner", "fdemri_select_modes", "fdemri_set_mode_mask",
-           "fdemri_get_stats", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_measure_fp64_peak_3reg", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
+           "fdemri_get_stats", "fdemri_get_item_evals", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_measure_fp64_peak_3reg", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
 
 
 class FdemriStats(C.Structure):
@@ -73,6 +73,8 @@ def lib() -> C.CDLL:
         L.fdemri_set_mode_mask.argtypes = [vp, vp]
         L.fdemri_get_stats.restype = C.c_int
         L.fdemri_get_stats.argtypes = [vp, C.POINTER(FdemriStats)]
+        L.fdemri_get_item_evals.restype = C.c_int
+        L.fdemri_get_item_evals.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.fdemri_get_coeffs.restype = C.c_int
         L.fdemri_get_coeffs.argtypes = [vp, dp, dp, dp]
         L.fdemri_get_kernel_ms.restype = C.c_int
@@ -192,6 +194,12 @@ def fdemri_get_stats(plan, check=True) -> dict:
     return out
 
 
+def fdemri_get_item_evals(plan, n_batch) -> np.ndarray:
+    out = np.zeros(int(n_batch), dtype=np.uint64)
+    _chk("fdemri_get_item_evals", lib().fdemri_get_item_evals(plan, out.ctypes.data_as(C.POINTER(C.c_uint64))))
+    return out
+
+
 def fdemri_get_coeffs(plan, shared_hi=None, shared_lo=None, amp_coef=None):
     _chk("fdemri_get_coeffs", lib().fdemri_get_coeffs(plan, _ptr(shared_hi), _ptr(shared_lo), _ptr(amp_coef)))
 
@@ -262,20 +270,9 @@ class Waveform:
         fdemri_set_workspace(self.plan, self.ws_view)
 
     def ensure_capacity(self, stream=None) -> bool:
-        """Synchronises.  If the last build reported FDEMRI_BAD_LIST_OVERFLOW (the per-tile work list did not fit),
-        allocates a work space with room for fdemri_stats.n_pairs entries and builds again.  Returns True if it
-        had to.  (Marshalling only: the C library never allocates.)"""
-        st = fdemri_get_stats(self.plan, check=False)
-        if not (st["flags"] & 16):
-            return False
-        extra = 4 * int(st["n_pairs"] * 1.1) + 4096
-        self._alloc_workspace(fdemri_workspace_bytes(self.plan) + extra)
-        assert self._inputs is not None
-        self._build(stream)
-        st = fdemri_get_stats(self.plan, check=False)
-        if st["flags"] & 16:
-            raise FdemriError("fdemri_build_splines (work list still does not fit)", 2)
-        return True
+        """Kept for callers of the first release: there is no work list that could outgrow the work space any more
+        (the sum kernels find their entries from the bands of the map), so there is never anything to grow."""
+        return False
 
     def _build(self, stream):
         if self.polar:
@@ -301,6 +298,9 @@ class Waveform:
 
     def stats(self, check=True):
         return fdemri_get_stats(self.plan, check=check)
+
+    def item_evals(self) -> np.ndarray:
+        return fdemri_get_item_evals(self.plan, self.n_batch)
 
     def coeffs(self):
         torch = self.torch

@@ -17,7 +17,6 @@
 #include "fdemri_common.cuh"
 #include "fdemri_map.cuh"
 #include "fdemri_splines.cuh"
-#include "fdemri_pairs.cuh"
 #include "fdemri_select.cuh"
 #include "fdemri_sum.cuh"
 
@@ -39,29 +38,31 @@ struct fdemri_plan_s {
     std::vector<int4> wmeta;
     std::vector<double> wcoef;
     double *sh_hi, *sh_lo, *rec;
-    int2* ent;
-    int* tile_cnt;                 // [B * n_tiles] pairs per tile, then [B * n_tiles] fill cursors
-    unsigned int* tile_off;        // [B * n_tiles + 1]
-    unsigned int* pairs;           // [pair_cap]
-    double* inner_part;            // [B * n_tiles][FDEMRI_CWARPS][4] partial inner products
-    double* inner_edge;            // [B * n_tiles][FDEMRI_CWARPS][4][4] edge bins for the Hann filter
+    int2* ent;                     // [B][V][2][3][S] bin intervals of the segment branches
+    int4* gband;                   // [B][V][2][G] bands of the groups of 32 segments
+    int2* vband;                   // [B][V][2] bands of the voice-signs
+    int* iband;                    // [B][2] {-lo, hi} of the item
+    unsigned long long* item_evals;// [B] mode-bin evaluations of the map, per batch item
+    double* inner_part;            // [ranges][4] partial inner products (a range: 64 bins of a consumer warp, or a block)
+    double* inner_edge;            // [ranges][4][4] edge bins for the Hann filter
     double* sel_total;             // [B][n_knots] total power per time step (mode selection)
     const unsigned char* mode_mask;// [B][V] borrowed from the caller, or NULL: every mode is summed
-    unsigned long long pair_cap;
     double4* wts;
     double* angles;
-    unsigned long long* stats;     // [0..5], [7], [8] = fdemri_stats, [6] = tile counter (low 32 bits); 16 slots
-    std::vector<double> angle_stage;
+    unsigned long long* stats;     // [0..5], [7], [8] = fdemri_stats, [6] = tile counter (low 32 bits), [9] = flags of the
+                                   // last sum; 16 slots
+    double* angle_stage;           // pinned host buffer [2 * n_batch]: the angles of the last sum, read by its async copy
     bool built;
     cudaStream_t last_stream;
     int sm_count;
-    bool spline_attr_set;
     int sum_blocks_per_sm;         // resident CTAs of k_tile_sum per SM (0: not queried yet)
     uint32_t flags;
     cudaEvent_t ev0, ev1;
     cudaStream_t side;             // the amplitude splines run beside the shared ones (fork/join on two events)
     cudaEvent_t ev_fork, ev_join;
     bool ev_valid;
+    cudaEvent_t ev_angles;         // the copy of the angles out of the pinned staging buffer has run
+    bool last_stream_valid;
 };
 
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -88,19 +89,19 @@ static size_t carve(fdemri_plan_s* p, char* base) {
     p->sh_lo = (double*)take(B * 4 * S * 4 * sizeof(double));
     p->rec = (double*)take(B * V * S * R_DOUBLES * sizeof(double));
     p->ent = (int2*)take(B * V * 2 * (size_t)d.ent_max * sizeof(int2));
+    p->gband = (int4*)take(B * V * 2 * (size_t)d.n_groups * sizeof(int4));
+    p->vband = (int2*)take(B * V * 2 * sizeof(int2));
+    p->iband = (int*)take(B * 2 * sizeof(int));
+    p->item_evals = (unsigned long long*)take(B * sizeof(unsigned long long));
     const size_t NT = B * (size_t)d.n_tiles;
-    p->tile_cnt = (int*)take(2 * NT * sizeof(int));
-    p->tile_off = (unsigned int*)take((NT + 1) * sizeof(unsigned int));
     p->wts = (double4*)take(B * V * sizeof(double4));
     p->angles = (double*)take(B * 2 * sizeof(double));
     p->stats = (unsigned long long*)take(16 * sizeof(unsigned long long));
     p->sel_total = (double*)take(B * (size_t)d.n_knots * sizeof(double));
-    // partial inner products of the tile-major kernel (the bin-major mode forms them from the waveform in memory)
-    const size_t NI = (d.tile_bins == 1) ? 0 : NT;
-    p->inner_part = (double*)take(NI * FDEMRI_CWARPS * 4 * sizeof(double));
-    p->inner_edge = (double*)take(NI * FDEMRI_CWARPS * 16 * sizeof(double));
-    // the pair list takes what is left of the work space (default: see fdemri_workspace_bytes)
-    p->pairs = (unsigned int*)take(0);
+    // partial inner products: one range per consumer warp of a tile, or per block of the bin-major kernel
+    const size_t NR = d.bin_major ? NT : NT * FDEMRI_CWARPS;
+    p->inner_part = (double*)take(NR * 4 * sizeof(double));
+    p->inner_edge = (double*)take(NR * 16 * sizeof(double));
     return off;
 }
 
@@ -151,6 +152,19 @@ static void build_weight_table(fdemri_plan_s* p) {
     }
 }
 
+// frees whatever the plan owns (streams, events, the pinned angle buffer); also the error paths of plan_impl
+static void release_plan(fdemri_plan_s* p) {
+    if (!p) return;
+    if (p->side) cudaStreamDestroy(p->side);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
+    if (p->ev0) cudaEventDestroy(p->ev0);
+    if (p->ev1) cudaEventDestroy(p->ev1);
+    if (p->ev_angles) cudaEventDestroy(p->ev_angles);
+    if (p->angle_stage) cudaFreeHost(p->angle_stage);
+    delete p;
+}
+
 static int plan_impl(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, const int32_t* k_host, int n_batch,
                      int n_knots, const double* t_knots_dev, int64_t n_freq, const double* freq_dev, double f0, double df,
                      uint32_t flags) {
@@ -171,19 +185,28 @@ static int plan_impl(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, c
     if ((flags & FDEMRI_FLAG_BIN_MAJOR) && (flags & FDEMRI_FLAG_TILE_MAJOR)) return FDEMRI_ERR_INVALID_ARG;
     const bool bin_major = (flags & FDEMRI_FLAG_BIN_MAJOR) ||
                            (!(flags & FDEMRI_FLAG_TILE_MAJOR) && n_freq < (int64_t)256 * (n_knots - 1));
-    const int tile_bins = bin_major ? 1 : FDEMRI_TILE;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    /* bin-major: the largest block of bins (32, 16, 8) that still gives every resident CTA (two per SM) four blocks:
+       a block costs a scan of all voice bands, so large blocks are cheap, but few blocks balance badly */
+    int tile_bins = bin_major ? FDEMRI_BIN_BLOCK : FDEMRI_TILE;
+    while (bin_major && tile_bins > 8 && (n_freq * (int64_t)n_batch) / tile_bins < (int64_t)8 * prop.multiProcessorCount)
+        tile_bins /= 2;
     int64_t n_tiles = (n_freq + tile_bins - 1) / tile_bins;
     if (n_tiles * (int64_t)n_batch >= ((int64_t)1 << 31)) return FDEMRI_ERR_INVALID_ARG;
     if ((int64_t)n_batch * n_modes * (n_knots - 1) >= ((int64_t)1 << 31)) return FDEMRI_ERR_INVALID_ARG;   /* 32-bit record index */
-    if ((int64_t)n_modes * 6 * (n_knots - 1) >= ((int64_t)1 << 32)) return FDEMRI_ERR_INVALID_ARG;          /* 32-bit work-list key */
+    if ((int64_t)n_modes * 6 * (n_knots + 31) >= ((int64_t)1 << 27)) return FDEMRI_ERR_INVALID_ARG;          /* 27-bit row index */
     fdemri_plan_s* p = new (std::nothrow) fdemri_plan_s();
     if (!p) return FDEMRI_ERR_INVALID_ARG;
     p->d.n_modes = n_modes;
     p->d.n_batch = n_batch;
     p->d.n_knots = n_knots;
     p->d.n_seg = n_knots - 1;
-    p->d.ent_max = 3 * (n_knots - 1);                 /* slot = 3*segment + branch */
+    p->d.n_groups = (n_knots - 1 + 31) / 32;
+    p->d.ent_max = 3 * 32 * p->d.n_groups;            /* key = vs * ent_max + branch * 32 n_groups + segment */
     p->d.n_freq = n_freq;
+    p->d.bin_major = bin_major ? 1 : 0;
     p->d.tile_bins = tile_bins;
     p->d.n_tiles = (int)n_tiles;
     p->d.f0 = f0;
@@ -197,30 +220,28 @@ static int plan_impl(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, c
     p->ws_bytes = 0;
     p->built = false;
     p->last_stream = nullptr;
-    int dev = 0;
-    cudaDeviceProp prop;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
-        delete p;
-        return FDEMRI_ERR_CUDA;
-    }
-    p->sm_count = prop.multiProcessorCount;
     p->sum_blocks_per_sm = 0;
-    p->spline_attr_set = false;
     p->mode_mask = nullptr;
     p->flags = flags;
     p->ev_valid = false;
     p->ev0 = p->ev1 = nullptr;
     p->side = nullptr;
     p->ev_fork = p->ev_join = nullptr;
+    p->angle_stage = nullptr;
+    p->ev_angles = nullptr;
+    p->last_stream_valid = false;
+    p->sm_count = prop.multiProcessorCount;
     if (cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-        cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming) != cudaSuccess) {
-        delete p;
+        cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&p->ev_angles, cudaEventDisableTiming) != cudaSuccess ||
+        cudaHostAlloc((void**)&p->angle_stage, (size_t)2 * n_batch * sizeof(double), cudaHostAllocDefault) != cudaSuccess) {
+        release_plan(p);
         return FDEMRI_ERR_CUDA;
     }
     if (flags & FDEMRI_FLAG_TIMING) {
         if (cudaEventCreate(&p->ev0) != cudaSuccess || cudaEventCreate(&p->ev1) != cudaSuccess) {
-            delete p;
+            release_plan(p);
             return FDEMRI_ERR_CUDA;
         }
     }
@@ -253,28 +274,20 @@ extern "C" int fdemri_plan_kerr(fdemri_plan_t* out, int n_modes, const int32_t* 
 extern "C" size_t fdemri_workspace_bytes(fdemri_plan_t p) {
     if (!p) return 0;
     fdemri_plan_s tmp = *p;
-    // default capacity of the pair list: every entry once plus an eighth of the band per (voice, sign)
-    const size_t pairs = (size_t)p->d.n_batch * p->d.n_modes * 2 * ((size_t)p->d.n_seg + (size_t)p->d.n_tiles / 8 + 1);
-    return carve(&tmp, nullptr) + align_up(pairs * sizeof(unsigned int));
+    return carve(&tmp, nullptr);
 }
 
-extern "C" size_t fdemri_workspace_bytes_min(fdemri_plan_t p) {
-    if (!p) return 0;
-    fdemri_plan_s tmp = *p;
-    return carve(&tmp, nullptr) + 256;
-}
+extern "C" size_t fdemri_workspace_bytes_min(fdemri_plan_t p) { return fdemri_workspace_bytes(p); }
 
 extern "C" int fdemri_set_workspace(fdemri_plan_t p, void* dev_ptr, size_t bytes) {
     if (!p || !dev_ptr) return FDEMRI_ERR_INVALID_ARG;
     if (((uintptr_t)dev_ptr & 255) != 0) return FDEMRI_ERR_INVALID_ARG;
     fdemri_plan_s tmp = *p;
     const size_t fixed = carve(&tmp, nullptr);
-    if (bytes < fixed + 256) return FDEMRI_ERR_WORKSPACE;
+    if (bytes < fixed) return FDEMRI_ERR_WORKSPACE;
     p->ws = dev_ptr;
     p->ws_bytes = bytes;
     carve(p, (char*)dev_ptr);
-    p->pair_cap = (bytes - fixed) / sizeof(unsigned int);
-    if (p->pair_cap > 0xffffffffull) p->pair_cap = 0xffffffffull;
     p->built = false;
     if (cudaMemcpy(p->lmn_dev, p->lmn.data(), p->lmn.size() * sizeof(int32_t), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(p->lm_index_dev, p->lm_index.data(), p->lm_index.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess ||
@@ -284,6 +297,24 @@ extern "C" int fdemri_set_workspace(fdemri_plan_t p, void* dev_ptr, size_t bytes
     if (p->k_dev && cudaMemcpy(p->k_dev, p->kk.data(), p->kk.size() * sizeof(int32_t), cudaMemcpyHostToDevice) != cudaSuccess)
         return FDEMRI_ERR_CUDA;
     if (cudaMemset(p->stats, 0, 16 * sizeof(unsigned long long)) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    return FDEMRI_OK;
+}
+
+// The dynamic shared memory limit of a kernel is an attribute of the function, per device and process-wide (not per
+// plan): set it once per device to what the largest plan (FDEMRI_MAX_KNOTS) can ask for.
+static int raise_spline_smem_limits() {
+    static bool done[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    if (dev >= 0 && dev < 64 && done[dev]) return FDEMRI_OK;
+    const int N = FDEMRI_MAX_KNOTS;
+    const size_t sm_sh = (size_t)(2 * N * FDEMRI_SH_ROW + 5 * N) * sizeof(double2);
+    const size_t sm_am = ((size_t)2 * N * FDEMRI_AMP_ROW + N + (N & 1)) * sizeof(double) +
+                         (size_t)2 * FDEMRI_AMP_VOICES * N * sizeof(double2);
+    if (cudaFuncSetAttribute(k_spline_shared, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_sh) != cudaSuccess ||
+        cudaFuncSetAttribute(k_spline_amp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_am) != cudaSuccess)
+        return FDEMRI_ERR_CUDA;
+    if (dev >= 0 && dev < 64) done[dev] = true;
     return FDEMRI_OK;
 }
 
@@ -297,50 +328,35 @@ static int build_impl(fdemri_plan_t p, const double* f_phi, const double* f_thet
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const FdemriDims& d = p->d;
     p->last_stream = st;
-    if (cudaMemsetAsync(p->stats, 0, 16 * sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
-    // S1: parallel cyclic reduction, one thread per knot
-    {
-        const int N = d.n_knots;
-        const int threads = (N + 31) & ~31;
-        const size_t sm_sh = (size_t)(2 * N * FDEMRI_SH_ROW + 5 * N) * sizeof(double2);
-        const size_t sm_am = ((size_t)2 * N * FDEMRI_AMP_ROW + N + (N & 1)) * sizeof(double) +
-                             (size_t)2 * FDEMRI_AMP_VOICES * N * sizeof(double2);
-        if (!p->spline_attr_set) {
-            if (cudaFuncSetAttribute(k_spline_shared, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_sh) != cudaSuccess ||
-                cudaFuncSetAttribute(k_spline_amp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_am) != cudaSuccess)
-                return FDEMRI_ERR_CUDA;
-            p->spline_attr_set = true;
-        }
-        // the two solves are independent: the amplitudes go to a side stream, joined before S2 reads them
-        const int groups = (d.n_modes + FDEMRI_AMP_VOICES - 1) / FDEMRI_AMP_VOICES;
-        if (cudaEventRecord(p->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(p->side, p->ev_fork, 0) != cudaSuccess)
-            return FDEMRI_ERR_CUDA;
-        k_spline_amp<<<(unsigned)((size_t)d.n_batch * groups), threads, sm_am, p->side>>>(d.n_modes, N, p->t_knots_dev, amp,
-                                                                                       p->rec, p->stats + 5);
-        k_spline_shared<<<dim3(d.n_batch, polar ? 2 : 1), threads, sm_sh, st>>>(N, p->t_knots_dev, f_phi, f_r, Phi_phi, Phi_r,
-                                                                               p->sh_hi, p->sh_lo, p->stats + 5, f_theta,
-                                                                               Phi_theta, p->sh2_hi, p->sh2_lo);
-        if (cudaEventRecord(p->ev_join, p->side) != cudaSuccess || cudaStreamWaitEvent(st, p->ev_join, 0) != cudaSuccess)
-            return FDEMRI_ERR_CUDA;
-    }
-    // S2: records, entries and tile counts; then the per-tile work lists (prefix sum, fill, sort)
-    const size_t NT = (size_t)d.n_batch * d.n_tiles;
-    if (cudaMemsetAsync(p->tile_cnt, 0, 2 * NT * sizeof(int), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
-    size_t nrec = (size_t)d.n_batch * d.n_modes * d.n_seg;
+    if (raise_spline_smem_limits() != FDEMRI_OK) return FDEMRI_ERR_CUDA;
+    if (cudaMemsetAsync(p->stats, 0, 16 * sizeof(unsigned long long), st) != cudaSuccess ||
+        cudaMemsetAsync(p->item_evals, 0, (size_t)d.n_batch * sizeof(unsigned long long), st) != cudaSuccess ||
+        cudaMemsetAsync(p->iband, 0x80, (size_t)d.n_batch * 2 * sizeof(int), st) != cudaSuccess)   /* very negative */
+        return FDEMRI_ERR_CUDA;
+    // S1: parallel cyclic reduction, one thread per knot.  The amplitude splines (Re/Im A of every voice) are
+    // independent of everything S2 needs: they run on the side stream beside the shared splines AND the map, and are
+    // joined before the stream goes on (the sum reads them).
+    const int N = d.n_knots;
+    const int threads = (N + 31) & ~31;
+    const size_t sm_sh = (size_t)(2 * N * FDEMRI_SH_ROW + 5 * N) * sizeof(double2);
+    const size_t sm_am = ((size_t)2 * N * FDEMRI_AMP_ROW + N + (N & 1)) * sizeof(double) +
+                         (size_t)2 * FDEMRI_AMP_VOICES * N * sizeof(double2);
+    const int groups = (d.n_modes + FDEMRI_AMP_VOICES - 1) / FDEMRI_AMP_VOICES;
+    if (cudaEventRecord(p->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(p->side, p->ev_fork, 0) != cudaSuccess)
+        return FDEMRI_ERR_CUDA;
+    k_spline_amp<<<(unsigned)((size_t)d.n_batch * groups), threads, sm_am, p->side>>>(d.n_modes, N, p->t_knots_dev, amp,
+                                                                                   p->rec, p->stats + 5);
+    if (cudaEventRecord(p->ev_join, p->side) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    k_spline_shared<<<dim3(d.n_batch, polar ? 2 : 1), threads, sm_sh, st>>>(N, p->t_knots_dev, f_phi, f_r, Phi_phi, Phi_r,
+                                                                           p->sh_hi, p->sh_lo, p->stats + 5, f_theta,
+                                                                           Phi_theta, p->sh2_hi, p->sh2_lo);
+    // S2: records, entries and their bands: one warp per (batch item, voice)
+    const size_t nvoice = (size_t)d.n_batch * d.n_modes;
     auto records = polar ? k_records<true> : k_records<false>;
-    records<<<(unsigned)((nrec + 127) / 128), 128, 0, st>>>(d, p->lmn_dev, p->t_knots_dev, p->sh_hi, p->sh_lo, f_phi, f_r,
-                                                            p->rec, p->ent, d.tile_bins == 1 ? nullptr : p->tile_cnt, p->mode_mask, p->stats,
-                                                            p->k_dev, p->sh2_hi, p->sh2_lo, f_theta);
-    const size_t nslots = (size_t)d.n_batch * d.n_modes * 2 * d.ent_max;
-    const unsigned nb = (unsigned)((nslots + 255) / 256);
-    if (d.tile_bins == 1)
-        k_pair_pass<0><<<nb, 256, 0, st>>>(d, p->ent, p->tile_cnt, p->tile_off, p->tile_cnt + NT, p->pairs, p->pair_cap);
-    k_pair_scan<<<1, 1024, 0, st>>>(NT, p->tile_cnt, p->tile_off, p->pair_cap, p->stats);
-    k_pair_pass<1><<<nb, 256, 0, st>>>(d, p->ent, p->tile_cnt, p->tile_off, p->tile_cnt + NT, p->pairs, p->pair_cap);
-    // per-bin lists are short (a few hundred keys): smaller CTAs, more of them resident
-    const unsigned sort_keys = d.tile_bins == 1 ? FDEMRI_SORT_CAP_BIN : FDEMRI_SORT_CAP_TILE;
-    k_pair_sort<<<(unsigned)NT, d.tile_bins == 1 ? FDEMRI_SORT_THREADS_BIN : FDEMRI_SORT_THREADS_TILE,
-                  sort_keys * sizeof(unsigned int), st>>>(NT, p->tile_off, p->pairs, p->pair_cap, sort_keys);
+    records<<<(unsigned)((nvoice + FDEMRI_REC_WARPS - 1) / FDEMRI_REC_WARPS), FDEMRI_REC_WARPS * 32, 0, st>>>(
+        d, p->lmn_dev, p->t_knots_dev, p->sh_hi, p->sh_lo, f_phi, f_r, p->rec, p->ent, p->gband, p->vband, p->iband,
+        p->mode_mask, p->stats, p->item_evals, p->k_dev, p->sh2_hi, p->sh2_lo, f_theta);
+    if (cudaStreamWaitEvent(st, p->ev_join, 0) != cudaSuccess) return FDEMRI_ERR_CUDA;
     if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
     p->built = true;
     return FDEMRI_OK;
@@ -371,29 +387,37 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
     const FdemriDims& d = p->d;
     if (n_angles != 1 && n_angles != d.n_batch) return FDEMRI_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    p->last_stream = st;
-    p->angle_stage.resize((size_t)2 * n_angles);
-    for (int i = 0; i < n_angles; ++i) {
+    for (int i = 0; i < n_angles; ++i)
         if (!std::isfinite(theta_host[i]) || !std::isfinite(phi_host[i])) return FDEMRI_ERR_INVALID_ARG;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    // the pinned staging buffer is read by the asynchronous copy below: wait for the copy of the previous sum
+    // (not while a graph is being captured: synchronising is not allowed there)
+    if (cap == cudaStreamCaptureStatusNone && p->last_stream_valid && cudaEventSynchronize(p->ev_angles) != cudaSuccess)
+        return FDEMRI_ERR_CUDA;
+    p->last_stream = st;
+    for (int i = 0; i < n_angles; ++i) {
         p->angle_stage[2 * i] = theta_host[i];
         p->angle_stage[2 * i + 1] = phi_host[i];
     }
-    if (cudaMemcpyAsync(p->angles, p->angle_stage.data(), p->angle_stage.size() * sizeof(double),
-                        cudaMemcpyHostToDevice, st) != cudaSuccess)
+    if (cudaMemcpyAsync(p->angles, p->angle_stage, (size_t)2 * n_angles * sizeof(double), cudaMemcpyHostToDevice, st) != cudaSuccess)
         return FDEMRI_ERR_CUDA;
+    // (a stream being captured into a CUDA graph: no event; a replay reads the buffer as the last call left it)
+    p->last_stream_valid = cap == cudaStreamCaptureStatusNone && cudaEventRecord(p->ev_angles, st) == cudaSuccess;
     // S0
     int nw = n_angles * d.n_modes;
     k_weights<<<(nw + 127) / 128, 128, 0, st>>>(n_angles, d.n_modes, p->lmn_dev, p->k_dev, p->lm_index_dev, p->wmeta_dev, p->wcoef_dev,
                                                 p->angles, p->wts);
-    // reset the per-sum counters: n_airy (slot 4) and the tile counter (slot 6)
+    // reset the per-sum counters: n_airy (slot 4), the tile counter (6), n_slow (7), n_pairs (8), the sum's flags (9)
     if (cudaMemsetAsync(p->stats + 4, 0, sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
-    if (cudaMemsetAsync(p->stats + 6, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    if (cudaMemsetAsync(p->stats + 6, 0, 4 * sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
     SumArgs a;
     a.d = d;
     a.rec = p->rec;
     a.ent = p->ent;
-    a.tile_off = p->tile_off;
-    a.pairs = p->pairs;
+    a.gband = p->gband;
+    a.vband = p->vband;
+    a.iband = p->iband;
     a.wts = p->wts;
     a.n_angles = n_angles;
     a.hp = hplus_dev;
@@ -406,10 +430,8 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
     a.dcross = dcross_dev;
     a.inner_part = inner_out_dev ? p->inner_part : nullptr;
     a.inner_edge = (inner_out_dev && hann) ? p->inner_edge : nullptr;
-    const bool bin_major = d.tile_bins == 1;
-    if (bin_major && !hplus_dev) return FDEMRI_ERR_UNSUPPORTED;      /* bin-major: inner products come from the waveform */
-    if (bin_major) a.inner_part = a.inner_edge = nullptr;
-    const size_t smem = bin_major ? (size_t)FDEMRI_BIN_WARPS * 32 * FDEMRI_BIN_STRIDE * sizeof(double) : sizeof(FdemriRing);
+    const bool bin_major = d.bin_major != 0;
+    const size_t smem = bin_major ? sizeof(FdemriBinSmem) : sizeof(FdemriTileSmem);
     const int threads = bin_major ? FDEMRI_BIN_WARPS * 32 : FDEMRI_SUM_THREADS;
     if (p->sum_blocks_per_sm == 0) {
         const void* fn = bin_major ? (const void*)k_bin_sum : (const void*)k_tile_sum;
@@ -424,8 +446,7 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
                     smem, per_sm);
     }
     long long grid = (long long)p->sm_count * p->sum_blocks_per_sm;
-    const long long units = bin_major ? (a.total_tiles + FDEMRI_BIN_WARPS - 1) / FDEMRI_BIN_WARPS : a.total_tiles;
-    if (grid > units) grid = units;
+    if (grid > a.total_tiles) grid = a.total_tiles;
     if (p->ev0) cudaEventRecord(p->ev0, st);
     if (bin_major) k_bin_sum<<<(unsigned)grid, threads, smem, st>>>(a);
     else k_tile_sum<<<(unsigned)grid, threads, smem, st>>>(a);
@@ -437,14 +458,10 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
             return FDEMRI_ERR_CUDA;
         }
     }
-    if (inner_out_dev && bin_major) {
-        k_inner_dense<<<d.n_batch, 1024, 0, st>>>(d.n_freq, hplus_dev, hcross_dev, weight_dev, dplus_dev, dcross_dev, hann,
-                                                  inner_out_dev);
-        return cudaGetLastError() == cudaSuccess ? FDEMRI_OK : FDEMRI_ERR_CUDA;
-    }
     if (inner_out_dev) {
-        k_inner_reduce<<<d.n_batch, 256, 0, st>>>(d.n_tiles, d.n_freq, p->inner_part, a.inner_edge, weight_dev, dplus_dev,
-                                                  dcross_dev, inner_out_dev);
+        const size_t n_ranges = bin_major ? (size_t)d.n_tiles : (size_t)d.n_tiles * FDEMRI_CWARPS;
+        k_inner_reduce<<<d.n_batch, 256, 0, st>>>(n_ranges, bin_major ? d.tile_bins : 32 * FDEMRI_BPL, d.n_freq, p->inner_part,
+                                                  a.inner_edge, weight_dev, dplus_dev, dcross_dev, inner_out_dev);
         if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
     }
     return FDEMRI_OK;
@@ -493,14 +510,24 @@ extern "C" int fdemri_get_stats(fdemri_plan_t p, fdemri_stats* out) {
     if (cudaStreamSynchronize(p->last_stream) != cudaSuccess) return FDEMRI_ERR_CUDA;
     if (cudaMemcpy(h, p->stats, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess) return FDEMRI_ERR_CUDA;
     out->n_items = h[0];
+    out->reserved = 0;
     out->n_evals = h[2];
     out->n_turnover = h[3];
     out->n_airy = h[4];
-    out->flags = h[5];
+    out->flags = h[5] | h[9];                          /* build flags | flags of the last sum */
     out->n_slow = h[7];
     out->n_pairs = h[8];
-    if (h[5] & FDEMRI_BAD_LIST_OVERFLOW) return FDEMRI_ERR_WORKSPACE;
-    if (h[5] & FDEMRI_BAD_NONFINITE) return FDEMRI_ERR_INVALID_ARG;
+    if (out->flags & FDEMRI_BAD_NONFINITE) return FDEMRI_ERR_INVALID_ARG;
+    return FDEMRI_OK;
+}
+
+extern "C" int fdemri_get_item_evals(fdemri_plan_t p, uint64_t* out_host) {
+    if (!p || !out_host) return FDEMRI_ERR_INVALID_ARG;
+    if (!p->ws) return FDEMRI_ERR_WORKSPACE;
+    if (!p->built) return FDEMRI_ERR_NOT_BUILT;
+    if (cudaStreamSynchronize(p->last_stream) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    if (cudaMemcpy(out_host, p->item_evals, (size_t)p->d.n_batch * sizeof(uint64_t), cudaMemcpyDeviceToHost) != cudaSuccess)
+        return FDEMRI_ERR_CUDA;
     return FDEMRI_OK;
 }
 
@@ -601,12 +628,7 @@ extern "C" int fdemri_measure_fp64_peak_3reg(int n_iters, double* tflops_out) { 
 
 extern "C" int fdemri_destroy(fdemri_plan_t p) {
     if (!p) return FDEMRI_ERR_INVALID_ARG;
-    if (p->side) cudaStreamDestroy(p->side);
-    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
-    if (p->ev_join) cudaEventDestroy(p->ev_join);
-    if (p->ev0) cudaEventDestroy(p->ev0);
-    if (p->ev1) cudaEventDestroy(p->ev1);
-    delete p;
+    release_plan(p);
     return FDEMRI_OK;
 }
 
@@ -617,7 +639,7 @@ extern "C" const char* fdemri_strerror(int status) {
         case FDEMRI_ERR_WORKSPACE: return "work space missing or too small";
         case FDEMRI_ERR_CUDA: return "CUDA error";
         case FDEMRI_ERR_NOT_BUILT: return "splines not built";
-        case FDEMRI_ERR_UNSUPPORTED: return "input violates an assumption of the method";
+        case FDEMRI_ERR_UNSUPPORTED: return "call not available in this configuration";
         default: return "unknown status";
     }
 }

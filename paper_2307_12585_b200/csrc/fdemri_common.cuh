@@ -9,13 +9,13 @@
 #define FDEMRI_CWARPS 12             // consumer (evaluating) warps per CTA of the sum kernel
 #endif
 #define FDEMRI_BPL 2                 // bins per lane: a consumer warp owns 32*FDEMRI_BPL consecutive bins
-#define FDEMRI_TILE (FDEMRI_CWARPS * 32 * FDEMRI_BPL)     // bins per tile (512)
+#define FDEMRI_TILE (FDEMRI_CWARPS * 32 * FDEMRI_BPL)     // bins per tile (768)
+#define FDEMRI_BIN_BLOCK 32          // bins per block of the bin-major sum kernel (one CTA at a time)
 #define FDEMRI_SUM_THREADS ((FDEMRI_CWARPS + 1) * 32)     // + one producer warp
 #define FDEMRI_CHUNK 32              // staged items per ring stage (one per producer lane)
 #ifndef FDEMRI_STAGES
 #define FDEMRI_STAGES 8              // ring depth
 #endif
-#define FDEMRI_BAD_LIST_OVERFLOW_BIT 16ull   // = FDEMRI_BAD_LIST_OVERFLOW of fdemri.h
 
 // ------------------------------------------------------------------------------------------------
 // Record of one (voice, segment) in global memory: everything the sum needs about that piece of
@@ -82,10 +82,12 @@ enum {
 
 struct FdemriDims {
     int n_modes, n_batch, n_knots, n_seg;   // n_seg = n_knots - 1
-    int ent_max;                            // entry slots per (voice, sign) = 3 * n_seg (segment, branch)
+    int ent_max;                            // entry slots per (voice, sign) = 3 * 32 n_groups: key = vs * ent_max + branch * 32 n_groups + segment
+    int n_groups;                           // groups of 32 consecutive segments = ceil(n_seg / 32)
     int64_t n_freq;
-    int tile_bins;                          // bins per work-list tile: FDEMRI_TILE (tile-major sum) or 1 (bin-major sum)
-    int n_tiles;                            // tiles per batch item = ceil(n_freq / tile_bins)
+    int bin_major;                          // 1: the bin-major sum kernel (sparse grids), 0: the tile-major one
+    int tile_bins;                          // bins a CTA owns at a time: FDEMRI_TILE (tile-major) or 8, 16, FDEMRI_BIN_BLOCK = 32 (bin-major)
+    int n_tiles;                            // tiles (blocks) per batch item = ceil(n_freq / tile_bins)
     double f0, df;
     const double* freq;                     // NULL => uniform grid
 };

@@ -142,186 +142,241 @@ __device__ int64_t fdemri_first_gt(const FdemriDims& d, double x) {
     return i;
 }
 
-// ent: [B][V][2][ent_max] int2 {first bin, last bin}, slot = 3*seg + branch (time order); empty slots have last < first.  tile_cnt: [B][n_tiles] entries per tile, counted here for the tile-major lists (NULL: the
-// per-bin lists of the bin-major mode are counted by k_pair_pass<0>, which shares wide entries among the lanes).
+// ------------------------------------------------------------------------------------------------
+// S2: one WARP per (batch item, voice); its lanes take the segments 32 at a time ("groups" of 32 consecutive
+// segments).  Per segment: the record (F cubic, phase cubic, inversion seed or extrema) and, for both signs and up
+// to three monotone branches, the interval of bins the branch covers ("entry").  Per group and per voice-sign the
+// union of those intervals ("bands"): the sum kernels find the entries that meet a tile of bins by walking
+//     voice-sign band  ->  group bands  ->  the 32 entries of a group row
+// in ascending key order -- no per-tile list is ever built, sorted or stored (the paper: "the spline segment in
+// which each value of f falls is predetermined before the summation", L105; here the predetermined map is the
+// entries plus two levels of bands over them).
+//   ent   [B][V][2][3][Sp] int2 {first bin, last bin}; empty: last < first; Sp = 32 G (rows padded with empty entries to
+//         whole groups: a group row is 256 aligned bytes).   key = ((v*2+sign)*3 + branch)*Sp + segment
+//   gband [B][V][2][G] int4 {lo, hi of the branch-0 entries of the group; lo, hi of its branch-1/2 entries}
+//   vband [B][V][2]    int2 {lo, hi} over all entries of the voice-sign
+//   iband [B]          int2 {max of -lo, max of hi} over the item (atomicMax; memset to 0x80 bytes before)
 // POLAR: general voices (l, m, k, n) -- kk[v] = k, sh2_hi/sh2_lo the splines of (f_theta, Phi_theta) (components
 // 0 and 1 of a second [B][4][n_seg][4] array), f_theta the knot values.
+// ------------------------------------------------------------------------------------------------
+#define FDEMRI_REC_WARPS 4           // warps (voices) per CTA of k_records
+
 template <bool POLAR>
-__global__ void k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ t_knots,
-                          const double* __restrict__ sh_hi, const double* __restrict__ sh_lo,
-                          const double* __restrict__ f_phi, const double* __restrict__ f_r, double* __restrict__ rec,
-                          int2* __restrict__ ent, int* __restrict__ tile_cnt, const unsigned char* __restrict__ mode_mask,
-                          unsigned long long* __restrict__ stats, const int* __restrict__ kk,
-                          const double* __restrict__ sh2_hi, const double* __restrict__ sh2_lo,
-                          const double* __restrict__ f_theta) {
-    size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    size_t total = (size_t)d.n_batch * d.n_modes * d.n_seg;
-    if (id >= total) return;
-    int k = (int)(id % d.n_seg);
-    size_t bv = id / d.n_seg;
-    int v = (int)(bv % d.n_modes);
-    int b = (int)(bv / d.n_modes);
-    int m = lmn[3 * v + 1], n = lmn[3 * v + 2];
-    const size_t per = (size_t)d.n_seg * 4;
-    // coefficients (a, b, c, d) of f_phi, f_r, Phi_phi, Phi_r on this segment, hi and lo parts: eight 32-byte loads
-    const double4* H4 = reinterpret_cast<const double4*>(sh_hi + (size_t)b * 4 * per) + k;
-    const double4* L4 = reinterpret_cast<const double4*>(sh_lo + (size_t)b * 4 * per) + k;
-    const double4 h0 = H4[0], h1 = H4[d.n_seg], h2 = H4[2 * (size_t)d.n_seg], h3 = H4[3 * (size_t)d.n_seg];
-    const double4 l0 = L4[0], l1 = L4[d.n_seg], l2 = L4[2 * (size_t)d.n_seg], l3 = L4[3 * (size_t)d.n_seg];
-    double* R = rec + id * R_DOUBLES;
-    // F cubic (Eq. 6)
-    double FA = fdemri_knotF(m, n, h0.x, h1.x);
-    dd FBd = fdemri_combine(m, n, h0.y, l0.y, h1.y, l1.y);
-    dd FCd = fdemri_combine(m, n, h0.z, l0.z, h1.z, l1.z);
-    dd FDd = fdemri_combine(m, n, h0.w, l0.w, h1.w, l1.w);
-    // phase spline of the voice, in cycles (R9)
+__global__ void __launch_bounds__(FDEMRI_REC_WARPS * 32)
+k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ t_knots,
+          const double* __restrict__ sh_hi, const double* __restrict__ sh_lo,
+          const double* __restrict__ f_phi, const double* __restrict__ f_r, double* __restrict__ rec,
+          int2* __restrict__ ent, int4* __restrict__ gband, int2* __restrict__ vband, int* __restrict__ iband,
+          const unsigned char* __restrict__ mode_mask, unsigned long long* __restrict__ stats,
+          unsigned long long* __restrict__ item_evals, const int* __restrict__ kk,
+          const double* __restrict__ sh2_hi, const double* __restrict__ sh2_lo,
+          const double* __restrict__ f_theta) {
+    const int lane = threadIdx.x & 31;
+    const size_t bv = (size_t)blockIdx.x * FDEMRI_REC_WARPS + (threadIdx.x >> 5);
+    if (bv >= (size_t)d.n_batch * d.n_modes) return;                 // whole warp
+    const unsigned full = 0xffffffffu;
+    const int v = (int)(bv % d.n_modes);
+    const int b = (int)(bv / d.n_modes);
+    const int m = lmn[3 * v + 1], n = lmn[3 * v + 2];
+    const int S = d.n_seg, G = d.n_groups;
+    const size_t per = (size_t)S * 4;
+    const int kq = POLAR ? kk[v] : 0;
+    const bool masked = mode_mask && !mode_mask[bv];                 // a mode the selection dropped has no entries
+    const int64_t first_pos = fdemri_first_gt(d, 0.0);               // bins with f > 0 only (R13)
     const dd inv2pi = dd{FDEMRI_INV2PI_HI, FDEMRI_INV2PI_LO};
-    dd Pa = dd_add(two_prod((double)m, h2.x), two_prod((double)n, h3.x));   // knot values: exact
-    dd Pb = fdemri_combine(m, n, h2.y, l2.y, h3.y, l3.y);
-    dd Pc = fdemri_combine(m, n, h2.z, l2.z, h3.z, l3.z);
-    dd Pd = fdemri_combine(m, n, h2.w, l2.w, h3.w, l3.w);
-    int kq = 0;
-    const double4* G4 = nullptr;
-    if (POLAR) {                                            // the polar terms k f_theta, k Phi_theta (Eq. 1)
-        kq = kk[v];
-        G4 = reinterpret_cast<const double4*>(sh2_hi + (size_t)b * 4 * per) + k;
-        const double4* GL = reinterpret_cast<const double4*>(sh2_lo + (size_t)b * 4 * per) + k;
-        const double4 g0 = G4[0], g1 = G4[d.n_seg], e0 = GL[0], e1 = GL[d.n_seg];
-        const double kd = (double)kq;
-        FA = fdemri_knotF3(m, kq, n, h0.x, g0.x, h1.x);
-        FBd = dd_add(FBd, dd_mul_d(dd{g0.y, e0.y}, kd));
-        FCd = dd_add(FCd, dd_mul_d(dd{g0.z, e0.z}, kd));
-        FDd = dd_add(FDd, dd_mul_d(dd{g0.w, e0.w}, kd));
-        Pa = dd_add(Pa, two_prod(kd, g1.x));
-        Pb = dd_add(Pb, dd_mul_d(dd{g1.y, e1.y}, kd));
-        Pc = dd_add(Pc, dd_mul_d(dd{g1.z, e1.z}, kd));
-        Pd = dd_add(Pd, dd_mul_d(dd{g1.w, e1.w}, kd));
-    }
-    double FB = FBd.hi, FC = FCd.hi, FD = FDd.hi;
-    double pc = -dd_frac(dd_mul(Pa, inv2pi));
-    dd bq = dd_mul(Pb, inv2pi);
-    double tk = t_knots[(size_t)b * d.n_knots + k];
-    double h = __dadd_rn(t_knots[(size_t)b * d.n_knots + k + 1], -tk);
-    // the record is written as four 32-byte stores at the end (slots 8..15 belong to k_spline_amp)
-    double rQ1, rQ2, rQ3, rTYPE, rSF;
-    // interior extrema of F on (0, h): roots of FB + 2 FC t + 3 FD t^2
-    double ext[2]; int ne = 0;
-    {
-        double qa = 3.0 * FD, qb = 2.0 * FC, qc = FB;
-        if (qa == 0.0) {
-            if (qb != 0.0) { double r = -qc / qb; if (r > 0.0 && r < h) ext[ne++] = r; }
-        } else {
-            double disc = qb * qb - 4.0 * qa * qc;
-            if (disc > 0.0) {
-                double sq = sqrt(disc);
-                double qq = -0.5 * (qb + (qb >= 0.0 ? sq : -sq));
-                double r1 = qq / qa, r2 = (qq != 0.0) ? qc / qq : r1;
-                if (r1 > r2) { double tmp = r1; r1 = r2; r2 = tmp; }
-                if (r1 > 0.0 && r1 < h) ext[ne++] = r1;
-                if (r2 > 0.0 && r2 < h && r2 != r1) ext[ne++] = r2;
-            }
-        }
-    }
-    bool bad = !(isfinite(FA) && isfinite(FB) && isfinite(FC) && isfinite(FD) && isfinite(pc) && isfinite(bq.hi));
-    if (ne == 0) {
-        // seed of the inverse: cubic through tau(x) at x = dF {0, 1/3, 2/3, 1}, x = s f - FA
-        double dF = h * (FB + h * (FC + h * FD));
-        double q1 = 0.0, q2 = 0.0, q3 = 0.0;
-        if (dF != 0.0 && isfinite(dF)) {
-            double t1 = fdemri_root_build(FB, FC, FD, dF * (1.0 / 3.0), h);
-            double t2 = fdemri_root_build(FB, FC, FD, dF * (2.0 / 3.0), h);
-            double g1 = 3.0 * t1, g2 = 1.5 * t2, g3 = h;
-            double gam = 4.5 * (g1 - 2.0 * g2 + g3);
-            double bet = 3.0 * (g2 - g1) - gam;
-            double alp = g1 - bet * (1.0 / 3.0) - gam * (1.0 / 9.0);
-            double idF = 1.0 / dF;
-            q1 = alp * idF; q2 = bet * idF * idF; q3 = gam * idF * idF * idF;
-        }
-        rQ1 = q1; rQ2 = q2; rQ3 = q3; rTYPE = 0.0;
-        rSF = (dF < 0.0) ? -1.0 : 1.0;
-    } else if (ne == 1) {
-        double te = ext[0];
-        rQ1 = te;
-        rQ2 = FA + te * (FB + te * (FC + te * FD));          // F_e (R7)
-        rQ3 = 0.0;
-        rTYPE = 1.0;
-        rSF = 0.0;
-        atomicAdd(stats + 3, 1ull);
-    } else {
-        // two interior extrema (the paper assumes at most one, L105; R5): three monotone branches
-        const double t1 = ext[0], t2 = ext[1];
-        rQ1 = t1;
-        rQ2 = FA + t1 * (FB + t1 * (FC + t1 * FD));          // F_e1
-        rQ3 = t2;
-        rTYPE = 2.0;
-        rSF = FA + t2 * (FB + t2 * (FC + t2 * FD));          // F_e2 (the slot of the sign, which type 0 alone needs)
-        atomicAdd(stats + 3, 1ull);
-    }
-    if (bad) atomicOr(stats + 5, 4ull);
-    // ---- bin intervals of the branches of this segment, for both signs (L105) ----
-    {
-        double4* R4 = reinterpret_cast<double4*>(R);        // rec is 256-byte aligned, records are 192 bytes
-        R4[0] = make_double4(FA, FB, FC, FD);
-        R4[1] = make_double4(rQ1, rQ2, rQ3, h);
-        R4[4] = make_double4(pc, bq.hi, bq.lo, -dd_mul(Pc, inv2pi).hi);
-        R4[5] = make_double4(-dd_mul(Pd, inv2pi).hi, tk, rTYPE, rSF);
-    }
-    const int type = (int)rTYPE;
-    const double Fk = FA;
     const size_t last = (size_t)b * d.n_knots + d.n_knots - 1;
-    double Fk1;
-    if (POLAR) Fk1 = (k + 1 < d.n_seg) ? fdemri_knotF3(m, kq, n, H4[1].x, G4[1].x, H4[d.n_seg + 1].x)
-                                    : fdemri_knotF3(m, kq, n, f_phi[last], f_theta[last], f_r[last]);
-    else    Fk1 = (k + 1 < d.n_seg) ? fdemri_knotF(m, n, H4[1].x, H4[d.n_seg + 1].x)
-                                    : fdemri_knotF(m, n, f_phi[last], f_r[last]);
-    const int64_t first_pos = fdemri_first_gt(d, 0.0);      // bins with f > 0 only (R13)
-    unsigned long long evals = 0, items = 0;
-    // branch j of the segment runs from V[j] to V[j+1]: knot value, extremum values, next knot value; a branch includes
-    // its start iff that is the knot and its end iff that is an extremum (R6, R7)
-    const double Vv[4] = {Fk, type >= 1 ? rQ2 : Fk1, type == 2 ? rSF : Fk1, Fk1};
-    const int nbr = (mode_mask && !mode_mask[bv]) ? 0 : type + 1;        // a mode the selection dropped has no entries
-    for (int sg = 0; sg < 2; ++sg) {
-        int2* E = ent + ((bv * 2 + sg) * (size_t)d.ent_max) + 3 * k;
-        for (int br = 0; br < 3; ++br) {
-            int2 e4 = make_int2(0, -1);                     // empty: last < first
-            if (br < nbr) {
-                const double Va = Vv[br], Vb = Vv[br + 1];
-                const bool a_incl = (br == 0), b_incl = (br + 1 < nbr);
-                if (Va != Vb) {
-                    const double lo_v = fmin(Va, Vb), hi_v = fmax(Va, Vb);
-                    const bool lo_incl = (Va < Vb) ? a_incl : b_incl;
-                    const bool hi_incl = (Va < Vb) ? b_incl : a_incl;
-                    const double flo = sg ? -hi_v : lo_v, fhi = sg ? -lo_v : hi_v;
-                    const bool flo_incl = sg ? hi_incl : lo_incl, fhi_incl = sg ? lo_incl : hi_incl;
-                    if (fhi > 0.0) {
-                        int64_t lo_b = flo_incl ? fdemri_first_ge(d, flo) : fdemri_first_gt(d, flo);
-                        const int64_t hi1 = fhi_incl ? fdemri_first_gt(d, fhi) : fdemri_first_ge(d, fhi);
-                        if (lo_b < first_pos) lo_b = first_pos;
-                        if (lo_b < hi1) {
-                            e4.x = (int)lo_b; e4.y = (int)(hi1 - 1);
-                            evals += (unsigned long long)(hi1 - lo_b);
-                            ++items;
-                            if (tile_cnt) {                 // tile-major lists: an entry meets a handful of tiles
-                                const int t0 = e4.x / d.tile_bins, t1 = e4.y / d.tile_bins;
-                                for (int t = t0; t <= t1; ++t) atomicAdd(tile_cnt + (size_t)b * d.n_tiles + t, 1);
+    unsigned long long evals = 0;
+    unsigned items = 0, turnovers = 0;
+    bool bad = false;
+    int vlo[2] = {0x7fffffff, 0x7fffffff}, vhi[2] = {-1, -1};
+    for (int g = 0; g < G; ++g) {
+        const int k = 32 * g + lane;
+        const bool active = k < S;
+        int2 e[2][3];
+#pragma unroll
+        for (int sg = 0; sg < 2; ++sg)
+#pragma unroll
+            for (int br = 0; br < 3; ++br) e[sg][br] = make_int2(0, -1);       // empty: last < first
+        if (active) {
+            // coefficients (a, b, c, d) of f_phi, f_r, Phi_phi, Phi_r on this segment, hi and lo parts
+            const double4* H4 = reinterpret_cast<const double4*>(sh_hi + (size_t)b * 4 * per) + k;
+            const double4* L4 = reinterpret_cast<const double4*>(sh_lo + (size_t)b * 4 * per) + k;
+            const double4 h0 = H4[0], h1 = H4[S], h2 = H4[2 * (size_t)S], h3 = H4[3 * (size_t)S];
+            const double4 l0 = L4[0], l1 = L4[S], l2 = L4[2 * (size_t)S], l3 = L4[3 * (size_t)S];
+            // F cubic (Eq. 6)
+            double FA = fdemri_knotF(m, n, h0.x, h1.x);
+            dd FBd = fdemri_combine(m, n, h0.y, l0.y, h1.y, l1.y);
+            dd FCd = fdemri_combine(m, n, h0.z, l0.z, h1.z, l1.z);
+            dd FDd = fdemri_combine(m, n, h0.w, l0.w, h1.w, l1.w);
+            // phase spline of the voice, in cycles (R9)
+            dd Pa = dd_add(two_prod((double)m, h2.x), two_prod((double)n, h3.x));   // knot values: exact
+            dd Pb = fdemri_combine(m, n, h2.y, l2.y, h3.y, l3.y);
+            dd Pc = fdemri_combine(m, n, h2.z, l2.z, h3.z, l3.z);
+            dd Pd = fdemri_combine(m, n, h2.w, l2.w, h3.w, l3.w);
+            const double4* G4 = nullptr;
+            if (POLAR) {                                            // the polar terms k f_theta, k Phi_theta (Eq. 1)
+                G4 = reinterpret_cast<const double4*>(sh2_hi + (size_t)b * 4 * per) + k;
+                const double4* GL = reinterpret_cast<const double4*>(sh2_lo + (size_t)b * 4 * per) + k;
+                const double4 g0 = G4[0], g1 = G4[S], e0 = GL[0], e1 = GL[S];
+                const double kd = (double)kq;
+                FA = fdemri_knotF3(m, kq, n, h0.x, g0.x, h1.x);
+                FBd = dd_add(FBd, dd_mul_d(dd{g0.y, e0.y}, kd));
+                FCd = dd_add(FCd, dd_mul_d(dd{g0.z, e0.z}, kd));
+                FDd = dd_add(FDd, dd_mul_d(dd{g0.w, e0.w}, kd));
+                Pa = dd_add(Pa, two_prod(kd, g1.x));
+                Pb = dd_add(Pb, dd_mul_d(dd{g1.y, e1.y}, kd));
+                Pc = dd_add(Pc, dd_mul_d(dd{g1.z, e1.z}, kd));
+                Pd = dd_add(Pd, dd_mul_d(dd{g1.w, e1.w}, kd));
+            }
+            const double FB = FBd.hi, FC = FCd.hi, FD = FDd.hi;
+            const double pc = -dd_frac(dd_mul(Pa, inv2pi));
+            const dd bq = dd_mul(Pb, inv2pi);
+            const double tk = t_knots[(size_t)b * d.n_knots + k];
+            const double h = __dadd_rn(t_knots[(size_t)b * d.n_knots + k + 1], -tk);
+            double rQ1, rQ2, rQ3, rTYPE, rSF;
+            // interior extrema of F on (0, h): roots of FB + 2 FC t + 3 FD t^2
+            double ext[2]; int ne = 0;
+            {
+                const double qa = 3.0 * FD, qb = 2.0 * FC, qc = FB;
+                if (qa == 0.0) {
+                    if (qb != 0.0) { const double r = -qc / qb; if (r > 0.0 && r < h) ext[ne++] = r; }
+                } else {
+                    const double disc = qb * qb - 4.0 * qa * qc;
+                    if (disc > 0.0) {
+                        const double sq = sqrt(disc);
+                        const double qq = -0.5 * (qb + (qb >= 0.0 ? sq : -sq));
+                        double r1 = qq / qa, r2 = (qq != 0.0) ? qc / qq : r1;
+                        if (r1 > r2) { const double tmp = r1; r1 = r2; r2 = tmp; }
+                        if (r1 > 0.0 && r1 < h) ext[ne++] = r1;
+                        if (r2 > 0.0 && r2 < h && r2 != r1) ext[ne++] = r2;
+                    }
+                }
+            }
+            if (!(isfinite(FA) && isfinite(FB) && isfinite(FC) && isfinite(FD) && isfinite(pc) && isfinite(bq.hi))) bad = true;
+            if (ne == 0) {
+                // seed of the inverse: cubic through tau(x) at x = dF {0, 1/3, 2/3, 1}, x = s f - FA
+                const double dF = h * (FB + h * (FC + h * FD));
+                double q1 = 0.0, q2 = 0.0, q3 = 0.0;
+                if (dF != 0.0 && isfinite(dF)) {
+                    const double t1 = fdemri_root_build(FB, FC, FD, dF * (1.0 / 3.0), h);
+                    const double t2 = fdemri_root_build(FB, FC, FD, dF * (2.0 / 3.0), h);
+                    const double g1 = 3.0 * t1, g2 = 1.5 * t2, g3 = h;
+                    const double gam = 4.5 * (g1 - 2.0 * g2 + g3);
+                    const double bet = 3.0 * (g2 - g1) - gam;
+                    const double alp = g1 - bet * (1.0 / 3.0) - gam * (1.0 / 9.0);
+                    const double idF = 1.0 / dF;
+                    q1 = alp * idF; q2 = bet * idF * idF; q3 = gam * idF * idF * idF;
+                }
+                rQ1 = q1; rQ2 = q2; rQ3 = q3; rTYPE = 0.0;
+                rSF = (dF < 0.0) ? -1.0 : 1.0;
+            } else if (ne == 1) {
+                const double te = ext[0];
+                rQ1 = te;
+                rQ2 = FA + te * (FB + te * (FC + te * FD));          // F_e (R7)
+                rQ3 = 0.0;
+                rTYPE = 1.0;
+                rSF = 0.0;
+                ++turnovers;
+            } else {
+                // two interior extrema (the paper assumes at most one, L105; R5): three monotone branches
+                const double t1 = ext[0], t2 = ext[1];
+                rQ1 = t1;
+                rQ2 = FA + t1 * (FB + t1 * (FC + t1 * FD));          // F_e1
+                rQ3 = t2;
+                rTYPE = 2.0;
+                rSF = FA + t2 * (FB + t2 * (FC + t2 * FD));          // F_e2 (the slot of the sign, which type 0 alone needs)
+                ++turnovers;
+            }
+            {
+                // the record: four 32-byte stores (slots 8..15 belong to k_spline_amp)
+                double4* R4 = reinterpret_cast<double4*>(rec + (bv * S + k) * R_DOUBLES);
+                R4[0] = make_double4(FA, FB, FC, FD);
+                R4[1] = make_double4(rQ1, rQ2, rQ3, h);
+                R4[4] = make_double4(pc, bq.hi, bq.lo, -dd_mul(Pc, inv2pi).hi);
+                R4[5] = make_double4(-dd_mul(Pd, inv2pi).hi, tk, rTYPE, rSF);
+            }
+            // ---- bin intervals of the branches of this segment, for both signs (L105) ----
+            const int type = (int)rTYPE;
+            const double Fk = FA;
+            double Fk1;
+            if (POLAR) Fk1 = (k + 1 < S) ? fdemri_knotF3(m, kq, n, H4[1].x, G4[1].x, H4[S + 1].x)
+                                         : fdemri_knotF3(m, kq, n, f_phi[last], f_theta[last], f_r[last]);
+            else    Fk1 = (k + 1 < S) ? fdemri_knotF(m, n, H4[1].x, H4[S + 1].x)
+                                      : fdemri_knotF(m, n, f_phi[last], f_r[last]);
+            // branch j of the segment runs from V[j] to V[j+1]: knot value, extremum values, next knot value; a branch
+            // includes its start iff that is the knot and its end iff that is an extremum (R6, R7)
+            const double Vv[4] = {Fk, type >= 1 ? rQ2 : Fk1, type == 2 ? rSF : Fk1, Fk1};
+            const int nbr = masked ? 0 : type + 1;
+#pragma unroll
+            for (int sg = 0; sg < 2; ++sg) {
+#pragma unroll
+                for (int br = 0; br < 3; ++br) {
+                    if (br < nbr) {
+                        const double Va = Vv[br], Vb = Vv[br + 1];
+                        const bool a_incl = (br == 0), b_incl = (br + 1 < nbr);
+                        if (Va != Vb) {
+                            const double lo_v = fmin(Va, Vb), hi_v = fmax(Va, Vb);
+                            const bool lo_incl = (Va < Vb) ? a_incl : b_incl;
+                            const bool hi_incl = (Va < Vb) ? b_incl : a_incl;
+                            const double flo = sg ? -hi_v : lo_v, fhi = sg ? -lo_v : hi_v;
+                            const bool flo_incl = sg ? hi_incl : lo_incl, fhi_incl = sg ? lo_incl : hi_incl;
+                            if (fhi > 0.0) {
+                                int64_t lo_b = flo_incl ? fdemri_first_ge(d, flo) : fdemri_first_gt(d, flo);
+                                const int64_t hi1 = fhi_incl ? fdemri_first_gt(d, fhi) : fdemri_first_ge(d, fhi);
+                                if (lo_b < first_pos) lo_b = first_pos;
+                                if (lo_b < hi1) {
+                                    e[sg][br] = make_int2((int)lo_b, (int)(hi1 - 1));
+                                    evals += (unsigned long long)(hi1 - lo_b);
+                                    ++items;
+                                }
                             }
                         }
                     }
                 }
             }
-            E[br] = e4;
+        }
+        // entries (coalesced rows of the group) and the bands over them
+#pragma unroll
+        for (int sg = 0; sg < 2; ++sg) {
+            int lo0 = 0x7fffffff, hi0 = -1, lo12 = 0x7fffffff, hi12 = -1;
+#pragma unroll
+            for (int br = 0; br < 3; ++br) {
+                const int2 q = e[sg][br];
+                ent[((bv * 2 + sg) * 3 + br) * (size_t)(32 * G) + k] = q;       // (lanes past the last segment: empty)
+                if (q.y >= q.x) {
+                    if (br == 0) { lo0 = q.x; hi0 = q.y; }
+                    else { lo12 = min(lo12, q.x); hi12 = max(hi12, q.y); }
+                }
+            }
+            lo0 = __reduce_min_sync(full, lo0); hi0 = __reduce_max_sync(full, hi0);
+            lo12 = __reduce_min_sync(full, lo12); hi12 = __reduce_max_sync(full, hi12);
+            if (lane == 0) gband[(bv * 2 + sg) * (size_t)G + g] = make_int4(lo0, hi0, lo12, hi12);
+            vlo[sg] = min(vlo[sg], min(lo0, lo12));
+            vhi[sg] = max(vhi[sg], max(hi0, hi12));
         }
     }
-    // counters: one atomic per warp (every thread of a warp adding to the same word serialises in L2)
-    {
-        const unsigned mask = __activemask();
-        const unsigned it_w = __reduce_add_sync(mask, (unsigned)items);
-        const unsigned lo_w = __reduce_add_sync(mask, (unsigned)(evals & 0xffffu));
-        const unsigned hi_w = __reduce_add_sync(mask, (unsigned)(evals >> 16));
-        if ((threadIdx.x & 31) == __ffs(mask) - 1) {
-            if (it_w) atomicAdd(stats + 0, (unsigned long long)it_w);
-            const unsigned long long ev = ((unsigned long long)hi_w << 16) + lo_w;
-            if (ev) atomicAdd(stats + 2, ev);
+    // bands of the voice, of the item; counters: one atomic per warp
+    const unsigned it_w = __reduce_add_sync(full, items);
+    const unsigned tv_w = __reduce_add_sync(full, turnovers);
+    const unsigned lo_w = __reduce_add_sync(full, (unsigned)(evals & 0xffffu));
+    const unsigned mi_w = __reduce_add_sync(full, (unsigned)((evals >> 16) & 0xffffu));
+    const unsigned hi_w = __reduce_add_sync(full, (unsigned)(evals >> 32));
+    const bool any_bad = __any_sync(full, bad);
+    if (lane == 0) {
+        vband[bv * 2 + 0] = make_int2(vlo[0], vhi[0]);
+        vband[bv * 2 + 1] = make_int2(vlo[1], vhi[1]);
+        const int ilo = min(vlo[0], vlo[1]), ihi = max(vhi[0], vhi[1]);
+        if (ihi >= ilo) {
+            atomicMax(iband + 2 * b, -ilo);
+            atomicMax(iband + 2 * b + 1, ihi);
         }
+        if (it_w) atomicAdd(stats + 0, (unsigned long long)it_w);
+        if (tv_w) atomicAdd(stats + 3, (unsigned long long)tv_w);
+        const unsigned long long ev = ((unsigned long long)hi_w << 32) + ((unsigned long long)mi_w << 16) + lo_w;
+        if (ev) {
+            atomicAdd(stats + 2, ev);
+            atomicAdd(item_evals + b, ev);
+        }
+        if (any_bad) atomicOr(stats + 5, 4ull);
     }
 }

@@ -2,10 +2,11 @@
 //
 // A CTA owns a tile of FDEMRI_TILE consecutive bins of one batch item at a time (tiles are handed out by an
 // atomic counter).  It is warp-specialised:
-//   * one PRODUCER warp walks the tile's work list (fdemri_pairs.cuh: the entries -- (voice, sign, segment-branch)
-//     -- that intersect the tile, in the fixed order (voice, sign, time)), reads their records and weights
-//     from global memory, folds everything that does not depend on the bin into a 256-byte staged item, and
-//     pushes chunks of staged items through a shared-memory ring (full/empty mbarriers);
+//   * one PRODUCER warp finds the entries -- (voice, sign, segment-branch) -- that intersect the tile by walking the
+//     bands of fdemri_map.cuh (voice-sign band -> group bands -> the 32 entries of a group row) in ascending key
+//     order, reads their records and weights from global memory, folds everything that does not depend on the bin
+//     into a 256-byte staged item, and pushes chunks of staged items through a shared-memory ring (full/empty
+//     mbarriers).  No per-tile list exists anywhere: the walk is the list;
 //   * FDEMRI_CWARPS CONSUMER warps each own 64 consecutive bins of the tile, two per lane (lane, lane + 32),
 //     with the eight accumulators in registers.  For every staged item that overlaps its bins a consumer warp
 //     evaluates the term of Eq. 9 for both of its bins at once (two independent
@@ -37,9 +38,10 @@
 struct SumArgs {
     FdemriDims d;
     const double* rec;        // [B][V][S][R_DOUBLES]
-    const int2* ent;          // [B][V][2][ent_max] {first bin, last bin}; slot = 3*segment + branch
-    const unsigned int* tile_off;   // [B * n_tiles + 1] first pair of every tile
-    const unsigned int* pairs;      // sorted keys (voice*2+sign)*ent_max + e of every tile
+    const int2* ent;          // [B][V][2][3][Sp] {first bin, last bin}, Sp = 32 G; key = ((v*2+sign)*3 + branch)*Sp + segment
+    const int4* gband;        // [B][V][2][G] bands of the groups of 32 segments {lo, hi (branch 0), lo, hi (branches 1, 2)}
+    const int2* vband;        // [B][V][2] band of the voice-sign
+    const int* iband;         // [B][2] {-lo, hi} of the item
     const double4* wts;       // [n_angles][V]
     int n_angles;
     double* hp;               // [B][n_freq][2]
@@ -51,9 +53,10 @@ struct SumArgs {
     const double* weight;     // [n_freq] w_k = 4 df / S_n(f_k), or NULL for w = 1
     const double* dplus;      // [n_freq][2] data, + polarisation (NULL: only <h|h>)
     const double* dcross;     // [n_freq][2]
-    double* inner_part;       // [total_tiles][FDEMRI_CWARPS][4] partial sums {<h|h>, Re<d|h>, Im<d|h>, 0}
-    double* inner_edge;       // Hann filter (L145): [total_tiles][FDEMRI_CWARPS][4][4] h at the first two and last two bins
-                              // of every warp range; NULL: no window
+    double* inner_part;       // [ranges][4] partial sums {<h|h>, Re<d|h>, Im<d|h>, 0}; a range = the 64 bins of a consumer
+                              // warp (tile-major: total_tiles * FDEMRI_CWARPS ranges) or a block of bins (bin-major)
+    double* inner_edge;       // Hann filter (L145): [ranges][4][4] h at the first two and last two bins of every range;
+                              // NULL: no window
 };
 
 // asymptotic series of g(X) e^{+i pi/4 sgn X} = sum_k i^k a_k u^k, u = 1/X, a_k = prod_j (4/9-(2j-1)^2)/(k! 8^k)
@@ -426,13 +429,171 @@ __device__ __forceinline__ void fdemri_stage_item(double* dst, const double* __r
     fdemri_stage_regs(dst, fdemri_load_rec(R), w, lo, hi, sg, br);
 }
 
-// Producer: walks the sorted pair list of every tile it draws (S2c, fdemri_pairs.cuh), one ring stage per
-// 32 keys: key -> entry (bin interval, segment, branch) -> record + weights -> staged item.
-__device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ring, int lane) {
+// ---------------------------------------------------------------------------------------------------------
+// The item scan: the entries of one batch item that meet a range of bins [b0, b1], produced in ascending key
+// order by ONE warp, a step at a time (fdemri_map.cuh has the tables):
+//   level 1  voice-sign bands, L1U x 32 at a time (coalesced int2 loads)      -> queue q1 of voice-signs that meet the range
+//   level 2  the group bands of up to 32 queued voice-signs, a lane each      -> queue q2 of rows (vs, branch, group)
+//   level 3  the 32 entries of up to 32 queued rows, a lane per row (16 x 16 B)  -> emit(entry) in order
+// A deeper level runs whenever it has input, a shallower one only when its output queue is empty: the queues are
+// FIFO, so the emitted order is (voice, sign, branch, segment) = ascending key, and every load is issued in
+// batches of independent requests (latency is paid per step, not per entry).  All control flow is warp-uniform.
+// ---------------------------------------------------------------------------------------------------------
+struct FdemriScan {
+    const int2* vband;        // tables of the batch item
+    const int4* gband;
+    const int2* ent;
+    int Sp, G, nb2;           // Sp = 32 G: entries per (voice, sign, branch) row, padded; nb2: voice-signs per level-2 step
+                              // (their rows must fit q2)
+    int b0, b1;
+    int vs_next, vs_end;      // voice-signs still to look at
+    unsigned q1_head, q1_tail, q2_head, q2_tail;
+};
+
+template <int Q2CAP>
+__device__ __forceinline__ void fdemri_scan_init(FdemriScan& c, const SumArgs& a, int b, int vs0, int vs1, int b0, int b1) {
+    const FdemriDims& d = a.d;
+    const size_t nvs = (size_t)2 * d.n_modes;
+    c.vband = a.vband + (size_t)b * nvs;
+    c.gband = a.gband + (size_t)b * nvs * d.n_groups;
+    c.ent = a.ent + (size_t)b * nvs * d.ent_max;
+    c.Sp = 32 * d.n_groups; c.G = d.n_groups;
+    c.nb2 = min(32, Q2CAP / (3 * d.n_groups));
+    c.b0 = b0; c.b1 = b1;
+    c.vs_next = vs0; c.vs_end = vs1;
+    c.q1_head = c.q1_tail = c.q2_head = c.q2_tail = 0u;
+}
+
+// One step.  Returns 0: exhausted, 1: progressed, 2: level 3 has input but emit has no room for a row (32 entries).
+// emit.room() -> free places (warp-uniform); emit.store(offset, vsbr, seg, lo, hi): the entry goes to the offset-th free
+// place; emit.advance(n): n places have been filled.
+template <int Q1CAP, int Q2CAP, int L1U, class Emit>
+__device__ __forceinline__ int fdemri_scan_step(FdemriScan& c, unsigned* __restrict__ q1, unsigned* __restrict__ q2, int lane,
+                                                Emit& emit) {
+    const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
+    if (c.q2_tail != c.q2_head) {                                   // ---- level 3: a lane per row of 32 entries ----
+        const int room = emit.room();
+        if (room < 32) return 2;
+        const int nr = (int)min(c.q2_tail - c.q2_head, 32u);
+        unsigned row = 0u, hits = 0u;
+        int4 e2[16];                                                // the row: 32 x {first bin, last bin}
+        if (lane < nr) {
+            row = q2[(c.q2_head + (unsigned)lane) & (Q2CAP - 1)];
+            const int4* src = reinterpret_cast<const int4*>(c.ent + (size_t)(row >> 4) * c.Sp + 32 * (row & 15u));
+#pragma unroll
+            for (int j = 0; j < 16; ++j) e2[j] = __ldg(src + j);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                hits |= (unsigned)(e2[j].y >= e2[j].x && e2[j].x <= c.b1 && e2[j].y >= c.b0) << (2 * j);
+                hits |= (unsigned)(e2[j].w >= e2[j].z && e2[j].z <= c.b1 && e2[j].w >= c.b0) << (2 * j + 1);
+            }
+        }
+        const int cnt = __popc(hits);
+        int incl = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(full, incl, o);
+            if (lane >= o) incl += t;
+        }
+        // rows are taken in order as long as their entries fit (the first always does: room >= 32)
+        const int nok = __popc(__ballot_sync(full, lane < nr && incl <= room));
+        if (lane < nok && hits) {
+            int off = incl - cnt;
+            const int vsbr = (int)(row >> 4), seg0 = 32 * (int)(row & 15u);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                if (hits & (1u << (2 * j))) emit.store(off++, vsbr, seg0 + 2 * j, e2[j].x, e2[j].y);
+                if (hits & (2u << (2 * j))) emit.store(off++, vsbr, seg0 + 2 * j + 1, e2[j].z, e2[j].w);
+            }
+        }
+        emit.advance(__shfl_sync(full, incl, nok - 1));
+        c.q2_head += (unsigned)nok;
+        __syncwarp();
+        return 1;
+    }
+    if (c.q1_tail != c.q1_head) {                                   // ---- level 2: a lane per voice-sign ----
+        const int nb = (int)min(c.q1_tail - c.q1_head, (unsigned)c.nb2);
+        unsigned m0 = 0u, m12 = 0u;
+        unsigned vs = 0u;
+        if (lane < nb) {
+            vs = q1[(c.q1_head + lane) & (Q1CAP - 1)];
+            const int4* gb = c.gband + (size_t)vs * c.G;
+            for (int g = 0; g < c.G; ++g) {
+                const int4 q = __ldg(gb + g);
+                m0 |= (unsigned)(q.x <= c.b1 && q.y >= c.b0) << g;
+                m12 |= (unsigned)(q.z <= c.b1 && q.w >= c.b0) << g;
+            }
+        }
+        const int cnt = __popc(m0) + 2 * __popc(m12);
+        int incl = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(full, incl, o);
+            if (lane >= o) incl += t;
+        }
+        unsigned pos = c.q2_tail + (unsigned)(incl - cnt);
+#pragma unroll
+        for (int br = 0; br < 3; ++br) {
+            unsigned mk = br ? m12 : m0;
+            while (mk) {
+                const int g = __ffs(mk) - 1;
+                mk &= mk - 1;
+                q2[pos++ & (Q2CAP - 1)] = ((vs * 3u + (unsigned)br) << 4) | (unsigned)g;
+            }
+        }
+        c.q2_tail += (unsigned)__shfl_sync(full, incl, 31);
+        c.q1_head += (unsigned)nb;
+        __syncwarp();
+        return 1;
+    }
+    if (c.vs_next < c.vs_end) {                                     // ---- level 1: L1U x 32 voice-signs ----
+        int2 vb[L1U];
+#pragma unroll
+        for (int u = 0; u < L1U; ++u) {
+            const int vs = c.vs_next + 32 * u + lane;
+            vb[u] = (vs < c.vs_end) ? __ldg(c.vband + vs) : make_int2(1, 0);
+        }
+#pragma unroll
+        for (int u = 0; u < L1U; ++u) {
+            const bool stab = vb[u].y >= vb[u].x && vb[u].x <= c.b1 && vb[u].y >= c.b0;
+            const unsigned mk = __ballot_sync(full, stab);
+            if (stab) q1[(c.q1_tail + __popc(mk & lt)) & (Q1CAP - 1)] = (unsigned)(c.vs_next + 32 * u + lane);
+            c.q1_tail += (unsigned)__popc(mk);
+        }
+        c.vs_next += 32 * L1U;
+        __syncwarp();
+        return 1;
+    }
+    return 0;
+}
+
+// ---- the producer warp of the tile-major kernel -------------------------------------------------------------
+#define FDEMRI_PQ1 512          // voice-signs waiting for level 2   (>= 32 * L1U)
+#define FDEMRI_PQ2 2048         // rows waiting for level 3           (>= 32 * 3 * 16 groups)
+#define FDEMRI_PQ3 512          // entries waiting to be staged
+struct FdemriProdQueues {
+    unsigned q1[FDEMRI_PQ1];
+    unsigned q2[FDEMRI_PQ2];
+    int4 q3[FDEMRI_PQ3];        // {(vs*3 + branch), segment, first bin, last bin}
+};
+struct FdemriProdEmit {
+    int4* q3;
+    unsigned head, tail;
+    __device__ __forceinline__ int room() const { return (int)(FDEMRI_PQ3 - (tail - head)); }
+    __device__ __forceinline__ void store(int off, int vsbr, int seg, int lo, int hi) {
+        q3[(tail + (unsigned)off) & (FDEMRI_PQ3 - 1)] = make_int4(vsbr, seg, lo, hi);
+    }
+    __device__ __forceinline__ void advance(int n) { tail += (unsigned)n; }
+};
+
+// Producer: for every tile it draws, the entries that meet the tile (the scan above), one ring stage per 32 of them:
+// entry -> record + weights -> staged item.
+__device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ring, FdemriProdQueues* pq, int lane) {
     const FdemriDims& d = a.d;
     const int V = d.n_modes;
     int stage = 0;
     unsigned phase = 0;
+    unsigned long long n_items = 0;
     for (;;) {
         int gt = 0;
         if (lane == 0) gt = (int)atomicAdd(a.tile_counter, 1u);
@@ -442,58 +603,53 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
         const int64_t bin0 = (int64_t)tile * FDEMRI_TILE;
         const int tile_lo = (int)bin0;
         const int tile_hi = (int)min(bin0 + FDEMRI_TILE - 1, d.n_freq - 1);
-        const unsigned int off = a.tile_off[gt];
-        const int n = (int)(a.tile_off[gt + 1] - off);
         const int wbase = (a.n_angles > 1 ? b : 0) * V;
         const size_t rbase = (size_t)b * V * d.n_seg;
-        const int2* ent_b = a.ent + (size_t)b * 2 * V * d.ent_max;
-        int base = 0;
-        // The loads of a chunk form a chain key -> entry -> record (three trips to L2).  They run ahead of the ring:
-        // the keys two chunks ahead, the entries one chunk ahead, the records of this chunk before the wait for its slot.
-        unsigned int key0 = 0u, key1 = 0u;
-        int2 en0 = make_int2(0, -1);
-        if (lane < n) {
-            key0 = a.pairs[off + lane];
-            en0 = ent_b[key0];                                          // key = (voice*2+sign)*ent_max + 3*segment + branch
-        }
-        if (FDEMRI_CHUNK + lane < n) key1 = a.pairs[off + FDEMRI_CHUNK + lane];
+        // tiles outside the band of the item have no entry: nothing to scan
+        const bool in_band = tile_lo <= __ldg(a.iband + 2 * b + 1) && tile_hi >= -__ldg(a.iband + 2 * b);
+        FdemriScan sc;
+        fdemri_scan_init<FDEMRI_PQ2>(sc, a, b, 0, in_band ? 2 * V : 0, tile_lo, tile_hi);
+        FdemriProdEmit em;
+        em.q3 = pq->q3; em.head = em.tail = 0u;
+        bool last;
         do {
-            const int cnt = min(n - base, FDEMRI_CHUNK);
-            const int vs = (int)(key0 / (unsigned)d.ent_max);
-            const int slot = (int)(key0 - (unsigned)vs * (unsigned)d.ent_max);
-            const int seg = slot / 3, br = slot - 3 * seg;
-            const int v = vs >> 1;
+            // at least 33 entries queued, or all that are left: the stage knows whether it is the tile's last
+            while (em.tail - em.head <= 32u && fdemri_scan_step<FDEMRI_PQ1, FDEMRI_PQ2, 8>(sc, pq->q1, pq->q2, lane, em) == 1) {}
+            __syncwarp();
+            const int cnt = (int)min(em.tail - em.head, 32u);
+            int4 en = make_int4(0, 0, 0, -1);
             FdemriRecRegs q;
             double4 w4 = make_double4(0.0, 0.0, 0.0, 0.0);
             if (lane < cnt) {
-                q = fdemri_load_rec(a.rec + (rbase + (size_t)v * d.n_seg + seg) * R_DOUBLES);
+                en = pq->q3[(em.head + (unsigned)lane) & (FDEMRI_PQ3 - 1)];
+                const int v = en.x / 6;                                  // en.x = (v*2 + sign)*3 + branch
+                q = fdemri_load_rec(a.rec + (rbase + (size_t)v * d.n_seg + en.y) * R_DOUBLES);
                 w4 = a.wts[wbase + v];
             }
-            int2 en1 = make_int2(0, -1);
-            unsigned int key2 = 0u;
-            if (base + FDEMRI_CHUNK + lane < n) en1 = ent_b[key1];
-            if (base + 2 * FDEMRI_CHUNK + lane < n) key2 = a.pairs[off + base + 2 * FDEMRI_CHUNK + lane];
+            em.head += (unsigned)cnt;
+            last = (em.tail == em.head);
+            n_items += (unsigned)cnt;
             fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, FDEMRI_PROD_BACKOFF);
             if (lane < cnt) {
-                const int lo_e = max(en0.x, tile_lo) - tile_lo;
-                const int hi_e = min(en0.y, tile_hi) - tile_lo;
+                const int vs = en.x / 3, br = en.x - 3 * vs;
+                const int lo_e = max(en.z, tile_lo) - tile_lo;
+                const int hi_e = min(en.w, tile_hi) - tile_lo;
                 fdemri_stage_regs(ring->st[stage].items[lane], q, w4, lo_e, hi_e, (unsigned)(vs & 1), (unsigned)br);
             }
-            key0 = key1; en0 = en1; key1 = key2;
-            base += FDEMRI_CHUNK;
             __syncwarp();
             if (lane == 0) {
-                ring->st[stage].hdr[0] = gt; ring->st[stage].hdr[1] = cnt; ring->st[stage].hdr[2] = (base >= n);
+                ring->st[stage].hdr[0] = gt; ring->st[stage].hdr[1] = cnt; ring->st[stage].hdr[2] = last;
                 fdemri_mbar_arrive(&ring->full[stage]);
             }
             if (++stage == FDEMRI_STAGES) { stage = 0; phase ^= 1u; }
-        } while (base < n);
+        } while (!last);
     }
     // no more work
     fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, FDEMRI_PROD_BACKOFF);
     if (lane == 0) {
         ring->st[stage].hdr[0] = -1; ring->st[stage].hdr[1] = 0; ring->st[stage].hdr[2] = 1;
         fdemri_mbar_arrive(&ring->full[stage]);
+        if (n_items) atomicAdd(a.stats + 8, n_items);              // (entry, tile) pairs staged
     }
 }
 
@@ -675,7 +831,7 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
     if (lane == 0) {
         if (n_airy) atomicAdd(a.stats + 4, (unsigned long long)n_airy);
         if (n_slow) atomicAdd(a.stats + 7, (unsigned long long)n_slow);
-        if (errs) atomicOr(a.stats + 5, (unsigned long long)errs);
+        if (errs) atomicOr(a.stats + 9, (unsigned long long)errs);
     }
 }
 
@@ -683,9 +839,14 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
 #ifndef FDEMRI_MAXNREG
 #define FDEMRI_MAXNREG 128
 #endif
+struct FdemriTileSmem {
+    FdemriRing ring;
+    FdemriProdQueues pq;
+};
 __global__ void __maxnreg__(FDEMRI_MAXNREG) k_tile_sum(SumArgs a) {
     extern __shared__ __align__(16) unsigned char fdemri_smem[];
-    FdemriRing* ring = reinterpret_cast<FdemriRing*>(fdemri_smem);
+    FdemriTileSmem* sm = reinterpret_cast<FdemriTileSmem*>(fdemri_smem);
+    FdemriRing* ring = &sm->ring;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     if (tid == 0) {
         for (int i = 0; i < FDEMRI_STAGES; ++i) {
@@ -694,31 +855,14 @@ __global__ void __maxnreg__(FDEMRI_MAXNREG) k_tile_sum(SumArgs a) {
         }
     }
     __syncthreads();
-    if (*(volatile const unsigned long long*)(a.stats + 5) & FDEMRI_BAD_LIST_OVERFLOW_BIT) {
-        // the work list did not fit the work space: fail loudly (NaN everywhere; see fdemri_get_stats)
-        const size_t n = (size_t)a.d.n_batch * a.d.n_freq * 2;
-        const double nan = __longlong_as_double(0x7ff8000000000000ll);
-        if (a.hp) {
-            for (size_t i = (size_t)blockIdx.x * blockDim.x + tid; i < n; i += (size_t)gridDim.x * blockDim.x) {
-                a.hp[i] = nan;
-                a.hx[i] = nan;
-            }
-        }
-        if (a.inner_part) {
-            const size_t m = (size_t)a.total_tiles * FDEMRI_CWARPS * 4;
-            for (size_t i = (size_t)blockIdx.x * blockDim.x + tid; i < m; i += (size_t)gridDim.x * blockDim.x) a.inner_part[i] = nan;
-            if (a.inner_edge)
-                for (size_t i = (size_t)blockIdx.x * blockDim.x + tid; i < 4 * m; i += (size_t)gridDim.x * blockDim.x) a.inner_edge[i] = nan;
-        }
-        return;
-    }
-    if (wid == FDEMRI_CWARPS) fdemri_producer(a, ring, lane);
+    if (wid == FDEMRI_CWARPS) fdemri_producer(a, ring, &sm->pq, lane);
     else fdemri_consumer(a, ring, wid, lane);
 }
 
-// Fixed-order sum of the per-(tile, warp) partial inner products of one batch item.  One CTA per item.
-// With the Hann filter (edge != NULL) it also adds the first and the last bin of every warp range, whose filtered
-// values need a bin of the neighbouring range: range i covers bins 64 i .. 64 i + 63 of the item.
+// Fixed-order sum of the per-range partial inner products of one batch item.  One CTA per item.  A range is the
+// 64 bins of a consumer warp of the tile-major kernel or a block of bins of the bin-major one (range_bins).
+// With the Hann filter (edge != NULL) it also adds the first and the last bin of every range, whose filtered
+// values need a bin of the neighbouring range: range i covers bins range_bins i .. range_bins (i + 1) - 1 of the item.
 // out: [B][4] = {<h|h>, Re<d|h>, Im<d|h>, 0}
 __device__ __forceinline__ void fdemri_inner_bin(const double4 h, int64_t k, const double* __restrict__ weight,
                                                  const double* __restrict__ dplus, const double* __restrict__ dcross,
@@ -737,13 +881,13 @@ __device__ __forceinline__ double4 fdemri_hann3(const double4 l, const double4 c
                         0.5 * c.w - 0.25 * (l.w + r.w));
 }
 
-__global__ void __launch_bounds__(256) k_inner_reduce(int n_tiles, int64_t n_freq, const double* __restrict__ part,
-                                                      const double* __restrict__ edge, const double* __restrict__ weight,
-                                                      const double* __restrict__ dplus, const double* __restrict__ dcross,
-                                                      double* __restrict__ out) {
+__global__ void __launch_bounds__(256) k_inner_reduce(size_t n_ranges, int range_bins, int64_t n_freq,
+                                                      const double* __restrict__ part, const double* __restrict__ edge,
+                                                      const double* __restrict__ weight, const double* __restrict__ dplus,
+                                                      const double* __restrict__ dcross, double* __restrict__ out) {
     __shared__ double s_r[3][256];
     const int b = blockIdx.x, tid = threadIdx.x;
-    const size_t n = (size_t)n_tiles * FDEMRI_CWARPS;
+    const size_t n = n_ranges;
     const double4* p = reinterpret_cast<const double4*>(part) + (size_t)b * n;
     const double4* e = edge ? reinterpret_cast<const double4*>(edge) + (size_t)b * n * 4 : nullptr;
     const double4 zero = make_double4(0.0, 0.0, 0.0, 0.0);
@@ -752,7 +896,7 @@ __global__ void __launch_bounds__(256) k_inner_reduce(int n_tiles, int64_t n_fre
         const double4 v = p[i];
         hh += v.x; dr += v.y; di += v.z;
         if (e) {
-            const int64_t k0 = (int64_t)i * 64, k1 = k0 + 63;
+            const int64_t k0 = (int64_t)i * range_bins, k1 = k0 + range_bins - 1;
             if (k0 < n_freq) {
                 const double4 left = (i > 0) ? e[(i - 1) * 4 + 3] : zero;
                 fdemri_inner_bin(fdemri_hann3(left, e[i * 4 + 0], e[i * 4 + 1]), k0, weight, dplus, dcross, hh, dr, di);
@@ -776,122 +920,198 @@ __global__ void __launch_bounds__(256) k_inner_reduce(int n_tiles, int64_t n_fre
 
 // ---------------------------------------------------------------------------------------------------------
 // Bin-major sum (sparse or down-sampled frequency arrays, section 3.3 / L218-242): when a (voice,
-// segment) covers only a few bins, a tile of bins would run every item for a handful of lanes.  Here the work
-// lists are per BIN (d.tile_bins = 1): one warp per bin, the lanes take the entries that cover it 32 at a time,
-// each lane stages its own item (same 256-byte layout, a 272-byte lane stride keeps 128-bit shared accesses
-// conflict-free), evaluates the same fast / slow term functions, and a fixed butterfly adds the lanes: every bin is
-// still written once, with no atomics, in a data-determined order.  This is the paper's own map -- the segment of
-// every (f, voice) predetermined (L105) -- with the threads over the voices of a frequency instead of over the
-// frequencies of a voice.
+// segment) covers only a few bins, a tile of bins would run every item for a handful of lanes.  Here a CTA owns a
+// BLOCK of d.tile_bins (8, 16 or 32: the plan takes the largest that still gives every resident CTA a few blocks)
+// consecutive bins at a time (blocks are handed out by an atomic counter):
+//   A  its eight warps run the item scan (above) over an eighth of the voice-signs each and collect the entries that
+//      meet the block, in key order, in shared memory (a round takes what fits; further rounds take the rest);
+//   B  every warp takes bins of the block in turn: its lanes filter the collected entries for those that cover the
+//      bin, 32 at a time each lane stages its own item (same 256-byte layout, a 272-byte lane stride keeps 128-bit
+//      shared accesses conflict-free) and evaluates the same fast / slow term functions, a fixed butterfly adds the
+//      lanes, and lane 0 adds the round's sum to the bin's accumulator.
+// Every bin is written once, with no atomics and no list in global memory, in an order that depends on the data only.
+// This is the paper's own map -- the segment of every (f, voice) predetermined (L105) -- with the threads over the
+// voices of a frequency instead of over the frequencies of a voice.  The Eq. 12 inner products are formed from the
+// block's accumulators (one range per block for k_inner_reduce).
 // ---------------------------------------------------------------------------------------------------------
 #define FDEMRI_BIN_WARPS 8
-#define FDEMRI_BIN_STRIDE 34         // doubles per lane slot
+#define FDEMRI_BIN_STRIDE 34         // doubles per lane slot of the staging area
+#define FDEMRI_BQ1 256               // per warp: voice-signs waiting for level 2 (= 32 * L1U)
+#define FDEMRI_BQ2 256               // per warp: rows waiting for level 3
+#define FDEMRI_BREG 256              // per warp: entries collected per round
 
-__device__ __forceinline__ bool fdemri_overflow_poison(const SumArgs& a) {
-    if (!(*(volatile const unsigned long long*)(a.stats + 5) & FDEMRI_BAD_LIST_OVERFLOW_BIT)) return false;
-    // the work list did not fit the work space: fail loudly (NaN everywhere; see fdemri_get_stats)
-    const size_t n = (size_t)a.d.n_batch * a.d.n_freq * 2;
-    const double nan = __longlong_as_double(0x7ff8000000000000ll);
-    const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nt = (size_t)gridDim.x * blockDim.x;
-    if (a.hp) {
-        for (size_t i = tid; i < n; i += nt) {
-            a.hp[i] = nan;
-            a.hx[i] = nan;
-        }
+struct FdemriBinWarpQ {
+    unsigned q1[FDEMRI_BQ1];
+    unsigned q2[FDEMRI_BQ2];
+    uint2 reg[FDEMRI_BREG];          // {key, first bin | last bin << 8, both relative to the block}
+};
+struct FdemriBinSmem {
+    double stage[FDEMRI_BIN_WARPS * 32 * FDEMRI_BIN_STRIDE];
+    double4 acc[FDEMRI_BIN_BLOCK];
+    FdemriBinWarpQ wq[FDEMRI_BIN_WARPS];
+    unsigned short wlist[FDEMRI_BIN_WARPS][64];
+    int reg_cnt[FDEMRI_BIN_WARPS];
+    int cur_block;
+};
+struct FdemriBinEmit {
+    uint2* reg;
+    int n, Sp, b0, b1;
+    __device__ __forceinline__ int room() const { return FDEMRI_BREG - n; }
+    __device__ __forceinline__ void store(int off, int vsbr, int seg, int lo, int hi) {
+        reg[n + off] = make_uint2((unsigned)(vsbr * Sp + seg), (unsigned)(max(lo, b0) - b0) | ((unsigned)(min(hi, b1) - b0) << 8));
     }
-    return true;
-}
+    __device__ __forceinline__ void advance(int k) { n += k; }
+};
 
 __global__ void __launch_bounds__(FDEMRI_BIN_WARPS * 32, 2) k_bin_sum(SumArgs a) {
-    extern __shared__ __align__(16) double fdemri_bin_smem[];
-    if (fdemri_overflow_poison(a)) return;
+    extern __shared__ __align__(16) unsigned char fdemri_bin_smem[];
+    FdemriBinSmem* sm = reinterpret_cast<FdemriBinSmem*>(fdemri_bin_smem);
     const FdemriDims& d = a.d;
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    double* it = fdemri_bin_smem + ((size_t)wid * 32 + lane) * FDEMRI_BIN_STRIDE;
-    const int V = d.n_modes;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
+    double* it = sm->stage + ((size_t)wid * 32 + lane) * FDEMRI_BIN_STRIDE;
+    const int V = d.n_modes, S = d.n_seg, Sp = 32 * d.n_groups, NB = d.tile_bins;     // NB <= FDEMRI_BIN_BLOCK
+    const int part = ((2 * V + FDEMRI_BIN_WARPS - 1) / FDEMRI_BIN_WARPS + 31) & ~31;     // voice-signs per warp
     unsigned n_airy = 0, n_slow = 0, errs = 0;
+    unsigned long long n_acc = 0;
     for (;;) {
-        int gb = 0;
-        if (lane == 0) gb = (int)atomicAdd(a.tile_counter, 1u);
-        gb = __shfl_sync(0xffffffffu, gb, 0);
+        __syncthreads();                                             // the previous block's accumulators have been read
+        if (tid == 0) sm->cur_block = (int)atomicAdd(a.tile_counter, 1u);
+        if (tid < FDEMRI_BIN_BLOCK) sm->acc[tid] = make_double4(0.0, 0.0, 0.0, 0.0);
+        __syncthreads();
+        const int gb = sm->cur_block;
         if (gb >= a.total_tiles) break;
-        const int b = gb / d.n_tiles, bin = gb - b * d.n_tiles;           // n_tiles = n_freq in this mode
-        const double f = fdemri_freq(d, bin);
-        const unsigned int off = a.tile_off[gb];
-        const int n = (int)(a.tile_off[gb + 1] - off);
+        const int b = gb / d.n_tiles, blk = gb - b * d.n_tiles;
+        const int i0 = blk * NB;
+        const int i1 = (int)min((int64_t)i0 + NB - 1, d.n_freq - 1);
         const int wbase = (a.n_angles > 1 ? b : 0) * V;
-        const size_t rbase = (size_t)b * V * d.n_seg;
-        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-        for (int base = 0; base < n; base += 32) {
-            if (base + lane < n) {
-                const unsigned int key = a.pairs[off + base + lane];
-                const int vs = (int)(key / (unsigned)d.ent_max);              // key = (voice*2+sign)*ent_max + 3*segment + branch
-                const int slot = (int)(key - (unsigned)vs * (unsigned)d.ent_max);
-                const int seg = slot / 3, br = slot - 3 * seg;
-                const int v = vs >> 1;
-                fdemri_stage_item(it, a.rec + (rbase + (size_t)v * d.n_seg + seg) * R_DOUBLES, a.wts[wbase + v], 0, 0,
-                                  (unsigned)(vs & 1), (unsigned)br);
-                const unsigned flags = (unsigned)(*reinterpret_cast<const int2*>(it)).y;
-                const double sf = fdemri_xorsign(f, (flags & 4u) << 29);
-                double Tr = 0.0, Ti = 0.0;
-                bool ok = false;
-                if (!(flags & 1u)) ok = fdemri_term_fast(it, sf, Tr, Ti);
-                if (!ok) {
-                    const FdemriSlowOut o = fdemri_term_slow(it, sf, flags);
-                    Tr = o.tre; Ti = o.tim;
-                    n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+        const size_t rbase = (size_t)b * V * S;
+        const bool in_band = i0 <= __ldg(a.iband + 2 * b + 1) && i1 >= -__ldg(a.iband + 2 * b);
+        FdemriScan sc;
+        const int vs0 = min(wid * part, 2 * V), vs1 = min(vs0 + part, 2 * V);
+        fdemri_scan_init<FDEMRI_BQ2>(sc, a, b, vs0, in_band ? vs1 : vs0, i0, i1);
+        FdemriBinWarpQ* wq = &sm->wq[wid];
+        int more;
+        do {
+            // ---- A: this warp's part of the voice range: entries that meet the block, as many as fit ----
+            FdemriBinEmit em;
+            em.reg = wq->reg; em.n = 0; em.Sp = Sp; em.b0 = i0; em.b1 = i1;
+            int rc;
+            while ((rc = fdemri_scan_step<FDEMRI_BQ1, FDEMRI_BQ2, 8>(sc, wq->q1, wq->q2, lane, em)) == 1) {}
+            if (lane == 0) sm->reg_cnt[wid] = em.n;
+            more = __syncthreads_or(rc != 0);
+            // ---- B: bins of the block, a warp each ----
+            for (int t = wid; i0 + t <= i1; t += FDEMRI_BIN_WARPS) {
+                const double f = fdemri_freq(d, i0 + t);
+                double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+                unsigned wl_head = 0u, wl_tail = 0u;
+                bool any = false;
+                // evaluates the first `nl` waiting entries, a lane each
+                auto evaluate = [&](int nl) {
+                    if (lane < nl) {
+                        const unsigned idx = sm->wlist[wid][(wl_head + (unsigned)lane) & 63u];
+                        const unsigned key = sm->wq[idx / FDEMRI_BREG].reg[idx % FDEMRI_BREG].x;
+                        const int vsbr = (int)(key / (unsigned)Sp), seg = (int)(key - (unsigned)vsbr * (unsigned)Sp);
+                        const int vs = vsbr / 3, br = vsbr - 3 * vs;
+                        const int v = vs >> 1;
+                        fdemri_stage_item(it, a.rec + (rbase + (size_t)v * S + seg) * R_DOUBLES, a.wts[wbase + v], 0, 0,
+                                          (unsigned)(vs & 1), (unsigned)br);
+                        const unsigned flags = (unsigned)(*reinterpret_cast<const int2*>(it)).y;
+                        const double sf = fdemri_xorsign(f, (flags & 4u) << 29);
+                        double Tr = 0.0, Ti = 0.0;
+                        bool ok = false;
+                        if (!(flags & 1u)) ok = fdemri_term_fast(it, sf, Tr, Ti);
+                        if (!ok) {
+                            const FdemriSlowOut o = fdemri_term_slow(it, sf, flags);
+                            Tr = o.tre; Ti = o.tim;
+                            n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                        }
+                        a0 = fma(it[S_WP], Tr, a0); a1 = fma(it[S_SWP], Ti, a1); a2 = fma(it[S_NWX], Ti, a2); a3 = fma(it[S_SWX], Tr, a3);
+                        ++n_acc;
+                    }
+                    wl_head += (unsigned)nl;
+                    any = true;
+                };
+                for (int r = 0; r < FDEMRI_BIN_WARPS; ++r) {
+                    const int cnt = sm->reg_cnt[r];
+                    for (int j0 = 0; j0 < cnt; j0 += 32) {
+                        const int j = j0 + lane;
+                        bool hit = false;
+                        if (j < cnt) {
+                            const unsigned span = sm->wq[r].reg[j].y;
+                            hit = t >= (int)(span & 255u) && t <= (int)(span >> 8);
+                        }
+                        const unsigned mk = __ballot_sync(full, hit);
+                        if (hit) sm->wlist[wid][(wl_tail + (unsigned)__popc(mk & lt)) & 63u] = (unsigned short)(r * FDEMRI_BREG + j);
+                        wl_tail += (unsigned)__popc(mk);
+                        __syncwarp();
+                        if (wl_tail - wl_head >= 32u) evaluate(32);
+                    }
                 }
-                a0 = fma(it[S_WP], Tr, a0); a1 = fma(it[S_SWP], Ti, a1); a2 = fma(it[S_NWX], Ti, a2); a3 = fma(it[S_SWX], Tr, a3);
-            }
-        }
+                if (wl_tail != wl_head) evaluate((int)(wl_tail - wl_head));
+                if (any) {                                           // (warp-uniform)
 #pragma unroll
-        for (int o = 16; o; o >>= 1) {
-            a0 += __shfl_xor_sync(0xffffffffu, a0, o); a1 += __shfl_xor_sync(0xffffffffu, a1, o);
-            a2 += __shfl_xor_sync(0xffffffffu, a2, o); a3 += __shfl_xor_sync(0xffffffffu, a3, o);
-        }
-        if (lane == 0) {
-            const size_t o = ((size_t)b * d.n_freq + bin) * 2;
-            *reinterpret_cast<double2*>(a.hp + o) = make_double2(a0, a1);
-            *reinterpret_cast<double2*>(a.hx + o) = make_double2(a2, a3);
+                    for (int o = 16; o; o >>= 1) {
+                        a0 += __shfl_xor_sync(full, a0, o); a1 += __shfl_xor_sync(full, a1, o);
+                        a2 += __shfl_xor_sync(full, a2, o); a3 += __shfl_xor_sync(full, a3, o);
+                    }
+                    if (lane == 0) {
+                        double4 s4 = sm->acc[t];
+                        s4.x += a0; s4.y += a1; s4.z += a2; s4.w += a3;
+                        sm->acc[t] = s4;
+                    }
+                }
+            }
+            __syncthreads();                                         // the collected entries may be overwritten
+        } while (more);
+        // ---- outputs of the block: the waveform (S4) and / or its share of the inner products of Eq. 12 ----
+        if (wid == 0) {
+            const int64_t bin = (int64_t)i0 + lane;
+            const bool valid = lane < NB && bin <= i1;
+            const double4 h = sm->acc[lane];                          // (zero past the block and past the grid)
+            if (a.hp && valid) {
+                const size_t o = ((size_t)b * d.n_freq + bin) * 2;
+                *reinterpret_cast<double2*>(a.hp + o) = make_double2(h.x, h.y);
+                *reinterpret_cast<double2*>(a.hx + o) = make_double2(h.z, h.w);
+            }
+            if (a.inner_part) {
+                double4 u = h;
+                bool use = valid;
+                if (a.inner_edge) {
+                    // Hann window as the 3-point filter h_k/2 - h_{k-1}/4 - h_{k+1}/4 (L145): the first and the last bin
+                    // of the block need a bin of a neighbouring block and are left to k_inner_reduce
+                    if (lane < 2 || (lane >= NB - 2 && lane < NB))
+                        *reinterpret_cast<double4*>(a.inner_edge + ((size_t)gb * 4 + (lane < 2 ? lane : lane - (NB - 4))) * 4) = h;
+                    double4 l, r;
+                    l.x = __shfl_up_sync(full, h.x, 1); l.y = __shfl_up_sync(full, h.y, 1);
+                    l.z = __shfl_up_sync(full, h.z, 1); l.w = __shfl_up_sync(full, h.w, 1);
+                    r.x = __shfl_down_sync(full, h.x, 1); r.y = __shfl_down_sync(full, h.y, 1);
+                    r.z = __shfl_down_sync(full, h.z, 1); r.w = __shfl_down_sync(full, h.w, 1);
+                    u = fdemri_hann3(l, h, r);
+                    use = valid && lane != 0 && lane != NB - 1;
+                }
+                double hh = 0.0, dr = 0.0, di = 0.0;
+                if (use) fdemri_inner_bin(u, bin, a.weight, a.dplus, a.dcross, hh, dr, di);
+#pragma unroll
+                for (int o = 16; o; o >>= 1) {
+                    hh += __shfl_xor_sync(full, hh, o);
+                    dr += __shfl_xor_sync(full, dr, o);
+                    di += __shfl_xor_sync(full, di, o);
+                }
+                if (lane == 0) *reinterpret_cast<double4*>(a.inner_part + (size_t)gb * 4) = make_double4(hh, dr, di, 0.0);
+            }
         }
     }
     for (int o = 16; o; o >>= 1) {
-        n_airy += __shfl_xor_sync(0xffffffffu, n_airy, o);
-        n_slow += __shfl_xor_sync(0xffffffffu, n_slow, o);
-        errs |= __shfl_xor_sync(0xffffffffu, errs, o);
+        n_airy += __shfl_xor_sync(full, n_airy, o);
+        n_slow += __shfl_xor_sync(full, n_slow, o);
+        errs |= __shfl_xor_sync(full, errs, o);
+        n_acc += __shfl_xor_sync(full, n_acc, o);
     }
     if (lane == 0) {
         if (n_airy) atomicAdd(a.stats + 4, (unsigned long long)n_airy);
         if (n_slow) atomicAdd(a.stats + 7, (unsigned long long)n_slow);
-        if (errs) atomicOr(a.stats + 5, (unsigned long long)errs);
+        if (errs) atomicOr(a.stats + 9, (unsigned long long)errs);
+        if (n_acc) atomicAdd(a.stats + 8, n_acc);                  // accumulated terms (= n_evals of the map, P9)
     }
-}
-
-// Inner products of Eq. 12 from a waveform in memory (bin-major mode): one CTA per batch item, fixed order.
-__global__ void __launch_bounds__(1024) k_inner_dense(int64_t n_freq, const double* __restrict__ hp, const double* __restrict__ hx,
-                                                       const double* __restrict__ weight, const double* __restrict__ dplus,
-                                                       const double* __restrict__ dcross, int hann, double* __restrict__ out) {
-    __shared__ double s_r[3][1024];
-    const int b = blockIdx.x, tid = threadIdx.x;
-    const double4 zero = make_double4(0.0, 0.0, 0.0, 0.0);
-    const double* p = hp + (size_t)b * n_freq * 2;
-    const double* x = hx + (size_t)b * n_freq * 2;
-    auto at = [&](int64_t k) {
-        if (k < 0 || k >= n_freq) return zero;
-        return make_double4(p[2 * k], p[2 * k + 1], x[2 * k], x[2 * k + 1]);
-    };
-    double hh = 0.0, dr = 0.0, di = 0.0;
-    for (int64_t k = tid; k < n_freq; k += 1024) {
-        const double4 h = hann ? fdemri_hann3(at(k - 1), at(k), at(k + 1)) : at(k);
-        fdemri_inner_bin(h, k, weight, dplus, dcross, hh, dr, di);
-    }
-    s_r[0][tid] = hh; s_r[1][tid] = dr; s_r[2][tid] = di;
-    __syncthreads();
-    for (int o = 512; o; o >>= 1) {
-        if (tid < o) {
-            s_r[0][tid] += s_r[0][tid + o]; s_r[1][tid] += s_r[1][tid + o]; s_r[2][tid] += s_r[2][tid + o];
-        }
-        __syncthreads();
-    }
-    if (tid == 0) *reinterpret_cast<double4*>(out + 4 * (size_t)b) = make_double4(s_r[0][0], s_r[1][0], s_r[2][0], 0.0);
 }
