@@ -6,10 +6,12 @@
 
 #define FDEMRI_MAX_KNOTS 512
 #ifndef FDEMRI_CWARPS
-#define FDEMRI_CWARPS 12             // consumer (evaluating) warps per CTA of the sum kernel
+#define FDEMRI_CWARPS 15             // consumer (evaluating) warps per CTA of the sum kernel: with the producer warp 16 warps,
+                                     // four per SM sub-partition -- the producer shares its sub-partition with three
+                                     // consumers, the other three carry four, so its instructions never set the pace
 #endif
 #define FDEMRI_BPL 2                 // bins per lane: a consumer warp owns 32*FDEMRI_BPL consecutive bins
-#define FDEMRI_TILE (FDEMRI_CWARPS * 32 * FDEMRI_BPL)     // bins per tile (768)
+#define FDEMRI_TILE (FDEMRI_CWARPS * 32 * FDEMRI_BPL)     // bins per tile (960)
 #define FDEMRI_BIN_BLOCK 32          // bins per block of the bin-major sum kernel (one CTA at a time)
 #define FDEMRI_SUM_THREADS ((FDEMRI_CWARPS + 1) * 32)     // + one producer warp
 #define FDEMRI_CHUNK 32              // staged items per ring stage (one per producer lane)

@@ -32,7 +32,7 @@
 #define FDEMRI_CONS_BACKOFF 64u     // ns between polls of a consumer warp waiting for a stage
 #endif
 #ifndef FDEMRI_PROD_BACKOFF
-#define FDEMRI_PROD_BACKOFF 256u    // ns between polls of the producer warp waiting for a free stage
+#define FDEMRI_PROD_BACKOFF 1000u   // ns between polls of the producer warp waiting for a free stage (it runs stages ahead)
 #endif
 
 struct SumArgs {
@@ -434,10 +434,9 @@ __device__ __forceinline__ void fdemri_stage_item(double* dst, const double* __r
 // order by ONE warp, a step at a time (fdemri_map.cuh has the tables):
 //   level 1  voice-sign bands, L1U x 32 at a time (coalesced int2 loads)      -> queue q1 of voice-signs that meet the range
 //   level 2  the group bands of up to 32 queued voice-signs, a lane each      -> queue q2 of rows (vs, branch, group)
-//   level 3  the 32 entries of up to 32 queued rows, a lane per row (16 x 16 B)  -> emit(entry) in order
-// A deeper level runs whenever it has input, a shallower one only when its output queue is empty: the queues are
-// FIFO, so the emitted order is (voice, sign, branch, segment) = ascending key, and every load is issued in
-// batches of independent requests (latency is paid per step, not per entry).  All control flow is warp-uniform.
+//   level 3  the 32 entries of up to 32 queued rows, a lane per row (16 x 16 B)      -> emit(entry) in order
+// The queues are FIFO, so the emitted order is (voice, sign, branch, segment) = ascending key, and every load is
+// issued in batches of independent requests (latency is paid per step, not per entry).  Control flow is warp-uniform.
 // ---------------------------------------------------------------------------------------------------------
 struct FdemriScan {
     const int2* vband;        // tables of the batch item
@@ -458,7 +457,7 @@ __device__ __forceinline__ void fdemri_scan_init(FdemriScan& c, const SumArgs& a
     c.gband = a.gband + (size_t)b * nvs * d.n_groups;
     c.ent = a.ent + (size_t)b * nvs * d.ent_max;
     c.Sp = 32 * d.n_groups; c.G = d.n_groups;
-    c.nb2 = min(32, Q2CAP / (3 * d.n_groups));
+    c.nb2 = min(32, (Q2CAP - 32) / (3 * d.n_groups));          // level 2 runs with < 32 rows queued: its output must fit
     c.b0 = b0; c.b1 = b1;
     c.vs_next = vs0; c.vs_end = vs1;
     c.q1_head = c.q1_tail = c.q2_head = c.q2_tail = 0u;
@@ -471,21 +470,32 @@ template <int Q1CAP, int Q2CAP, int L1U, class Emit>
 __device__ __forceinline__ int fdemri_scan_step(FdemriScan& c, unsigned* __restrict__ q1, unsigned* __restrict__ q2, int lane,
                                                 Emit& emit) {
     const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
-    if (c.q2_tail != c.q2_head) {                                   // ---- level 3: a lane per row of 32 entries ----
+    // Which level: a deeper one as soon as it has a full batch of 32 inputs (all lanes busy), a shallower one to make
+    // more input, a partial batch only when nothing shallower is left.  (Queue sizes make one of them always possible.)
+    const unsigned n2 = c.q2_tail - c.q2_head, n1 = c.q1_tail - c.q1_head;
+    const bool more1 = c.vs_next < c.vs_end;
+    int level;
+    if (n2 >= 32u) level = 3;
+    else if (n1 >= 32u || (n1 > 0u && !more1)) level = 2;
+    else if (more1) level = 1;
+    else if (n2 > 0u) level = 3;
+    else return 0;
+    if (level == 3) {                                               // ---- level 3: up to 32 rows, a lane per row ----
         const int room = emit.room();
         if (room < 32) return 2;
         const int nr = (int)min(c.q2_tail - c.q2_head, 32u);
         unsigned row = 0u, hits = 0u;
-        int4 e2[16];                                                // the row: 32 x {first bin, last bin}
+        const int2* src = c.ent;
         if (lane < nr) {
+            // pass 1: which of the row's 32 entries meet the range (16 x 16-byte loads, nothing kept but the mask)
             row = q2[(c.q2_head + (unsigned)lane) & (Q2CAP - 1)];
-            const int4* src = reinterpret_cast<const int4*>(c.ent + (size_t)(row >> 4) * c.Sp + 32 * (row & 15u));
-#pragma unroll
-            for (int j = 0; j < 16; ++j) e2[j] = __ldg(src + j);
+            src = c.ent + (size_t)(row >> 4) * c.Sp + 32 * (row & 15u);
+            const int4* s4 = reinterpret_cast<const int4*>(src);
 #pragma unroll
             for (int j = 0; j < 16; ++j) {
-                hits |= (unsigned)(e2[j].y >= e2[j].x && e2[j].x <= c.b1 && e2[j].y >= c.b0) << (2 * j);
-                hits |= (unsigned)(e2[j].w >= e2[j].z && e2[j].z <= c.b1 && e2[j].w >= c.b0) << (2 * j + 1);
+                const int4 q = __ldg(s4 + j);
+                hits |= (unsigned)(q.y >= q.x && q.x <= c.b1 && q.y >= c.b0) << (2 * j);
+                hits |= (unsigned)(q.w >= q.z && q.z <= c.b1 && q.w >= c.b0) << (2 * j + 1);
             }
         }
         const int cnt = __popc(hits);
@@ -497,13 +507,15 @@ __device__ __forceinline__ int fdemri_scan_step(FdemriScan& c, unsigned* __restr
         }
         // rows are taken in order as long as their entries fit (the first always does: room >= 32)
         const int nok = __popc(__ballot_sync(full, lane < nr && incl <= room));
-        if (lane < nok && hits) {
+        if (lane < nok) {
+            // pass 2: the few entries that hit, read again (they are in L1 now)
             int off = incl - cnt;
             const int vsbr = (int)(row >> 4), seg0 = 32 * (int)(row & 15u);
-#pragma unroll
-            for (int j = 0; j < 16; ++j) {
-                if (hits & (1u << (2 * j))) emit.store(off++, vsbr, seg0 + 2 * j, e2[j].x, e2[j].y);
-                if (hits & (2u << (2 * j))) emit.store(off++, vsbr, seg0 + 2 * j + 1, e2[j].z, e2[j].w);
+            while (hits) {
+                const int j = __ffs(hits) - 1;
+                hits &= hits - 1;
+                const int2 q = __ldg(src + j);
+                emit.store(off++, vsbr, seg0 + j, q.x, q.y);
             }
         }
         emit.advance(__shfl_sync(full, incl, nok - 1));
@@ -511,7 +523,7 @@ __device__ __forceinline__ int fdemri_scan_step(FdemriScan& c, unsigned* __restr
         __syncwarp();
         return 1;
     }
-    if (c.q1_tail != c.q1_head) {                                   // ---- level 2: a lane per voice-sign ----
+    if (level == 2) {                                               // ---- level 2: a lane per voice-sign ----
         const int nb = (int)min(c.q1_tail - c.q1_head, (unsigned)c.nb2);
         unsigned m0 = 0u, m12 = 0u;
         unsigned vs = 0u;
@@ -546,7 +558,7 @@ __device__ __forceinline__ int fdemri_scan_step(FdemriScan& c, unsigned* __restr
         __syncwarp();
         return 1;
     }
-    if (c.vs_next < c.vs_end) {                                     // ---- level 1: L1U x 32 voice-signs ----
+    {                                                               // ---- level 1: L1U x 32 voice-signs ----
         int2 vb[L1U];
 #pragma unroll
         for (int u = 0; u < L1U; ++u) {
@@ -564,12 +576,11 @@ __device__ __forceinline__ int fdemri_scan_step(FdemriScan& c, unsigned* __restr
         __syncwarp();
         return 1;
     }
-    return 0;
 }
 
 // ---- the producer warp of the tile-major kernel -------------------------------------------------------------
-#define FDEMRI_PQ1 512          // voice-signs waiting for level 2   (>= 32 * L1U)
-#define FDEMRI_PQ2 2048         // rows waiting for level 3           (>= 32 * 3 * 16 groups)
+#define FDEMRI_PQ1 512          // voice-signs waiting for level 2   (>= 31 + 32 * L1U, L1U = 8)
+#define FDEMRI_PQ2 2048         // rows waiting for level 3           (>= 32 + 32 * 3 * 16 groups)
 #define FDEMRI_PQ3 512          // entries waiting to be staged
 struct FdemriProdQueues {
     unsigned q1[FDEMRI_PQ1];
@@ -629,7 +640,19 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
             em.head += (unsigned)cnt;
             last = (em.tail == em.head);
             n_items += (unsigned)cnt;
-            fdemri_mbar_wait(&ring->empty[stage], phase ^ 1u, FDEMRI_PROD_BACKOFF);
+            // wait for the ring slot; meanwhile scan ahead for the next stages (nothing to do: back off)
+            {
+                const unsigned addr = fdemri_smem_addr(&ring->empty[stage]);
+                bool can_scan = true;                                // false: exhausted, or the entry queue is full
+                (void)can_scan;
+                while (!fdemri_mbar_try(addr, phase ^ 1u)) {
+#ifdef FDEMRI_SCAN_AHEAD        /* measured: scanning ahead while waiting costs the consumers more than it saves (profiles/) */
+                    if (can_scan) can_scan = fdemri_scan_step<FDEMRI_PQ1, FDEMRI_PQ2, 8>(sc, pq->q1, pq->q2, lane, em) == 1;
+                    else
+#endif
+                    __nanosleep(FDEMRI_PROD_BACKOFF);
+                }
+            }
             if (lane < cnt) {
                 const int vs = en.x / 3, br = en.x - 3 * vs;
                 const int lo_e = max(en.z, tile_lo) - tile_lo;
@@ -936,8 +959,8 @@ __global__ void __launch_bounds__(256) k_inner_reduce(size_t n_ranges, int range
 // ---------------------------------------------------------------------------------------------------------
 #define FDEMRI_BIN_WARPS 8
 #define FDEMRI_BIN_STRIDE 34         // doubles per lane slot of the staging area
-#define FDEMRI_BQ1 256               // per warp: voice-signs waiting for level 2 (= 32 * L1U)
-#define FDEMRI_BQ2 256               // per warp: rows waiting for level 3
+#define FDEMRI_BQ1 256               // per warp: voice-signs waiting for level 2 (>= 31 + 32 * L1U, L1U = 4)
+#define FDEMRI_BQ2 512               // per warp: rows waiting for level 3
 #define FDEMRI_BREG 256              // per warp: entries collected per round
 
 struct FdemriBinWarpQ {
@@ -997,7 +1020,7 @@ __global__ void __launch_bounds__(FDEMRI_BIN_WARPS * 32, 2) k_bin_sum(SumArgs a)
             FdemriBinEmit em;
             em.reg = wq->reg; em.n = 0; em.Sp = Sp; em.b0 = i0; em.b1 = i1;
             int rc;
-            while ((rc = fdemri_scan_step<FDEMRI_BQ1, FDEMRI_BQ2, 8>(sc, wq->q1, wq->q2, lane, em)) == 1) {}
+            while ((rc = fdemri_scan_step<FDEMRI_BQ1, FDEMRI_BQ2, 4>(sc, wq->q1, wq->q2, lane, em)) == 1) {}
             if (lane == 0) sm->reg_cnt[wid] = em.n;
             more = __syncthreads_or(rc != 0);
             // ---- B: bins of the block, a warp each ----
