@@ -191,7 +191,11 @@ static int plan_impl(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, c
     /* bin-major: the largest block of bins (32, 16, 8) that still gives every resident CTA (two per SM) four blocks:
        a block costs a scan of all voice bands, so large blocks are cheap, but few blocks balance badly */
     int tile_bins = bin_major ? FDEMRI_BIN_BLOCK : FDEMRI_TILE;
-    while (bin_major && tile_bins > 8 && (n_freq * (int64_t)n_batch) / tile_bins < (int64_t)8 * prop.multiProcessorCount)
+#ifndef FDEMRI_BIN_BLOCKS_PER_SM
+#define FDEMRI_BIN_BLOCKS_PER_SM 8
+#endif
+    while (bin_major && tile_bins > 8 &&
+           (n_freq * (int64_t)n_batch) / tile_bins < (int64_t)FDEMRI_BIN_BLOCKS_PER_SM * prop.multiProcessorCount)
         tile_bins /= 2;
     int64_t n_tiles = (n_freq + tile_bins - 1) / tile_bins;
     if (n_tiles * (int64_t)n_batch >= ((int64_t)1 << 31)) return FDEMRI_ERR_INVALID_ARG;
@@ -211,6 +215,7 @@ static int plan_impl(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, c
     p->d.n_tiles = (int)n_tiles;
     p->d.f0 = f0;
     p->d.df = df;
+    p->d.inv_df = (df > 0.0) ? 1.0 / df : 0.0;
     p->d.freq = freq_dev;
     p->lmn.assign(lmn_host, lmn_host + (size_t)3 * n_modes);
     if (k_host) p->kk.assign(k_host, k_host + n_modes);
@@ -308,10 +313,11 @@ static int raise_spline_smem_limits() {
     if (cudaGetDevice(&dev) != cudaSuccess) return FDEMRI_ERR_CUDA;
     if (dev >= 0 && dev < 64 && done[dev]) return FDEMRI_OK;
     const int N = FDEMRI_MAX_KNOTS;
-    const size_t sm_sh = (size_t)(2 * N * FDEMRI_SH_ROW + 5 * N) * sizeof(double2);
+    const size_t sm_sh = (size_t)(2 * N * FDEMRI_SH_ROW + 6 * N) * sizeof(double2);
     const size_t sm_am = ((size_t)2 * N * FDEMRI_AMP_ROW + N + (N & 1)) * sizeof(double) +
                          (size_t)2 * FDEMRI_AMP_VOICES * N * sizeof(double2);
-    if (cudaFuncSetAttribute(k_spline_shared, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_sh) != cudaSuccess ||
+    if (cudaFuncSetAttribute(k_spline_shared<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_sh) != cudaSuccess ||
+        cudaFuncSetAttribute(k_spline_shared<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_sh) != cudaSuccess ||
         cudaFuncSetAttribute(k_spline_amp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_am) != cudaSuccess)
         return FDEMRI_ERR_CUDA;
     if (dev >= 0 && dev < 64) done[dev] = true;
@@ -338,7 +344,7 @@ static int build_impl(fdemri_plan_t p, const double* f_phi, const double* f_thet
     // joined before the stream goes on (the sum reads them).
     const int N = d.n_knots;
     const int threads = (N + 31) & ~31;
-    const size_t sm_sh = (size_t)(2 * N * FDEMRI_SH_ROW + 5 * N) * sizeof(double2);
+    const size_t sm_sh = (size_t)(2 * N * FDEMRI_SH_ROW + 6 * N) * sizeof(double2);
     const size_t sm_am = ((size_t)2 * N * FDEMRI_AMP_ROW + N + (N & 1)) * sizeof(double) +
                          (size_t)2 * FDEMRI_AMP_VOICES * N * sizeof(double2);
     const int groups = (d.n_modes + FDEMRI_AMP_VOICES - 1) / FDEMRI_AMP_VOICES;
@@ -347,9 +353,13 @@ static int build_impl(fdemri_plan_t p, const double* f_phi, const double* f_thet
     k_spline_amp<<<(unsigned)((size_t)d.n_batch * groups), threads, sm_am, p->side>>>(d.n_modes, N, p->t_knots_dev, amp,
                                                                                    p->rec, p->stats + 5);
     if (cudaEventRecord(p->ev_join, p->side) != cudaSuccess) return FDEMRI_ERR_CUDA;
-    k_spline_shared<<<dim3(d.n_batch, polar ? 2 : 1), threads, sm_sh, st>>>(N, p->t_knots_dev, f_phi, f_r, Phi_phi, Phi_r,
-                                                                           p->sh_hi, p->sh_lo, p->stats + 5, f_theta,
-                                                                           Phi_theta, p->sh2_hi, p->sh2_lo);
+    // four threads per knot (a component each) up to 256 knots, two above
+    if (N <= 256)
+        k_spline_shared<4><<<dim3(d.n_batch, polar ? 2 : 1), (4 * N + 31) & ~31, sm_sh, st>>>(
+            N, p->t_knots_dev, f_phi, f_r, Phi_phi, Phi_r, p->sh_hi, p->sh_lo, p->stats + 5, f_theta, Phi_theta, p->sh2_hi, p->sh2_lo);
+    else
+        k_spline_shared<2><<<dim3(d.n_batch, polar ? 2 : 1), (2 * N + 31) & ~31, sm_sh, st>>>(
+            N, p->t_knots_dev, f_phi, f_r, Phi_phi, Phi_r, p->sh_hi, p->sh_lo, p->stats + 5, f_theta, Phi_theta, p->sh2_hi, p->sh2_lo);
     // S2: records, entries and their bands: one warp per (batch item, voice)
     const size_t nvoice = (size_t)d.n_batch * d.n_modes;
     auto records = polar ? k_records<true> : k_records<false>;

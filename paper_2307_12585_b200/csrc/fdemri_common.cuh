@@ -90,7 +90,7 @@ struct FdemriDims {
     int bin_major;                          // 1: the bin-major sum kernel (sparse grids), 0: the tile-major one
     int tile_bins;                          // bins a CTA owns at a time: FDEMRI_TILE (tile-major) or 8, 16, FDEMRI_BIN_BLOCK = 32 (bin-major)
     int n_tiles;                            // tiles (blocks) per batch item = ceil(n_freq / tile_bins)
-    double f0, df;
+    double f0, df, inv_df;                  // inv_df = 1 / df: only to guess a bin index, which is then fixed up exactly
     const double* freq;                     // NULL => uniform grid
 };
 

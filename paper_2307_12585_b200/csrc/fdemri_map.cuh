@@ -93,35 +93,44 @@ __device__ __forceinline__ double fdemri_knotF3(int m, int k, int n, double fphi
     return __dadd_rn(__dadd_rn(__dmul_rn((double)m, fphi), __dmul_rn((double)k, fth)), __dmul_rn((double)n, fr));
 }
 
-// root of the monotone cubic  FB t + FC t^2 + FD t^3 = x  on [0, h]  (safeguarded Newton; build time only)
-__device__ double fdemri_root_build(double FB, double FC, double FD, double x, double h) {
-    double lo = 0.0, hi = h;
-    double Gh = h * (FB + h * (FC + h * FD)) - x;
-    bool inc = Gh > -x;                      // G(h) > G(0)
-    double t = (Gh != -x) ? h * (x / (Gh + x)) : 0.5 * h;   // secant seed
-    t = fmin(fmax(t, 0.0), h);
-    for (int it = 0; it < 8; ++it) {                               // a seed: a handful of safeguarded steps is plenty
-        double G = t * (FB + t * (FC + t * FD)) - x;
-        double dG = FB + t * (2.0 * FC + 3.0 * FD * t);
-        if (G == 0.0) break;
-        if ((G > 0.0) == inc) hi = t; else lo = t;
-        double tn = t - G / dG;
-        if (!(tn > lo && tn < hi)) tn = 0.5 * (lo + hi);
-        if (fabs(tn - t) <= 1e-9 * h) { t = tn; break; }          // the points only shape the seed of the inverse
-        t = tn;
+// roots of the monotone cubic  FB t + FC t^2 + FD t^3 = x  on [0, h]  for x = x1 and x = x2 (build time only: the two
+// points shape the seed of the inverse, whose own interpolation error is ~1e-4 h, so four safeguarded Newton steps from
+// the secant point are plenty).  Both roots advance together: two independent dependency chains, no divergent loop.
+__device__ __forceinline__ void fdemri_root_build2(double FB, double FC, double FD, double x1, double x2, double h,
+                                                   double& t1, double& t2) {
+    const double Gh = h * (FB + h * (FC + h * FD));                // G(h) + x
+    const bool inc = Gh > 0.0;                                     // G(h) > G(0)
+    const double ih = (Gh != 0.0) ? h / Gh : 0.0;
+    double lo1 = 0.0, hi1 = h, lo2 = 0.0, hi2 = h;
+    t1 = fmin(fmax(x1 * ih, 0.0), h);                              // secant seeds
+    t2 = fmin(fmax(x2 * ih, 0.0), h);
+#pragma unroll
+    for (int it = 0; it < 4; ++it) {
+        const double G1 = t1 * (FB + t1 * (FC + t1 * FD)) - x1, G2 = t2 * (FB + t2 * (FC + t2 * FD)) - x2;
+        const double d1 = FB + t1 * (2.0 * FC + 3.0 * FD * t1), d2 = FB + t2 * (2.0 * FC + 3.0 * FD * t2);
+        if ((G1 > 0.0) == inc) hi1 = t1; else lo1 = t1;
+        if ((G2 > 0.0) == inc) hi2 = t2; else lo2 = t2;
+        double n1 = t1 - G1 / d1, n2 = t2 - G2 / d2;
+        if (!(n1 > lo1 && n1 < hi1)) n1 = 0.5 * (lo1 + hi1);
+        if (!(n2 > lo2 && n2 < hi2)) n2 = 0.5 * (lo2 + hi2);
+        t1 = (G1 == 0.0) ? t1 : n1;
+        t2 = (G2 == 0.0) ? t2 : n2;
     }
-    return t;
 }
 
 // first bin index with f_i >= x  (n_freq if none)
 __device__ int64_t fdemri_first_ge(const FdemriDims& d, double x) {
     int64_t n = d.n_freq;
     if (d.freq) {
+        // binary search down to a window of 8, then the window at once (independent loads: one trip instead of three)
         int64_t lo = 0, hi = n;
-        while (lo < hi) { int64_t mid = (lo + hi) >> 1; if (__ldg(d.freq + mid) < x) lo = mid + 1; else hi = mid; }
-        return lo;
+        while (hi - lo > 8) { int64_t mid = (lo + hi) >> 1; if (__ldg(d.freq + mid) < x) lo = mid + 1; else hi = mid; }
+        int below = 0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) below += (lo + j < hi && __ldg(d.freq + lo + j) < x) ? 1 : 0;
+        return lo + below;
     }
-    double g = ceil((x - d.f0) / d.df);
+    double g = ceil((x - d.f0) * d.inv_df);
     int64_t i = (g <= 0.0) ? 0 : (g >= (double)n ? n : (int64_t)g);
     while (i > 0 && fdemri_freq(d, i - 1) >= x) --i;
     while (i < n && fdemri_freq(d, i) < x) ++i;
@@ -135,7 +144,7 @@ __device__ int64_t fdemri_first_gt(const FdemriDims& d, double x) {
         while (lo < hi) { int64_t mid = (lo + hi) >> 1; if (__ldg(d.freq + mid) <= x) lo = mid + 1; else hi = mid; }
         return lo;
     }
-    double g = floor((x - d.f0) / d.df) + 1.0;
+    double g = floor((x - d.f0) * d.inv_df) + 1.0;
     int64_t i = (g <= 0.0) ? 0 : (g >= (double)n ? n : (int64_t)g);
     while (i > 0 && fdemri_freq(d, i - 1) > x) --i;
     while (i < n && fdemri_freq(d, i) <= x) ++i;
@@ -197,6 +206,8 @@ k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ 
         for (int sg = 0; sg < 2; ++sg)
 #pragma unroll
             for (int br = 0; br < 3; ++br) e[sg][br] = make_int2(0, -1);       // empty: last < first
+        double V0 = 0.0, V1 = 0.0, V2 = 0.0, V3 = 0.0;
+        int nbr = 0;
         if (active) {
             // coefficients (a, b, c, d) of f_phi, f_r, Phi_phi, Phi_r on this segment, hi and lo parts
             const double4* H4 = reinterpret_cast<const double4*>(sh_hi + (size_t)b * 4 * per) + k;
@@ -258,8 +269,8 @@ k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ 
                 const double dF = h * (FB + h * (FC + h * FD));
                 double q1 = 0.0, q2 = 0.0, q3 = 0.0;
                 if (dF != 0.0 && isfinite(dF)) {
-                    const double t1 = fdemri_root_build(FB, FC, FD, dF * (1.0 / 3.0), h);
-                    const double t2 = fdemri_root_build(FB, FC, FD, dF * (2.0 / 3.0), h);
+                    double t1, t2;
+                    fdemri_root_build2(FB, FC, FD, dF * (1.0 / 3.0), dF * (2.0 / 3.0), h, t1, t2);
                     const double g1 = 3.0 * t1, g2 = 1.5 * t2, g3 = h;
                     const double gam = 4.5 * (g1 - 2.0 * g2 + g3);
                     const double bet = 3.0 * (g2 - g1) - gam;
@@ -305,24 +316,71 @@ k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ 
                                       : fdemri_knotF(m, n, f_phi[last], f_r[last]);
             // branch j of the segment runs from V[j] to V[j+1]: knot value, extremum values, next knot value; a branch
             // includes its start iff that is the knot and its end iff that is an extremum (R6, R7)
-            const double Vv[4] = {Fk, type >= 1 ? rQ2 : Fk1, type == 2 ? rSF : Fk1, Fk1};
-            const int nbr = masked ? 0 : type + 1;
+            V0 = Fk; V1 = type >= 1 ? rQ2 : Fk1; V2 = type == 2 ? rSF : Fk1; V3 = Fk1;
+            nbr = masked ? 0 : type + 1;
+        }
+        // One search per knot: g = first bin >= |F_k|, and whether that bin equals |F_k| (then first bin > |F_k| is g + 1).
+        // The next knot's pair comes from the next lane; the last lane of the group looks its own up.  (Scalars and
+        // selects, no indexed arrays: those would live in local memory.)
+        int g0, g1, g2, g3;
+        bool q0, q1, q2, q3;
+        {
+            const double a0 = fabs(V0);
+            const int64_t s0 = active ? fdemri_first_ge(d, a0) : 0;
+            g0 = (int)s0;
+            q0 = active && s0 < d.n_freq && fdemri_freq(d, s0) == a0;
+            g3 = __shfl_down_sync(full, g0, 1);
+            q3 = __shfl_down_sync(full, (int)q0, 1) != 0;
+            if (active && (lane == 31 || k + 1 >= S)) {              // no next lane holds the knot k + 1
+                const double a3 = fabs(V3);
+                const int64_t s3 = fdemri_first_ge(d, a3);
+                g3 = (int)s3;
+                q3 = s3 < d.n_freq && fdemri_freq(d, s3) == a3;
+            }
+            g1 = g2 = g3; q1 = q2 = q3;
+            if (active && nbr > 1) {                                 // extremum values (turnover segments only)
+                const double a1 = fabs(V1);
+                const int64_t s1 = fdemri_first_ge(d, a1);
+                g1 = (int)s1;
+                q1 = s1 < d.n_freq && fdemri_freq(d, s1) == a1;
+            }
+            if (active && nbr > 2) {
+                const double a2 = fabs(V2);
+                const int64_t s2 = fdemri_first_ge(d, a2);
+                g2 = (int)s2;
+                q2 = s2 < d.n_freq && fdemri_freq(d, s2) == a2;
+            }
+        }
+        if (active) {
 #pragma unroll
             for (int sg = 0; sg < 2; ++sg) {
 #pragma unroll
                 for (int br = 0; br < 3; ++br) {
                     if (br < nbr) {
-                        const double Va = Vv[br], Vb = Vv[br + 1];
-                        const bool a_incl = (br == 0), b_incl = (br + 1 < nbr);
+                        // end values of the branch: start (index br) and end (index br + 1, or 3 = the next knot)
+                        const bool to_knot = !(br + 1 < nbr);
+                        const double Va = br == 0 ? V0 : (br == 1 ? V1 : V2);
+                        const int ga = br == 0 ? g0 : (br == 1 ? g1 : g2);
+                        const bool qa = br == 0 ? q0 : (br == 1 ? q1 : q2);
+                        const double Vb = to_knot ? V3 : (br == 0 ? V1 : V2);
+                        const int gb = to_knot ? g3 : (br == 0 ? g1 : g2);
+                        const bool qb = to_knot ? q3 : (br == 0 ? q1 : q2);
+                        const bool a_incl = (br == 0), b_incl = !to_knot;
                         if (Va != Vb) {
-                            const double lo_v = fmin(Va, Vb), hi_v = fmax(Va, Vb);
-                            const bool lo_incl = (Va < Vb) ? a_incl : b_incl;
-                            const bool hi_incl = (Va < Vb) ? b_incl : a_incl;
-                            const double flo = sg ? -hi_v : lo_v, fhi = sg ? -lo_v : hi_v;
+                            const bool up = Va < Vb;
+                            const double Vlo = up ? Va : Vb, Vhi = up ? Vb : Va;      // lower / higher end value
+                            const int glo = up ? ga : gb, ghi = up ? gb : ga;
+                            const bool qlo = up ? qa : qb, qhi = up ? qb : qa;
+                            const bool lo_incl = up ? a_incl : b_incl, hi_incl = up ? b_incl : a_incl;
+                            // in terms of f = s x:  s = +1: f in [Vlo, Vhi];  s = -1: f in [-Vhi, -Vlo]
+                            const double flo = sg ? -Vhi : Vlo, fhi = sg ? -Vlo : Vhi;
+                            const int gflo = sg ? ghi : glo, gfhi = sg ? glo : ghi;
+                            const bool qflo = sg ? qhi : qlo, qfhi = sg ? qlo : qhi;
                             const bool flo_incl = sg ? hi_incl : lo_incl, fhi_incl = sg ? lo_incl : hi_incl;
                             if (fhi > 0.0) {
-                                int64_t lo_b = flo_incl ? fdemri_first_ge(d, flo) : fdemri_first_gt(d, flo);
-                                const int64_t hi1 = fhi_incl ? fdemri_first_gt(d, fhi) : fdemri_first_ge(d, fhi);
+                                // first bin >= x (incl) or > x (excl); x <= 0: every bin qualifies (clipped to f > 0 below)
+                                int64_t lo_b = (flo > 0.0) ? (int64_t)gflo + ((!flo_incl && qflo) ? 1 : 0) : 0;
+                                const int64_t hi1 = (int64_t)gfhi + ((fhi_incl && qfhi) ? 1 : 0);
                                 if (lo_b < first_pos) lo_b = first_pos;
                                 if (lo_b < hi1) {
                                     e[sg][br] = make_int2((int)lo_b, (int)(hi1 - 1));
