@@ -203,6 +203,12 @@ int fdemri_measure_fp64_peak(int n_iters, double* tflops_out);
  * general FP64 kernel can reach; on B200 about 2/3 of the figure above (register-file read bandwidth). */
 int fdemri_measure_fp64_peak_3reg(int n_iters, double* tflops_out);
 
+/* Issue-cost microbenchmarks behind the roofline discussion of DESIGN.md (what an FP64 instruction costs on a B200
+ * sub-partition as a function of its distinct register operands, and whether integer / FP32 instructions issue in its
+ * shadow).  variant 0..9: see csrc/fdemri.cu; ns_out = time per group of instructions per warp and sub-partition.
+ * Synchronous; n_iters ~ 1 << 15. */
+int fdemri_measure_issue_ns(int variant, int n_iters, double* ns_out);
+
 int fdemri_destroy(fdemri_plan_t plan);
 const char* fdemri_strerror(int status);
 /* Library version string, e.g. "fdemri 0.1 sm_100a". */

@@ -21,7 +21,7 @@ STATUS = {0: "FDEMRI_OK", 1: "FDEMRI_ERR_INVALID_ARG", 2: "FDEMRI_ERR_WORKSPACE"
           4: "FDEMRI_ERR_NOT_BUILT", 5: "FDEMRI_ERR_UNSUPPORTED"}
 
 EXPORTS = ["fdemri_plan", "fdemri_plan_kerr", "fdemri_build_splines_kerr", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum", "fdemri_sum_inner", "fdemri_select_modes", "fdemri_set_mode_mask",
-           "fdemri_get_stats", "fdemri_get_item_evals", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_measure_fp64_peak_3reg", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
+           "fdemri_get_stats", "fdemri_get_item_evals", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_measure_fp64_peak_3reg", "fdemri_measure_issue_ns", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
 
 
 class FdemriStats(C.Structure):
@@ -83,6 +83,8 @@ def lib() -> C.CDLL:
         L.fdemri_measure_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
         L.fdemri_measure_fp64_peak_3reg.restype = C.c_int
         L.fdemri_measure_fp64_peak_3reg.argtypes = [C.c_int, C.POINTER(C.c_double)]
+        L.fdemri_measure_issue_ns.restype = C.c_int
+        L.fdemri_measure_issue_ns.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.fdemri_destroy.restype = C.c_int
         L.fdemri_destroy.argtypes = [vp]
         L.fdemri_strerror.restype = C.c_char_p
@@ -220,6 +222,12 @@ def fdemri_measure_fp64_peak_3reg(n_iters=1 << 16) -> float:
     tf = C.c_double()
     _chk("fdemri_measure_fp64_peak_3reg", lib().fdemri_measure_fp64_peak_3reg(int(n_iters), C.byref(tf)))
     return float(tf.value)
+
+
+def fdemri_measure_issue_ns(variant, n_iters=1 << 15) -> float:
+    ns = C.c_double()
+    _chk("fdemri_measure_issue_ns", lib().fdemri_measure_issue_ns(int(variant), int(n_iters), C.byref(ns)))
+    return float(ns.value)
 
 
 def fdemri_destroy(plan):

@@ -633,6 +633,102 @@ static int measure_peak(int n_iters, double* tflops_out) {
     return FDEMRI_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Issue-cost microbenchmarks (profiles/r2_dispatch_model.md): 8 independent chains per thread, 16 warps per SM
+// sub-partition; the measured quantity is the time per group of instructions per warp and sub-partition, in ns.
+//   0  DFMA a_i <- a_i * m + c            one distinct register operand, two shared ones (.reuse)
+//   1  DFMA a_i <- a_i * b_i + c          two distinct register operands, one shared
+//   2  DFMA a_i <- a_i * b_i + const-bank two distinct register operands and a constant-bank operand
+//   3  DFMA a_i <- a_i * b_i + b_j        three distinct register operands
+//   4  DMUL a_i <- a_i * b_i              5  DADD a_i <- a_i + b_i
+//   6  variant 1 + two integer instructions (xor, add) per DFMA
+//   7  variant 1 + four integer instructions per DFMA
+//   8  variant 0 + one FFMA (one distinct register operand) per DFMA
+//   9  variant 3 + one FFMA (one distinct register operand) per DFMA
+// ---------------------------------------------------------------------------------------------------------
+__constant__ double c_issue_k[2] = {0.999999, 1e-9};
+
+template <int V>
+__global__ void __launch_bounds__(512) k_issue(int n_iters, double seed, double* sink) {
+    double a[8], b[8];
+    float fa[8];
+    int ia[8], ib[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        a[i] = seed + threadIdx.x + i; b[i] = 0.999999 + 1e-9 * (threadIdx.x + i); fa[i] = (float)a[i];
+        ia[i] = threadIdx.x * (i + 3); ib[i] = threadIdx.x + i * 7;
+    }
+    const double m = 0.999999 + seed * 1e-12, c = 1e-9 + seed * 1e-13;
+    const float fm = (float)m, fc = (float)c;
+    for (int it = 0; it < n_iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            if (V == 0 || V == 8) a[i] = fma(a[i], m, c);
+            if (V == 1 || V == 6 || V == 7) a[i] = fma(a[i], b[i], c);
+            if (V == 2) a[i] = fma(a[i], b[i], c_issue_k[1]);
+            if (V == 3 || V == 9) a[i] = fma(a[i], b[i], b[(i + 3) & 7]);
+            if (V == 4) a[i] = a[i] * b[i];
+            if (V == 5) a[i] = a[i] + b[i];
+            if (V == 6 || V == 7) ia[i] = (ia[i] ^ ib[i]) + 1;
+            if (V == 7) ib[i] = (ib[i] & ia[i]) | 5;
+            if (V == 8 || V == 9) fa[i] = fmaf(fa[i], fm, fc);
+        }
+    }
+    double r = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) r += a[i] + b[i] + (double)fa[i] + (double)(ia[i] + ib[i]);
+    if (r == 12345.678) sink[0] = r;     // never true; keeps the chains alive
+}
+
+template <int V>
+static int run_issue(int n_iters, double* ns_out) {
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    double* sink = nullptr;
+    if (cudaMalloc(&sink, sizeof(double)) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int threads = 512, per_sm = 4, blocks = prop.multiProcessorCount * per_sm;
+    k_issue<V><<<blocks, threads>>>(n_iters / 8 + 1, 1.0, sink);
+    float best = 1e30f;
+    for (int rep = 0; rep < 3; ++rep) {
+        cudaEventRecord(e0);
+        k_issue<V><<<blocks, threads>>>(n_iters, 1.0, sink);
+        cudaEventRecord(e1);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
+    // groups issued per sub-partition: 8 per iteration and warp, threads / 32 * per_sm / 4 warps per sub-partition
+    const double groups = 8.0 * (double)n_iters * (threads / 32) * per_sm / 4.0;
+    *ns_out = (double)best * 1e6 / groups;
+    return FDEMRI_OK;
+}
+
+extern "C" int fdemri_measure_issue_ns(int variant, int n_iters, double* ns_out) {
+    if (!ns_out || n_iters < 1) return FDEMRI_ERR_INVALID_ARG;
+    switch (variant) {
+        case 0: return run_issue<0>(n_iters, ns_out);
+        case 1: return run_issue<1>(n_iters, ns_out);
+        case 2: return run_issue<2>(n_iters, ns_out);
+        case 3: return run_issue<3>(n_iters, ns_out);
+        case 4: return run_issue<4>(n_iters, ns_out);
+        case 5: return run_issue<5>(n_iters, ns_out);
+        case 6: return run_issue<6>(n_iters, ns_out);
+        case 7: return run_issue<7>(n_iters, ns_out);
+        case 8: return run_issue<8>(n_iters, ns_out);
+        case 9: return run_issue<9>(n_iters, ns_out);
+        default: return FDEMRI_ERR_INVALID_ARG;
+    }
+}
+
 extern "C" int fdemri_measure_fp64_peak(int n_iters, double* tflops_out) { return measure_peak<false>(n_iters, tflops_out); }
 extern "C" int fdemri_measure_fp64_peak_3reg(int n_iters, double* tflops_out) { return measure_peak<true>(n_iters, tflops_out); }
 
