@@ -171,33 +171,52 @@ def test_deterministic_bitwise(fd):
     wf.close()
 
 
-def test_batched_config4_subset(fd, orc):
-    """Config 4 on a seeded subset of its 1024 parameter sets spanning the M range, per-item angles."""
+def test_batched_config4_eight_items(fd, orc):
+    """BASELINE config 4 on the inputs bench.py times (substeps = 200, the seeded parameter sets): 8 of the 1024 items
+    spanning the M range (1e5 .. 1e7: 3.9e9 .. 2e6 evaluations each) in one plan, per-item viewing angles.
+      * >= 1e5 random (item, bin) samples in total against the oracle, bar 1e-10 per bin relative to the item's max|h|;
+      * the three cheapest items (2e6, 1.5e7 and 1e8 evaluations) element by element over EVERY bin, with the per-item
+        evaluation count of the map (fdemri_get_item_evals) equal to the oracle's count of accumulated terms (P9)."""
     from paper_2307_12585_b200 import synth
     M, e0, _ = synth.config4_params()
     order = np.argsort(M)
-    items = [int(order[3]), int(order[len(order) // 2]), int(order[-3])]
-    w = synth.config4(items=items, substeps=40)
+    pick = [0, 146, 292, 438, 585, 731, 877, 1023]
+    items = [int(order[i]) for i in pick]
+    w = synth.config4(items=items)                                   # substeps = 200, as bench.py --config 4
     wf = fd.waveform_from_workload(w)
-    th = np.array([w.theta, 1.0, 2.5])
-    ph = np.array([w.phi, -2.0, 0.3])
+    rng = np.random.default_rng(404)
+    th = np.concatenate([[w.theta], rng.uniform(0.2, 2.9, len(items) - 1)])
+    ph = np.concatenate([[w.phi], rng.uniform(-3.0, 3.0, len(items) - 1)])
     wf.sum(th, ph)
     hp, hx = wf.result()
     st = wf.stats()
-    total = 0
+    per_item = wf.item_evals()
+    assert st["flags"] == 0 and int(per_item.sum()) == st["n_evals"] and np.all(per_item > 0)
+    # the three cheapest items (fewest evaluations): every bin
+    cheap = [int(i) for i in np.argsort(per_item)[:3]]
+    n_samples = 0
+    freq_all = w.freq_array()
     for b in range(len(items)):
-        idx = _sampled_bins(w.n_freq, 1500, 20 + b, hi_frac=0.9)
-        freq = w.freq_array()[idx]
-        ref = orc.waveform(w.lmn, w.t_knots[b], w.f_phi[b], w.f_r[b], w.Phi_phi[b], w.Phi_r[b], w.amp[b], freq,
+        full = b in cheap
+        idx = np.arange(w.n_freq) if full else _sampled_bins(w.n_freq, 14000, 40 + b, hi_frac=0.95)
+        ref = orc.waveform(w.lmn, w.t_knots[b], w.f_phi[b], w.f_r[b], w.Phi_phi[b], w.Phi_r[b], w.amp[b], freq_all[idx],
                            float(th[b]), float(ph[b]))
         scale = max(np.abs(hp[b]).max(), np.abs(hx[b]).max())
         keep = ref["ambiguous"] == 0
+        assert (~keep).sum() <= MAX_AMBIGUOUS
         err = max(np.abs(hp[b][idx] - ref["hplus"])[keep].max(), np.abs(hx[b][idx] - ref["hcross"])[keep].max()) / scale
         mm = one_minus_overlap(hp[b][idx][keep], hx[b][idx][keep], ref["hplus"][keep], ref["hcross"][keep])
-        print(f"[parity] config4 item {items[b]} (M={M[items[b]]:.3g}): {err:.3e}, mismatch {mm:.3e}")
+        zero = (ref["nterms"] == 0) & keep
+        assert np.all(hp[b][idx][zero] == 0) and np.all(hx[b][idx][zero] == 0)
+        counts = f"map count {int(per_item[b])}"
+        if full:
+            assert int(per_item[b]) == ref["n_evals"], (items[b], int(per_item[b]), ref["n_evals"])
+            counts += f" = oracle count {ref['n_evals']} (every bin)"
+        print(f"[parity] config4 item {items[b]} (M = {M[items[b]]:.3g}, e0 = {e0[items[b]]:.2f}): max|dh|/max|h| = {err:.3e}, "
+              f"1-overlap = {mm:.3e}, {len(idx)} bins, {counts}")
         assert err <= TOL_BIN and mm <= TOL_MISMATCH
-        total += 1
-    assert total == 3 and st["n_evals"] > 0
+        n_samples += len(idx)
+    assert n_samples >= 100000
     wf.close()
 
 
