@@ -23,14 +23,18 @@ _ip = C.POINTER(C.c_int32)
 
 
 def build(force: bool = False) -> str:
-    """g++ -O2 -std=c++17 -fopenmp -ffp-contract=off -> oracle/libfdemri_oracle.so"""
-    stale = (not os.path.exists(_LIB)) or any(
-        os.path.getmtime(s) > os.path.getmtime(_LIB) for s in (_SRC, _HDR))
+    """g++ -O2 -std=c++17 -fopenmp -ffp-contract=off -> oracle/libfdemri_oracle.so
+    With FDEMRI_ORACLE_SANITIZE=1 in the environment: -O1 -g -fsanitize=address,undefined into
+    oracle/libfdemri_oracle_san.so (run the tests with LD_PRELOAD=$(g++ -print-file-name=libasan.so))."""
+    san = os.environ.get("FDEMRI_ORACLE_SANITIZE", "") not in ("", "0")
+    lib = _LIB.replace(".so", "_san.so") if san else _LIB
+    stale = (not os.path.exists(lib)) or any(
+        os.path.getmtime(s) > os.path.getmtime(lib) for s in (_SRC, _HDR))
     if force or stale:
-        cmd = ["g++", "-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC",
-               "-o", _LIB, _SRC]
+        opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-omit-frame-pointer"] if san else ["-O2"]
+        cmd = ["g++", *opt, "-std=c++17", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC", "-o", lib, _SRC]
         subprocess.run(cmd, check=True, cwd=_HERE)
-    return _LIB
+    return lib
 
 
 def _d(a):

@@ -805,3 +805,54 @@ def test_step_is_capturable_in_a_cuda_graph(fd, orc):
     check(hp1[0] / -2.0, hx1[0] / -2.0, ref, "graph replay")
     del g
     wf.close()
+
+
+@pytest.mark.parametrize("mode", ["tile", "bin"])
+def test_guard_bands_and_garbage_in_the_work_space(fd, orc, mode):
+    """compute-sanitizer is closed on this pool, so the library is checked with means of its own.  (memcheck) the work
+    space and both output buffers sit between guard bands of a known byte pattern, which must be intact after build +
+    sum + fused inner products on three cases (small turnover case, the zig-zag with a two-extrema segment, 2000 voices
+    in one tile / block -- more than the scan queues hold); (initcheck) the work space is filled with garbage (0xFF: NaN
+    as doubles, -1 as integers) or with zeros before the plan touches it, and both runs must give the same bits, equal to
+    the oracle within the bar: nothing is read before it is written."""
+    import torch
+    from helpers import zigzag_case
+    from paper_2307_12585_b200 import synth
+    flag = fd.FDEMRI_FLAG_BIN_MAJOR if mode == "bin" else fd.FDEMRI_FLAG_TILE_MAJOR
+    many = synth.small_case(seed=3, n_knots=6, n_freq=3000, modes=((2, 2, 0),), turnover=False)
+    many.f0 = 4.0e-3
+    many.lmn = np.repeat(many.lmn, 2000, axis=0)
+    many.amp = np.ascontiguousarray(np.repeat(many.amp, 2000, axis=1))
+    G = 1 << 16                                                   # guard bytes on either side
+    for label, w in (("small", synth.small_case(seed=2, n_knots=14)), ("zigzag", zigzag_case()), ("2000 voices", many)):
+        ref = oracle_c(orc, w, w.freq_array())
+        results = []
+        for fill in (0xFF, 0x00):
+            wf = fd.Waveform(w.lmn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df, flags=flag)
+            need = fd.fdemri_workspace_bytes(wf.plan)
+            raw = torch.full((need + 2 * G + 512,), 0xA5, dtype=torch.uint8, device=wf.dev)
+            off = G + ((-(raw.data_ptr() + G)) % 256)
+            raw[off:off + need] = fill
+            wf.ws, wf.ws_view = raw, raw[off:off + need]
+            fd.fdemri_set_workspace(wf.plan, wf.ws_view)
+            nout = w.n_freq * 2
+            obuf = torch.full((2 * nout + 3 * (G // 8),), float("inf"), dtype=torch.float64, device=wf.dev)
+            g8 = G // 8
+            hp = obuf[g8:g8 + nout].view(1, w.n_freq, 2)
+            hx = obuf[2 * g8 + nout:2 * g8 + 2 * nout].view(1, w.n_freq, 2)
+            wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)
+            fd.fdemri_sum(wf.plan, w.theta, w.phi, hp, hx)
+            inner = torch.zeros((1, 4), dtype=torch.float64, device=wf.dev)
+            fd.fdemri_sum_inner(wf.plan, w.theta, w.phi, inner, hann=True, hplus=hp, hcross=hx)
+            torch.cuda.synchronize()
+            assert bool((raw[:off] == 0xA5).all()) and bool((raw[off + need:] == 0xA5).all()), f"{label}: work-space guard"
+            guards = torch.cat([obuf[:g8], obuf[g8 + nout:2 * g8 + nout], obuf[2 * g8 + 2 * nout:]])
+            assert bool(torch.isinf(guards).all()), f"{label}: output guard"
+            a = hp.cpu().numpy().view(np.complex128)[0, :, 0]
+            b = hx.cpu().numpy().view(np.complex128)[0, :, 0]
+            check(a, b, ref, f"{label}, {mode}-major, work space pre-filled with {fill:#04x}")
+            assert wf.stats()["n_evals"] == ref["n_evals"]
+            results.append((a.copy(), b.copy(), inner.cpu().numpy().copy()))
+            wf.close()
+        for x, y in zip(results[0], results[1]):
+            assert np.array_equal(x.view(np.uint64) if x.dtype != np.float64 else x, y.view(np.uint64) if y.dtype != np.float64 else y)
