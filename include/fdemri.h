@@ -162,17 +162,25 @@ int fdemri_sum_inner(fdemri_plan_t plan, int n_angles, const double* theta_host,
                      const double* weight_dev, const double* data_plus_dev, const double* data_cross_dev, int hann,
                      double* hplus_dev, double* hcross_dev, double* inner_out_dev, void* cuda_stream);
 
-/* Mode selection by power threshold: "Within each time step of the sparse array,
- * we take |A_lmkn(t)|^2 and sort the individual modes in descending order and compute a cumulative summation.  From this
- * sorted array, we check whether the additional power contributed by an individual mode falls below the threshold eps
- * related to the total power emitted. ... The selected modes are given by the union of all contributing modes across
- * all time steps."  Reading (R15): a mode contributes at a time step iff |A|^2 >= eps * (sum over all modes of
- * |A|^2 at that step); keep = union over the time steps.
+/* Mode selection by power threshold: per time step of the sparse trajectory the
+ * modes are sorted by |A_lmkn(t)|^2 in descending order, a cumulative sum is formed, and the modes whose "additional
+ * power" stays above "the threshold eps related to the total power emitted" contribute; "the selected modes are given
+ * by the union of all contributing modes across all time steps".  The rule itself is not printed (the paper defers to
+ * Katz et al. 2021): both readings of DESIGN.md R15 are available.
+ *   FDEMRI_SELECT_OWN_POWER   a mode contributes at a time step iff |A|^2 >= eps * (sum over all modes of |A|^2 there);
+ *   FDEMRI_SELECT_CUMULATIVE  the contributing modes are the shortest prefix of the sorted array whose cumulative sum
+ *                             reaches (1 - eps) * total: the discarded power is at most eps * total per time step
+ *                             (a sort per (item, time step) in shared memory: n_modes <= 16384, else
+ *                             FDEMRI_ERR_UNSUPPORTED).
  *  amp_dev     [n_batch][n_modes][n_knots][2], as in fdemri_build_splines
- *  eps         >= 0 (0 keeps every mode)
+ *  eps         >= 0
  *  keep_dev    [n_batch][n_modes] bytes, out: 1 = selected
  *  n_keep_dev  [n_batch] int32, out: number of selected modes
- * Needs the work space (a [n_batch][n_knots] scratch of total powers).  Enqueued on cuda_stream. */
+ * Needs the work space (a [n_batch][n_knots] scratch of total powers).  Enqueued on cuda_stream.
+ * fdemri_select_modes is fdemri_select_modes_rule with FDEMRI_SELECT_OWN_POWER. */
+enum { FDEMRI_SELECT_OWN_POWER = 0, FDEMRI_SELECT_CUMULATIVE = 1 };
+int fdemri_select_modes_rule(fdemri_plan_t plan, const double* amp_dev, double eps, int rule, unsigned char* keep_dev,
+                             int32_t* n_keep_dev, void* cuda_stream);
 int fdemri_select_modes(fdemri_plan_t plan, const double* amp_dev, double eps, unsigned char* keep_dev,
                         int32_t* n_keep_dev, void* cuda_stream);
 /* Modes with keep_dev[b][v] == 0 get no entries in the next fdemri_build_splines and so never reach the sum.

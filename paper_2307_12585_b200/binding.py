@@ -20,7 +20,7 @@ FDEMRI_FLAG_TIMING, FDEMRI_FLAG_BIN_MAJOR, FDEMRI_FLAG_TILE_MAJOR = 1, 2, 4
 STATUS = {0: "FDEMRI_OK", 1: "FDEMRI_ERR_INVALID_ARG", 2: "FDEMRI_ERR_WORKSPACE", 3: "FDEMRI_ERR_CUDA",
           4: "FDEMRI_ERR_NOT_BUILT", 5: "FDEMRI_ERR_UNSUPPORTED"}
 
-EXPORTS = ["fdemri_plan", "fdemri_plan_kerr", "fdemri_build_splines_kerr", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum", "fdemri_sum_inner", "fdemri_select_modes", "fdemri_set_mode_mask",
+EXPORTS = ["fdemri_plan", "fdemri_plan_kerr", "fdemri_build_splines_kerr", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum", "fdemri_sum_inner", "fdemri_select_modes", "fdemri_select_modes_rule", "fdemri_set_mode_mask",
            "fdemri_get_stats", "fdemri_get_item_evals", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_measure_fp64_peak_3reg", "fdemri_measure_issue_ns", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
 
 
@@ -69,6 +69,8 @@ def lib() -> C.CDLL:
                                        vp]
         L.fdemri_select_modes.restype = C.c_int
         L.fdemri_select_modes.argtypes = [vp, dp, C.c_double, vp, vp, vp]
+        L.fdemri_select_modes_rule.restype = C.c_int
+        L.fdemri_select_modes_rule.argtypes = [vp, dp, C.c_double, C.c_int, vp, vp, vp]
         L.fdemri_set_mode_mask.restype = C.c_int
         L.fdemri_set_mode_mask.argtypes = [vp, vp]
         L.fdemri_get_stats.restype = C.c_int
@@ -180,6 +182,17 @@ def fdemri_select_modes(plan, amp, eps, keep, n_keep, stream=None):
     assert n_keep.is_cuda and n_keep.is_contiguous() and n_keep.element_size() == 4
     _chk("fdemri_select_modes", lib().fdemri_select_modes(plan, _ptr(amp), float(eps), C.c_void_p(keep.data_ptr()),
                                                           C.c_void_p(n_keep.data_ptr()), _stream_ptr(stream)))
+
+
+FDEMRI_SELECT_OWN_POWER, FDEMRI_SELECT_CUMULATIVE = 0, 1
+
+
+def fdemri_select_modes_rule(plan, amp, eps, rule, keep, n_keep, stream=None):
+    """As fdemri_select_modes with the reading of L60 chosen by `rule` (FDEMRI_SELECT_OWN_POWER / _CUMULATIVE)."""
+    assert keep.is_cuda and keep.is_contiguous() and keep.element_size() == 1
+    assert n_keep.is_cuda and n_keep.is_contiguous() and n_keep.element_size() == 4
+    _chk("fdemri_select_modes_rule", lib().fdemri_select_modes_rule(plan, _ptr(amp), float(eps), int(rule), C.c_void_p(keep.data_ptr()),
+                                                                    C.c_void_p(n_keep.data_ptr()), _stream_ptr(stream)))
 
 
 def fdemri_set_mode_mask(plan, keep):

@@ -492,18 +492,38 @@ extern "C" int fdemri_sum_inner(fdemri_plan_t p, int n_angles, const double* the
 }
 
 
-extern "C" int fdemri_select_modes(fdemri_plan_t p, const double* amp_dev, double eps, unsigned char* keep_dev,
-                                   int32_t* n_keep_dev, void* cuda_stream) {
+extern "C" int fdemri_select_modes_rule(fdemri_plan_t p, const double* amp_dev, double eps, int rule, unsigned char* keep_dev,
+                                        int32_t* n_keep_dev, void* cuda_stream) {
     if (!p || !amp_dev || !keep_dev || !n_keep_dev || !(eps >= 0.0)) return FDEMRI_ERR_INVALID_ARG;
+    if (rule != FDEMRI_SELECT_OWN_POWER && rule != FDEMRI_SELECT_CUMULATIVE) return FDEMRI_ERR_INVALID_ARG;
     if (!p->ws) return FDEMRI_ERR_WORKSPACE;
     const FdemriDims& d = p->d;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (cudaMemsetAsync(n_keep_dev, 0, d.n_batch * sizeof(int32_t), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
-    k_select_total<<<d.n_batch * d.n_knots, 256, 0, st>>>(d.n_modes, d.n_knots, amp_dev, p->sel_total);
-    const size_t n = (size_t)d.n_batch * d.n_modes;
-    k_select_keep<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(d.n_batch, d.n_modes, d.n_knots, amp_dev, p->sel_total, eps, keep_dev,
-                                                               n_keep_dev);
+    if (rule == FDEMRI_SELECT_OWN_POWER) {
+        if (cudaMemsetAsync(n_keep_dev, 0, d.n_batch * sizeof(int32_t), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
+        k_select_total<<<d.n_batch * d.n_knots, 256, 0, st>>>(d.n_modes, d.n_knots, amp_dev, p->sel_total);
+        const size_t n = (size_t)d.n_batch * d.n_modes;
+        k_select_keep<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(d.n_batch, d.n_modes, d.n_knots, amp_dev, p->sel_total, eps,
+                                                                   keep_dev, n_keep_dev);
+        return cudaGetLastError() == cudaSuccess ? FDEMRI_OK : FDEMRI_ERR_CUDA;
+    }
+    /* cumulative cut: a sort per (item, time step) in shared memory */
+    if (d.n_modes > FDEMRI_SELECT_MAX_MODES) return FDEMRI_ERR_UNSUPPORTED;
+    int Vp = 1024;
+    while (Vp < d.n_modes) Vp <<= 1;
+    const size_t smem = (size_t)Vp * 12 + 1024 * sizeof(double);
+    if (cudaFuncSetAttribute(k_select_cumulative, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             FDEMRI_SELECT_MAX_MODES * 12 + 1024 * (int)sizeof(double)) != cudaSuccess)
+        return FDEMRI_ERR_CUDA;
+    if (cudaMemsetAsync(keep_dev, 0, (size_t)d.n_batch * d.n_modes, st) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    k_select_cumulative<<<d.n_batch * d.n_knots, 1024, smem, st>>>(d.n_modes, d.n_knots, Vp, amp_dev, eps, keep_dev);
+    k_select_count<<<d.n_batch, 256, 0, st>>>(d.n_modes, keep_dev, n_keep_dev);
     return cudaGetLastError() == cudaSuccess ? FDEMRI_OK : FDEMRI_ERR_CUDA;
+}
+
+extern "C" int fdemri_select_modes(fdemri_plan_t p, const double* amp_dev, double eps, unsigned char* keep_dev,
+                                   int32_t* n_keep_dev, void* cuda_stream) {
+    return fdemri_select_modes_rule(p, amp_dev, eps, FDEMRI_SELECT_OWN_POWER, keep_dev, n_keep_dev, cuda_stream);
 }
 
 extern "C" int fdemri_set_mode_mask(fdemri_plan_t p, const unsigned char* keep_dev) {

@@ -856,3 +856,72 @@ def test_guard_bands_and_garbage_in_the_work_space(fd, orc, mode):
             wf.close()
         for x, y in zip(results[0], results[1]):
             assert np.array_equal(x.view(np.uint64) if x.dtype != np.float64 else x, y.view(np.uint64) if y.dtype != np.float64 else y)
+
+
+def _cumulative_margin(amp, eps):
+    """Modes whose cumulative-cut decision is clear at every time step: |sum before the mode - (1 - eps) total| > 1e-12 total."""
+    power = amp[..., 0] ** 2 + amp[..., 1] ** 2
+    sure = np.ones(power.shape[0], dtype=bool)
+    for k in range(power.shape[1]):
+        order = np.argsort(-power[:, k], kind="stable")
+        cum = np.cumsum(power[order, k])
+        before = np.concatenate([[0.0], cum[:-1]])
+        sure[order[np.abs(before - (1.0 - eps) * cum[-1]) <= 1e-12 * cum[-1]]] = False
+    return sure
+
+
+def test_mode_selection_cumulative_cut(fd, orc):
+    """The second reading of L60 (R15 (b)): fdemri_select_modes_rule(FDEMRI_SELECT_CUMULATIVE) -- a descending sort
+    and a cumulative sum per (item, time step) on the device -- against oracle.select_modes(rule="cumulative") on config 1
+    (252 modes) and on config 2's amplitudes (3843 modes, 150 time steps), two batch items with different amplitudes; the
+    two readings differ; the cumulative mask feeds the sum like the other one."""
+    import torch
+    import oracle
+    for idx in (1, 2):
+        w = workload(idx)
+        amp2 = np.stack([w.amp[0], w.amp[0][::-1] * 0.5 + 0.1 * w.amp[0]])          # a second item with other amplitudes
+        tk = np.repeat(w.t_knots, 2, axis=0)
+        wf = fd.Waveform(w.lmn, tk, 4096, f0=0.0, df=w.df)
+        d_amp = torch.from_numpy(np.ascontiguousarray(amp2)).to(wf.dev)
+        keep = torch.zeros((2, w.lmn.shape[0]), dtype=torch.uint8, device=wf.dev)
+        n_keep = torch.zeros(2, dtype=torch.int32, device=wf.dev)
+        for eps in (1e-5, 1e-2, 0.3):
+            fd.fdemri_select_modes_rule(wf.plan, d_amp, eps, fd.FDEMRI_SELECT_CUMULATIVE, keep, n_keep)
+            torch.cuda.synchronize()
+            for b in range(2):
+                got = keep.cpu().numpy()[b].astype(bool)
+                want, _ = oracle.select_modes(amp2[b], eps, rule="cumulative")
+                sure = _cumulative_margin(amp2[b], eps)
+                assert np.array_equal(got[sure], want[sure]) and sure.sum() >= len(sure) - 3, (idx, eps, b)
+                assert int(n_keep.cpu().numpy()[b]) == int(got.sum())
+                own, _ = oracle.select_modes(amp2[b], eps, rule="own")
+                assert want.sum() >= own.sum()
+            print(f"[select] config {idx} amplitudes, eps = {eps}: cumulative cut keeps {int(got.sum())} of {len(got)} modes "
+                  f"(own-power rule: {int(own.sum())})")
+        wf.close()
+    # the mask feeds the sum
+    w = workload(1)
+    wf = fd.Waveform(w.lmn, w.t_knots, w.n_freq, freqs=w.freqs, f0=w.f0, df=w.df)
+    d_amp = torch.from_numpy(np.ascontiguousarray(w.amp)).to(wf.dev)
+    keep = torch.zeros((1, w.lmn.shape[0]), dtype=torch.uint8, device=wf.dev)
+    n_keep = torch.zeros(1, dtype=torch.int32, device=wf.dev)
+    fd.fdemri_select_modes_rule(wf.plan, d_amp, 1e-2, fd.FDEMRI_SELECT_CUMULATIVE, keep, n_keep)
+    fd.fdemri_set_mode_mask(wf.plan, keep)
+    wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)
+    wf.sum(w.theta, w.phi)
+    hp, hx = wf.result()
+    sel = np.flatnonzero(keep.cpu().numpy()[0])
+    assert 0 < len(sel) < w.lmn.shape[0]
+    ref = orc.waveform(w.lmn[sel], w.t_knots[0], w.f_phi[0], w.f_r[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0][sel], w.freq_array(),
+                       w.theta, w.phi)
+    check(hp[0], hx[0], ref, f"config1 with the cumulative cut at eps = 1e-2 ({len(sel)} of {w.lmn.shape[0]} modes)")
+    assert wf.stats()["n_evals"] == ref["n_evals"]
+    # more modes than the shared-memory sort takes: the call says so
+    big = fd.Waveform(np.repeat(w.lmn, 70, axis=0), w.t_knots, 1024, f0=0.0, df=w.df)
+    k2 = torch.zeros((1, 70 * w.lmn.shape[0]), dtype=torch.uint8, device=wf.dev)
+    with pytest.raises(fd.FdemriError) as ei:
+        fd.fdemri_select_modes_rule(big.plan, d_amp, 1e-2, fd.FDEMRI_SELECT_CUMULATIVE, k2, n_keep)
+    assert ei.value.status == 5
+    big.close()
+    fd.fdemri_set_mode_mask(wf.plan, None)
+    wf.close()
