@@ -162,6 +162,19 @@ int fdemri_sum_inner(fdemri_plan_t plan, int n_angles, const double* theta_host,
                      const double* weight_dev, const double* data_plus_dev, const double* data_cross_dev, int hann,
                      double* hplus_dev, double* hcross_dev, double* inner_out_dev, void* cuda_stream);
 
+/* The time-domain voice sum of Eq. 1 / Eq. 2 from the splines of the last
+ * fdemri_build_splines: the signal whose Fourier transform (Eq. 3) the stationary-phase sum of fdemri_sum
+ * approximates, on the uniform time grid t_j = t0 + (double)j * dt, j = 0 .. n_samples - 1:
+ *     h(t) = h+ - i hx = sum_v A_v(t) Y_lm e^{-i Phi_v(t)}  +  [m > 0]  (-1)^(l+k) conj(A_v(t)) Y_l,-m e^{+i Phi_v(t)}.
+ * Samples outside [t_0, t_{N-1}) of the batch item's trajectory are 0.  Modes dropped by fdemri_set_mode_mask are
+ * left out.  (With N_s samples and Delta t = dt:  h~+(f_i) ~ N_s dt ifft(h+)_i  for f_i = i / (N_s dt): the sign
+ * convention of Eq. 3.)
+ *  theta_host, phi_host      as in fdemri_sum
+ *  hplus_td_dev, hcross_td_dev  [n_batch][n_samples] real FP64, fully overwritten
+ * One thread per sample, all voices in list order: the work is n_samples x n_modes (the paper's time-domain cost, L210). */
+int fdemri_td_sum(fdemri_plan_t plan, int n_angles, const double* theta_host, const double* phi_host, int64_t n_samples,
+                  double t0, double dt, double* hplus_td_dev, double* hcross_td_dev, void* cuda_stream);
+
 /* Mode selection by power threshold: per time step of the sparse trajectory the
  * modes are sorted by |A_lmkn(t)|^2 in descending order, a cumulative sum is formed, and the modes whose "additional
  * power" stays above "the threshold eps related to the total power emitted" contribute; "the selected modes are given

@@ -181,6 +181,26 @@ class Oracle:
                     n_evals=int(ne.value), nterms=nterms, ambiguous=amb, max_roots=int(mr.value))
 
 
+    def td(self, lmkn, t, Phi_phi, Phi_r, amp, n_samples, t0, dt, theta, phi, Phi_theta=None, n_threads=0):
+        """Eq. 1 / Eq. 2: the time-domain voice sum on t_j = t0 + j dt.  lmkn: [n_modes][4] (l, m, k, n) or [n_modes][3]
+        (l, m, n).  Returns (hplus, hcross) real arrays [n_samples]."""
+        lm = np.ascontiguousarray(lmkn, dtype=np.int32)
+        if lm.shape[1] == 3:
+            lm = np.ascontiguousarray(np.stack([lm[:, 0], lm[:, 1], np.zeros_like(lm[:, 0]), lm[:, 2]], axis=1))
+        t, tp = _d(t)
+        a1, p1 = _d(Phi_phi); a3, p3 = _d(Phi_r)
+        p2 = None
+        if Phi_theta is not None:
+            a2, p2 = _d(Phi_theta)
+        amp, ap = _d(amp)
+        hp = np.empty(int(n_samples)); hx = np.empty(int(n_samples))
+        rc = self.lib.fdemri_oracle_td(C.c_int(lm.shape[0]), lm.ctypes.data_as(_ip), C.c_int(t.shape[0]), tp, p1, p2, p3, ap,
+                                       C.c_int64(int(n_samples)), C.c_double(t0), C.c_double(dt), C.c_double(theta),
+                                       C.c_double(phi), hp.ctypes.data_as(_dp), hx.ctypes.data_as(_dp), C.c_int(n_threads))
+        if rc:
+            raise ValueError(f"fdemri_oracle_td -> {rc}")
+        return hp, hx
+
     def inner(self, hplus, hcross, dplus=None, dcross=None, w=None, hann=False):
         """Eq. 12 as a sum over the grid: (<h|h>, <d|h>) with <a|b> = sum_k w_k (a+ conj b+ + ax conj bx)."""
         hp = np.ascontiguousarray(hplus, dtype=np.complex128)

@@ -636,6 +636,65 @@ extern "C" int fdemri_oracle_waveform_kerr(int n_modes, const int32_t* lmkn, int
                     theta, phi, hplus, hcross, n_evals, nterms, ambiguous, max_roots, n_threads);
 }
 
+// Eq. 1 / Eq. 2 (L62-74): the time-domain voice sum, sample by sample, voice by voice.
+extern "C" int fdemri_oracle_td(int n_modes, const int32_t* lmkn, int n_knots, const double* t,
+                                const double* Phi_phi, const double* Phi_theta, const double* Phi_r, const double* amp,
+                                int64_t n_samples, double t0, double dt, double theta, double phi,
+                                double* hplus, double* hcross, int n_threads) {
+    if (!knots_ok(n_knots, t) || !lmkn || !Phi_phi || !Phi_r || !amp || n_modes < 0 || n_samples < 0 || !hplus || !hcross)
+        return 1;
+    const int N = n_knots, S = N - 1;
+    const size_t per = (size_t)S * 4;
+    KnotSystem ks(N, t);
+    std::vector<ld> sp(3 * per, 0.0L), am((size_t)n_modes * 2 * per);
+    ks.solve(Phi_phi, &sp[0 * per]);
+    ks.solve(Phi_r, &sp[1 * per]);
+    if (Phi_theta) ks.solve(Phi_theta, &sp[2 * per]);
+    std::vector<double> y(N);
+    std::vector<cld> Yp(n_modes), Ym(n_modes);
+    for (int v = 0; v < n_modes; ++v) {
+        const int l = lmkn[4 * v], m = lmkn[4 * v + 1], k = lmkn[4 * v + 2];
+        if (l < 2 || m < 0 || m > l || (k != 0 && !Phi_theta)) return 1;
+        for (int c = 0; c < 2; ++c) {
+            for (int q = 0; q < N; ++q) y[q] = amp[((size_t)v * N + q) * 2 + c];
+            ks.solve(y.data(), &am[((size_t)v * 2 + c) * per]);
+        }
+        Yp[v] = ylm_m2(l, m, theta, phi);
+        const ld sg = ((l + k) & 1) ? -1.0L : 1.0L;                      // (-1)^(l+k), R16
+        Ym[v] = (m > 0) ? sg * ylm_m2(l, -m, theta, phi) : cld(0.0L, 0.0L);
+    }
+#ifdef _OPENMP
+    omp_set_num_threads(n_threads > 0 ? n_threads : omp_get_num_procs());
+#endif
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < n_samples; ++j) {
+        const double tj = t0 + (double)j * dt;                           // the sample time as a double (product, then sum)
+        hplus[j] = 0.0; hcross[j] = 0.0;
+        if (!(tj >= t[0]) || !(tj < t[N - 1])) continue;                 // R14
+        int seg = (int)(std::upper_bound(t, t + N, tj) - t) - 1;
+        seg = std::min(std::max(seg, 0), S - 1);
+        const ld tau = (ld)tj - (ld)t[seg];
+        cld h(0.0L, 0.0L);
+        for (int v = 0; v < n_modes; ++v) {
+            const int m = lmkn[4 * v + 1], k = lmkn[4 * v + 2], n = lmkn[4 * v + 3];
+            ld cP[4];
+            for (int q = 0; q < 4; ++q)                                  // L103: coefficient-wise
+                cP[q] = (ld)m * sp[0 * per + 4 * seg + q] + (ld)n * sp[1 * per + 4 * seg + q] + (ld)k * sp[2 * per + 4 * seg + q];
+            const ld Phi = horner3(cP, tau);
+            ld cyc = Phi / TWO_PI_L;
+            cyc -= rintl(cyc);
+            const ld ang = TWO_PI_L * cyc;
+            const cld A(horner3(&am[((size_t)v * 2 + 0) * per + 4 * seg], tau), horner3(&am[((size_t)v * 2 + 1) * per + 4 * seg], tau));
+            const cld E(cosl(ang), -sinl(ang));                          // e^{-i Phi}
+            h += A * Yp[v] * E;
+            if (m > 0) h += std::conj(A) * Ym[v] * std::conj(E);
+        }
+        hplus[j] = (double)h.real();                                     // h = h+ - i hx (L64)
+        hcross[j] = (double)(-h.imag());
+    }
+    return 0;
+}
+
 extern "C" int fdemri_oracle_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

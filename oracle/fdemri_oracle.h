@@ -89,6 +89,18 @@ int fdemri_oracle_waveform_kerr(int n_modes, const int32_t* lmkn, int n_knots, c
 int fdemri_oracle_inner(int64_t n_freq, const double* w, const double* hplus, const double* hcross,
                         const double* dplus, const double* dcross, int hann, double* out);
 
+/* The time-domain voice sum the stationary-phase sum approximates (Eq. 1 / Eq. 2): on the uniform
+ * time grid t_j = t0 + j dt, j = 0..n_samples-1,
+ *     h(t) = h+ - i hx = sum over the list voices of  A_v(t) Y_lm e^{-i Phi_v(t)}
+ *                        + for m > 0 the implied partner (l,-m,-k,-n):  (-1)^(l+k) conj(A_v(t)) Y_l,-m e^{+i Phi_v(t)},
+ * with the not-a-knot splines of Phi_phi, Phi_r (, Phi_theta), Re A_v, Im A_v evaluated in long double, Phi_v formed
+ * coefficient-wise (L103).  Samples outside [t_0, t_{N-1}) are 0 (R14).  lmkn [n_modes][4] (l, m, k, n); Phi_theta may be
+ * NULL when every k is 0.  hplus, hcross: [n_samples] real. */
+int fdemri_oracle_td(int n_modes, const int32_t* lmkn, int n_knots, const double* t,
+                     const double* Phi_phi, const double* Phi_theta, const double* Phi_r, const double* amp,
+                     int64_t n_samples, double t0, double dt, double theta, double phi,
+                     double* hplus, double* hcross, int n_threads);
+
 int fdemri_oracle_num_threads(void);
 /* Test switch for pin P7: list voices stand for themselves only (m of either sign, no implied partner). */
 void fdemri_oracle_set_explicit(int on);

@@ -20,7 +20,7 @@ FDEMRI_FLAG_TIMING, FDEMRI_FLAG_BIN_MAJOR, FDEMRI_FLAG_TILE_MAJOR = 1, 2, 4
 STATUS = {0: "FDEMRI_OK", 1: "FDEMRI_ERR_INVALID_ARG", 2: "FDEMRI_ERR_WORKSPACE", 3: "FDEMRI_ERR_CUDA",
           4: "FDEMRI_ERR_NOT_BUILT", 5: "FDEMRI_ERR_UNSUPPORTED"}
 
-EXPORTS = ["fdemri_plan", "fdemri_plan_kerr", "fdemri_build_splines_kerr", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum", "fdemri_sum_inner", "fdemri_select_modes", "fdemri_select_modes_rule", "fdemri_set_mode_mask",
+EXPORTS = ["fdemri_plan", "fdemri_plan_kerr", "fdemri_build_splines_kerr", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum", "fdemri_td_sum", "fdemri_sum_inner", "fdemri_select_modes", "fdemri_select_modes_rule", "fdemri_set_mode_mask",
            "fdemri_get_stats", "fdemri_get_item_evals", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_measure_fp64_peak_3reg", "fdemri_measure_issue_ns", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
 
 
@@ -64,6 +64,9 @@ def lib() -> C.CDLL:
         L.fdemri_build_splines_kerr.argtypes = [vp, dp, dp, dp, dp, dp, dp, dp, vp]
         L.fdemri_sum.restype = C.c_int
         L.fdemri_sum.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), dp, dp, vp]
+        L.fdemri_td_sum.restype = C.c_int
+        L.fdemri_td_sum.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int64, C.c_double, C.c_double,
+                                    dp, dp, vp]
         L.fdemri_sum_inner.restype = C.c_int
         L.fdemri_sum_inner.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), dp, dp, dp, C.c_int, dp, dp, dp,
                                        vp]
@@ -163,6 +166,16 @@ def fdemri_sum(plan, theta, phi, hplus, hcross, stream=None):
     dp = C.POINTER(C.c_double)
     _chk("fdemri_sum", lib().fdemri_sum(plan, th.shape[0], th.ctypes.data_as(dp), ph.ctypes.data_as(dp), _ptr(hplus),
                                         _ptr(hcross), _stream_ptr(stream)))
+
+
+def fdemri_td_sum(plan, theta, phi, n_samples, t0, dt, hplus_td, hcross_td, stream=None):
+    """hplus_td, hcross_td: float64 CUDA tensors [n_batch][n_samples]."""
+    th = np.atleast_1d(np.asarray(theta, dtype=np.float64))
+    ph = np.atleast_1d(np.asarray(phi, dtype=np.float64))
+    assert th.shape == ph.shape
+    dp = C.POINTER(C.c_double)
+    _chk("fdemri_td_sum", lib().fdemri_td_sum(plan, th.shape[0], th.ctypes.data_as(dp), ph.ctypes.data_as(dp), int(n_samples),
+                                              float(t0), float(dt), _ptr(hplus_td), _ptr(hcross_td), _stream_ptr(stream)))
 
 
 def fdemri_sum_inner(plan, theta, phi, inner_out, weight=None, data_plus=None, data_cross=None, hann=False, hplus=None,

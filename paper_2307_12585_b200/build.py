@@ -9,7 +9,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libfdemri.so")
 SOURCES = ["fdemri.cu"]
-DEPS = ["fdemri.cu", "fdemri_common.cuh", "fdemri_map.cuh", "fdemri_splines.cuh", "fdemri_sum.cuh", "fdemri_select.cuh", "airy_tables.inc", "poly_tables.inc", os.path.join("..", "..", "include", "fdemri.h")]
+DEPS = ["fdemri.cu", "fdemri_common.cuh", "fdemri_map.cuh", "fdemri_splines.cuh", "fdemri_sum.cuh", "fdemri_td.cuh", "fdemri_select.cuh", "airy_tables.inc", "poly_tables.inc", os.path.join("..", "..", "include", "fdemri.h")]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "--fmad=true"]

@@ -19,6 +19,7 @@
 #include "fdemri_splines.cuh"
 #include "fdemri_select.cuh"
 #include "fdemri_sum.cuh"
+#include "fdemri_td.cuh"
 
 struct fdemri_plan_s {
     FdemriDims d;
@@ -384,19 +385,9 @@ extern "C" int fdemri_build_splines_kerr(fdemri_plan_t p, const double* f_phi, c
     return build_impl(p, f_phi, f_theta, f_r, Phi_phi, Phi_theta, Phi_r, amp, cuda_stream);
 }
 
-// S0 + S3 + S4 (+ the fused inner products when inner_out_dev is given)
-static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, const double* phi_host, double* hplus_dev,
-                       double* hcross_dev, const double* weight_dev, const double* dplus_dev, const double* dcross_dev,
-                       int hann, double* inner_out_dev, void* cuda_stream) {
-    if (!p || !theta_host || !phi_host) return FDEMRI_ERR_INVALID_ARG;
-    if ((hplus_dev == nullptr) != (hcross_dev == nullptr)) return FDEMRI_ERR_INVALID_ARG;
-    if (!hplus_dev && !inner_out_dev) return FDEMRI_ERR_INVALID_ARG;
-    if ((dplus_dev == nullptr) != (dcross_dev == nullptr)) return FDEMRI_ERR_INVALID_ARG;
-    if (!p->ws) return FDEMRI_ERR_WORKSPACE;
-    if (!p->built) return FDEMRI_ERR_NOT_BUILT;
+// S0: the viewing angles go through the plan's pinned buffer to the device, then k_weights.  Shared by the sums.
+static int stage_weights(fdemri_plan_t p, int n_angles, const double* theta_host, const double* phi_host, cudaStream_t st) {
     const FdemriDims& d = p->d;
-    if (n_angles != 1 && n_angles != d.n_batch) return FDEMRI_ERR_INVALID_ARG;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
     for (int i = 0; i < n_angles; ++i)
         if (!std::isfinite(theta_host[i]) || !std::isfinite(phi_host[i])) return FDEMRI_ERR_INVALID_ARG;
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
@@ -414,10 +405,29 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
         return FDEMRI_ERR_CUDA;
     // (a stream being captured into a CUDA graph: no event; a replay reads the buffer as the last call left it)
     p->last_stream_valid = cap == cudaStreamCaptureStatusNone && cudaEventRecord(p->ev_angles, st) == cudaSuccess;
-    // S0
-    int nw = n_angles * d.n_modes;
+    const int nw = n_angles * d.n_modes;
     k_weights<<<(nw + 127) / 128, 128, 0, st>>>(n_angles, d.n_modes, p->lmn_dev, p->k_dev, p->lm_index_dev, p->wmeta_dev, p->wcoef_dev,
                                                 p->angles, p->wts);
+    return FDEMRI_OK;
+}
+
+// S0 + S3 + S4 (+ the fused inner products when inner_out_dev is given)
+static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, const double* phi_host, double* hplus_dev,
+                       double* hcross_dev, const double* weight_dev, const double* dplus_dev, const double* dcross_dev,
+                       int hann, double* inner_out_dev, void* cuda_stream) {
+    if (!p || !theta_host || !phi_host) return FDEMRI_ERR_INVALID_ARG;
+    if ((hplus_dev == nullptr) != (hcross_dev == nullptr)) return FDEMRI_ERR_INVALID_ARG;
+    if (!hplus_dev && !inner_out_dev) return FDEMRI_ERR_INVALID_ARG;
+    if ((dplus_dev == nullptr) != (dcross_dev == nullptr)) return FDEMRI_ERR_INVALID_ARG;
+    if (!p->ws) return FDEMRI_ERR_WORKSPACE;
+    if (!p->built) return FDEMRI_ERR_NOT_BUILT;
+    const FdemriDims& d = p->d;
+    if (n_angles != 1 && n_angles != d.n_batch) return FDEMRI_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    {
+        const int rc = stage_weights(p, n_angles, theta_host, phi_host, st);
+        if (rc != FDEMRI_OK) return rc;
+    }
     // reset the per-sum counters: n_airy (slot 4), the tile counter (6), n_slow (7), n_pairs (8), the sum's flags (9)
     if (cudaMemsetAsync(p->stats + 4, 0, sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
     if (cudaMemsetAsync(p->stats + 6, 0, 4 * sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
@@ -475,6 +485,24 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
         if (cudaGetLastError() != cudaSuccess) return FDEMRI_ERR_CUDA;
     }
     return FDEMRI_OK;
+}
+
+extern "C" int fdemri_td_sum(fdemri_plan_t p, int n_angles, const double* theta_host, const double* phi_host, int64_t n_samples,
+                             double t0, double dt, double* hplus_td_dev, double* hcross_td_dev, void* cuda_stream) {
+    if (!p || !theta_host || !phi_host || !hplus_td_dev || !hcross_td_dev || n_samples < 1 || !(dt > 0.0) ||
+        !std::isfinite(t0) || !std::isfinite(dt))
+        return FDEMRI_ERR_INVALID_ARG;
+    if (!p->ws) return FDEMRI_ERR_WORKSPACE;
+    if (!p->built) return FDEMRI_ERR_NOT_BUILT;
+    const FdemriDims& d = p->d;
+    if (n_angles != 1 && n_angles != d.n_batch) return FDEMRI_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int rc = stage_weights(p, n_angles, theta_host, phi_host, st);
+    if (rc != FDEMRI_OK) return rc;
+    const dim3 grid((unsigned)((n_samples + 255) / 256), (unsigned)d.n_batch);
+    k_td_sum<<<grid, 256, 0, st>>>(d, p->rec, p->t_knots_dev, p->wts, n_angles, p->mode_mask, (long long)n_samples, t0, dt,
+                                   hplus_td_dev, hcross_td_dev);
+    return cudaGetLastError() == cudaSuccess ? FDEMRI_OK : FDEMRI_ERR_CUDA;
 }
 
 extern "C" int fdemri_sum(fdemri_plan_t p, int n_angles, const double* theta_host, const double* phi_host,

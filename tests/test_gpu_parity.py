@@ -925,3 +925,74 @@ def test_mode_selection_cumulative_cut(fd, orc):
     big.close()
     fd.fdemri_set_mode_mask(wf.plan, None)
     wf.close()
+
+
+# ---- the time-domain voice sum of Eq. 1 / Eq. 2: fdemri_td_sum ---------------------------------
+def test_td_sum_parity_and_fd_against_fft_of_td(fd, orc):
+    """(1) fdemri_td_sum element by element against the oracle's time-domain sum (fdemri_oracle_td) on a 2^19-sample
+    case with nine voices (F < 0, m = 0 and turnover voices among them), on a ragged general-voice case with two batch
+    items and per-item angles, and with a mode mask.  (2) On the box, the check the paper makes (L141-147): the
+    frequency-domain waveform of fdemri_sum against the FFT of the time-domain one (cuFFT through torch.fft, Eq. 3's sign:
+    N dt ifft), mismatch with and without the Hann window, at the levels of the oracle's own convention check P6."""
+    import dataclasses
+    import torch
+    from paper_2307_12585_b200 import synth
+    N, dt = 2 ** 19, 10.0
+    modes = [(2, 2, 0), (2, 1, 1), (2, 2, -2), (3, 0, 2), (3, 3, -1), (2, 1, -4), (4, 2, 1), (2, 0, -1), (3, 1, -2)]
+    w = synth.small_case(seed=3, n_knots=24, n_freq=N // 2 + 1, modes=modes, T_s=N * dt)
+    wf = fd.waveform_from_workload(w)
+    wf.sum(w.theta, w.phi)
+    Hp, Hx = wf.result()
+    tp = torch.full((1, N), float("nan"), dtype=torch.float64, device=wf.dev)
+    tx = torch.full_like(tp, float("nan"))
+    fd.fdemri_td_sum(wf.plan, w.theta, w.phi, N, 0.0, dt, tp, tx)
+    torch.cuda.synchronize()
+    ref_p, ref_x = orc.td(w.lmn, w.t_knots[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0], N, 0.0, dt, w.theta, w.phi)
+    scale = max(np.abs(ref_p).max(), np.abs(ref_x).max())
+    err = max(np.abs(tp.cpu().numpy()[0] - ref_p).max(), np.abs(tx.cpu().numpy()[0] - ref_x).max()) / scale
+    print(f"[parity] time-domain sum, 2^19 samples x 9 voices: max|dh|/max|h| = {err:.3e}")
+    assert err <= TOL_BIN
+    # (2) FD against N dt ifft(TD), on the device
+    win = 0.5 * (1.0 - torch.cos(2.0 * math.pi * torch.arange(N, dtype=torch.float64, device=wf.dev) / N))
+    fft = lambda x: (N * dt * torch.fft.ifft(x)).cpu().numpy()[: N // 2 + 1]
+    sl = slice(1, N // 2)
+    m_raw = one_minus_overlap(Hp[0][sl], Hx[0][sl], fft(tp[0])[sl], fft(tx[0])[sl])
+    filt = lambda H: 0.5 * H[1:-1] - 0.25 * H[:-2] - 0.25 * H[2:]
+    m_win = one_minus_overlap(filt(Hp[0]), filt(Hx[0]), fft(tp[0] * win)[1:-1], fft(tx[0] * win)[1:-1])
+    print(f"[fd vs fft(td)] mismatch without window {m_raw:.3e}, with the Hann window {m_win:.3e} (paper, one system: 8e-4 -> 4e-6, L147)")
+    assert m_raw < 1e-2 and m_win < 2e-3 and m_win < m_raw
+    assert one_minus_overlap(np.conj(Hp[0][sl]), Hx[0][sl], fft(tp[0])[sl], fft(tx[0])[sl]) > 0.2
+    # with a mode mask: the masked voices are left out of the time-domain sum too
+    keep = torch.ones((1, len(modes)), dtype=torch.uint8, device=wf.dev)
+    keep[0, 1] = 0; keep[0, 4] = 0
+    fd.fdemri_set_mode_mask(wf.plan, keep)
+    wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)
+    a = torch.empty((1, 4096), dtype=torch.float64, device=wf.dev); b = torch.empty_like(a)
+    fd.fdemri_td_sum(wf.plan, w.theta, w.phi, 4096, 1.0e5, 777.0, a, b)
+    torch.cuda.synchronize()
+    sel = [i for i in range(len(modes)) if i not in (1, 4)]
+    rp, rx = orc.td(w.lmn[sel], w.t_knots[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0][sel], 4096, 1.0e5, 777.0, w.theta, w.phi)
+    assert max(np.abs(a.cpu().numpy()[0] - rp).max(), np.abs(b.cpu().numpy()[0] - rx).max()) <= TOL_BIN * scale
+    fd.fdemri_set_mode_mask(wf.plan, None)
+    wf.close()
+    # general voices, two batch items, per-item angles, a grid that starts before t_0 and runs past t_{N-1}
+    modes4 = ((2, 2, 1, 0), (2, 1, -1, 1), (3, 2, 3, -2), (3, 3, -3, 1), (4, 1, 2, 0), (2, 0, 1, -1))
+    a_ = synth.small_case_kerr(seed=8, n_knots=16, modes=modes4)
+    b_ = synth.small_case_kerr(seed=9, n_knots=16, modes=modes4)
+    cat = lambda x, y: np.concatenate([x, y], axis=0)
+    w2 = dataclasses.replace(a_, t_knots=cat(a_.t_knots, b_.t_knots), f_phi=cat(a_.f_phi, b_.f_phi), f_r=cat(a_.f_r, b_.f_r),
+                             Phi_phi=cat(a_.Phi_phi, b_.Phi_phi), Phi_r=cat(a_.Phi_r, b_.Phi_r), amp=cat(a_.amp, b_.amp),
+                             f_theta=cat(a_.f_theta, b_.f_theta), Phi_theta=cat(a_.Phi_theta, b_.Phi_theta))
+    wf2 = fd.waveform_from_workload(w2)
+    ns, t0s, dts = 5001, -3.0e4, 613.7
+    th, ph = np.array([0.7, 2.2]), np.array([-1.0, 0.4])
+    o1 = torch.empty((2, ns), dtype=torch.float64, device=wf2.dev); o2 = torch.empty_like(o1)
+    fd.fdemri_td_sum(wf2.plan, th, ph, ns, t0s, dts, o1, o2)
+    torch.cuda.synchronize()
+    for i in range(2):
+        rp, rx = orc.td(w2.lmkn, w2.t_knots[i], w2.Phi_phi[i], w2.Phi_r[i], w2.amp[i], ns, t0s, dts, float(th[i]), float(ph[i]),
+                        Phi_theta=w2.Phi_theta[i])
+        sc = max(np.abs(rp).max(), np.abs(rx).max())
+        e = max(np.abs(o1.cpu().numpy()[i] - rp).max(), np.abs(o2.cpu().numpy()[i] - rx).max()) / sc
+        assert e <= TOL_BIN and np.all(o1.cpu().numpy()[i][rp == 0] == 0) and (rp == 0).sum() > 40
+    wf2.close()

@@ -308,3 +308,50 @@ def test_kerr_brute_force_fft(orc):
     lm0 = w.lmkn.copy(); lm0[:, 2] = 0
     bad = _run_kerr(orc, w, lmkn=lm0)
     assert one_minus_overlap(filt(bad["hplus"]), filt(bad["hcross"]), Hpw[1:-1], Hxw[1:-1]) > 0.2
+
+
+# ---- the time-domain voice sum (Eq. 1 / Eq. 2) of the oracle -----------------------------------------------------
+def test_td_sum_against_numpy_and_fft(orc):
+    """fdemri_oracle_td (long double, C++) against the plain numpy sum with scipy's not-a-knot splines used by P6 above
+    (phases reach 1e5 rad, so the double-precision scipy splines limit the agreement to ~1e-10); zero outside
+    [t_0, t_{N-1}); h+ = Re h, hx = -Im h; and the FFT of the oracle's own time series against its own stationary-phase
+    sum at the convention-check level of P6 (Hann-filtered mismatch < 2e-3)."""
+    w, N, dt = _td_case()
+    h = _td_waveform(w, N, dt, TH, PH, orc)
+    hp, hx = orc.td(w.lmn, w.t_knots[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0], N, 0.0, dt, TH, PH)
+    scale = np.abs(h).max()
+    assert np.max(np.abs(hp - h.real)) < 3e-10 * scale and np.max(np.abs(hx + h.imag)) < 3e-10 * scale
+    # samples before t_0 and from t_{N-1} on are exactly zero; inside they are not
+    hp2, hx2 = orc.td(w.lmn, w.t_knots[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0], 64, -20 * dt, dt, TH, PH)
+    assert np.all(hp2[:20] == 0) and np.all(hx2[:20] == 0) and np.all(hp2[20:] != 0)
+    T = w.t_knots[0][-1]
+    hp3, _ = orc.td(w.lmn, w.t_knots[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0], 8, T - 4 * dt, dt, TH, PH)
+    assert np.all(hp3[:4] != 0) and np.all(hp3[4:] == 0)
+    # Eq. 3 convention and the Hann filter, now from the oracle's own time series
+    out = orc.waveform(w.lmn, w.t_knots[0], w.f_phi[0], w.f_r[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0], w.freq_array(), TH, PH)
+    hann = 0.5 * (1 - np.cos(2 * np.pi * np.arange(N) / N))
+    Hpw = (N * dt * np.fft.ifft(hp * hann))[: N // 2 + 1]
+    Hxw = (N * dt * np.fft.ifft(hx * hann))[: N // 2 + 1]
+    filt = lambda H: 0.5 * H[1:-1] - 0.25 * H[:-2] - 0.25 * H[2:]
+    assert one_minus_overlap(filt(out["hplus"]), filt(out["hcross"]), Hpw[1:-1], Hxw[1:-1]) < 2e-3
+
+
+def test_td_sum_general_voices(orc):
+    """The k Phi_theta term and the (-1)^(l+k) of the partner in the time-domain sum: against the numpy sum of
+    test_kerr_brute_force_fft's kind on a small case."""
+    w = synth.small_case_kerr(seed=3, n_knots=16, n_freq=1024)
+    t = w.t_knots[0]
+    N, dt = 4096, t[-1] / 4096
+    tj = np.arange(N) * dt
+    sp = lambda y: CubicSpline(t, y, bc_type="not-a-knot")(tj)
+    Pp, Pt, Pr = sp(w.Phi_phi[0]), sp(w.Phi_theta[0]), sp(w.Phi_r[0])
+    h = np.zeros(N, complex)
+    for v, (l, m, k, n) in enumerate(w.lmkn):
+        A = sp(w.amp[0, v, :, 0]) + 1j * sp(w.amp[0, v, :, 1])
+        Phi = m * Pp + k * Pt + n * Pr
+        h += A * orc.ylm(int(l), int(m), TH, PH) * np.exp(-1j * Phi)
+        if m > 0:
+            h += (-1) ** (l + k) * np.conj(A) * orc.ylm(int(l), -int(m), TH, PH) * np.exp(+1j * Phi)
+    hp, hx = orc.td(w.lmkn, t, w.Phi_phi[0], w.Phi_r[0], w.amp[0], N, 0.0, dt, TH, PH, Phi_theta=w.Phi_theta[0])
+    scale = np.abs(h).max()
+    assert np.max(np.abs(hp - h.real)) < 3e-10 * scale and np.max(np.abs(hx + h.imag)) < 3e-10 * scale
