@@ -996,3 +996,25 @@ def test_td_sum_parity_and_fd_against_fft_of_td(fd, orc):
         e = max(np.abs(o1.cpu().numpy()[i] - rp).max(), np.abs(o2.cpu().numpy()[i] - rx).max()) / sc
         assert e <= TOL_BIN and np.all(o1.cpu().numpy()[i][rp == 0] == 0) and (rp == 0).sum() > 40
     wf2.close()
+
+
+def test_interleaved_builds_of_plans_with_different_knot_counts(fd, orc):
+    """The dynamic shared-memory limit of the spline kernels is an attribute of the kernel, not of a plan: two live plans
+    with 150 and 40 knots (and one with 400), built in turn and again, must all keep working (round-1 advice)."""
+    from paper_2307_12585_b200 import synth
+    cases = [synth.small_case(seed=21, n_knots=150, n_freq=20000), synth.small_case(seed=22, n_knots=40, n_freq=20000),
+             synth.small_case(seed=23, n_knots=400, n_freq=20000)]
+    wfs = [fd.Waveform(w.lmn, w.t_knots, w.n_freq, f0=w.f0, df=w.df) for w in cases]
+    refs = [oracle_c(orc, w, w.freq_array()) for w in cases]
+    for order in ((0, 1, 2), (1, 0, 2), (2, 1, 0)):
+        for i in order:
+            w, wf = cases[i], wfs[i]
+            wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)
+        for i in order:
+            w, wf = cases[i], wfs[i]
+            wf.sum(w.theta, w.phi)
+            hp, hx = wf.result()
+            check(hp[0], hx[0], refs[i], f"plan with {w.n_knots} knots, build order {order}")
+            assert wf.stats()["n_evals"] == refs[i]["n_evals"]
+    for wf in wfs:
+        wf.close()
