@@ -248,12 +248,18 @@ __device__ __noinline__ FdemriSlowOut fdemri_term_slow(const double* it, double 
         tau = fmin(fmax(tau, 0.0), h);
         double dG = 0.0, c2 = 0.0;
         int n = 0;
+        double prev = h;
         for (; n < 60; ++n) {
             const double b2 = fma(tau, FD, FC), b1 = fma(tau, b2, FB), G = fma(tau, b1, -x);
             c2 = fma(tau, FD, b2); dG = fma(tau, c2, b1);
             const double delta = G / dG;
             if (!(fabs(delta) > 1e-14 * h)) { if (fabs(delta) <= h) tau -= delta; break; }
-            tau = fmin(fmax(tau - delta, 0.0), h);
+            const double tn = fmin(fmax(tau - delta, 0.0), h);
+            // no progress any more: the root sits on an end of the segment (the step is clamped away), or the step has
+            // reached its rounding floor -- the iterate is as good as it gets
+            if (tn == tau || (fabs(delta) >= prev && fabs(delta) <= 1e-9 * h)) { tau = tn; break; }
+            prev = fabs(delta);
+            tau = tn;
         }
         if (n == 60) out.info |= (8u << 4);
         tau = fmin(fmax(tau, 0.0), h);
@@ -274,6 +280,7 @@ __device__ __noinline__ FdemriSlowOut fdemri_term_slow(const double* it, double 
         if (0.5 * (ta + tb) < te) z = -z;
         const double tol = 1e-14 * h;
         int n = 0;
+        double prev = h;
         for (; n < 40; ++n) {
             const double H = fma(z * z, fma(FD, z, c2), -Delta);
             const double dH = z * fma(3.0 * FD, z, 2.0 * c2);
@@ -281,6 +288,8 @@ __device__ __noinline__ FdemriSlowOut fdemri_term_slow(const double* it, double 
             const double delta = H / dH;
             z -= delta;
             if (fabs(delta) <= tol) break;
+            if (fabs(delta) >= prev && fabs(delta) <= 1e-9 * h) break;       // rounding floor of the step
+            prev = fabs(delta);
         }
         if (n == 40) out.info |= (8u << 4);
         tau = fmin(fmax(te + z, ta), tb);

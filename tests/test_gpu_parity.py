@@ -414,7 +414,7 @@ def test_random_small_cases_sweep(fd, orc):
         wf.sum(w.theta, w.phi)
         hp, hx = wf.result()
         st = wf.stats()
-        assert st["status"] == 0 and (st["flags"] & ~8) == 0     # (8 = FDEMRI_BAD_NEWTON: informational, parity decides)
+        assert st["status"] == 0 and (st["flags"] & ~8) == 0     # (8 = FDEMRI_BAD_NEWTON: counted below)
         newton += bool(st["flags"] & 8)
         ref = oracle_c(orc, w, w.freq_array())
         assert st["n_evals"] == ref["n_evals"], (case, modes)
@@ -430,6 +430,7 @@ def test_random_small_cases_sweep(fd, orc):
             worst = max(worst, err)
         wf.close()
     print(f"[parity] 20 random small cases: worst max|dh|/max|h| = {worst:.3e}; iteration cap reported in {newton} of them")
+    assert newton == 0
 
 
 @pytest.mark.parametrize("mode", ["bin", "tile"])
