@@ -973,7 +973,9 @@ struct FdemriBinWarpQ {
     uint2 reg[FDEMRI_BREG];          // {key, first bin | last bin << 8, both relative to the block}
 };
 struct FdemriBinSmem {
+#ifdef FDEMRI_BIN_STAGE_SMEM
     double stage[FDEMRI_BIN_WARPS * 32 * FDEMRI_BIN_STRIDE];
+#endif
     double4 acc[FDEMRI_BIN_BLOCK];
     FdemriBinWarpQ wq[FDEMRI_BIN_WARPS];
     unsigned short wlist[FDEMRI_BIN_WARPS][64];
@@ -996,7 +998,9 @@ __global__ void __launch_bounds__(FDEMRI_BIN_WARPS * 32, 2) k_bin_sum(SumArgs a)
     const FdemriDims& d = a.d;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
+#ifdef FDEMRI_BIN_STAGE_SMEM
     double* it = sm->stage + ((size_t)wid * 32 + lane) * FDEMRI_BIN_STRIDE;
+#endif
     const int V = d.n_modes, S = d.n_seg, Sp = 32 * d.n_groups, NB = d.tile_bins;     // NB <= FDEMRI_BIN_BLOCK
     const int part = ((2 * V + FDEMRI_BIN_WARPS - 1) / FDEMRI_BIN_WARPS + 31) & ~31;     // voice-signs per warp
     unsigned n_airy = 0, n_slow = 0, errs = 0;
@@ -1041,19 +1045,33 @@ __global__ void __launch_bounds__(FDEMRI_BIN_WARPS * 32, 2) k_bin_sum(SumArgs a)
                         const int vsbr = (int)(key / (unsigned)Sp), seg = (int)(key - (unsigned)vsbr * (unsigned)Sp);
                         const int vs = vsbr / 3, br = vsbr - 3 * vs;
                         const int v = vs >> 1;
+#ifdef FDEMRI_BIN_STAGE_SMEM
                         fdemri_stage_item(it, a.rec + (rbase + (size_t)v * S + seg) * R_DOUBLES, a.wts[wbase + v], 0, 0,
                                           (unsigned)(vs & 1), (unsigned)br);
-                        const unsigned flags = (unsigned)(*reinterpret_cast<const int2*>(it)).y;
+                        const double* item = it;
+#else
+                        // the lane's item stays in registers (every index below is a constant after inlining); only the
+                        // rare slow path gets a copy in shared memory, which its out-of-line function reads
+                        __align__(16) double item[S_DOUBLES];
+                        fdemri_stage_item(item, a.rec + (rbase + (size_t)v * S + seg) * R_DOUBLES, a.wts[wbase + v], 0, 0,
+                                          (unsigned)(vs & 1), (unsigned)br);
+#endif
+                        const unsigned flags = (unsigned)(*reinterpret_cast<const int2*>(item)).y;
                         const double sf = fdemri_xorsign(f, (flags & 4u) << 29);
                         double Tr = 0.0, Ti = 0.0;
                         bool ok = false;
-                        if (!(flags & 1u)) ok = fdemri_term_fast(it, sf, Tr, Ti);
+                        if (!(flags & 1u)) ok = fdemri_term_fast(item, sf, Tr, Ti);
                         if (!ok) {
+#ifndef FDEMRI_BIN_STAGE_SMEM
+                            __align__(16) double it[S_DOUBLES];          // a copy on the thread's stack (local memory)
+#pragma unroll
+                            for (int q = 0; q < S_DOUBLES; ++q) it[q] = item[q];
+#endif
                             const FdemriSlowOut o = fdemri_term_slow(it, sf, flags);
                             Tr = o.tre; Ti = o.tim;
                             n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
                         }
-                        a0 = fma(it[S_WP], Tr, a0); a1 = fma(it[S_SWP], Ti, a1); a2 = fma(it[S_NWX], Ti, a2); a3 = fma(it[S_SWX], Tr, a3);
+                        a0 = fma(item[S_WP], Tr, a0); a1 = fma(item[S_SWP], Ti, a1); a2 = fma(item[S_NWX], Ti, a2); a3 = fma(item[S_SWX], Tr, a3);
                         ++n_acc;
                     }
                     wl_head += (unsigned)nl;
