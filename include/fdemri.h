@@ -16,8 +16,8 @@
  * Conventions
  *   - "dev" pointers are CUDA device pointers, "host" pointers are host pointers.  The caller owns every
  *     buffer, including the work space; the plan owns only small host metadata.
- *   - No call allocates device memory except the two fdemri_measure_* microbenchmarks (8 bytes, freed before they
- *     return); a plan owns a small pinned host buffer.  build_splines / sum do not synchronise: they enqueue
+ *   - No call allocates device memory except the fdemri_measure_* microbenchmarks (8 bytes, freed before they
+ *     return); a plan owns a small pinned host buffer (fdemri_select_modes_static needs neither plan nor work space).  build_splines / sum do not synchronise: they enqueue
  *     kernels on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default stream).
  *     build_splines runs one of its kernels on a stream of the plan, forked from and joined back into
  *     `cuda_stream` with events, so ordering on `cuda_stream` is all a caller needs.
@@ -39,7 +39,8 @@ enum {
     FDEMRI_ERR_WORKSPACE = 2,   /* work space missing or smaller than fdemri_workspace_bytes                        */
     FDEMRI_ERR_CUDA = 3,        /* a CUDA runtime call or kernel failed                                   */
     FDEMRI_ERR_NOT_BUILT = 4,   /* fdemri_sum / get_coeffs before fdemri_build_splines                    */
-    FDEMRI_ERR_UNSUPPORTED = 5  /* the call is not available in this configuration (not returned at present)   */
+    FDEMRI_ERR_UNSUPPORTED = 5, /* the call is not available in this configuration                                 */
+    FDEMRI_ERR_STATIC_SCRATCH = 6 /* fdemri_select_modes_static: n_batch * n_knots > FDEMRI_STATIC_MAX_TOTALS         */
 };
 
 /* plan flags */
@@ -196,6 +197,23 @@ int fdemri_select_modes_rule(fdemri_plan_t plan, const double* amp_dev, double e
                              int32_t* n_keep_dev, void* cuda_stream);
 int fdemri_select_modes(fdemri_plan_t plan, const double* amp_dev, double eps, unsigned char* keep_dev,
                         int32_t* n_keep_dev, void* cuda_stream);
+/* fdemri_select_modes (FDEMRI_SELECT_OWN_POWER) for callers that cannot allocate device memory or hold a plan: code
+ * between other work under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  No plan, no work
+ * space: the [n_batch][n_knots] scratch of total powers is a static device array inside the library
+ * (FDEMRI_STATIC_MAX_TOTALS doubles = 256 KB, held by every GPU that loads the library until the process exits).  The
+ * call allocates nothing on the device or the host (no cudaMalloc / cudaFree / cudaHostAlloc, no plan): its first use
+ * on a device asks the runtime for the array's address, later calls only enqueue one memset of n_keep_dev and two
+ * kernels on cuda_stream.
+ *  n_batch, n_modes, n_knots  >= 1;  n_batch * n_knots <= FDEMRI_STATIC_MAX_TOTALS, else FDEMRI_ERR_STATIC_SCRATCH
+ *                             (nothing is enqueued); devices with ordinal >= FDEMRI_STATIC_MAX_DEVICES:
+ *                             FDEMRI_ERR_UNSUPPORTED
+ *  amp_dev, eps, keep_dev, n_keep_dev, cuda_stream   as in fdemri_select_modes; results are bit-identical to it.
+ * Every call on a device shares the one array, which keeps the last call's totals (a call overwrites all it reads, so
+ * nothing has to be cleared but n_keep_dev, which the call clears): two calls that overlap on the GPU -- different
+ * streams, or the same graph launched twice concurrently -- race.  Serialise them (one stream, or events). */
+enum { FDEMRI_STATIC_MAX_TOTALS = 32768, FDEMRI_STATIC_MAX_DEVICES = 64 };
+int fdemri_select_modes_static(int n_batch, int n_modes, int n_knots, const double* amp_dev, double eps,
+                               unsigned char* keep_dev, int32_t* n_keep_dev, void* cuda_stream);
 /* Modes with keep_dev[b][v] == 0 get no entries in the next fdemri_build_splines and so never reach the sum.
  * keep_dev is borrowed until it is replaced or the plan is destroyed (every later build reads it, from a kernel that
  * runs after the call has returned); NULL: every mode of the list is summed.  The mode list of the plan is unchanged. */

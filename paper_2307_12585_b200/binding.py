@@ -18,9 +18,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 FDEMRI_OK = 0
 FDEMRI_FLAG_TIMING, FDEMRI_FLAG_BIN_MAJOR, FDEMRI_FLAG_TILE_MAJOR = 1, 2, 4
 STATUS = {0: "FDEMRI_OK", 1: "FDEMRI_ERR_INVALID_ARG", 2: "FDEMRI_ERR_WORKSPACE", 3: "FDEMRI_ERR_CUDA",
-          4: "FDEMRI_ERR_NOT_BUILT", 5: "FDEMRI_ERR_UNSUPPORTED"}
+          4: "FDEMRI_ERR_NOT_BUILT", 5: "FDEMRI_ERR_UNSUPPORTED", 6: "FDEMRI_ERR_STATIC_SCRATCH"}
+FDEMRI_STATIC_MAX_TOTALS = 32768
 
-EXPORTS = ["fdemri_plan", "fdemri_plan_kerr", "fdemri_build_splines_kerr", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum", "fdemri_td_sum", "fdemri_sum_inner", "fdemri_select_modes", "fdemri_select_modes_rule", "fdemri_set_mode_mask",
+EXPORTS = ["fdemri_plan", "fdemri_plan_kerr", "fdemri_build_splines_kerr", "fdemri_workspace_bytes", "fdemri_workspace_bytes_min", "fdemri_set_workspace", "fdemri_build_splines", "fdemri_sum", "fdemri_td_sum", "fdemri_sum_inner", "fdemri_select_modes", "fdemri_select_modes_rule", "fdemri_select_modes_static", "fdemri_set_mode_mask",
            "fdemri_get_stats", "fdemri_get_item_evals", "fdemri_get_coeffs", "fdemri_get_kernel_ms", "fdemri_measure_fp64_peak", "fdemri_measure_fp64_peak_3reg", "fdemri_measure_issue_ns", "fdemri_destroy", "fdemri_strerror", "fdemri_version"]
 
 
@@ -74,6 +75,8 @@ def lib() -> C.CDLL:
         L.fdemri_select_modes.argtypes = [vp, dp, C.c_double, vp, vp, vp]
         L.fdemri_select_modes_rule.restype = C.c_int
         L.fdemri_select_modes_rule.argtypes = [vp, dp, C.c_double, C.c_int, vp, vp, vp]
+        L.fdemri_select_modes_static.restype = C.c_int
+        L.fdemri_select_modes_static.argtypes = [C.c_int, C.c_int, C.c_int, dp, C.c_double, vp, vp, vp]
         L.fdemri_set_mode_mask.restype = C.c_int
         L.fdemri_set_mode_mask.argtypes = [vp, vp]
         L.fdemri_get_stats.restype = C.c_int
@@ -206,6 +209,19 @@ def fdemri_select_modes_rule(plan, amp, eps, rule, keep, n_keep, stream=None):
     assert n_keep.is_cuda and n_keep.is_contiguous() and n_keep.element_size() == 4
     _chk("fdemri_select_modes_rule", lib().fdemri_select_modes_rule(plan, _ptr(amp), float(eps), int(rule), C.c_void_p(keep.data_ptr()),
                                                                     C.c_void_p(n_keep.data_ptr()), _stream_ptr(stream)))
+
+
+def fdemri_select_modes_static(amp, eps, keep, n_keep, stream=None):
+    """fdemri_select_modes without a plan or a work space: the scratch is a static device array of the library, so the call
+    allocates nothing (include/fdemri.h).  amp: float64 CUDA tensor [n_batch][n_modes][n_knots][2]; keep, n_keep as there.
+    Raises FdemriError(FDEMRI_ERR_STATIC_SCRATCH) when n_batch * n_knots > FDEMRI_STATIC_MAX_TOTALS."""
+    assert amp.dim() == 4 and amp.shape[3] == 2
+    n_batch, n_modes, n_knots = (int(x) for x in amp.shape[:3])
+    assert keep.is_cuda and keep.is_contiguous() and keep.element_size() == 1 and keep.numel() == n_batch * n_modes
+    assert n_keep.is_cuda and n_keep.is_contiguous() and n_keep.element_size() == 4 and n_keep.numel() == n_batch
+    _chk("fdemri_select_modes_static", lib().fdemri_select_modes_static(n_batch, n_modes, n_knots, _ptr(amp), float(eps),
+                                                                        C.c_void_p(keep.data_ptr()), C.c_void_p(n_keep.data_ptr()),
+                                                                        _stream_ptr(stream)))
 
 
 def fdemri_set_mode_mask(plan, keep):

@@ -10,6 +10,7 @@
 #include <cstdlib>
 #include <algorithm>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <unordered_map>
 #include <vector>
@@ -554,6 +555,48 @@ extern "C" int fdemri_select_modes(fdemri_plan_t p, const double* amp_dev, doubl
     return fdemri_select_modes_rule(p, amp_dev, eps, FDEMRI_SELECT_OWN_POWER, keep_dev, n_keep_dev, cuda_stream);
 }
 
+// ---- mode selection for callers that cannot allocate (fdemri.h: fdemri_select_modes_static) ----------------------
+// The [n_batch][n_knots] scratch of total powers that fdemri_select_modes keeps in the caller's work space lives here in
+// a file-scope device array: every GPU that loads the library holds FDEMRI_STATIC_MAX_TOTALS doubles (256 KB) until the
+// process exits.  In host code the array's name is a stand-in of the host side, not a device address: the address the
+// kernels get comes from cudaGetSymbolAddress, asked once per device with that device current.
+static __device__ __align__(256) double g_select_total_static[FDEMRI_STATIC_MAX_TOTALS];
+
+static int select_static_scratch(double** out) {
+    static std::mutex mu;
+    static double* ptr_of_device[FDEMRI_STATIC_MAX_DEVICES] = {};
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    if (dev < 0 || dev >= FDEMRI_STATIC_MAX_DEVICES) return FDEMRI_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr_of_device[dev]) {
+        void* q = nullptr;
+        if (cudaGetSymbolAddress(&q, g_select_total_static) != cudaSuccess || !q) return FDEMRI_ERR_CUDA;
+        ptr_of_device[dev] = static_cast<double*>(q);
+    }
+    *out = ptr_of_device[dev];
+    return FDEMRI_OK;
+}
+
+extern "C" int fdemri_select_modes_static(int n_batch, int n_modes, int n_knots, const double* amp_dev, double eps,
+                                          unsigned char* keep_dev, int32_t* n_keep_dev, void* cuda_stream) {
+    if (n_batch < 1 || n_modes < 1 || n_knots < 1 || !amp_dev || !keep_dev || !n_keep_dev || !(eps >= 0.0))
+        return FDEMRI_ERR_INVALID_ARG;
+    if ((int64_t)n_batch * n_knots > FDEMRI_STATIC_MAX_TOTALS) return FDEMRI_ERR_STATIC_SCRATCH;
+    const size_t n = (size_t)n_batch * n_modes;
+    if ((n + 127) / 128 > 0x7fffffffu) return FDEMRI_ERR_INVALID_ARG;
+    double* total = nullptr;
+    const int rc = select_static_scratch(&total);
+    if (rc != FDEMRI_OK) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    /* n_keep is accumulated with atomicAdd and must start at zero; the totals this call reads are all written by
+       k_select_total first, so what the last call left in the scratch is never seen */
+    if (cudaMemsetAsync(n_keep_dev, 0, (size_t)n_batch * sizeof(int32_t), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
+    k_select_total<<<n_batch * n_knots, 256, 0, st>>>(n_modes, n_knots, amp_dev, total);
+    k_select_keep<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(n_batch, n_modes, n_knots, amp_dev, total, eps, keep_dev, n_keep_dev);
+    return cudaGetLastError() == cudaSuccess ? FDEMRI_OK : FDEMRI_ERR_CUDA;
+}
+
 extern "C" int fdemri_set_mode_mask(fdemri_plan_t p, const unsigned char* keep_dev) {
     if (!p) return FDEMRI_ERR_INVALID_ARG;
     p->mode_mask = keep_dev;
@@ -794,6 +837,7 @@ extern "C" const char* fdemri_strerror(int status) {
         case FDEMRI_ERR_CUDA: return "CUDA error";
         case FDEMRI_ERR_NOT_BUILT: return "splines not built";
         case FDEMRI_ERR_UNSUPPORTED: return "call not available in this configuration";
+        case FDEMRI_ERR_STATIC_SCRATCH: return "size beyond the library's static scratch (n_batch * n_knots > FDEMRI_STATIC_MAX_TOTALS)";
         default: return "unknown status";
     }
 }

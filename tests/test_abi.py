@@ -72,3 +72,20 @@ def test_plan_argument_validation_without_gpu():
     assert L.fdemri_plan_kerr(None, 1, None, 1, 10, fake, 1000, None, 0.0, 1e-6, 0) == INVALID
     assert L.fdemri_build_splines_kerr(None, fake, fake, fake, fake, fake, fake, fake, None) == INVALID
     assert L.fdemri_build_splines(None, fake, fake, fake, fake, fake, None) == INVALID
+
+
+def test_select_modes_static_validates_before_touching_the_device():
+    """fdemri_select_modes_static (the entry point that allocates nothing): bad arguments and sizes beyond its static
+    scratch are refused on the host, before any CUDA call."""
+    L = binding.lib()
+    fake = ctypes.c_void_p(256)
+    INVALID, STATIC_SCRATCH = 1, 6
+    assert L.fdemri_select_modes_static(0, 4, 10, fake, 0.1, fake, fake, None) == INVALID
+    assert L.fdemri_select_modes_static(1, 4, 10, None, 0.1, fake, fake, None) == INVALID
+    assert L.fdemri_select_modes_static(1, 4, 10, fake, -1.0, fake, fake, None) == INVALID
+    assert L.fdemri_select_modes_static(1, 4, 10, fake, float("nan"), fake, fake, None) == INVALID
+    lim = binding.FDEMRI_STATIC_MAX_TOTALS
+    assert L.fdemri_select_modes_static(lim // 100 + 1, 4, 100, fake, 0.1, fake, fake, None) == STATIC_SCRATCH
+    assert L.fdemri_select_modes_static(1 << 20, 4, 1 << 20, fake, 0.1, fake, fake, None) == STATIC_SCRATCH
+    assert b"static scratch" in L.fdemri_strerror(STATIC_SCRATCH)
+    assert binding.STATUS[STATIC_SCRATCH] == "FDEMRI_ERR_STATIC_SCRATCH"
