@@ -659,6 +659,30 @@ def test_many_knots(fd, orc):
     wf.close()
 
 
+def test_tile_major_merged_passes_short_segments(fd, orc):
+    """Segments much shorter than a consumer warp's 64 bins (300 knots, ~18 bins per segment of the (2,2,0) voice; fewer
+    for the slow voices), tile-major forced: every warp range holds several segment boundaries, so the consumers' merged
+    passes -- consecutive items with disjoint bins evaluated in one pass, each (lane, slot) with the item that covers its
+    bin -- run with runs of two and more items, rising and falling voices, both signs."""
+    from paper_2307_12585_b200 import synth
+    modes = ((2, 2, 0), (2, 1, -2), (3, 0, 1), (2, 2, -3), (4, 3, 2), (5, 1, -4), (3, 2, -1))
+    for seed, nk in ((13, 300), (14, 97)):
+        w = synth.small_case(seed=seed, n_knots=nk, n_freq=30000, modes=modes)
+        wf = fd.waveform_from_workload(w, flags=fd.FDEMRI_FLAG_TILE_MAJOR)
+        wf.sum(w.theta, w.phi)
+        hp, hx = wf.result()
+        st = wf.stats()
+        ref = oracle_c(orc, w, w.freq_array())
+        check(hp[0], hx[0], ref, f"short segments, {nk} knots, tile-major")
+        assert st["n_evals"] == ref["n_evals"] and st["flags"] == 0
+        assert st["n_evals"] / st["n_items"] < 64            # on average several entries per warp range
+        again = [x.copy() for x in (hp, hx)]
+        wf.sum(w.theta, w.phi)
+        hp2, hx2 = wf.result()
+        assert np.array_equal(again[0].view(np.uint64), hp2.view(np.uint64)) and np.array_equal(again[1].view(np.uint64), hx2.view(np.uint64))
+        wf.close()
+
+
 # ---- general voices (l, m, k, n) of Eq. 1: fdemri_plan_kerr / fdemri_build_splines_kerr (SURVEY 8(f) rank 4) -----------
 def test_kerr_voices_small(fd, orc):
     from paper_2307_12585_b200 import synth
