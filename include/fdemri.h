@@ -99,8 +99,11 @@ int fdemri_plan(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, int n_
                 uint32_t flags);
 
 /* Device work space the plan needs (bytes); the caller allocates it (256-byte aligned) and hands it over.
- * The work space holds the spline records, the segment->bin map and its bands; it must stay valid and untouched
- * between build_splines and the last sum.  fdemri_set_workspace returns FDEMRI_ERR_WORKSPACE for a smaller buffer;
+ * The work space holds the plan's tables (written by fdemri_set_workspace), the spline records, the segment->bin map
+ * and its bands; it must stay valid and untouched from fdemri_set_workspace to the last sum.  A plan with an explicit
+ * frequency array also keeps a bucket table of that array there, written by the first fdemri_build_splines after
+ * fdemri_set_workspace: every lookup through it is checked against the array itself, so changing the array later
+ * costs time, never a bin.  fdemri_set_workspace returns FDEMRI_ERR_WORKSPACE for a smaller buffer;
  * it may be called again with another buffer, fdemri_build_splines must then be repeated.
  * One stream at a time: the per-call scratch (angles, weights, counters, partial inner products) lives in the work
  * space, so two fdemri_sum calls on one plan must not run concurrently on different streams. */

@@ -62,6 +62,7 @@ struct fdemri_plan_s {
     cudaEvent_t ev0, ev1;
     cudaStream_t side;             // the amplitude splines run beside the shared ones (fork/join on two events)
     cudaEvent_t ev_fork, ev_join;
+    bool lut_built;                // explicit grids: the bucket table of the frequency array has been enqueued
     bool ev_valid;
     cudaEvent_t ev_angles;         // the copy of the angles out of the pinned staging buffer has run
     bool last_stream_valid;
@@ -100,6 +101,7 @@ static size_t carve(fdemri_plan_s* p, char* base) {
     p->angles = (double*)take(B * 2 * sizeof(double));
     p->stats = (unsigned long long*)take(16 * sizeof(unsigned long long));
     p->sel_total = (double*)take(B * (size_t)d.n_knots * sizeof(double));
+    p->d.lut = d.lut_n ? (const int*)take(((size_t)d.lut_n + 1 + FDEMRI_LUT_HDR) * sizeof(int)) : nullptr;
     // partial inner products: one range per consumer warp of a tile, or per block of the bin-major kernel
     const size_t NR = d.bin_major ? NT : NT * FDEMRI_CWARPS;
     p->inner_part = (double*)take(NR * 4 * sizeof(double));
@@ -219,6 +221,9 @@ static int plan_impl(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, c
     p->d.df = df;
     p->d.inv_df = (df > 0.0) ? 1.0 / df : 0.0;
     p->d.freq = freq_dev;
+    p->d.lut = nullptr;
+    /* explicit grids: four buckets per bin (a log-spaced array puts many bins into its lowest buckets), at most 4 M */
+    p->d.lut_n = freq_dev ? (int)std::min<int64_t>(4 * n_freq, (int64_t)1 << 22) : 0;
     p->lmn.assign(lmn_host, lmn_host + (size_t)3 * n_modes);
     if (k_host) p->kk.assign(k_host, k_host + n_modes);
     build_weight_table(p);
@@ -234,6 +239,7 @@ static int plan_impl(fdemri_plan_t* out, int n_modes, const int32_t* lmn_host, c
     p->ev0 = p->ev1 = nullptr;
     p->side = nullptr;
     p->ev_fork = p->ev_join = nullptr;
+    p->lut_built = false;
     p->angle_stage = nullptr;
     p->ev_angles = nullptr;
     p->last_stream_valid = false;
@@ -296,6 +302,7 @@ extern "C" int fdemri_set_workspace(fdemri_plan_t p, void* dev_ptr, size_t bytes
     p->ws_bytes = bytes;
     carve(p, (char*)dev_ptr);
     p->built = false;
+    p->lut_built = false;
     if (cudaMemcpy(p->lmn_dev, p->lmn.data(), p->lmn.size() * sizeof(int32_t), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(p->lm_index_dev, p->lm_index.data(), p->lm_index.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(p->wmeta_dev, p->wmeta.data(), p->wmeta.size() * sizeof(int4), cudaMemcpyHostToDevice) != cudaSuccess ||
@@ -341,6 +348,12 @@ static int build_impl(fdemri_plan_t p, const double* f_phi, const double* f_thet
         cudaMemsetAsync(p->item_evals, 0, (size_t)d.n_batch * sizeof(unsigned long long), st) != cudaSuccess ||
         cudaMemsetAsync(p->iband, 0x80, (size_t)d.n_batch * 2 * sizeof(int), st) != cudaSuccess)   /* very negative */
         return FDEMRI_ERR_CUDA;
+    if (d.lut && !p->lut_built) {
+        // explicit frequency array: its bucket table, once per work space (the lookups check every answer against the
+        // array itself, so a table that has gone stale or been overwritten costs time, never a bin)
+        k_freq_lut<<<(d.lut_n + 1 + 255) / 256, 256, 0, st>>>(d, const_cast<int*>(d.lut));
+        p->lut_built = true;
+    }
     // S1: parallel cyclic reduction, one thread per knot.  The amplitude splines (Re/Im A of every voice) are
     // independent of everything S2 needs: they run on the side stream beside the shared splines AND the map, and are
     // joined before the stream goes on (the sum reads them).

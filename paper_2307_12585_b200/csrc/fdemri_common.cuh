@@ -92,6 +92,8 @@ struct FdemriDims {
     int n_tiles;                            // tiles (blocks) per batch item = ceil(n_freq / tile_bins)
     double f0, df, inv_df;                  // inv_df = 1 / df: only to guess a bin index, which is then fixed up exactly
     const double* freq;                     // NULL => uniform grid
+    const int* lut;                         // explicit grids: bucket table of fdemri_map.cuh (k_freq_lut), else NULL
+    int lut_n;                              // its buckets
 };
 
 // frequency of bin i: explicit array, or the uniform grid f0 + i*df with a rounded product and a rounded sum

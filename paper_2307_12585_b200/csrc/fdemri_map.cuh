@@ -118,17 +118,61 @@ __device__ __forceinline__ void fdemri_root_build2(double FB, double FC, double 
     }
 }
 
+// ---- explicit frequency arrays: a bucket table instead of a full binary search per knot value ----------------------------
+// lut = { double f_lo = freq[0], double inv_w, int64 first bin with f > 0, int64 0,  int first[lut_n + 1] }:
+// first[j] = first bin with freq >= f_lo + j w,  w = (freq[n-1] - f_lo) / lut_n,  first[lut_n] = n_freq.
+// A search takes the window [first[j-1], first[j+2]] around its bucket j = floor((x - f_lo) inv_w) -- one bucket of
+// slack either side for the rounding of j -- finishes there, and CHECKS the answer against its two neighbours (falling back
+// to the plain binary search, which never happened in any test): the table only ever saves time, it cannot move a bin.
+// Built by the first fdemri_build_splines after fdemri_set_workspace; if the array changes afterwards, or the table is
+// overwritten, the lookups fall back to the plain search one by one (indices read from the table are clamped first).
+#define FDEMRI_LUT_HDR 8                    // ints in front of first[]
+
+__device__ __forceinline__ int64_t fdemri_bsearch_ge(const double* __restrict__ f, int64_t lo, int64_t hi, double x) {
+    // first i in [lo, hi] with f[i] >= x (hi if none in [lo, hi)): binary search down to a window of 8, then the window
+    // at once (independent loads: one trip instead of three)
+    while (hi - lo > 8) { int64_t mid = (lo + hi) >> 1; if (__ldg(f + mid) < x) lo = mid + 1; else hi = mid; }
+    int below = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) below += (lo + j < hi && __ldg(f + lo + j) < x) ? 1 : 0;
+    return lo + below;
+}
+
+__global__ void k_freq_lut(FdemriDims d, int* __restrict__ lut) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t n = d.n_freq;
+    const double f_lo = __ldg(d.freq), f_hi = __ldg(d.freq + n - 1);
+    const double w = (f_hi - f_lo) / (double)d.lut_n;
+    if (j == 0) {
+        double* hd = reinterpret_cast<double*>(lut);
+        hd[0] = f_lo;
+        hd[1] = (w > 0.0) ? 1.0 / w : 0.0;
+        int64_t lo = 0, hi = n;                                     // first bin with f > 0 (R13)
+        while (lo < hi) { int64_t mid = (lo + hi) >> 1; if (__ldg(d.freq + mid) <= 0.0) lo = mid + 1; else hi = mid; }
+        reinterpret_cast<long long*>(lut)[2] = lo;
+        reinterpret_cast<long long*>(lut)[3] = 0;
+    }
+    if (j > d.lut_n) return;
+    lut[FDEMRI_LUT_HDR + j] = (j == d.lut_n) ? (int)n : (int)fdemri_bsearch_ge(d.freq, 0, n, f_lo + (double)j * w);
+}
+
 // first bin index with f_i >= x  (n_freq if none)
 __device__ int64_t fdemri_first_ge(const FdemriDims& d, double x) {
     int64_t n = d.n_freq;
     if (d.freq) {
-        // binary search down to a window of 8, then the window at once (independent loads: one trip instead of three)
-        int64_t lo = 0, hi = n;
-        while (hi - lo > 8) { int64_t mid = (lo + hi) >> 1; if (__ldg(d.freq + mid) < x) lo = mid + 1; else hi = mid; }
-        int below = 0;
-#pragma unroll
-        for (int j = 0; j < 8; ++j) below += (lo + j < hi && __ldg(d.freq + lo + j) < x) ? 1 : 0;
-        return lo + below;
+        if (d.lut) {
+            const double* hd = reinterpret_cast<const double*>(d.lut);
+            const double t = (x - __ldg(hd)) * __ldg(hd + 1);
+            if (t >= 0.0 && t < (double)d.lut_n) {                  // (NaN and the two ends take the plain search)
+                const int j = (int)t;
+                const int64_t lo = min(max((int64_t)__ldg(d.lut + FDEMRI_LUT_HDR + max(j - 1, 0)), (int64_t)0), n);
+                const int64_t hi = min(max((int64_t)__ldg(d.lut + FDEMRI_LUT_HDR + min(j + 2, d.lut_n)), lo), n);
+                const int64_t i = fdemri_bsearch_ge(d.freq, lo, hi, x);
+                const bool ok = (i == 0 || __ldg(d.freq + i - 1) < x) && (i == n || __ldg(d.freq + i) >= x);
+                if (ok) return i;
+            }
+        }
+        return fdemri_bsearch_ge(d.freq, 0, n, x);
     }
     double g = ceil((x - d.f0) * d.inv_df);
     int64_t i = (g <= 0.0) ? 0 : (g >= (double)n ? n : (int64_t)g);
@@ -136,18 +180,22 @@ __device__ int64_t fdemri_first_ge(const FdemriDims& d, double x) {
     while (i < n && fdemri_freq(d, i) < x) ++i;
     return i;
 }
-// first bin index with f_i > x
-__device__ int64_t fdemri_first_gt(const FdemriDims& d, double x) {
+// first bin index with f_i > 0 (R13: only bins with f > 0 carry signal)
+__device__ int64_t fdemri_first_positive(const FdemriDims& d) {
     int64_t n = d.n_freq;
     if (d.freq) {
+        if (d.lut) {
+            const int64_t i = min(max((int64_t)reinterpret_cast<const long long*>(d.lut)[2], (int64_t)0), n);
+            if ((i == 0 || __ldg(d.freq + i - 1) <= 0.0) && (i == n || __ldg(d.freq + i) > 0.0)) return i;
+        }
         int64_t lo = 0, hi = n;
-        while (lo < hi) { int64_t mid = (lo + hi) >> 1; if (__ldg(d.freq + mid) <= x) lo = mid + 1; else hi = mid; }
+        while (lo < hi) { int64_t mid = (lo + hi) >> 1; if (__ldg(d.freq + mid) <= 0.0) lo = mid + 1; else hi = mid; }
         return lo;
     }
-    double g = floor((x - d.f0) * d.inv_df) + 1.0;
+    double g = floor((0.0 - d.f0) * d.inv_df) + 1.0;
     int64_t i = (g <= 0.0) ? 0 : (g >= (double)n ? n : (int64_t)g);
-    while (i > 0 && fdemri_freq(d, i - 1) > x) --i;
-    while (i < n && fdemri_freq(d, i) <= x) ++i;
+    while (i > 0 && fdemri_freq(d, i - 1) > 0.0) --i;
+    while (i < n && fdemri_freq(d, i) <= 0.0) ++i;
     return i;
 }
 
@@ -191,7 +239,7 @@ k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ 
     const size_t per = (size_t)S * 4;
     const int kq = POLAR ? kk[v] : 0;
     const bool masked = mode_mask && !mode_mask[bv];                 // a mode the selection dropped has no entries
-    const int64_t first_pos = fdemri_first_gt(d, 0.0);               // bins with f > 0 only (R13)
+    const int64_t first_pos = fdemri_first_positive(d);              // bins with f > 0 only (R13)
     const dd inv2pi = dd{FDEMRI_INV2PI_HI, FDEMRI_INV2PI_LO};
     const size_t last = (size_t)b * d.n_knots + d.n_knots - 1;
     unsigned long long evals = 0;

@@ -657,15 +657,15 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
             // wait for the ring slot; meanwhile scan ahead for the next stages (nothing to do: back off)
             {
                 const unsigned addr = fdemri_smem_addr(&ring->empty[stage]);
-                bool can_scan = true;                                // false: exhausted, or the entry queue is full
-                (void)can_scan;
-                while (!fdemri_mbar_try(addr, phase ^ 1u)) {
 #ifdef FDEMRI_SCAN_AHEAD        /* measured: scanning ahead while waiting costs the consumers more than it saves (profiles/) */
+                bool can_scan = true;                                // false: exhausted, or the entry queue is full
+                while (!fdemri_mbar_try(addr, phase ^ 1u)) {
                     if (can_scan) can_scan = fdemri_scan_step<FDEMRI_PQ1, FDEMRI_PQ2, 8>(sc, pq->q1, pq->q2, lane, em) == 1;
-                    else
-#endif
-                    __nanosleep(FDEMRI_PROD_BACKOFF);
+                    else __nanosleep(FDEMRI_PROD_BACKOFF);
                 }
+#else
+                while (!fdemri_mbar_try(addr, phase ^ 1u)) __nanosleep(FDEMRI_PROD_BACKOFF);
+#endif
             }
             if (lane < cnt) {
                 const int vs = en.x / 3, br = en.x - 3 * vs;
@@ -770,15 +770,18 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
                     double T0r, T0i, T1r, T1i;
                     const bool ok0 = fdemri_term_fast(it0, sf0, T0r, T0i);
                     const bool ok1 = fdemri_term_fast(it1, sf1, T1r, T1i);
-                    if (m0 && !ok0) {
-                        const FdemriSlowOut o = fdemri_term_slow(it0, sf0, fl0);
-                        T0r = o.tre; T0i = o.tim;
-                        n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
-                    }
-                    if (m1 && !ok1) {
-                        const FdemriSlowOut o = fdemri_term_slow(it1, sf1, fl1);
-                        T1r = o.tre; T1i = o.tim;
-                        n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                    const bool bad0 = m0 && !ok0, bad1 = m1 && !ok1;
+                    if (__any_sync(0xffffffffu, bad0 || bad1)) {
+                        if (bad0) {
+                            const FdemriSlowOut o = fdemri_term_slow(it0, sf0, fl0);
+                            T0r = o.tre; T0i = o.tim;
+                            n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                        }
+                        if (bad1) {
+                            const FdemriSlowOut o = fdemri_term_slow(it1, sf1, fl1);
+                            T1r = o.tre; T1i = o.tim;
+                            n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                        }
                     }
                     if (m0) {
                         a00 = fma(it0[S_WP], T0r, a00); a01 = fma(it0[S_SWP], T0i, a01);
@@ -793,26 +796,39 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
             }
 #endif
             const double sf0 = fdemri_xorsign(f0, sbit), sf1 = fdemri_xorsign(f1, sbit);
-            double T0r = 0.0, T0i = 0.0, T1r = 0.0, T1i = 0.0;
-            bool ok0 = false, ok1 = false;
+            double T0r, T0i, T1r, T1i;
             if (!(flags & 1u)) {
                 // both slots always, also for an item that ends inside this warp's 64 bins and leaves one of them without
                 // a lane: skipping the empty slot (three copies of the fast path behind a warp-uniform branch) was
                 // measured 2 % slower than the few wasted evaluations
-                ok0 = fdemri_term_fast(it, sf0, T0r, T0i);
-                ok1 = fdemri_term_fast(it, sf1, T1r, T1i);
+                const bool ok0 = fdemri_term_fast(it, sf0, T0r, T0i);
+                const bool ok1 = fdemri_term_fast(it, sf1, T1r, T1i);
+                const bool bad0 = act0 && !ok0, bad1 = act1 && !ok1;
+                if (__any_sync(0xffffffffu, bad0 || bad1)) {             // one warp-uniform branch: under 1 % of the passes
+                    if (bad0) {
+                        const FdemriSlowOut o = fdemri_term_slow(it, sf0, flags);
+                        T0r = o.tre; T0i = o.tim;
+                        n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                    }
+                    if (bad1) {
+                        const FdemriSlowOut o = fdemri_term_slow(it, sf1, flags);
+                        T1r = o.tre; T1i = o.tim;
+                        n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                    }
+                }
+            } else {
+                T0r = T0i = T1r = T1i = 0.0;
+                if (act0) {
+                    const FdemriSlowOut o = fdemri_term_slow(it, sf0, flags);
+                    T0r = o.tre; T0i = o.tim;
+                    n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                }
+                if (act1) {
+                    const FdemriSlowOut o = fdemri_term_slow(it, sf1, flags);
+                    T1r = o.tre; T1i = o.tim;
+                    n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                }
             }
-            if (act0 && !ok0) {
-                const FdemriSlowOut o = fdemri_term_slow(it, sf0, flags);
-                T0r = o.tre; T0i = o.tim;
-                n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
-            }
-            if (act1 && !ok1) {
-                const FdemriSlowOut o = fdemri_term_slow(it, sf1, flags);
-                T1r = o.tre; T1i = o.tim;
-                n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
-            }
-            // weights (O2): s=+1: h+ += w+ T, hx += i wx T;  s=-1: h+ += w+ conj(T), hx += conj(i wx T)
             const double wp = it[S_WP], swp = it[S_SWP], nwx = it[S_NWX], swx = it[S_SWX];
             if (act0) {
                 a00 = fma(wp, T0r, a00); a01 = fma(swp, T0i, a01); a02 = fma(nwx, T0i, a02); a03 = fma(swx, T0r, a03);

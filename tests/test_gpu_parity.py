@@ -683,6 +683,32 @@ def test_tile_major_merged_passes_short_segments(fd, orc):
         wf.close()
 
 
+@pytest.mark.parametrize("mode", ["bin", "tile"])
+def test_explicit_grid_changed_between_builds(fd, orc, mode):
+    """Explicit frequency arrays go through a bucket table that the first build after fdemri_set_workspace writes into the
+    work space (fdemri_map.cuh).  The array is then replaced IN PLACE by a different one -- other spacing, other range -- and
+    the splines rebuilt: the table is stale, every lookup through it is checked against the array and repeated by plain
+    search where the check fails, so the result is at parity for the new array (and the counts are the oracle's)."""
+    import torch
+    from paper_2307_12585_b200 import synth
+    w = synth.small_case(seed=21, n_knots=40)
+    n = 6000
+    grids = [np.geomspace(2e-4, 9e-3, n), np.concatenate([[0.0], np.linspace(1.1e-3, 7e-3, n - 1) ** 1.0]),
+             np.sort(np.random.default_rng(5).uniform(5e-4, 8e-3, n))]
+    flag = fd.FDEMRI_FLAG_BIN_MAJOR if mode == "bin" else fd.FDEMRI_FLAG_TILE_MAJOR
+    wf = fd.Waveform(w.lmn, w.t_knots, n, freqs=grids[0], flags=flag)
+    for i, g in enumerate(grids):
+        wf.freqs.copy_(torch.from_numpy(g))
+        wf.build_splines(w.f_phi, w.f_r, w.Phi_phi, w.Phi_r, w.amp)
+        wf.sum(w.theta, w.phi)
+        hp, hx = wf.result()
+        st = wf.stats()
+        ref = orc.waveform(w.lmn, w.t_knots[0], w.f_phi[0], w.f_r[0], w.Phi_phi[0], w.Phi_r[0], w.amp[0], g, w.theta, w.phi)
+        check(hp[0], hx[0], ref, f"explicit grid {i} ({mode}-major), table built for grid 0")
+        assert st["n_evals"] == ref["n_evals"] and st["flags"] == 0
+    wf.close()
+
+
 # ---- general voices (l, m, k, n) of Eq. 1: fdemri_plan_kerr / fdemri_build_splines_kerr (SURVEY 8(f) rank 4) -----------
 def test_kerr_voices_small(fd, orc):
     from paper_2307_12585_b200 import synth
