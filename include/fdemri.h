@@ -140,9 +140,10 @@ int fdemri_build_splines_kerr(fdemri_plan_t plan, const double* f_phi, const dou
                               void* cuda_stream);
 
 /* S0 + S3 + S4 (S2 is part of fdemri_build_splines).
- *  theta_host, phi_host  source-frame viewing angles (L66), [n_angles] on the host, n_angles = 1 or n_batch; copied
- *                        into a pinned buffer of the plan before the call returns.  (When the call is captured into a
- *                        CUDA graph, a replay uses the angles of the most recent fdemri_sum call on the plan.)
+ *  theta_host, phi_host  source-frame viewing angles (L66), [n_angles] on the host, n_angles = 1 or n_batch; read
+ *                        before the call returns.  n_angles = 1: the pair travels as kernel arguments (a call captured
+ *                        into a CUDA graph replays the angles of the capture).  n_angles = n_batch: copied through a
+ *                        pinned buffer of the plan (a replay uses the angles of the most recent such call on the plan).
  *  hplus_dev, hcross_dev [n_batch][n_freq][2] (re, im) FP64, fully overwritten (zeros where no voice has
  *                        support, L147; the bin f = 0 is always zero) */
 int fdemri_sum(fdemri_plan_t plan, int n_angles, const double* theta_host, const double* phi_host,

@@ -43,8 +43,9 @@ struct fdemri_plan_s {
     int2* ent;                     // [B][V][2][3][S] bin intervals of the segment branches
     int4* gband;                   // [B][V][2][G] bands of the groups of 32 segments
     int2* vband;                   // [B][V][2] bands of the voice-signs
-    int* iband;                    // [B][2] {-lo, hi} of the item
+    int* iband;                    // [B][2] {0x7fffffff - lo, hi + 1} of the item ({0, 0}: empty)
     unsigned long long* item_evals;// [B] mode-bin evaluations of the map, per batch item
+    size_t build_clear_bytes;      // stats .. item_evals, cleared by one memset per build
     double* inner_part;            // [ranges][4] partial inner products (a range: 64 bins of a consumer warp, or a block)
     double* inner_edge;            // [ranges][4][4] edge bins for the Hann filter
     double* sel_total;             // [B][n_knots] total power per time step (mode selection)
@@ -94,12 +95,14 @@ static size_t carve(fdemri_plan_s* p, char* base) {
     p->ent = (int2*)take(B * V * 2 * (size_t)d.ent_max * sizeof(int2));
     p->gband = (int4*)take(B * V * 2 * (size_t)d.n_groups * sizeof(int4));
     p->vband = (int2*)take(B * V * 2 * sizeof(int2));
+    // cleared together by one memset at the head of every build: keep the three adjacent and in this order
+    p->stats = (unsigned long long*)take(16 * sizeof(unsigned long long));
     p->iband = (int*)take(B * 2 * sizeof(int));
     p->item_evals = (unsigned long long*)take(B * sizeof(unsigned long long));
+    p->build_clear_bytes = base ? (size_t)((char*)p->item_evals - (char*)p->stats) + B * sizeof(unsigned long long) : 0;
     const size_t NT = B * (size_t)d.n_tiles;
     p->wts = (double4*)take(B * V * sizeof(double4));
     p->angles = (double*)take(B * 2 * sizeof(double));
-    p->stats = (unsigned long long*)take(16 * sizeof(unsigned long long));
     p->sel_total = (double*)take(B * (size_t)d.n_knots * sizeof(double));
     p->d.lut = d.lut_n ? (const int*)take(((size_t)d.lut_n + 1 + FDEMRI_LUT_HDR) * sizeof(int)) : nullptr;
     // partial inner products: one range per consumer warp of a tile, or per block of the bin-major kernel
@@ -344,10 +347,7 @@ static int build_impl(fdemri_plan_t p, const double* f_phi, const double* f_thet
     const FdemriDims& d = p->d;
     p->last_stream = st;
     if (raise_spline_smem_limits() != FDEMRI_OK) return FDEMRI_ERR_CUDA;
-    if (cudaMemsetAsync(p->stats, 0, 16 * sizeof(unsigned long long), st) != cudaSuccess ||
-        cudaMemsetAsync(p->item_evals, 0, (size_t)d.n_batch * sizeof(unsigned long long), st) != cudaSuccess ||
-        cudaMemsetAsync(p->iband, 0x80, (size_t)d.n_batch * 2 * sizeof(int), st) != cudaSuccess)   /* very negative */
-        return FDEMRI_ERR_CUDA;
+    if (cudaMemsetAsync(p->stats, 0, p->build_clear_bytes, st) != cudaSuccess) return FDEMRI_ERR_CUDA;   /* stats, iband, item_evals */
     if (d.lut && !p->lut_built) {
         // explicit frequency array: its bucket table, once per work space (the lookups check every answer against the
         // array itself, so a table that has gone stale or been overwritten costs time, never a bin)
@@ -400,10 +400,20 @@ extern "C" int fdemri_build_splines_kerr(fdemri_plan_t p, const double* f_phi, c
 }
 
 // S0: the viewing angles go through the plan's pinned buffer to the device, then k_weights.  Shared by the sums.
-static int stage_weights(fdemri_plan_t p, int n_angles, const double* theta_host, const double* phi_host, cudaStream_t st) {
+static int stage_weights(fdemri_plan_t p, int n_angles, const double* theta_host, const double* phi_host, cudaStream_t st,
+                         bool reset_sum_counters) {
     const FdemriDims& d = p->d;
     for (int i = 0; i < n_angles; ++i)
         if (!std::isfinite(theta_host[i]) || !std::isfinite(phi_host[i])) return FDEMRI_ERR_INVALID_ARG;
+    const int nw = n_angles * d.n_modes;
+    unsigned long long* counters = reset_sum_counters ? p->stats : nullptr;
+    if (n_angles == 1) {
+        // one viewing direction for the whole batch: the two angles travel as kernel arguments
+        p->last_stream = st;
+        k_weights<<<(nw + 127) / 128, 128, 0, st>>>(1, d.n_modes, p->lmn_dev, p->k_dev, p->lm_index_dev, p->wmeta_dev, p->wcoef_dev,
+                                                    nullptr, theta_host[0], phi_host[0], p->wts, counters);
+        return FDEMRI_OK;
+    }
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) return FDEMRI_ERR_CUDA;
     // the pinned staging buffer is read by the asynchronous copy below: wait for the copy of the previous sum
@@ -419,9 +429,8 @@ static int stage_weights(fdemri_plan_t p, int n_angles, const double* theta_host
         return FDEMRI_ERR_CUDA;
     // (a stream being captured into a CUDA graph: no event; a replay reads the buffer as the last call left it)
     p->last_stream_valid = cap == cudaStreamCaptureStatusNone && cudaEventRecord(p->ev_angles, st) == cudaSuccess;
-    const int nw = n_angles * d.n_modes;
     k_weights<<<(nw + 127) / 128, 128, 0, st>>>(n_angles, d.n_modes, p->lmn_dev, p->k_dev, p->lm_index_dev, p->wmeta_dev, p->wcoef_dev,
-                                                p->angles, p->wts);
+                                                p->angles, 0.0, 0.0, p->wts, counters);
     return FDEMRI_OK;
 }
 
@@ -439,12 +448,10 @@ static int enqueue_sum(fdemri_plan_t p, int n_angles, const double* theta_host, 
     if (n_angles != 1 && n_angles != d.n_batch) return FDEMRI_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     {
-        const int rc = stage_weights(p, n_angles, theta_host, phi_host, st);
+        // (k_weights also resets the per-sum counters: n_airy, the tile counter, n_slow, n_pairs, the sum's flags)
+        const int rc = stage_weights(p, n_angles, theta_host, phi_host, st, true);
         if (rc != FDEMRI_OK) return rc;
     }
-    // reset the per-sum counters: n_airy (slot 4), the tile counter (6), n_slow (7), n_pairs (8), the sum's flags (9)
-    if (cudaMemsetAsync(p->stats + 4, 0, sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
-    if (cudaMemsetAsync(p->stats + 6, 0, 4 * sizeof(unsigned long long), st) != cudaSuccess) return FDEMRI_ERR_CUDA;
     SumArgs a;
     a.d = d;
     a.rec = p->rec;
@@ -511,7 +518,7 @@ extern "C" int fdemri_td_sum(fdemri_plan_t p, int n_angles, const double* theta_
     const FdemriDims& d = p->d;
     if (n_angles != 1 && n_angles != d.n_batch) return FDEMRI_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const int rc = stage_weights(p, n_angles, theta_host, phi_host, st);
+    const int rc = stage_weights(p, n_angles, theta_host, phi_host, st, false);
     if (rc != FDEMRI_OK) return rc;
     const dim3 grid((unsigned)((n_samples + 255) / 256), (unsigned)d.n_batch);
     k_td_sum<<<grid, 256, 0, st>>>(d, p->rec, p->t_knots_dev, p->wts, n_angles, p->mode_mask, (long long)n_samples, t0, dt,

@@ -50,13 +50,20 @@ __device__ __forceinline__ double fdemri_wigner_sum(const int4 meta, const doubl
 __global__ void k_weights(int n_angles, int V, const int* __restrict__ lmn, const int* __restrict__ kk,
                           const int* __restrict__ lm_index,
                           const int4* __restrict__ wmeta, const double* __restrict__ wcoef,
-                          const double* __restrict__ angles, double4* __restrict__ wts) {
+                          const double* __restrict__ angles, double theta0, double phi0, double4* __restrict__ wts,
+                          unsigned long long* __restrict__ sum_counters) {
     int id = blockIdx.x * blockDim.x + threadIdx.x;
+    // the counters of the sum that follows on the stream: n_airy (slot 4), the tile counter (6), n_slow (7), n_pairs (8),
+    // the sum's flags (9) -- cleared here instead of by two memsets in front of every sum
+    if (sum_counters && id == 0) {
+        sum_counters[4] = 0ull; sum_counters[6] = 0ull; sum_counters[7] = 0ull; sum_counters[8] = 0ull; sum_counters[9] = 0ull;
+    }
     if (id >= n_angles * V) return;
     int a = id / V, v = id - a * V;
     const int m = lmn[3 * v + 1];
     const int lm = lm_index[v];
-    double theta = angles[2 * a], phi = angles[2 * a + 1];
+    // one pair of angles for the whole batch travels as kernel arguments (no copy); per-item angles come from `angles`
+    double theta = angles ? angles[2 * a] : theta0, phi = angles ? angles[2 * a + 1] : phi0;
     double ch = cos(0.5 * theta), sh = sin(0.5 * theta);
     const double yp = fdemri_wigner_sum(wmeta[2 * lm], wcoef, ch, sh);            // -2Y_{l,m}(theta, 0)
     double wp, wx;
@@ -212,7 +219,7 @@ __device__ int64_t fdemri_first_positive(const FdemriDims& d) {
 //         whole groups: a group row is 256 aligned bytes).   key = ((v*2+sign)*3 + branch)*Sp + segment
 //   gband [B][V][2][G] int4 {lo, hi of the branch-0 entries of the group; lo, hi of its branch-1/2 entries}
 //   vband [B][V][2]    int2 {lo, hi} over all entries of the voice-sign
-//   iband [B]          int2 {max of -lo, max of hi} over the item (atomicMax; memset to 0x80 bytes before)
+//   iband [B]          int2 {max of 0x7fffffff - lo, max of hi + 1} over the item (atomicMax; zeroed before: {0, 0} = empty)
 // POLAR: general voices (l, m, k, n) -- kk[v] = k, sh2_hi/sh2_lo the splines of (f_theta, Phi_theta) (components
 // 0 and 1 of a second [B][4][n_seg][4] array), f_theta the knot values.
 // ------------------------------------------------------------------------------------------------
@@ -473,8 +480,8 @@ k_records(FdemriDims d, const int* __restrict__ lmn, const double* __restrict__ 
         vband[bv * 2 + 1] = make_int2(vlo[1], vhi[1]);
         const int ilo = min(vlo[0], vlo[1]), ihi = max(vhi[0], vhi[1]);
         if (ihi >= ilo) {
-            atomicMax(iband + 2 * b, -ilo);
-            atomicMax(iband + 2 * b + 1, ihi);
+            atomicMax(iband + 2 * b, 0x7fffffff - ilo);
+            atomicMax(iband + 2 * b + 1, ihi + 1);
         }
         if (it_w) atomicAdd(stats + 0, (unsigned long long)it_w);
         if (tv_w) atomicAdd(stats + 3, (unsigned long long)tv_w);

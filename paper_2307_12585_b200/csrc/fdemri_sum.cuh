@@ -41,7 +41,7 @@ struct SumArgs {
     const int2* ent;          // [B][V][2][3][Sp] {first bin, last bin}, Sp = 32 G; key = ((v*2+sign)*3 + branch)*Sp + segment
     const int4* gband;        // [B][V][2][G] bands of the groups of 32 segments {lo, hi (branch 0), lo, hi (branches 1, 2)}
     const int2* vband;        // [B][V][2] band of the voice-sign
-    const int* iband;         // [B][2] {-lo, hi} of the item
+    const int* iband;         // [B][2] {0x7fffffff - lo, hi + 1} of the item ({0, 0}: empty)
     const double4* wts;       // [n_angles][V]
     int n_angles;
     double* hp;               // [B][n_freq][2]
@@ -631,7 +631,7 @@ __device__ __forceinline__ void fdemri_producer(const SumArgs& a, FdemriRing* ri
         const int wbase = (a.n_angles > 1 ? b : 0) * V;
         const size_t rbase = (size_t)b * V * d.n_seg;
         // tiles outside the band of the item have no entry: nothing to scan
-        const bool in_band = tile_lo <= __ldg(a.iband + 2 * b + 1) && tile_hi >= -__ldg(a.iband + 2 * b);
+        const bool in_band = tile_lo <= __ldg(a.iband + 2 * b + 1) - 1 && tile_hi >= 0x7fffffff - __ldg(a.iband + 2 * b);
         FdemriScan sc;
         fdemri_scan_init<FDEMRI_PQ2>(sc, a, b, 0, in_band ? 2 * V : 0, tile_lo, tile_hi);
         FdemriProdEmit em;
@@ -1093,7 +1093,7 @@ __global__ void __launch_bounds__(FDEMRI_BIN_WARPS * 32, 2) k_bin_sum(SumArgs a)
         const int i1 = (int)min((int64_t)i0 + NB - 1, d.n_freq - 1);
         const int wbase = (a.n_angles > 1 ? b : 0) * V;
         const size_t rbase = (size_t)b * V * S;
-        const bool in_band = i0 <= __ldg(a.iband + 2 * b + 1) && i1 >= -__ldg(a.iband + 2 * b);
+        const bool in_band = i0 <= __ldg(a.iband + 2 * b + 1) - 1 && i1 >= 0x7fffffff - __ldg(a.iband + 2 * b);
         FdemriScan sc;
         const int vs0 = min(wid * part, 2 * V), vs1 = min(vs0 + part, 2 * V);
         fdemri_scan_init<FDEMRI_BQ2>(sc, a, b, vs0, in_band ? vs1 : vs0, i0, i1);
