@@ -1029,16 +1029,15 @@ __global__ void __launch_bounds__(256) k_inner_reduce(size_t n_ranges, int range
 //   A  its eight warps run the item scan (above) over an eighth of the voice-signs each and collect the entries that
 //      meet the block, in key order, in shared memory (a round takes what fits; further rounds take the rest);
 //   B  every warp takes bins of the block in turn: its lanes filter the collected entries for those that cover the
-//      bin, 32 at a time each lane stages its own item (same 256-byte layout, a 272-byte lane stride keeps 128-bit
-//      shared accesses conflict-free) and evaluates the same fast / slow term functions, a fixed butterfly adds the
-//      lanes, and lane 0 adds the round's sum to the bin's accumulator.
+//      bin, 32 at a time each lane stages its own item IN REGISTERS (same layout as the ring's items; only the rare slow
+//      path gets a copy on the thread's stack) and evaluates the same fast / slow term functions, a fixed butterfly adds
+//      the lanes, and lane 0 adds the round's sum to the bin's accumulator.
 // Every bin is written once, with no atomics and no list in global memory, in an order that depends on the data only.
 // This is the paper's own map -- the segment of every (f, voice) predetermined (L105) -- with the threads over the
 // voices of a frequency instead of over the frequencies of a voice.  The Eq. 12 inner products are formed from the
 // block's accumulators (one range per block for k_inner_reduce).
 // ---------------------------------------------------------------------------------------------------------
 #define FDEMRI_BIN_WARPS 8
-#define FDEMRI_BIN_STRIDE 34         // doubles per lane slot of the staging area
 #define FDEMRI_BQ1 256               // per warp: voice-signs waiting for level 2 (>= 31 + 32 * L1U, L1U = 4)
 #define FDEMRI_BQ2 512               // per warp: rows waiting for level 3
 #define FDEMRI_BREG 256              // per warp: entries collected per round
@@ -1049,9 +1048,6 @@ struct FdemriBinWarpQ {
     uint2 reg[FDEMRI_BREG];          // {key, first bin | last bin << 8, both relative to the block}
 };
 struct FdemriBinSmem {
-#ifdef FDEMRI_BIN_STAGE_SMEM
-    double stage[FDEMRI_BIN_WARPS * 32 * FDEMRI_BIN_STRIDE];
-#endif
     double4 acc[FDEMRI_BIN_BLOCK];
     FdemriBinWarpQ wq[FDEMRI_BIN_WARPS];
     unsigned short wlist[FDEMRI_BIN_WARPS][64];
@@ -1074,9 +1070,6 @@ __global__ void __launch_bounds__(FDEMRI_BIN_WARPS * 32, 2) k_bin_sum(SumArgs a)
     const FdemriDims& d = a.d;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
-#ifdef FDEMRI_BIN_STAGE_SMEM
-    double* it = sm->stage + ((size_t)wid * 32 + lane) * FDEMRI_BIN_STRIDE;
-#endif
     const int V = d.n_modes, S = d.n_seg, Sp = 32 * d.n_groups, NB = d.tile_bins;     // NB <= FDEMRI_BIN_BLOCK
     const int part = ((2 * V + FDEMRI_BIN_WARPS - 1) / FDEMRI_BIN_WARPS + 31) & ~31;     // voice-signs per warp
     unsigned n_airy = 0, n_slow = 0, errs = 0;
@@ -1086,9 +1079,14 @@ __global__ void __launch_bounds__(FDEMRI_BIN_WARPS * 32, 2) k_bin_sum(SumArgs a)
         if (tid == 0) sm->cur_block = (int)atomicAdd(a.tile_counter, 1u);
         if (tid < FDEMRI_BIN_BLOCK) sm->acc[tid] = make_double4(0.0, 0.0, 0.0, 0.0);
         __syncthreads();
-        const int gb = sm->cur_block;
-        if (gb >= a.total_tiles) break;
-        const int b = gb / d.n_tiles, blk = gb - b * d.n_tiles;
+        if (sm->cur_block >= a.total_tiles) break;
+        // A CTA gets only a few blocks (config 3: 1250 for 296 CTAs), so the blocks handed out last decide how long the
+        // last CTA runs alone.  The blocks of an item go out from the TOP of the grid down: the expensive terms -- the
+        // slow path near the extrema of F and at small |X|, where the inspiral ends -- sit at the
+        // highest frequencies a voice reaches, so the tail is made of the cheap blocks (config 3: 0.273 -> 0.251 ms;
+        // sorting the blocks by the number of voice bands that cover them was measured too: 0.260 ms plus 27 us of sort).
+        const int b = sm->cur_block / d.n_tiles, blk = d.n_tiles - 1 - (sm->cur_block - b * d.n_tiles);
+        const int gb = b * d.n_tiles + blk;
         const int i0 = blk * NB;
         const int i1 = (int)min((int64_t)i0 + NB - 1, d.n_freq - 1);
         const int wbase = (a.n_angles > 1 ? b : 0) * V;
@@ -1121,28 +1119,20 @@ __global__ void __launch_bounds__(FDEMRI_BIN_WARPS * 32, 2) k_bin_sum(SumArgs a)
                         const int vsbr = (int)(key / (unsigned)Sp), seg = (int)(key - (unsigned)vsbr * (unsigned)Sp);
                         const int vs = vsbr / 3, br = vsbr - 3 * vs;
                         const int v = vs >> 1;
-#ifdef FDEMRI_BIN_STAGE_SMEM
-                        fdemri_stage_item(it, a.rec + (rbase + (size_t)v * S + seg) * R_DOUBLES, a.wts[wbase + v], 0, 0,
-                                          (unsigned)(vs & 1), (unsigned)br);
-                        const double* item = it;
-#else
                         // the lane's item stays in registers (every index below is a constant after inlining); only the
-                        // rare slow path gets a copy in shared memory, which its out-of-line function reads
+                        // rare slow path gets a copy on the thread's stack, which its out-of-line function reads
                         __align__(16) double item[S_DOUBLES];
                         fdemri_stage_item(item, a.rec + (rbase + (size_t)v * S + seg) * R_DOUBLES, a.wts[wbase + v], 0, 0,
                                           (unsigned)(vs & 1), (unsigned)br);
-#endif
                         const unsigned flags = (unsigned)(*reinterpret_cast<const int2*>(item)).y;
                         const double sf = fdemri_xorsign(f, (flags & 4u) << 29);
                         double Tr = 0.0, Ti = 0.0;
                         bool ok = false;
                         if (!(flags & 1u)) ok = fdemri_term_fast(item, sf, Tr, Ti);
                         if (!ok) {
-#ifndef FDEMRI_BIN_STAGE_SMEM
                             __align__(16) double it[S_DOUBLES];          // a copy on the thread's stack (local memory)
 #pragma unroll
                             for (int q = 0; q < S_DOUBLES; ++q) it[q] = item[q];
-#endif
                             const FdemriSlowOut o = fdemri_term_slow(it, sf, flags);
                             Tr = o.tre; Ti = o.tim;
                             n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
