@@ -716,41 +716,91 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
             f1 = (bin_a + 32 < d.n_freq) ? fdemri_freq(d, bin_a + 32) : 0.0;
             a00 = a01 = a02 = a03 = a10 = a11 = a12 = a13 = 0.0;
         }
-        // items of the chunk that overlap this warp's bins: lane j looks at item j, one ballot, then the set
-        // bits are walked in ascending (= list) order
-        unsigned todo;
+        // items of the chunk that overlap this warp's bins: lane j looks at item j, two ballots (overlaps; is monotone and
+        // covers all 64 bins), then the set bits are walked in ascending (= list) order
+        unsigned todo, fullm;
         {
-            bool mine = false;
+            bool mine = false, whole = false;
             if (lane < cnt) {
-                const int mx = *reinterpret_cast<const int*>(S->items[lane]);       // lo | hi << 16
-                mine = !((mx >> 16) < wb || (mx & 0xffff) > wb + 32 * FDEMRI_BPL - 1);
+                const int2 mx = *reinterpret_cast<const int2*>(S->items[lane]);     // {lo | hi << 16, flags}
+                const int lo = mx.x & 0xffff, hi = mx.x >> 16;
+                mine = !(hi < wb || lo > wb + 32 * FDEMRI_BPL - 1);
+                whole = lo <= wb && hi >= wb + 32 * FDEMRI_BPL - 1 && !(mx.y & 1);
             }
             todo = __ballot_sync(0xffffffffu, mine);
+            fullm = __ballot_sync(0xffffffffu, whole);
         }
         while (todo) {
             const int j = __ffs(todo) - 1;
             todo &= todo - 1;
             const double* it = S->items[j];
+            if ((fullm >> j) & 1u) {
+                // ---- the common pass: a monotone item that covers every bin of this warp -- no masks ----
+                const unsigned sbit = ((unsigned)reinterpret_cast<const int*>(it)[1] & 4u) << 29;
+                const double sf0 = fdemri_xorsign(f0, sbit), sf1 = fdemri_xorsign(f1, sbit);
+                double T0r, T0i, T1r, T1i;
+                const bool ok0 = fdemri_term_fast(it, sf0, T0r, T0i);
+                const bool ok1 = fdemri_term_fast(it, sf1, T1r, T1i);
+                if (__any_sync(0xffffffffu, !(ok0 && ok1))) {            // one warp-uniform branch: under 1 % of the passes
+                    const unsigned flags = (unsigned)reinterpret_cast<const int*>(it)[1];
+                    if (!ok0) {
+                        const FdemriSlowOut o = fdemri_term_slow(it, sf0, flags);
+                        T0r = o.tre; T0i = o.tim;
+                        n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                    }
+                    if (!ok1) {
+                        const FdemriSlowOut o = fdemri_term_slow(it, sf1, flags);
+                        T1r = o.tre; T1i = o.tim;
+                        n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                    }
+                }
+                // weights (O2): s=+1: h+ += w+ T, hx += i wx T;  s=-1: h+ += w+ conj(T), hx += conj(i wx T)
+                const double wp = it[S_WP], swp = it[S_SWP], nwx = it[S_NWX], swx = it[S_SWX];
+                a00 = fma(wp, T0r, a00); a01 = fma(swp, T0i, a01); a02 = fma(nwx, T0i, a02); a03 = fma(swx, T0r, a03);
+                a10 = fma(wp, T1r, a10); a11 = fma(swp, T1i, a11); a12 = fma(nwx, T1i, a12); a13 = fma(swx, T1r, a13);
+                continue;
+            }
+            // ---- an item that covers part of this warp's bins, or a branch of a segment with extrema ----
             const int2 meta = *reinterpret_cast<const int2*>(it);        // {lo | hi << 16, flags}
             const int lo = meta.x & 0xffff, hi = meta.x >> 16;
             const unsigned flags = (unsigned)meta.y;
-            const unsigned sbit = (flags & 4u) << 29;
-            const bool act0 = rel0 >= lo && rel0 <= hi;          // (one unsigned compare each was measured: slower)
-            const bool act1 = rel1 >= lo && rel1 <= hi;
+            const bool act0 = rel0 >= lo && rel0 <= hi, act1 = rel1 >= lo && rel1 <= hi;
+            if (flags & 1u) {
+                const unsigned sbit = (flags & 4u) << 29;
+                const double sf0 = fdemri_xorsign(f0, sbit), sf1 = fdemri_xorsign(f1, sbit);
+                double T0r = 0.0, T0i = 0.0, T1r = 0.0, T1i = 0.0;
+                if (act0) {
+                    const FdemriSlowOut o = fdemri_term_slow(it, sf0, flags);
+                    T0r = o.tre; T0i = o.tim;
+                    n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                }
+                if (act1) {
+                    const FdemriSlowOut o = fdemri_term_slow(it, sf1, flags);
+                    T1r = o.tre; T1i = o.tim;
+                    n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                }
+                const double wp = it[S_WP], swp = it[S_SWP], nwx = it[S_NWX], swx = it[S_SWX];
+                if (act0) {
+                    a00 = fma(wp, T0r, a00); a01 = fma(swp, T0i, a01); a02 = fma(nwx, T0i, a02); a03 = fma(swx, T0r, a03);
+                }
+                if (act1) {
+                    a10 = fma(wp, T1r, a10); a11 = fma(swp, T1i, a11); a12 = fma(nwx, T1i, a12); a13 = fma(swx, T1r, a13);
+                }
+                continue;
+            }
+            // A monotone item that ends (or starts) inside this warp's 64 bins.  The items that follow it in the list and
+            // whose bins lie entirely beside what has been gathered so far -- the usual case: the next segment of the
+            // same voice, which starts at the following bin -- share ONE pass with it: every (lane, slot) evaluates the
+            // item that covers its bin, with its own item constants (per-lane addresses; FDEMRI_ITEM_STRIDE keeps
+            // neighbouring items on different banks).  Without this each of them would take a whole pass with part of
+            // the lanes idle: 5.70 M passes instead of 5.18 M on config 2, where 5.15 M would use every lane.  A bin
+            // still receives its terms in list order, so the sums are the same bit for bit.
+            const double* it0 = it;
+            const double* it1 = it;
+            unsigned fl0 = flags, fl1 = flags;
+            bool m0 = act0, m1 = act1;
 #ifndef FDEMRI_NO_MERGE
-            // Consecutive items of the list whose bins are disjoint -- the usual case: a segment of a voice ends inside
-            // this warp's 64 bins and the next segment of the same voice starts at the following bin -- share ONE pass:
-            // every (lane, slot) evaluates the item that covers its bin, with its own item constants (per-lane
-            // addresses; FDEMRI_ITEM_STRIDE keeps neighbouring items on different banks).  Without this each of them
-            // would take a whole pass with part of the lanes idle: 5.70 M passes instead of 5.18 M on config 2, where
-            // 5.15 M would use every lane.  A bin still receives its terms in list order, so the sums are the same bit
-            // for bit.  (Measured with the merged pass out of line, for pairs only, with and without the test on the
-            // first item's extent: this form was the fastest.)
-            if (!(flags & 1u) && (lo > wb || hi < wb + 32 * FDEMRI_BPL - 1)) {
-                const double* it0 = it;
-                const double* it1 = it;
-                unsigned fl0 = flags, fl1 = flags;
-                bool m0 = act0, m1 = act1;
+            {
                 int run_lo = lo, run_hi = hi, jn = j + 1;
                 while (jn < FDEMRI_CHUNK && ((todo >> jn) & 1u)) {
                     const double* itB = S->items[jn];
@@ -765,76 +815,34 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
                     if (b1) { it1 = itB; fl1 = (unsigned)metaB.y; }
                     m0 = m0 || b0; m1 = m1 || b1;
                 }
-                if (jn > j + 1) {
-                    const double sf0 = fdemri_xorsign(f0, (fl0 & 4u) << 29), sf1 = fdemri_xorsign(f1, (fl1 & 4u) << 29);
-                    double T0r, T0i, T1r, T1i;
-                    const bool ok0 = fdemri_term_fast(it0, sf0, T0r, T0i);
-                    const bool ok1 = fdemri_term_fast(it1, sf1, T1r, T1i);
-                    const bool bad0 = m0 && !ok0, bad1 = m1 && !ok1;
-                    if (__any_sync(0xffffffffu, bad0 || bad1)) {
-                        if (bad0) {
-                            const FdemriSlowOut o = fdemri_term_slow(it0, sf0, fl0);
-                            T0r = o.tre; T0i = o.tim;
-                            n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
-                        }
-                        if (bad1) {
-                            const FdemriSlowOut o = fdemri_term_slow(it1, sf1, fl1);
-                            T1r = o.tre; T1i = o.tim;
-                            n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
-                        }
-                    }
-                    if (m0) {
-                        a00 = fma(it0[S_WP], T0r, a00); a01 = fma(it0[S_SWP], T0i, a01);
-                        a02 = fma(it0[S_NWX], T0i, a02); a03 = fma(it0[S_SWX], T0r, a03);
-                    }
-                    if (m1) {
-                        a10 = fma(it1[S_WP], T1r, a10); a11 = fma(it1[S_SWP], T1i, a11);
-                        a12 = fma(it1[S_NWX], T1i, a12); a13 = fma(it1[S_SWX], T1r, a13);
-                    }
-                    continue;
-                }
             }
 #endif
-            const double sf0 = fdemri_xorsign(f0, sbit), sf1 = fdemri_xorsign(f1, sbit);
-            double T0r, T0i, T1r, T1i;
-            if (!(flags & 1u)) {
-                // both slots always, also for an item that ends inside this warp's 64 bins and leaves one of them without
-                // a lane: skipping the empty slot (three copies of the fast path behind a warp-uniform branch) was
-                // measured 2 % slower than the few wasted evaluations
-                const bool ok0 = fdemri_term_fast(it, sf0, T0r, T0i);
-                const bool ok1 = fdemri_term_fast(it, sf1, T1r, T1i);
-                const bool bad0 = act0 && !ok0, bad1 = act1 && !ok1;
-                if (__any_sync(0xffffffffu, bad0 || bad1)) {             // one warp-uniform branch: under 1 % of the passes
+            {
+                const double sf0 = fdemri_xorsign(f0, (fl0 & 4u) << 29), sf1 = fdemri_xorsign(f1, (fl1 & 4u) << 29);
+                double T0r, T0i, T1r, T1i;
+                const bool ok0 = fdemri_term_fast(it0, sf0, T0r, T0i);
+                const bool ok1 = fdemri_term_fast(it1, sf1, T1r, T1i);
+                const bool bad0 = m0 && !ok0, bad1 = m1 && !ok1;
+                if (__any_sync(0xffffffffu, bad0 || bad1)) {
                     if (bad0) {
-                        const FdemriSlowOut o = fdemri_term_slow(it, sf0, flags);
+                        const FdemriSlowOut o = fdemri_term_slow(it0, sf0, fl0);
                         T0r = o.tre; T0i = o.tim;
                         n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
                     }
                     if (bad1) {
-                        const FdemriSlowOut o = fdemri_term_slow(it, sf1, flags);
+                        const FdemriSlowOut o = fdemri_term_slow(it1, sf1, fl1);
                         T1r = o.tre; T1i = o.tim;
                         n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
                     }
                 }
-            } else {
-                T0r = T0i = T1r = T1i = 0.0;
-                if (act0) {
-                    const FdemriSlowOut o = fdemri_term_slow(it, sf0, flags);
-                    T0r = o.tre; T0i = o.tim;
-                    n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                if (m0) {
+                    a00 = fma(it0[S_WP], T0r, a00); a01 = fma(it0[S_SWP], T0i, a01);
+                    a02 = fma(it0[S_NWX], T0i, a02); a03 = fma(it0[S_SWX], T0r, a03);
                 }
-                if (act1) {
-                    const FdemriSlowOut o = fdemri_term_slow(it, sf1, flags);
-                    T1r = o.tre; T1i = o.tim;
-                    n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                if (m1) {
+                    a10 = fma(it1[S_WP], T1r, a10); a11 = fma(it1[S_SWP], T1i, a11);
+                    a12 = fma(it1[S_NWX], T1i, a12); a13 = fma(it1[S_SWX], T1r, a13);
                 }
-            }
-            const double wp = it[S_WP], swp = it[S_SWP], nwx = it[S_NWX], swx = it[S_SWX];
-            if (act0) {
-                a00 = fma(wp, T0r, a00); a01 = fma(swp, T0i, a01); a02 = fma(nwx, T0i, a02); a03 = fma(swx, T0r, a03);
-            }
-            if (act1) {
-                a10 = fma(wp, T1r, a10); a11 = fma(swp, T1i, a11); a12 = fma(nwx, T1i, a12); a13 = fma(swx, T1r, a13);
             }
         }
         if (last) {
