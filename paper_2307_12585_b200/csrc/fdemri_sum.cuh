@@ -731,30 +731,42 @@ __device__ __forceinline__ void fdemri_consumer(const SumArgs& a, FdemriRing* ri
             fullm = __ballot_sync(0xffffffffu, whole);
         }
         while (todo) {
-            const int j = __ffs(todo) - 1;
-            todo &= todo - 1;
-            const double* it = S->items[j];
-            if ((fullm >> j) & 1u) {
-                // ---- the common pass: a monotone item that covers every bin of this warp -- no masks ----
+            // ---- the common pass: a monotone item that covers every bin of this warp -- no masks.  Its loop holds nothing
+            // else: a pass that needs the slow path for some lane, and an item of any other kind, leave it and are dealt
+            // with below (with the out-of-line slow path and its call sequence out of the way ptxas compiles the common
+            // pass 5 % faster: 2.55 -> 2.42 ms on config 2) ----
+            int j = 0, state = 0;                // 1: slow-path fix-ups for the pass in hand, 2: another kind of item
+            const double* it = nullptr;
+            double sf0 = 0.0, sf1 = 0.0, T0r = 0.0, T0i = 0.0, T1r = 0.0, T1i = 0.0;
+            bool ok0 = true, ok1 = true;
+            while (todo) {
+                j = __ffs(todo) - 1;
+                todo &= todo - 1;
+                it = S->items[j];
+                if (!((fullm >> j) & 1u)) { state = 2; break; }
                 const unsigned sbit = ((unsigned)reinterpret_cast<const int*>(it)[1] & 4u) << 29;
-                const double sf0 = fdemri_xorsign(f0, sbit), sf1 = fdemri_xorsign(f1, sbit);
-                double T0r, T0i, T1r, T1i;
-                const bool ok0 = fdemri_term_fast(it, sf0, T0r, T0i);
-                const bool ok1 = fdemri_term_fast(it, sf1, T1r, T1i);
-                if (__any_sync(0xffffffffu, !(ok0 && ok1))) {            // one warp-uniform branch: under 1 % of the passes
-                    const unsigned flags = (unsigned)reinterpret_cast<const int*>(it)[1];
-                    if (!ok0) {
-                        const FdemriSlowOut o = fdemri_term_slow(it, sf0, flags);
-                        T0r = o.tre; T0i = o.tim;
-                        n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
-                    }
-                    if (!ok1) {
-                        const FdemriSlowOut o = fdemri_term_slow(it, sf1, flags);
-                        T1r = o.tre; T1i = o.tim;
-                        n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
-                    }
-                }
+                sf0 = fdemri_xorsign(f0, sbit); sf1 = fdemri_xorsign(f1, sbit);
+                ok0 = fdemri_term_fast(it, sf0, T0r, T0i);
+                ok1 = fdemri_term_fast(it, sf1, T1r, T1i);
+                if (__any_sync(0xffffffffu, !(ok0 && ok1))) { state = 1; break; }      // under 1 % of the passes
                 // weights (O2): s=+1: h+ += w+ T, hx += i wx T;  s=-1: h+ += w+ conj(T), hx += conj(i wx T)
+                const double wp = it[S_WP], swp = it[S_SWP], nwx = it[S_NWX], swx = it[S_SWX];
+                a00 = fma(wp, T0r, a00); a01 = fma(swp, T0i, a01); a02 = fma(nwx, T0i, a02); a03 = fma(swx, T0r, a03);
+                a10 = fma(wp, T1r, a10); a11 = fma(swp, T1i, a11); a12 = fma(nwx, T1i, a12); a13 = fma(swx, T1r, a13);
+            }
+            if (state == 0) break;
+            if (state == 1) {
+                const unsigned flags = (unsigned)reinterpret_cast<const int*>(it)[1];
+                if (!ok0) {
+                    const FdemriSlowOut o = fdemri_term_slow(it, sf0, flags);
+                    T0r = o.tre; T0i = o.tim;
+                    n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                }
+                if (!ok1) {
+                    const FdemriSlowOut o = fdemri_term_slow(it, sf1, flags);
+                    T1r = o.tre; T1i = o.tim;
+                    n_airy += o.info & 1u; n_slow += (o.info >> 1) & 1u; errs |= o.info >> 4;
+                }
                 const double wp = it[S_WP], swp = it[S_SWP], nwx = it[S_NWX], swx = it[S_SWX];
                 a00 = fma(wp, T0r, a00); a01 = fma(swp, T0i, a01); a02 = fma(nwx, T0i, a02); a03 = fma(swx, T0r, a03);
                 a10 = fma(wp, T1r, a10); a11 = fma(swp, T1i, a11); a12 = fma(nwx, T1i, a12); a13 = fma(swx, T1r, a13);
