@@ -48,10 +48,10 @@ enum {
     FDEMRI_FLAG_NONE = 0,
     FDEMRI_FLAG_TIMING = 1,    /* record CUDA events around the S3 sum kernel of every fdemri_sum (see
                                   fdemri_get_kernel_ms); costs two event records per call                  */
-    FDEMRI_FLAG_BIN_MAJOR = 2, /* force the bin-major sum kernel (a CTA owns 32 consecutive bins, one warp per bin at a
+    FDEMRI_FLAG_BIN_MAJOR = 2, /* force the bin-major sum kernel (a CTA owns 8, 16 or 32 consecutive bins, one warp per bin at a
                                   time, lanes over the entries that cover it): the right shape when a (voice, segment)
                                   covers only a few bins -- sparse or down-sampled frequency arrays (PAPER.md 3.3)   */
-    FDEMRI_FLAG_TILE_MAJOR = 4 /* force the tile-major sum kernel (a CTA owns 768 consecutive bins): dense grids.
+    FDEMRI_FLAG_TILE_MAJOR = 4 /* force the tile-major sum kernel (a CTA owns 960 consecutive bins): dense grids.
                                   Default: bin-major iff n_freq < 256 (n_knots - 1)                         */
 };
 
