@@ -433,6 +433,52 @@ def test_random_small_cases_sweep(fd, orc):
     assert newton == 0
 
 
+def test_random_wide_sweep_both_kernels(fd, orc):
+    """Eighty seeded cases wider than the sweep above -- up to 24 modes (repeats allowed), 4 to 120 knots, 300 to 80 000 bins,
+    offset grids -- through BOTH sum kernels: per-bin parity on every bin the oracle does not mark boundary-ambiguous (R8),
+    exact zeros outside the support, no flag raised, and evaluation counts that differ from the oracle's by at most the
+    pair of roots an ambiguous bin may gain or lose.  With many voices that have a turnover, more than MAX_AMBIGUOUS bins
+    of a waveform can sit within 16 ulp of an extremum value; the allowance here is one per voice and sign."""
+    from paper_2307_12585_b200 import synth
+    rng = np.random.default_rng(230712585)
+    worst, n_amb, n_ev = 0.0, 0, 0
+    for case in range(80):
+        n_knots = int(rng.choice([rng.integers(4, 40), rng.integers(40, 121)]))
+        modes = []
+        for _ in range(int(rng.integers(1, 25))):
+            l = int(rng.integers(2, 11))
+            modes.append((l, int(rng.integers(0, l + 1)), int(rng.integers(-8, 9))))
+        n_freq = int(rng.choice([rng.integers(300, 5000), rng.integers(5000, 80000)]))
+        w = synth.small_case(seed=3000 + case, n_knots=n_knots, n_freq=n_freq, modes=tuple(modes), turnover=bool(rng.integers(0, 2)))
+        if case % 3 == 0:
+            w.f0 = float(rng.uniform(0.0, 2e-3))
+        w.theta, w.phi = float(rng.uniform(0.05, 3.0)), float(rng.uniform(-3.0, 3.0))
+        ref = oracle_c(orc, w, w.freq_array())
+        keep = ref["ambiguous"] == 0
+        amb = int((~keep).sum())
+        assert amb <= 2 * len(modes), (case, amb)
+        zero = (ref["nterms"] == 0) & keep
+        for flag in (fd.FDEMRI_FLAG_TILE_MAJOR, fd.FDEMRI_FLAG_BIN_MAJOR):
+            wf = fd.waveform_from_workload(w, flags=flag)
+            wf.sum(w.theta, w.phi)
+            hp, hx = wf.result()
+            st = wf.stats()
+            wf.close()
+            assert st["status"] == 0 and st["flags"] == 0, (case, flag, st["flags"])
+            assert abs(st["n_evals"] - ref["n_evals"]) <= 2 * amb, (case, flag, st["n_evals"], ref["n_evals"], amb)
+            if ref["n_evals"] == 0:
+                assert not hp.any() and not hx.any()
+                continue
+            err = max_rel_err(hp[0], hx[0], ref["hplus"], ref["hcross"], mask=keep)
+            assert np.all(hp[0][zero] == 0) and np.all(hx[0][zero] == 0), (case, flag)
+            assert err <= TOL_BIN, (case, flag, modes, err)
+            worst = max(worst, err)
+        n_amb += amb
+        n_ev += ref["n_evals"]
+    print(f"[parity] 80 random wide cases x 2 kernels ({n_ev:.3g} evaluations): worst max|dh|/max|h| = {worst:.3e}; "
+          f"{n_amb} boundary-ambiguous bins in all")
+
+
 @pytest.mark.parametrize("mode", ["bin", "tile"])
 def test_both_sum_kernels_on_the_same_inputs(fd, orc, mode):
     """The bin-major kernel (sparse grids, section 3.3) and the tile-major kernel forced on the same inputs:
